@@ -1,0 +1,155 @@
+"""ctypes loader for the CPU oracle (oracle/gs_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may
+import this package.  It imports nothing from paper_2502_02460_b200 and shares no code with the
+CUDA path.  Each wrapper converts its inputs to column-major (Fortran-order) numpy arrays, calls the
+plain-C routine, and returns new arrays; see gs_oracle.c for the passages each routine follows
+(PAPER.md:61-67).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gs_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp, no -ffast-math, no BLAS."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        i64, p = ctypes.c_int64, ctypes.c_void_p
+        for t in "dz":
+            getattr(lib, f"orc_cholesky_{t}").argtypes = [i64, p]
+            getattr(lib, f"orc_cholesky_{t}").restype = i64
+            getattr(lib, f"orc_invert_upper_{t}").argtypes = [i64, p, p]
+            getattr(lib, f"orc_invert_upper_{t}").restype = i64
+            getattr(lib, f"orc_to_standard_{t}").argtypes = [i64, p, p, p, p]
+            getattr(lib, f"orc_to_standard_{t}").restype = None
+            getattr(lib, f"orc_backtransform_{t}").argtypes = [i64, i64, p, p, p]
+            getattr(lib, f"orc_backtransform_{t}").restype = None
+            getattr(lib, f"orc_jacobi_{t}").argtypes = [i64, p, p, p]
+            getattr(lib, f"orc_jacobi_{t}").restype = i64
+        lib.orc_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+def _f(a, dtype=None) -> np.ndarray:
+    a = np.asarray(a)
+    if dtype is None:
+        dtype = np.complex128 if np.iscomplexobj(a) else np.float64
+    return np.array(a, dtype=dtype, order="F", copy=True)
+
+
+def _sfx(a: np.ndarray) -> str:
+    return "z" if a.dtype == np.complex128 else "d"
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+class NotPositiveDefinite(Exception):
+    def __init__(self, info: int):
+        super().__init__(f"pivot {info} is not positive")
+        self.info = info
+
+
+def cholesky(S) -> np.ndarray:
+    """O1: S = U^H U, returns U (upper, zeros below).  Raises NotPositiveDefinite(info)."""
+    U = _f(S)
+    N = U.shape[0]
+    assert U.shape == (N, N)
+    info = getattr(_load(), f"orc_cholesky_{_sfx(U)}")(N, _ptr(U))
+    if info != 0:
+        raise NotPositiveDefinite(int(info))
+    return U
+
+
+def invert_upper(U) -> np.ndarray:
+    """O2: V = U^-1 by back substitution (reads the upper triangle of U only)."""
+    U = _f(U)
+    N = U.shape[0]
+    V = np.zeros_like(U, order="F")
+    info = getattr(_load(), f"orc_invert_upper_{_sfx(U)}")(N, _ptr(U), _ptr(V))
+    if info != 0:
+        raise ZeroDivisionError(f"U({info},{info}) == 0")
+    return V
+
+
+def to_standard(H, V) -> np.ndarray:
+    """O3: H~ = V^H H V, FULL matrix (both triangles computed independently)."""
+    H = _f(H)
+    V = _f(V, H.dtype)
+    N = H.shape[0]
+    W = np.zeros_like(H, order="F")
+    Ht = np.zeros_like(H, order="F")
+    getattr(_load(), f"orc_to_standard_{_sfx(H)}")(N, _ptr(H), _ptr(V), _ptr(W), _ptr(Ht))
+    return Ht
+
+
+def backtransform(V, Ct) -> np.ndarray:
+    """O4: C = V C~ (no conjugation), C~ is N x nev."""
+    V = _f(V)
+    Ct = _f(Ct, V.dtype)
+    if np.iscomplexobj(Ct) and not np.iscomplexobj(V):
+        V = _f(V, np.complex128)
+    N, nev = Ct.shape
+    C = np.zeros_like(Ct, order="F")
+    if nev > 0:
+        getattr(_load(), f"orc_backtransform_{_sfx(V)}")(N, nev, _ptr(V), _ptr(Ct), _ptr(C))
+    return C
+
+
+def jacobi(A):
+    """O5: cyclic Jacobi, full Hermitian A -> (eps ascending, Q with eigenvectors as columns, sweeps)."""
+    A = _f(A)
+    N = A.shape[0]
+    eps = np.zeros(N, dtype=np.float64)
+    Q = np.zeros_like(A, order="F")
+    sweeps = getattr(_load(), f"orc_jacobi_{_sfx(A)}")(N, _ptr(A), _ptr(eps), _ptr(Q))
+    if sweeps < 0:
+        raise RuntimeError("Jacobi did not converge in 60 sweeps")
+    return eps, Q, int(sweeps)
+
+
+def hermitian_from_upper(Ht_upper) -> np.ndarray:
+    """Mirror the upper triangle (incl. diagonal) into a full Hermitian matrix."""
+    A = np.asarray(Ht_upper)
+    up = np.triu(A, 1)
+    d = np.diag(np.diag(A).real if np.iscomplexobj(A) else np.diag(A))
+    return up + up.conj().T + d
+
+
+def generalized_eigh(H, S, nev=None):
+    """O6: the whole path of PAPER.md:61-67 on the CPU: returns dict with U, V, Ht (full), eps
+    (lowest nev, ascending -- reading Q7), Ct, C."""
+    U = cholesky(S)
+    V = invert_upper(U)
+    Ht = to_standard(H, V)
+    eps, Q, sweeps = jacobi(hermitian_from_upper(Ht))
+    N = U.shape[0]
+    nev = N if nev is None else nev
+    Ct = np.asfortranarray(Q[:, :nev])
+    C = backtransform(V, Ct)
+    return {"U": U, "V": V, "Ht": Ht, "eps": eps[:nev], "Ct": Ct, "C": C, "sweeps": sweeps}
