@@ -1,0 +1,128 @@
+/*
+ * gs.h -- C ABI of libgs: reduction of the dense generalized eigenproblem  H C = eps S C
+ * (H symmetric / Hermitian, S positive definite; Eq. 2) to standard form and the
+ * eigenvector back-transformation, on ONE NVIDIA B200 (sm_100a), FP64.
+ *
+ * The four compute calls are the four steps of PAPER.md:61-67 ("Solving the generalized
+ * eigenproblem"), which ELPA also exposes one by one ("interfaces for each individual
+ * transformation step are also provided"):
+ *
+ *   gs_cholesky           1. Cholesky decomposition S = U^T U, U upper triangular
+ *   gs_invert_triangular  2. inversion of the upper triangular matrix U -> U^-1
+ *   gs_to_standard        3. two matrix products H~ = (U^-1)^T H U^-1
+ *   gs_backtransform         back-transformation C = U^-1 C~
+ *
+ * "A^T corresponds to the transpose or conjugate-transpose of a real- or complex-valued matrix"
+ * (PAPER.md:67).  The standard eigensolve H~ C~ = eps C~ between steps 3 and 4 is NOT part of
+ * this library.
+ *
+ * Conventions common to all calls
+ * -------------------------------
+ * Layout     Column-major, leading dimension = N (LAPACK/ELPA convention; eigenvectors are "stored
+ *            as matrix columns").  C~ and C are N x nev with leading dimension N.
+ *            GS_COMPLEX128 = interleaved (re, im) doubles.
+ * Pointers   Every matrix argument is a DEVICE pointer (cudaMalloc-class memory on the current
+ *            device), 16-byte aligned, caller-owned.  The library never allocates device memory
+ *            for matrices; scratch is the caller-provided workspace (gs_plan_set_workspace).
+ *            Outputs must not alias inputs except the documented in-place S_inout.
+ * Streams    `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *            Compute calls only enqueue work on it and return without synchronising.
+ * Errors     Every call returns a gs_status_t and never throws or exits.  Argument errors are
+ *            returned synchronously.  Numerical failure (a pivot that is not > 0, or NaN, in
+ *            gs_cholesky; a zero diagonal entry in gs_invert_triangular) is recorded in a
+ *            device-side flag as the 1-based index of the first bad pivot; all later compute
+ *            calls on the same plan become no-ops while the flag is set; gs_last_info synchronises
+ *            the stream and reports it.  gs_cholesky clears the flag when it starts.
+ * No CPU fallback exists: without a device of compute capability 10.x plan creation fails with
+ *            GS_ERR_UNSUPPORTED_DEVICE.
+ * Domain     N >= 1, 0 <= nev <= N.  Any N is accepted (ragged edges are handled in the kernels).
+ */
+#ifndef GS_H_
+#define GS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gs_plan gs_plan_t; /* opaque host object */
+
+typedef enum { GS_REAL64 = 0, GS_COMPLEX128 = 1 } gs_dtype_t;
+
+typedef enum {
+    GS_OK = 0,
+    GS_ERR_INVALID_ARG = 1,
+    GS_ERR_NOT_POSDEF = 2,         /* gs_last_info: pivot `info` of S is not positive          */
+    GS_ERR_SINGULAR = 3,           /* gs_last_info: U(info,info) == 0                            */
+    GS_ERR_CUDA = 4,               /* a CUDA runtime/driver call failed                          */
+    GS_ERR_WORKSPACE = 5,          /* workspace missing, too small or misaligned                 */
+    GS_ERR_UNSUPPORTED_DEVICE = 6  /* current device is not compute capability 10.x              */
+} gs_status_t;
+
+/* Create a plan for problems of order N, element type dtype, and nev wanted eigenvectors
+ * (BASELINE.json north_star: gs_plan_create(N, dtype, nev)).  Host-only state (tile schedule,
+ * TMA descriptors are built per call from the pointers).  *plan is set to NULL on failure. */
+gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_t nev);
+gs_status_t gs_plan_destroy(gs_plan_t* plan);
+
+/* Scratch the compute calls need: at most one N x N matrix plus O(N * 128) elements.  The caller
+ * allocates `bytes` of device memory (256-byte aligned) and hands it over; it stays caller-owned
+ * and must outlive every compute call enqueued on the plan.  Contents are undefined between calls. */
+gs_status_t gs_plan_workspace_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_plan_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t bytes);
+
+/* Step 1.  In place: on entry the upper triangle (incl. diagonal) of S_inout holds S
+ * (the strictly-lower part is never read); on exit the upper triangle holds U with real, strictly
+ * positive diagonal, S = U^H U, and the strictly-lower part is zero.
+ * Blocked right-looking POTRF: diagonal blocks factored in shared memory, panel solve and SYRK/HERK
+ * trailing update on FP64 tensor-core (DMMA) tiles. */
+gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream);
+
+/* Step 2.  Reads the upper triangle of U (N x N); writes Uinv = U^-1 (upper
+ * triangle) and zeros below the diagonal.  Uinv must not alias U.  Blocked TRTRI. */
+gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U, void* Uinv, void* cuda_stream);
+
+/* Step 3.  Htilde = Uinv^H * H * Uinv.  Reads all of H (both triangles must hold a
+ * consistent symmetric / Hermitian matrix) and the upper triangle of Uinv.  Writes the UPPER
+ * triangle (incl. diagonal) of Htilde; the strictly-lower part of the Htilde buffer is left
+ * untouched.  For GS_COMPLEX128 the diagonal of Htilde is exactly real.  Fused triangular product
+ * pair: exploits the triangularity of Uinv and forms one triangle of the symmetric result only. */
+gs_status_t gs_to_standard(gs_plan_t* plan, const void* H, const void* Uinv, void* Htilde,
+                           void* cuda_stream);
+
+/* Back-transformation.  C = Uinv * Ctilde over the nev columns of the plan (no
+ * conjugation).  Reads the upper triangle of Uinv and all of Ctilde (N x nev); writes C (N x nev).
+ * nev == 0 is a no-op. */
+gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C,
+                             void* cuda_stream);
+
+/* Synchronises `cuda_stream`, then reports the plan's numerical status: GS_OK with *info = 0, or
+ * GS_ERR_NOT_POSDEF / GS_ERR_SINGULAR with *info = 1-based index of the first bad pivot
+ * (LAPACK-style).  GS_ERR_CUDA if the stream reports an asynchronous error. */
+gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
+
+/* Host-buffer convenience wrapper for end-to-end measurement: copies S and H from HOST memory to
+ * device scratch inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3, copies the
+ * upper-triangular results back.  Any of the host output pointers may be NULL (not copied back).
+ * Scratch needed: gs_reduce_host_scratch_bytes().  Synchronises the stream before returning. */
+gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host_S,
+                           void* host_U, void* host_Uinv, void* host_Htilde,
+                           void* dev_scratch, size_t scratch_bytes, void* cuda_stream);
+gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Uinv, const void* host_Ctilde,
+                                  void* host_C, void* dev_scratch, size_t scratch_bytes,
+                                  void* cuda_stream);
+
+/* Number of kernels the library has launched on behalf of this plan since creation. */
+gs_status_t gs_plan_launch_count(const gs_plan_t* plan, int64_t* launches);
+
+const char* gs_status_string(gs_status_t status);
+/* Text of the last CUDA error seen by this plan ("" if none). */
+const char* gs_plan_last_cuda_error(const gs_plan_t* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GS_H_ */

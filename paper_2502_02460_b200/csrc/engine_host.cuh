@@ -1,0 +1,86 @@
+// engine_host.cuh -- host side of the tile engine: TMA descriptor construction and launch.
+#pragma once
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <cuda_runtime.h>
+
+#include <cstring>
+
+#include "tile_engine.cuh"
+
+namespace gs {
+
+// cuTensorMapEncodeTiled is a driver-API entry point; fetch it through the runtime so libgs does
+// not link libcuda directly.
+inline PFN_cuTensorMapEncodeTiled tensor_map_encoder()
+{
+    static PFN_cuTensorMapEncodeTiled fn = nullptr;
+    if (fn == nullptr) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(p);
+    }
+    return fn;
+}
+
+// Column-major FP64 matrix view: rows x cols, leading dimension ld (elements).  TMA needs a
+// 16-byte aligned base and a row pitch that is a multiple of 16 bytes (even ld).
+struct MatView {
+    const double* ptr;
+    long long rows, cols, ld;
+};
+
+inline bool tma_compatible(const MatView& m)
+{
+    return (reinterpret_cast<uintptr_t>(m.ptr) % 16 == 0) && (m.ld % 2 == 0);
+}
+
+// box = box_rows (contiguous dim, always 16 doubles = 128 B) x box_cols
+inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols)
+{
+    PFN_cuTensorMapEncodeTiled enc = tensor_map_encoder();
+    if (enc == nullptr) return false;
+    cuuint64_t dims[2] = {static_cast<cuuint64_t>(m.rows), static_cast<cuuint64_t>(m.cols)};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(m.ld) * 8};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(BK), static_cast<cuuint32_t>(box_cols)};
+    cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(m.ptr), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+inline int num_tiles(const EngineParams& p)
+{
+    const bool tri = p.order >= ORDER_TRI_ROW_DESC;
+    const int per = tri ? p.tiles_n * (p.tiles_n + 1) / 2 : p.tiles_m * p.tiles_n;
+    return per * p.batch;
+}
+
+inline cudaError_t engine_configure()
+{
+    static bool done = false;
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(tile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return e;
+    done = true;
+    return cudaSuccess;
+}
+
+// a_nn: A operand is m-contiguous (A stored M x K).  Returns cudaSuccess or the launch error.
+inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, cudaStream_t stream)
+{
+    const int grid = num_tiles(p);
+    if (grid <= 0) return cudaSuccess;
+    cudaError_t e = engine_configure();
+    if (e != cudaSuccess) return e;
+    if (a_nn) tile_engine_kernel<true><<<grid, kThreads, kSmemBytes, stream>>>(p);
+    else tile_engine_kernel<false><<<grid, kThreads, kSmemBytes, stream>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace gs
