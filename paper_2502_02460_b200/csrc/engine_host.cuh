@@ -63,23 +63,34 @@ inline cudaError_t engine_configure()
 {
     static bool done = false;
     if (done) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(tile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    cudaError_t e = cudaFuncSetAttribute(tile_engine_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(tile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    e = cudaFuncSetAttribute(tile_engine_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tile_engine_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tile_engine_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e != cudaSuccess) return e;
     done = true;
     return cudaSuccess;
 }
 
 // a_nn: A operand is m-contiguous (A stored M x K).  Returns cudaSuccess or the launch error.
-inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, cudaStream_t stream)
+// use_tma: every operand satisfies tma_compatible() and the tensor maps in p are valid; otherwise
+// the plain-load producer reads through p.raw*.
+inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, bool use_tma, cudaStream_t stream)
 {
     const int grid = num_tiles(p);
     if (grid <= 0) return cudaSuccess;
     cudaError_t e = engine_configure();
     if (e != cudaSuccess) return e;
-    if (a_nn) tile_engine_kernel<true><<<grid, kThreads, kSmemBytes, stream>>>(p);
-    else tile_engine_kernel<false><<<grid, kThreads, kSmemBytes, stream>>>(p);
+    if (use_tma) {
+        if (a_nn) tile_engine_kernel<true, true><<<grid, kThreads, kSmemBytes, stream>>>(p);
+        else tile_engine_kernel<false, true><<<grid, kThreads, kSmemBytes, stream>>>(p);
+    } else {
+        if (a_nn) tile_engine_kernel<true, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
+        else tile_engine_kernel<false, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
+    }
     return cudaGetLastError();
 }
 

@@ -64,8 +64,17 @@ struct OperandCoord {
     int bk, bx;     // per-batch increments
 };
 
+// Raw view of an operand matrix for the non-TMA loader (odd leading dimension: a row pitch that is
+// not a multiple of 16 bytes cannot be described by a tensor map).
+struct RawOperand {
+    const double* ptr;
+    long long ld;
+    int rows, cols;
+};
+
 struct EngineParams {
     CUtensorMap mapA, mapB, mapA2, mapB2;
+    RawOperand rawA, rawB, rawA2, rawB2;
     double* C;
     long long ldc;
     const int* info;              // device flag: non-zero => the whole launch is a no-op
@@ -149,7 +158,35 @@ __device__ __forceinline__ void mask_tile(unsigned char* tile, int k0, int x0, b
     }
 }
 
-template <bool kANN>
+// Non-TMA tile loaders (one warp): bounds-checked 8-byte global loads written into the same swizzled
+// shared-memory layout the TMA path produces; out-of-range elements are zero, as TMA's OOB fill.
+__device__ __forceinline__ void load_tile_kcontig(unsigned char* tile, const RawOperand& m, int k0, int x0, int lane)
+{
+    // element (k, x): global (row = k0 + k, col = x0 + x); smem offset x*128 + ((k>>1) ^ (x&7))*16 + (k&1)*8
+    for (int idx = lane; idx < BM * BK; idx += 32) {
+        const int x = idx >> 4, k = idx & 15;
+        const long long row = k0 + k, col = x0 + x;
+        double v = 0.0;
+        if (row >= 0 && col >= 0 && row < m.rows && col < m.cols) v = m.ptr[row + col * m.ld];
+        *reinterpret_cast<double*>(tile + x * 128 + (((k >> 1) ^ (x & 7)) * 16) + (k & 1) * 8) = v;
+    }
+}
+
+__device__ __forceinline__ void load_tile_mcontig(unsigned char* tile, const RawOperand& m, int k0, int x0, int lane)
+{
+    // element (mm, k): global (row = x0 + mm, col = k0 + k); box mb = mm>>4, mi = mm&15:
+    // smem offset mb*2048 + k*128 + ((mi>>1) ^ (k&7))*16 + (mi&1)*8
+    for (int idx = lane; idx < BM * BK; idx += 32) {
+        const int k = idx >> 7, mm = idx & 127;
+        const int mb = mm >> 4, mi = mm & 15;
+        const long long row = x0 + mm, col = k0 + k;
+        double v = 0.0;
+        if (row >= 0 && col >= 0 && row < m.rows && col < m.cols) v = m.ptr[row + col * m.ld];
+        *reinterpret_cast<double*>(tile + mb * 2048 + k * 128 + (((mi >> 1) ^ (k & 7)) * 16) + (mi & 1) * 8) = v;
+    }
+}
+
+template <bool kANN, bool kTMA>
 __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_constant__ EngineParams p)
 {
     if (p.info != nullptr && *p.info != 0) return;
@@ -190,6 +227,27 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
     const int b2_x = p.b2.x0 + b * p.b2.bx + BN * J, b2_k = p.b2.k0 + b * p.b2.bk;
 
     if (warp == kConsumerWarps) {
+        if (!kTMA) {
+            // ===================== plain-load producer (whole warp) =====================
+            for (int s = 0; s < nsteps; ++s) {
+                const int stage = s % kStages;
+                const uint32_t ph = (s / kStages) & 1;
+                mbar_wait(empty0 + 8 * stage, ph ^ 1);
+                unsigned char* st = smem + stage * kStageBytes;
+                const bool second = dual && (s & 1);
+                const int kt = k_lo + (dual ? (s >> 1) : s);
+                const RawOperand& rA = second ? p.rawA2 : p.rawA;
+                const RawOperand& rB = second ? p.rawB2 : p.rawB;
+                const int ax = second ? a2_x : a_x, ak = (second ? a2_k : a_k) + kt * BK;
+                const int bx = second ? b2_x : b_x, bk = (second ? b2_k : b_k) + kt * BK;
+                if (kANN) load_tile_mcontig(st, rA, ak, ax, lane);
+                else load_tile_kcontig(st, rA, ak, ax, lane);
+                load_tile_kcontig(st + kTileBytes, rB, bk, bx, lane);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full0 + 8 * stage);
+            }
+            return;
+        }
         // ===================== TMA producer (one elected lane) =====================
         if (lane == 0) {
             tma_prefetch_desc(&p.mapA);

@@ -1,0 +1,221 @@
+"""Thin ctypes binding of the C ABI in include/gs.h (same names, argument marshalling only).
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+libgs.so.  Loading fails loudly if the library has not been built -- there is no fallback.
+
+    plan = gs.Plan(N, nev=nev)                 # gs_plan_create + workspace from torch
+    plan.cholesky(S)                           # in place, S column-major torch tensor on the GPU
+    plan.invert_triangular(U, Uinv)
+    plan.to_standard(H, Uinv, Htilde)
+    plan.backtransform(Uinv, Ctilde, C)
+    plan.last_info()                           # synchronises; raises GsError on numerical failure
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from .workloads import is_colmajor
+
+GS_REAL64, GS_COMPLEX128 = 0, 1
+GS_OK = 0
+STATUS_NAMES = {
+    0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_NOT_POSDEF", 3: "GS_ERR_SINGULAR",
+    4: "GS_ERR_CUDA", 5: "GS_ERR_WORKSPACE", 6: "GS_ERR_UNSUPPORTED_DEVICE",
+}
+EXPORTS = (
+    "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
+    "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_last_info",
+    "gs_reduce_host_scratch_bytes", "gs_reduce_host", "gs_backtransform_host",
+    "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
+)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgs.so")
+PEAK_LIB_PATH = os.path.join(_HERE, "libgs_peak.so")
+_lib = None
+_peak = None
+
+
+class GsError(RuntimeError):
+    def __init__(self, status: int, info: int = 0, detail: str = ""):
+        self.status = status
+        self.info = info
+        name = STATUS_NAMES.get(status, f"status {status}")
+        super().__init__(f"{name}" + (f" (info={info})" if info else "") + (f": {detail}" if detail else ""))
+
+
+def lib() -> ctypes.CDLL:
+    """Load libgs.so.  Raises (never falls back) if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2502_02460_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t
+        L.gs_plan_create.argtypes = [ctypes.POINTER(vp), i64, ctypes.c_int, i64]
+        L.gs_plan_destroy.argtypes = [vp]
+        L.gs_plan_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        L.gs_plan_set_workspace.argtypes = [vp, vp, sz]
+        L.gs_cholesky.argtypes = [vp, vp, vp]
+        L.gs_invert_triangular.argtypes = [vp, vp, vp, vp]
+        L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
+        L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        L.gs_reduce_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.gs_backtransform_host.argtypes = [vp, vp, vp, vp, vp, sz, vp]
+        L.gs_plan_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
+        L.gs_status_string.argtypes = [ctypes.c_int]
+        L.gs_status_string.restype = ctypes.c_char_p
+        L.gs_plan_last_cuda_error.argtypes = [vp]
+        L.gs_plan_last_cuda_error.restype = ctypes.c_char_p
+        for name in EXPORTS:
+            if name not in ("gs_status_string", "gs_plan_last_cuda_error"):
+                getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def peak_lib() -> ctypes.CDLL:
+    global _peak
+    if _peak is None:
+        if not os.path.exists(PEAK_LIB_PATH):
+            raise FileNotFoundError(f"{PEAK_LIB_PATH} not found: run `python -m paper_2502_02460_b200.build`")
+        L = ctypes.CDLL(PEAK_LIB_PATH)
+        L.gs_peak_fp64.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double)]
+        L.gs_peak_fp64.restype = ctypes.c_double
+        _peak = L
+    return _peak
+
+
+def measure_fp64_peak(kind: int = 0, seconds: float = 1.0):
+    """(sustained TFLOP/s, burst TFLOP/s) of the FP64 tensor pipe (kind 0, DMMA) or DFMA (kind 1)."""
+    burst = ctypes.c_double(0.0)
+    sus = peak_lib().gs_peak_fp64(kind, seconds, ctypes.byref(burst))
+    if sus < 0:
+        raise RuntimeError("FP64 peak microbenchmark failed (CUDA error)")
+    return float(sus), float(burst.value)
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev_ptr(t: torch.Tensor, rows: int, cols: int, dtype) -> int:
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor")
+    if t.dtype != dtype or tuple(t.shape) != (rows, cols) or not is_colmajor(t):
+        raise ValueError(f"expected column-major {dtype} tensor of shape ({rows}, {cols}), got "
+                         f"{t.dtype} {tuple(t.shape)} strides {t.stride()}")
+    return t.data_ptr()
+
+
+class Plan:
+    """gs_plan_t plus its torch-owned workspace."""
+
+    def __init__(self, N: int, nev: int | None = None, dtype: int = GS_REAL64, device=None):
+        self.N = int(N)
+        self.nev = self.N if nev is None else int(nev)
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == GS_REAL64 else torch.complex128
+        self._h = ctypes.c_void_p()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        L = lib()
+        with torch.cuda.device(self.device):
+            self._check(L.gs_plan_create(ctypes.byref(self._h), self.N, dtype, self.nev))
+            n = ctypes.c_size_t(0)
+            self._check(L.gs_plan_workspace_bytes(self._h, ctypes.byref(n)))
+            self.workspace = torch.empty(n.value, dtype=torch.uint8, device=self.device)
+            self._check(L.gs_plan_set_workspace(self._h, self.workspace.data_ptr(), n.value))
+
+    def _check(self, status: int, info: int = 0):
+        if status != GS_OK:
+            detail = ""
+            if self._h:
+                detail = lib().gs_plan_last_cuda_error(self._h).decode()
+            raise GsError(status, info, detail)
+
+    def close(self):
+        if self._h:
+            lib().gs_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the four steps of PAPER.md:61-67 ----
+    def cholesky(self, S: torch.Tensor, stream=None):
+        self._check(lib().gs_cholesky(self._h, _dev_ptr(S, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+
+    def invert_triangular(self, U: torch.Tensor, Uinv: torch.Tensor, stream=None):
+        self._check(lib().gs_invert_triangular(self._h, _dev_ptr(U, self.N, self.N, self.tdtype),
+                                               _dev_ptr(Uinv, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+
+    def to_standard(self, H: torch.Tensor, Uinv: torch.Tensor, Htilde: torch.Tensor, stream=None):
+        self._check(lib().gs_to_standard(self._h, _dev_ptr(H, self.N, self.N, self.tdtype),
+                                         _dev_ptr(Uinv, self.N, self.N, self.tdtype),
+                                         _dev_ptr(Htilde, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+
+    def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, C: torch.Tensor, stream=None):
+        if self.nev == 0:
+            self._check(lib().gs_backtransform(self._h, None, None, None, _stream_ptr(stream)))
+            return
+        self._check(lib().gs_backtransform(self._h, _dev_ptr(Uinv, self.N, self.N, self.tdtype),
+                                           _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
+                                           _dev_ptr(C, self.N, self.nev, self.tdtype), _stream_ptr(stream)))
+
+    def last_info(self, stream=None, raise_on_failure: bool = True) -> int:
+        info = ctypes.c_int64(0)
+        status = lib().gs_last_info(self._h, _stream_ptr(stream), ctypes.byref(info))
+        if status != GS_OK and raise_on_failure:
+            self._check(status, int(info.value))
+        return int(info.value)
+
+    def launch_count(self) -> int:
+        n = ctypes.c_int64(0)
+        self._check(lib().gs_plan_launch_count(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    # ---- host-buffer entry points (end-to-end measurement) ----
+    def host_scratch_bytes(self) -> int:
+        n = ctypes.c_size_t(0)
+        self._check(lib().gs_reduce_host_scratch_bytes(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    def reduce_host(self, H: torch.Tensor, S: torch.Tensor, U, Uinv, Htilde, scratch: torch.Tensor, stream=None):
+        """H, S (and the optional outputs) are pinned HOST tensors, column-major."""
+        def hp(t):
+            return None if t is None else t.data_ptr()
+        self._check(lib().gs_reduce_host(self._h, hp(H), hp(S), hp(U), hp(Uinv), hp(Htilde), scratch.data_ptr(),
+                                         scratch.numel() * scratch.element_size(), _stream_ptr(stream)))
+
+    def backtransform_host(self, Uinv, Ctilde, C, scratch: torch.Tensor, stream=None):
+        self._check(lib().gs_backtransform_host(self._h, Uinv.data_ptr(), Ctilde.data_ptr(), C.data_ptr(),
+                                                scratch.data_ptr(), scratch.numel() * scratch.element_size(),
+                                                _stream_ptr(stream)))
+
+
+def generalized_to_standard(H: torch.Tensor, S: torch.Tensor, nev: int | None = None):
+    """Convenience: run steps 1-3 on fresh buffers.  Returns (plan, U, Uinv, Htilde); S is not modified."""
+    from .workloads import colmajor_empty, colmajor_zeros
+    N = H.shape[0]
+    plan = Plan(N, nev)
+    U = colmajor_empty(N, N, device=H.device)
+    U.copy_(S)
+    Uinv = colmajor_empty(N, N, device=H.device)
+    Ht = colmajor_zeros(N, N, device=H.device)
+    plan.cholesky(U)
+    plan.invert_triangular(U, Uinv)
+    plan.to_standard(H, Uinv, Ht)
+    plan.last_info()
+    return plan, U, Uinv, Ht
