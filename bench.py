@@ -1,0 +1,426 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the generalized -> standard reduction + back-transform.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (gs_cholesky, gs_invert_triangular, gs_to_standard,
+gs_backtransform: PAPER.md:61-67) over one seeded synthetic pencil of BASELINE.json `configs[2]`
+(N = 16384 real FP64, nev = 4096).  Metric: FP64 TFLOP/s with the nominal flop counts of
+BASELINE.json (N^3/3 + N^3/3 + N^3 + N^2 nev).  Prints ONE JSON line (rank 0).
+
+N > 1 GPUs: the path does not shard (replicas only) -- every rank reduces its
+own independent pencil (different seed; the paper's "trivial parallelism" over k-points / spin
+channels), no data-path collective; value = all ranks' flops / max-over-ranks time.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload; it is the reference arm of the contract for this tier.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "FP64 TFLOP/s of Cholesky+invert+transform+backtransform at N=16384; % FP64 peak"
+UNIT = "TFLOP/s"
+STAGES = ("cholesky", "invert", "to_standard", "backtransform")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2 = headline)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-sample", type=int, default=4096, help="order of the leading block the oracle is timed on")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-checks", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: sample SM clock and throttle reasons DURING the timed region (NVML, background thread)
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {
+        0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+        0x80: "hw_power_brake", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def start(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle timing (reported baseline / reference arm).  The oracle is timed as it stands.
+# ------------------------------------------------------------------------------------------------
+def oracle_step(k: int, inputs=None):
+    """One pass of the oracle's four stages on the BASELINE recipe at order k, nev = k/4.
+    Returns (seconds, per-stage seconds, inputs)."""
+    import oracle
+    from paper_2502_02460_b200 import workloads as wl
+
+    if inputs is None:
+        p = wl.make_pencil(k, wl.scaled_box(k), wl.BASE_SEED + 1)   # configs[1]'s seed when k = 4096
+        inputs = (p.H.numpy(), p.S.numpy(), wl.dense_rhs(k, k // 4, 1).numpy())
+    H, S, Ct = inputs
+    t0 = time.perf_counter()
+    U = oracle.cholesky(S)
+    t1 = time.perf_counter()
+    V = oracle.invert_upper(U)
+    t2 = time.perf_counter()
+    oracle.to_standard(H, V)
+    t3 = time.perf_counter()
+    oracle.backtransform(V, Ct)
+    t4 = time.perf_counter()
+    return t4 - t0, dict(zip(STAGES, (t1 - t0, t2 - t1, t3 - t2, t4 - t3))), inputs
+
+
+def cpu_baseline(k: int) -> dict:
+    import oracle
+    from paper_2502_02460_b200 import workloads as wl
+
+    sec, stages, _ = oracle_step(k)
+    fl = wl.nominal_flops(k, k // 4)["total"]
+    return {"value": fl / sec / 1e12, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"one pass of the four oracle stages on the BASELINE recipe at N={k}, nev={k // 4} "
+                      f"(configs[1] size; the full N=16384 oracle would take hours)",
+            "seconds": sec, "stage_seconds": stages}
+
+
+def run_reference(args):
+    """Reference arm: the CPU oracle on the host cores, rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    from paper_2502_02460_b200 import workloads as wl
+
+    # size the per-step sample so that the whole (warmup + steps) run ends within ~3 minutes:
+    # probe the oracle's rate at N=1024, then take the largest order whose predicted cost fits
+    probe_sec, _, _ = oracle_step(1024)
+    k = 1024
+    for cand in (args.cpu_sample, 3072, 2048):
+        if cand <= args.cpu_sample and probe_sec * (cand / 1024.0) ** 3 * (args.steps + args.warmup) <= 180.0:
+            k = cand
+            break
+    fl = wl.nominal_flops(k, k // 4)["total"]
+    inputs = None
+    warm = args.warmup
+    for _ in range(warm):
+        _, _, inputs = oracle_step(k, inputs)
+    total = 0.0
+    for _ in range(args.steps):
+        sec, _, inputs = oracle_step(k, inputs)
+        total += sec
+    value = fl * args.steps / total / 1e12
+    cfg = wl.CONFIGS[args.config]
+    sample = (f"each step = one pass of the four oracle stages on the BASELINE recipe at N={k}, nev={k // 4} "
+              f"(bounded sample of {cfg.name}); warm-up passes run: {warm}")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "sample_N": k, "sample_nev": k // 4},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------
+def _measured_peaks() -> dict:
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+def _ncu_traffic(label: str):
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    try:
+        d = json.load(open(os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")))
+        return d.get(label)
+    except Exception:
+        return None
+
+
+def _nvml_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+    ids = [v for v in vis.split(",") if v.strip()]
+    if local_rank < len(ids) and ids[local_rank].strip().isdigit():
+        return int(ids[local_rank])
+    return local_rank
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2502_02460_b200 import gs
+    from paper_2502_02460_b200 import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    cfg = wl.CONFIGS[args.config]
+    if cfg.complex:
+        raise SystemExit("bench.py: the complex (Hermitian) path is not built yet (DESIGN.md, out of scope this round)")
+    N, nev = cfg.N, cfg.nev
+    flops = wl.nominal_flops(N, nev)
+
+    # every rank reduces its own independent pencil (replicas; different seed per rank)
+    pencil = wl.make_pencil(N, cfg.box, cfg.seed + 100 * rank, device=dev)
+    H, S0 = pencil.H, pencil.S
+    U = wl.colmajor_empty(N, N, device=dev)
+    V = wl.colmajor_empty(N, N, device=dev)
+    Ht = wl.colmajor_zeros(N, N, device=dev)
+    Ct = wl.dense_rhs(N, nev, seed=rank, device=dev)
+    C = wl.colmajor_empty(N, nev, device=dev)
+    plan = gs.Plan(N, nev, device=dev)
+
+    # FP64 roofline denominator, measured on this device right now (MEASURED_PEAKS.json has no FP64 entry)
+    dmma_sus, dmma_burst = gs.measure_fp64_peak(0, 1.0)
+    dfma_sus, dfma_burst = gs.measure_fp64_peak(1, 0.5)
+    fp64_peak = max(dmma_sus, dfma_sus)
+
+    def one_step(ev=None):
+        U.copy_(S0)                       # restore S (outside the per-step events)
+        if ev is not None:
+            ev[0].record()
+        plan.cholesky(U)
+        if ev is not None:
+            ev[1].record()
+        plan.invert_triangular(U, V)
+        if ev is not None:
+            ev[2].record()
+        plan.to_standard(H, V, Ht)
+        if ev is not None:
+            ev[3].record()
+        plan.backtransform(V, Ct, C)
+        if ev is not None:
+            ev[4].record()
+
+    for _ in range(args.warmup):
+        one_step()
+    plan.last_info()
+    torch.cuda.synchronize()
+    barrier()
+
+    sampler = ClockSampler(_nvml_index(local_rank))
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    plan.set_timing(2)                    # CUDA events around the dominant kernel only (2 events / step)
+    launches0 = plan.launch_count()
+    sampler.start()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        one_step(events[k])
+    plan.last_info()                      # synchronises the stream, raises on numerical failure
+    torch.cuda.synchronize()
+    wall1 = time.perf_counter()
+    clocks = sampler.stop()
+    barrier()
+    launches = plan.launch_count() - launches0
+    dom = plan.launch_times().get("to_standard.syr2k", (0, 0.0))
+    plan.set_timing(0)
+
+    stage_ms = [sum(e[i].elapsed_time(e[i + 1]) for e in events) / args.steps for i in range(4)]
+    step_ms = max_over_ranks(sum(stage_ms))
+    value = world * flops["total"] / (step_ms * 1e-3) / 1e12
+
+    # per-kernel device times: one extra (untimed) step with events around every launch
+    plan.set_timing(1)
+    one_step()
+    plan.last_info()
+    kernels = {k: {"launches": n, "ms": round(ms, 3)} for k, (n, ms) in plan.launch_times().items()}
+    plan.set_timing(0)
+
+    # roofline of the dominant kernel: the SYR2K-shaped launch of gs_to_standard (2N^3/3 flop of the
+    # nominal 2.67 N^3-ish path: the largest single launch), timed live with CUDA events above
+    dom_flop = 2.0 * float(N) ** 3 / 3.0
+    dom_ms = dom[1] / max(dom[0], 1)
+    achieved = dom_flop / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else None
+    mp = _measured_peaks()
+    roofline = {
+        "bound": "tensor", "kernel": "tile_engine_kernel<TN,TMA> as to_standard.syr2k (FP64 DMMA)",
+        "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+        "frac": (achieved / fp64_peak) if achieved else None,
+        "traffic": _ncu_traffic("to_standard.syr2k"),
+        "algorithmic_flop_per_launch": dom_flop, "launch_ms": dom_ms, "launches_timed": dom[0],
+        "peak_source": "measured live on this device: sustained mma.sync.m8n8k4.f64 (DMMA) microbenchmark "
+                       "(libgs_peak.so); MEASURED_PEAKS.json has no FP64 entry",
+        "peaks": {"dmma_sustained": dmma_sus, "dmma_burst": dmma_burst, "dfma_sustained": dfma_sus,
+                  "dfma_burst": dfma_burst,
+                  "bf16_measured_x_nominal_ratio": (mp.get("bf16_tflops_sustained", 0.0) * 40.0 / 2250.0) or None,
+                  "hbm_gbs_measured": mp.get("hbm_gbs")},
+    }
+
+    stages = {}
+    for name, ms in zip(STAGES, stage_ms):
+        stages[name] = {"ms": round(ms, 3), "tflops": flops[name] / (ms * 1e-3) / 1e12,
+                        "frac_of_fp64_peak": flops[name] / (ms * 1e-3) / 1e12 / fp64_peak}
+
+    # ---- checks (off the timed region, plain torch FP64 on the device) ----
+    checks = None
+    if not args.no_checks and rank == 0:
+        Ut = torch.triu(U)
+        checks = {
+            "chol_resid_fro": ((Ut.t() @ Ut - S0).norm() / S0.norm()).item(),
+            "lower_U_max": torch.tril(U, -1).abs().max().item(),
+            "lower_Uinv_max": torch.tril(V, -1).abs().max().item(),
+        }
+        R = Ut @ V
+        R.diagonal().sub_(1.0)
+        checks["U_Uinv_minus_I_fro_over_sqrtN"] = R.norm().item() / N ** 0.5
+        del R
+        Href = V.t() @ (H @ V)
+        checks["Htilde_rel_fro_vs_torch"] = (torch.triu(Ht - Href).norm() / torch.triu(Href).norm()).item()
+        del Href
+        Cref = V @ Ct
+        checks["C_rel_fro_vs_torch"] = ((C - Cref).norm() / Cref.norm()).item()
+        del Cref, Ut
+        checks["ok"] = bool(checks["chol_resid_fro"] < 1e-13 and checks["U_Uinv_minus_I_fro_over_sqrtN"] < 1e-11 and
+                            checks["Htilde_rel_fro_vs_torch"] < 1e-11 and checks["C_rel_fro_vs_torch"] < 1e-11 and
+                            checks["lower_U_max"] == 0.0 and checks["lower_Uinv_max"] == 0.0)
+
+    # ---- end to end through the host-buffer C ABI calls (pinned host memory, copies inside the timing) ----
+    e2e = None
+    if not args.no_e2e:
+        del U, Ht, C
+        torch.cuda.empty_cache()
+        hH = torch.empty((N, N), dtype=torch.float64).pin_memory()
+        hS = torch.empty((N, N), dtype=torch.float64).pin_memory()
+        hHt = torch.empty((N, N), dtype=torch.float64).pin_memory()
+        hCt = torch.empty((nev, N), dtype=torch.float64).pin_memory()
+        hC = torch.empty((nev, N), dtype=torch.float64).pin_memory()
+        hH.copy_(H.t())           # buffers hold the column-major images
+        hS.copy_(S0.t())
+        hCt.copy_(Ct.t())
+        scratch = torch.empty(plan.host_scratch_bytes(), dtype=torch.uint8, device=dev)
+        e2e_steps = max(1, min(args.steps, 3))
+
+        def e2e_step():
+            plan.reduce_host(hH, hS, None, None, hHt, scratch)
+            plan.backtransform_host(hCt, hC, scratch)
+
+        e2e_step()
+        torch.cuda.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        barrier()
+        e2e_sec = max_over_ranks((t1 - t0) / e2e_steps)
+        e2e = {"value": world * flops["total"] / e2e_sec / 1e12, "unit": UNIT,
+               "h2d_bytes_per_step": 2 * N * N * 8 + N * nev * 8, "d2h_bytes_per_step": N * N * 8 + N * nev * 8,
+               "ms_per_step": e2e_sec * 1e3, "steps": e2e_steps,
+               "api": "gs_reduce_host + gs_backtransform_host (pinned host buffers in, H~ and C out)"}
+        if checks is not None:
+            # the host-buffer path must reproduce the device-buffer path bit for bit (same kernels, same order)
+            plan.to_standard(H, V, Ht2 := wl.colmajor_zeros(N, N, device=dev))
+            plan.last_info()
+            checks["e2e_Htilde_equals_device_path"] = bool(torch.equal(torch.triu(hHt.t().to(dev)), torch.triu(Ht2)))
+            del Ht2
+        del scratch, hH, hS, hHt, hCt, hC
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(args.cpu_sample)
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
+                       "recipe": "BASELINE.json configs[%d]: Gaussian-overlap S, H = -S(1+0.1g)+diag" % cfg.index,
+                       "parallelism": "replicas x%d (one independent pencil per GPU)" % world,
+                       "cache": "inputs_larger_than_L2 (each matrix %.1f GiB vs 126 MB L2)" % (N * N * 8 / 2 ** 30),
+                       "timing": "CUDA events per step on the launching stream; S restored between steps outside the events"},
+            "frac_of_fp64_peak": value / world / fp64_peak, "fp64_peak_tflops": fp64_peak,
+            "stages": stages, "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks, "checks": checks,
+            "wall_s_timed_region": wall1 - wall0,
+            "paper_context": "PAPER.md:133 Table 1 (ELPA 2024.05, NCCL, 4x A100-40GB, N=40960, nev=N): Cholesky 2.3 s, "
+                             "Invert 1.8 s, Multiply 18.8 s, Backtr. 6.8 s = 29.7 s, i.e. ~6.2 TFLOP/s on 4 GPUs (context only)",
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

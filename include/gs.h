@@ -103,17 +103,33 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctil
  * (LAPACK-style).  GS_ERR_CUDA if the stream reports an asynchronous error. */
 gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 
-/* Host-buffer convenience wrapper for end-to-end measurement: copies S and H from HOST memory to
- * device scratch inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3, copies the
- * upper-triangular results back.  Any of the host output pointers may be NULL (not copied back).
- * Scratch needed: gs_reduce_host_scratch_bytes().  Synchronises the stream before returning. */
+/* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
+ * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
+ * inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3 there and copies H~ (the whole
+ * N x N buffer; its upper triangle is the result, the strictly-lower part is zero) back to
+ * host_Htilde.  host_U / host_Uinv may be NULL (then they are not copied back).  U^-1 stays in the
+ * scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in, forms
+ * C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report numerical
+ * failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte aligned. */
 gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes);
 gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host_S,
                            void* host_U, void* host_Uinv, void* host_Htilde,
                            void* dev_scratch, size_t scratch_bytes, void* cuda_stream);
-gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Uinv, const void* host_Ctilde,
-                                  void* host_C, void* dev_scratch, size_t scratch_bytes,
-                                  void* cuda_stream);
+gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void* host_C,
+                                  void* dev_scratch, size_t scratch_bytes, void* cuda_stream);
+
+/* Optional per-launch device timing (CUDA events on the launching stream), for roofline reports.
+ * mode 0 = off (default); 1 = every kernel launch; 2 = only the dominant kernel (the SYR2K-shaped
+ * launch of gs_to_standard).  gs_plan_launch_times synchronises nothing: call it after the stream
+ * has been synchronised.  It fills up to `cap` entries (label, launches, total milliseconds)
+ * accumulated since the last gs_plan_set_timing call and returns the number of labels in *count. */
+typedef struct {
+    char label[32];
+    int64_t launches;
+    double ms;
+} gs_launch_time_t;
+gs_status_t gs_plan_set_timing(gs_plan_t* plan, int mode);
+gs_status_t gs_plan_launch_times(gs_plan_t* plan, gs_launch_time_t* out, int cap, int* count);
 
 /* Number of kernels the library has launched on behalf of this plan since creation. */
 gs_status_t gs_plan_launch_count(const gs_plan_t* plan, int64_t* launches);

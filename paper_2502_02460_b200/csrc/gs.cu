@@ -15,21 +15,38 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "engine_host.cuh"
 #include "leaf_kernels.cuh"
 
 using namespace gs;
 
+// launch labels for the optional per-launch timing (gs_plan_set_timing)
+enum LaunchLabel : int {
+    L_POTRF_LEAF = 0, L_POTRF_TRSM, L_POTRF_GEMM, L_POTRF_SYRK, L_ZERO_LOWER,
+    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_COUNT
+};
+static const char* const kLabelNames[L_COUNT] = {
+    "potrf.leaf", "potrf.trsm_leaf", "potrf.gemm", "potrf.syrk", "zero_lower",
+    "trtri.leaf", "trtri.w", "trtri.x", "to_standard.g", "to_standard.syr2k", "backtransform.trmm"};
+
+struct TimedLaunch {
+    int label;
+    cudaEvent_t e0, e1;
+};
+
 struct gs_plan {
-    int64_t N;
-    int64_t nev;
-    gs_dtype_t dtype;
-    int nblk;              // ceil(N / 128)
-    unsigned char* ws;     // caller-owned device workspace
-    size_t ws_bytes;
-    int64_t launches;
-    char cuda_error[256];
+    int64_t N = 0;
+    int64_t nev = 0;
+    gs_dtype_t dtype = GS_REAL64;
+    int nblk = 0;                    // ceil(N / 128)
+    unsigned char* ws = nullptr;     // caller-owned device workspace
+    size_t ws_bytes = 0;
+    int64_t launches = 0;
+    int timing_mode = 0;
+    std::vector<TimedLaunch> timed;
+    char cuda_error[256] = {0};
 };
 
 namespace {
@@ -48,6 +65,40 @@ gs_status_t cuda_fail(gs_plan* p, cudaError_t e)
 {
     if (p != nullptr) std::snprintf(p->cuda_error, sizeof(p->cuda_error), "%s", cudaGetErrorString(e));
     return GS_ERR_CUDA;
+}
+
+// Brackets one kernel launch with CUDA events on the launching stream when timing is enabled.
+struct LaunchTimer {
+    gs_plan* plan;
+    cudaStream_t stream;
+    bool on;
+    TimedLaunch t;
+    LaunchTimer(gs_plan* p, int label, cudaStream_t s) : plan(p), stream(s), on(false)
+    {
+        if (p->timing_mode == 1 || (p->timing_mode == 2 && label == L_TOSTD_SYR2K)) {
+            t.label = label;
+            if (cudaEventCreate(&t.e0) == cudaSuccess && cudaEventCreate(&t.e1) == cudaSuccess) {
+                on = true;
+                cudaEventRecord(t.e0, stream);
+            }
+        }
+    }
+    ~LaunchTimer()
+    {
+        if (on) {
+            cudaEventRecord(t.e1, stream);
+            plan->timed.push_back(t);
+        }
+    }
+};
+
+void clear_timed(gs_plan* p)
+{
+    for (TimedLaunch& t : p->timed) {
+        cudaEventDestroy(t.e0);
+        cudaEventDestroy(t.e1);
+    }
+    p->timed.clear();
 }
 
 #define GS_CUDA(plan, call)                                   \
@@ -86,8 +137,9 @@ bool set_operand(const Stage& st, EngineParams& p, int which, const MatView& m, 
     return make_tensor_map(map, m, mcontig ? 16 : BN);
 }
 
-gs_status_t launch(Stage& st, const EngineParams& p, bool a_nn)
+gs_status_t launch(Stage& st, const EngineParams& p, bool a_nn, int label)
 {
+    LaunchTimer timer(st.plan, label, st.stream);
     const cudaError_t e = engine_launch(p, a_nn, st.tma, st.stream);
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
     st.plan->launches += 1;
@@ -114,6 +166,7 @@ gs_status_t zero_lower(Stage& st, double* X)
     const int N = int(plan->N);
     if (N <= LB) return GS_OK;
     dim3 grid((N + 255) / 256, N);
+    LaunchTimer timer(st.plan, L_ZERO_LOWER, st.stream);
     zero_lower_blocks_kernel<<<grid, 256, 0, st.stream>>>(X, plan->N, N, info_ptr(plan));
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
@@ -136,6 +189,7 @@ struct Potrf {
     gs_status_t leaf(int b)
     {
         gs_plan* plan = st.plan;
+        LaunchTimer timer(plan, L_POTRF_LEAF, st.stream);
         potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(S, plan->N, int(plan->N), b * LB,
                                                                           winv_ptr(plan) + size_t(b) * LB * LB, info_ptr(plan));
         const cudaError_t e = cudaGetLastError();
@@ -155,7 +209,7 @@ struct Potrf {
         p.khi_c = LB / BK; p.kmax = LB / BK;
         p.a.k0 = 0; p.a.x0 = r0 * LB;          // W slot r0 = columns [128 r0, 128 r0 + 128) of vW
         p.b.k0 = r0 * LB; p.b.x0 = c0 * LB;
-        return launch(st, p, false);
+        return launch(st, p, false, L_POTRF_TRSM);
     }
 
     // S[h:r1, c0:c1] -= U[r0:h, h:r1]^T * S[r0:h, c0:c1]
@@ -170,7 +224,7 @@ struct Potrf {
         p.a.k0 = r0 * LB; p.a.x0 = h * LB;
         p.b.k0 = r0 * LB; p.b.x0 = c0 * LB;
         p.alpha = -1.0; p.beta = 1.0;
-        return launch(st, p, false);
+        return launch(st, p, false, L_POTRF_GEMM);
     }
 
     gs_status_t trsm(int r0, int r1, int c0, int c1)
@@ -196,7 +250,7 @@ struct Potrf {
         p.b.k0 = b0 * LB; p.b.x0 = mid * LB;
         p.alpha = -1.0; p.beta = 1.0;
         p.flags = F_STORE_UPPER;
-        return launch(st, p, false);
+        return launch(st, p, false, L_POTRF_SYRK);
     }
 
     gs_status_t potrf(int b0, int b1)
@@ -235,9 +289,8 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     int major = 0;
     if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return GS_ERR_UNSUPPORTED_DEVICE; }
     if (major != 10) return GS_ERR_UNSUPPORTED_DEVICE;
-    gs_plan* p = new (std::nothrow) gs_plan;
+    gs_plan* p = new (std::nothrow) gs_plan();
     if (p == nullptr) return GS_ERR_INVALID_ARG;
-    std::memset(p, 0, sizeof(*p));
     p->N = N;
     p->nev = nev;
     p->dtype = dtype;
@@ -249,6 +302,7 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
 gs_status_t gs_plan_destroy(gs_plan_t* plan)
 {
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    clear_timed(plan);
     delete plan;
     return GS_OK;
 }
@@ -306,7 +360,10 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
     const int N = int(plan->N), nblk = plan->nblk;
     Stage st{plan, stream, plan->N % 2 == 0};
 
-    trtri_leaf_kernel<<<nblk, kLeafThreads, kLeafSmemBytes, stream>>>(U, V, plan->N, N, info_ptr(plan));
+    {
+        LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
+        trtri_leaf_kernel<<<nblk, kLeafThreads, kLeafSmemBytes, stream>>>(U, V, plan->N, N, info_ptr(plan));
+    }
     GS_CUDA(plan, cudaGetLastError());
     plan->launches += 1;
     GS_TRY(zero_lower(st, V));
@@ -324,7 +381,7 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
             p.khi_c = LB / BK; p.khi_j = LB / BK; p.kmax = s * (LB / BK);
             p.a.x0 = 0; p.a.bx = stride; p.a.k0 = s * LB; p.a.bk = stride;
             p.b.k0 = s * LB; p.b.bk = stride; p.b.x0 = s * LB; p.b.bx = stride;
-            GS_TRY(launch(st, p, true));
+            GS_TRY(launch(st, p, true, L_TRTRI_W));
         }
         {   // X = -Ainv * W
             EngineParams p = blank_params(plan);
@@ -336,7 +393,7 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
             p.a.x0 = 0; p.a.bx = stride; p.a.k0 = 0; p.a.bk = stride;
             p.b.k0 = 0; p.b.bk = stride; p.b.x0 = s * LB; p.b.bx = stride;
             p.alpha = -1.0;
-            GS_TRY(launch(st, p, true));
+            GS_TRY(launch(st, p, true, L_TRTRI_X));
         }
     }
     return GS_OK;
@@ -366,7 +423,7 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         p.c_rows = N; p.c_cols = N;
         p.klo_i = kt; p.khi_c = kt; p.khi_j = kt; p.kmax = (N + BK - 1) / BK;
         p.flags = F_MASK_A | F_HALF_DIAG_A | F_MASK_B;
-        GS_TRY(launch(st, p, true));
+        GS_TRY(launch(st, p, true, L_TOSTD_G));
     }
     {
         EngineParams p = blank_params(plan);
@@ -378,7 +435,7 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         p.c_rows = N; p.c_cols = N;
         p.khi_c = kt; p.khi_i = kt; p.kmax = (N + BK - 1) / BK;
         p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER;
-        GS_TRY(launch(st, p, false));
+        GS_TRY(launch(st, p, false, L_TOSTD_SYR2K));
     }
     return GS_OK;
 }
@@ -401,7 +458,7 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
     p.c_rows = N; p.c_cols = nev;
     p.klo_i = LB / BK; p.khi_c = (N + BK - 1) / BK; p.kmax = p.khi_c;
     p.flags = F_MASK_A;
-    return launch(st, p, true);
+    return launch(st, p, true, L_BACK_TRMM);
 }
 
 gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)
@@ -422,7 +479,7 @@ gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes)
 {
     if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
     const size_t mat = ((size_t(plan->N) * size_t(plan->N) * sizeof(double) + 255) / 256) * 256;
-    *bytes = 4 * mat;   // S->U, H, Uinv, Htilde  (back-transform: Uinv, Ctilde, C fit in the same space)
+    *bytes = 4 * mat;   // S->U, H (later C~ and C), Uinv, Htilde
     return GS_OK;
 }
 
@@ -432,7 +489,7 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     GS_TRY(check_ready(plan));
     size_t need = 0;
     gs_reduce_host_scratch_bytes(plan, &need);
-    if (host_H == nullptr || host_S == nullptr || dev_scratch == nullptr || scratch_bytes < need ||
+    if (host_H == nullptr || host_S == nullptr || host_Htilde == nullptr || dev_scratch == nullptr || scratch_bytes < need ||
         (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
         return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -442,37 +499,73 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     void *dS = base, *dH = base + mat, *dV = base + 2 * mat, *dHt = base + 3 * mat;
     GS_CUDA(plan, cudaMemcpyAsync(dS, host_S, bytes, cudaMemcpyHostToDevice, stream));
     GS_CUDA(plan, cudaMemcpyAsync(dH, host_H, bytes, cudaMemcpyHostToDevice, stream));
+    GS_CUDA(plan, cudaMemsetAsync(dHt, 0, bytes, stream));
     GS_TRY(gs_cholesky(plan, dS, stream));
     GS_TRY(gs_invert_triangular(plan, dS, dV, stream));
     GS_TRY(gs_to_standard(plan, dH, dV, dHt, stream));
     if (host_U) GS_CUDA(plan, cudaMemcpyAsync(host_U, dS, bytes, cudaMemcpyDeviceToHost, stream));
     if (host_Uinv) GS_CUDA(plan, cudaMemcpyAsync(host_Uinv, dV, bytes, cudaMemcpyDeviceToHost, stream));
-    if (host_Htilde) GS_CUDA(plan, cudaMemcpyAsync(host_Htilde, dHt, bytes, cudaMemcpyDeviceToHost, stream));
+    GS_CUDA(plan, cudaMemcpyAsync(host_Htilde, dHt, bytes, cudaMemcpyDeviceToHost, stream));
     int64_t info = 0;
     return gs_last_info(plan, stream, &info);
 }
 
-gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Uinv, const void* host_Ctilde, void* host_C,
-                                  void* dev_scratch, size_t scratch_bytes, void* cuda_stream)
+gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void* host_C, void* dev_scratch,
+                                  size_t scratch_bytes, void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
     size_t need = 0;
     gs_reduce_host_scratch_bytes(plan, &need);
-    if (host_Uinv == nullptr || host_Ctilde == nullptr || host_C == nullptr || dev_scratch == nullptr || scratch_bytes < need ||
-        (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
+    if (dev_scratch == nullptr || scratch_bytes < need || (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
         return GS_ERR_INVALID_ARG;
+    if (plan->nev == 0) return GS_OK;
+    if (host_Ctilde == nullptr || host_C == nullptr) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const size_t mat = need / 4;
-    const size_t bytes = size_t(plan->N) * size_t(plan->N) * sizeof(double);
     const size_t cbytes = size_t(plan->N) * size_t(plan->nev) * sizeof(double);
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
-    void *dV = base, *dCt = base + mat, *dC = base + 2 * mat;
-    GS_CUDA(plan, cudaMemcpyAsync(dV, host_Uinv, bytes, cudaMemcpyHostToDevice, stream));
-    if (cbytes) GS_CUDA(plan, cudaMemcpyAsync(dCt, host_Ctilde, cbytes, cudaMemcpyHostToDevice, stream));
+    // U^-1 was left at base + 2*mat by gs_reduce_host; C~ and C reuse the S and H slots
+    void *dV = base + 2 * mat, *dCt = base, *dC = base + mat;
+    GS_CUDA(plan, cudaMemcpyAsync(dCt, host_Ctilde, cbytes, cudaMemcpyHostToDevice, stream));
     GS_TRY(gs_backtransform(plan, dV, dCt, dC, stream));
-    if (cbytes) GS_CUDA(plan, cudaMemcpyAsync(host_C, dC, cbytes, cudaMemcpyDeviceToHost, stream));
+    GS_CUDA(plan, cudaMemcpyAsync(host_C, dC, cbytes, cudaMemcpyDeviceToHost, stream));
     int64_t info = 0;
     return gs_last_info(plan, stream, &info);
+}
+
+gs_status_t gs_plan_set_timing(gs_plan_t* plan, int mode)
+{
+    if (plan == nullptr || mode < 0 || mode > 2) return GS_ERR_INVALID_ARG;
+    clear_timed(plan);
+    plan->timing_mode = mode;
+    return GS_OK;
+}
+
+gs_status_t gs_plan_launch_times(gs_plan_t* plan, gs_launch_time_t* out, int cap, int* count)
+{
+    if (plan == nullptr || count == nullptr || (out == nullptr && cap > 0)) return GS_ERR_INVALID_ARG;
+    double ms[L_COUNT] = {0};
+    int64_t n[L_COUNT] = {0};
+    for (const TimedLaunch& t : plan->timed) {
+        float f = 0.f;
+        const cudaError_t e = cudaEventElapsedTime(&f, t.e0, t.e1);
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+        ms[t.label] += f;
+        n[t.label] += 1;
+    }
+    clear_timed(plan);
+    int k = 0;
+    for (int l = 0; l < L_COUNT; ++l) {
+        if (n[l] == 0) continue;
+        if (k < cap) {
+            std::snprintf(out[k].label, sizeof(out[k].label), "%s", kLabelNames[l]);
+            out[k].launches = n[l];
+            out[k].ms = ms[l];
+        }
+        ++k;
+    }
+    *count = k;
+    return GS_OK;
 }
 
 gs_status_t gs_plan_launch_count(const gs_plan_t* plan, int64_t* launches)

@@ -30,7 +30,12 @@ EXPORTS = (
     "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_last_info",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
+    "gs_plan_set_timing", "gs_plan_launch_times",
 )
+
+
+class LaunchTime(ctypes.Structure):
+    _fields_ = [("label", ctypes.c_char * 32), ("launches", ctypes.c_int64), ("ms", ctypes.c_double)]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgs.so")
@@ -68,7 +73,9 @@ def lib() -> ctypes.CDLL:
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
         L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
-        L.gs_backtransform_host.argtypes = [vp, vp, vp, vp, vp, sz, vp]
+        L.gs_backtransform_host.argtypes = [vp, vp, vp, vp, sz, vp]
+        L.gs_plan_set_timing.argtypes = [vp, ctypes.c_int]
+        L.gs_plan_launch_times.argtypes = [vp, ctypes.POINTER(LaunchTime), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.gs_plan_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
         L.gs_status_string.argtypes = [ctypes.c_int]
         L.gs_status_string.restype = ctypes.c_char_p
@@ -199,10 +206,22 @@ class Plan:
         self._check(lib().gs_reduce_host(self._h, hp(H), hp(S), hp(U), hp(Uinv), hp(Htilde), scratch.data_ptr(),
                                          scratch.numel() * scratch.element_size(), _stream_ptr(stream)))
 
-    def backtransform_host(self, Uinv, Ctilde, C, scratch: torch.Tensor, stream=None):
-        self._check(lib().gs_backtransform_host(self._h, Uinv.data_ptr(), Ctilde.data_ptr(), C.data_ptr(),
+    def backtransform_host(self, Ctilde, C, scratch: torch.Tensor, stream=None):
+        """Uses the U^-1 that reduce_host left in `scratch`."""
+        self._check(lib().gs_backtransform_host(self._h, Ctilde.data_ptr(), C.data_ptr(),
                                                 scratch.data_ptr(), scratch.numel() * scratch.element_size(),
                                                 _stream_ptr(stream)))
+
+    # ---- optional per-launch timing (roofline reports) ----
+    def set_timing(self, mode: int):
+        self._check(lib().gs_plan_set_timing(self._h, mode))
+
+    def launch_times(self) -> dict:
+        """{label: (launches, total_ms)} since the last set_timing; call after a stream synchronise."""
+        buf = (LaunchTime * 16)()
+        n = ctypes.c_int(0)
+        self._check(lib().gs_plan_launch_times(self._h, buf, 16, ctypes.byref(n)))
+        return {buf[i].label.decode(): (int(buf[i].launches), float(buf[i].ms)) for i in range(min(n.value, 16))}
 
 
 def generalized_to_standard(H: torch.Tensor, S: torch.Tensor, nev: int | None = None):
