@@ -54,8 +54,9 @@ inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols)
 
 inline int num_tiles(const EngineParams& p)
 {
-    const bool tri = p.order >= ORDER_TRI_ROW_DESC;
-    const int per = tri ? p.tiles_n * (p.tiles_n + 1) / 2 : p.tiles_m * p.tiles_n;
+    int per = p.tiles_m * p.tiles_n;
+    if (p.order == ORDER_TRI_ROW_DESC || p.order == ORDER_TRI_DIAG_DESC) per = p.tiles_n * (p.tiles_n + 1) / 2;
+    else if (p.order == ORDER_TRAPEZOID) per = p.tiles_m * p.tiles_n - p.tiles_m * (p.tiles_m - 1) / 2;
     return per * p.batch;
 }
 

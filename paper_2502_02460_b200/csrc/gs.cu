@@ -13,6 +13,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -46,6 +47,11 @@ struct gs_plan {
     int64_t launches = 0;
     int timing_mode = 0;
     std::vector<TimedLaunch> timed;
+    // look-ahead of the blocked factorisation: a high-priority side stream owned by the plan, forked
+    // from and joined back into the caller's stream with events inside every call that uses it
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     char cuda_error[256] = {0};
 };
 
@@ -237,32 +243,96 @@ struct Potrf {
         return trsm(h, r1, c0, c1);
     }
 
-    // S[mid:b1, mid:b1] -= S[b0:mid, mid:b1]^T S[b0:mid, mid:b1], upper tiles only
-    gs_status_t syrk(int b0, int mid, int b1)
+    // S[c0:c1, c0:c1] -= S[k0:k1, c0:c1]^T S[k0:k1, c0:c1], upper tiles only
+    gs_status_t syrk(int k0, int k1, int c0, int c1)
     {
         EngineParams p = blank_params(st.plan);
         if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
         p.C = S; p.ldc = vS.ld;
-        p.tiles_m = b1 - mid; p.tiles_n = b1 - mid; p.order = ORDER_TRI_ROW_DESC;
-        p.c_row0 = mid * LB; p.c_col0 = mid * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
-        p.khi_c = (mid - b0) * (LB / BK); p.kmax = p.khi_c;
-        p.a.k0 = b0 * LB; p.a.x0 = mid * LB;
-        p.b.k0 = b0 * LB; p.b.x0 = mid * LB;
+        p.tiles_m = c1 - c0; p.tiles_n = c1 - c0; p.order = ORDER_TRI_ROW_DESC;
+        p.c_row0 = c0 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = (k1 - k0) * (LB / BK); p.kmax = p.khi_c;
+        p.a.k0 = k0 * LB; p.a.x0 = c0 * LB;
+        p.b.k0 = k0 * LB; p.b.x0 = c0 * LB;
         p.alpha = -1.0; p.beta = 1.0;
         p.flags = F_STORE_UPPER;
         return launch(st, p, false, L_POTRF_SYRK);
     }
 
+    // Block rows [r0, r1) of the trailing update (the next panel's rows), upper trapezoid:
+    // S[r0:r1, r0:n] -= S[k0:k1, r0:r1]^T S[k0:k1, r0:n]
+    gs_status_t update_rows(int k0, int k1, int r0, int r1, int n)
+    {
+        EngineParams p = blank_params(st.plan);
+        if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
+        p.C = S; p.ldc = vS.ld;
+        p.tiles_m = r1 - r0; p.tiles_n = n - r0; p.order = ORDER_TRAPEZOID;
+        p.c_row0 = r0 * LB; p.c_col0 = r0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = (k1 - k0) * (LB / BK); p.kmax = p.khi_c;
+        p.a.k0 = k0 * LB; p.a.x0 = r0 * LB;
+        p.b.k0 = k0 * LB; p.b.x0 = r0 * LB;
+        p.alpha = -1.0; p.beta = 1.0;
+        p.flags = F_STORE_UPPER;
+        return launch(st, p, false, L_POTRF_SYRK);
+    }
+
+    // recursive factorisation of the diagonal block [b0, b1) (touches nothing outside it)
     gs_status_t potrf(int b0, int b1)
     {
         if (b1 - b0 == 1) return leaf(b0);
         const int mid = b0 + (b1 - b0 + 1) / 2;
         GS_TRY(potrf(b0, mid));
         GS_TRY(trsm(b0, mid, mid, b1));
-        GS_TRY(syrk(b0, mid, b1));
+        GS_TRY(syrk(b0, mid, mid, b1));
         return potrf(mid, b1);
     }
+
+    // panel = block rows [b0, b1): factor the diagonal block, then solve the row panel to its right
+    gs_status_t panel(int b0, int b1, int n)
+    {
+        GS_TRY(potrf(b0, b1));
+        return trsm(b0, b1, b1, n);
+    }
+
+    // Right-looking over panels of NB blocks with one panel of look-ahead: while the caller's
+    // stream applies panel p to the trailing matrix beyond panel p+1, the plan's high-priority
+    // side stream applies it to the rows of panel p+1 and factors that panel.
+    gs_status_t factor(int n, int NB, cudaStream_t main_stream, cudaStream_t side, cudaEvent_t ev_fork, cudaEvent_t ev_join)
+    {
+        gs_plan* plan = st.plan;
+        st.stream = main_stream;
+        GS_TRY(panel(0, NB < n ? NB : n, n));
+        for (int b0 = 0; b0 + NB < n; b0 += NB) {
+            const int b1 = b0 + NB;
+            const int b2 = b1 + NB < n ? b1 + NB : n;
+            GS_CUDA(plan, cudaEventRecord(ev_fork, main_stream));
+            GS_CUDA(plan, cudaStreamWaitEvent(side, ev_fork, 0));
+            st.stream = side;
+            gs_status_t rc = update_rows(b0, b1, b1, b2, n);
+            if (rc == GS_OK) rc = panel(b1, b2, n);
+            st.stream = main_stream;
+            if (rc == GS_OK && b2 < n) rc = syrk(b0, b1, b2, n);
+            // always join the side stream back, also on failure
+            const cudaError_t e1 = cudaEventRecord(ev_join, side);
+            const cudaError_t e2 = cudaStreamWaitEvent(main_stream, ev_join, 0);
+            GS_TRY(rc);
+            GS_CUDA(plan, e1);
+            GS_CUDA(plan, e2);
+        }
+        return GS_OK;
+    }
 };
+
+gs_status_t ensure_side_stream(gs_plan* plan)
+{
+    if (plan->side != nullptr) return GS_OK;
+    int lo = 0, hi = 0;
+    GS_CUDA(plan, cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    GS_CUDA(plan, cudaStreamCreateWithPriority(&plan->side, cudaStreamNonBlocking, hi));
+    GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_fork, cudaEventDisableTiming));
+    GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_join, cudaEventDisableTiming));
+    return GS_OK;
+}
 
 gs_status_t configure_leaf(gs_plan* plan)
 {
@@ -295,6 +365,10 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     p->nev = nev;
     p->dtype = dtype;
     p->nblk = int((N + LB - 1) / LB);
+    if (const char* e = std::getenv("GS_POTRF_NB")) {
+        const int v = std::atoi(e);
+        if (v >= 1 && v <= 64) p->potrf_nb = v;
+    }
     *plan = p;
     return GS_OK;
 }
@@ -303,6 +377,9 @@ gs_status_t gs_plan_destroy(gs_plan_t* plan)
 {
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
     clear_timed(plan);
+    if (plan->ev_fork != nullptr) cudaEventDestroy(plan->ev_fork);
+    if (plan->ev_join != nullptr) cudaEventDestroy(plan->ev_join);
+    if (plan->side != nullptr) cudaStreamDestroy(plan->side);
     delete plan;
     return GS_OK;
 }
@@ -340,8 +417,9 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     f.S = S;
     f.vS = MatView{S, plan->N, plan->N, plan->N};
     f.vW = MatView{winv_ptr(plan), LB, (long long)LB * plan->nblk, LB};
-    GS_TRY(f.potrf(0, plan->nblk));
-    return zero_lower(f.st, S);
+    if (plan->nblk > plan->potrf_nb) GS_TRY(ensure_side_stream(plan));
+    GS_TRY(zero_lower(f.st, S));   // off-diagonal lower blocks: never touched by the factorisation
+    return f.factor(plan->nblk, plan->potrf_nb, stream, plan->side, plan->ev_fork, plan->ev_join);
 }
 
 // Block-recursive inversion by doubling: with U = [A B; 0 D],  U^-1 = [A^-1, -A^-1 B D^-1; 0, D^-1].

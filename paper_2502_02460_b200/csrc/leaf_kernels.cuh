@@ -5,24 +5,29 @@
 //                       tensor-core product.
 //   trtri_leaf_kernel : invert every diagonal block of U, one CTA per block.
 //
-// One CTA of 256 threads = a 16 x 16 grid of threads, thread (ty,tx) keeps the 8 x 8 sub-block
-// rows 8ty.., cols 8tx.. in registers.  Both factorisation and inversion are right-looking rank-1
-// sweeps: the pivot row is broadcast through a double-buffered shared-memory row (one
-// __syncthreads per step), the update is 64 register FMAs per thread.  Blocks shorter than 128
-// (ragged last block) are padded with the identity, which factors / inverts to itself.
+// One CTA of 256 threads = a 16 x 16 grid of threads.  The block is distributed 2-D CYCLICALLY:
+// thread (ty,tx) keeps the 64 elements (ty + 16 r, tx + 16 c), r,c = 0..7, in registers, so the
+// shrinking active region of a right-looking sweep stays spread over all threads and whole
+// register rows / columns drop out of the (unrolled) update statically: N^3/6 FMAs in total, not
+// N^3/2.  Both factorisation and inversion are rank-1 sweeps: the pivot row is broadcast through a
+// double-buffered shared-memory row (one __syncthreads per step).  Global traffic goes through a
+// padded shared-memory image of the block so that loads and stores are coalesced.  Blocks shorter
+// than 128 (ragged last block) are padded with the identity, which factors / inverts to itself.
 #pragma once
 #include <cuda_runtime.h>
 
 namespace gs {
 
 constexpr int LB = 128;                 // leaf block order
+constexpr int LP = LB + 1;              // padded shared-memory pitch (doubles)
 constexpr int kLeafThreads = 256;
-constexpr int kLeafSmemBytes = LB * LB * 8 + 2 * LB * 8 + LB * 8 + 16;   // Usm + rowbuf[2] + dvec + flag
+constexpr int kLeafSmemBytes = (LB * LP + 2 * LB + LB + LB) * 8 + 16;   // Usm + rowbuf[2] + dvec + dinv + flag
 
 struct LeafSmem {
-    double* U;        // LB x LB column-major, pitch LB
+    double* U;        // LB x LB column-major, pitch LP
     double* rowbuf;   // 2 x LB
     double* dvec;     // LB
+    double* dinv;     // LB : 1 / U(m,m)
     int* flag;
 };
 
@@ -30,46 +35,81 @@ __device__ __forceinline__ LeafSmem leaf_smem(unsigned char* raw)
 {
     LeafSmem s;
     s.U = reinterpret_cast<double*>(raw);
-    s.rowbuf = s.U + LB * LB;
+    s.rowbuf = s.U + LB * LP;
     s.dvec = s.rowbuf + 2 * LB;
-    s.flag = reinterpret_cast<int*>(s.dvec + LB);
+    s.dinv = s.dvec + LB;
+    s.flag = reinterpret_cast<int*>(s.dinv + LB);
     return s;
 }
 
-// V = Usm^-1 (upper), result left in registers v[r][c] of the upper thread blocks (ty <= tx).
-// Right-looking: for m = LB-1 .. 0: V(m,:) = acc(m,:) / U(m,m); acc(k,:) -= U(k,m) V(m,:) for k < m.
-__device__ __forceinline__ void invert_upper_from_smem(const LeafSmem& s, double (&v)[8][8], int tx, int ty)
+// Coalesced load of the upper triangle of a diagonal block into the padded shared image
+// (identity-padded beyond nb, zero below the diagonal).
+__device__ __forceinline__ void leaf_load_upper(const LeafSmem& s, const double* blk, long long ld, int nb, int t)
 {
+    for (int idx = t; idx < LB * LB; idx += kLeafThreads) {
+        const int row = idx & (LB - 1), col = idx >> 7;
+        double v = (row == col) ? 1.0 : 0.0;
+        if (row <= col && col < nb) v = blk[row + (long long)col * ld];
+        s.U[row + col * LP] = v;
+    }
+}
+
+// Coalesced store of the whole shared image (rows, cols < nb) to a column-major destination.
+__device__ __forceinline__ void leaf_store_all(const LeafSmem& s, double* dst, long long ld, int nb, int t)
+{
+    for (int idx = t; idx < LB * LB; idx += kLeafThreads) {
+        const int row = idx & (LB - 1), col = idx >> 7;
+        if (row < nb && col < nb) dst[row + (long long)col * ld] = s.U[row + col * LP];
+    }
+}
+
+// V = U^-1 (upper) for the U held in s.U (pitch LP) with s.dinv[m] = 1 / U(m,m).  On return the
+// shared image holds V (upper = inverse, strictly lower = 0).  Right-looking, backwards:
+//   for m = LB-1 .. 0:  V(m,:) = acc(m,:) * dinv(m);  acc(k,:) -= U(k,m) V(m,:)  for k < m.
+__device__ __forceinline__ void leaf_invert_upper(const LeafSmem& s, int tx, int ty)
+{
+    double v[8][8];
 #pragma unroll
     for (int r = 0; r < 8; ++r)
 #pragma unroll
-        for (int c = 0; c < 8; ++c) v[r][c] = (ty == tx && r == c) ? 1.0 : 0.0;
+        for (int c = 0; c < 8; ++c) v[r][c] = (r == c && ty == tx) ? 1.0 : 0.0;
 
-    for (int m = LB - 1; m >= 0; --m) {
-        const int mb = m >> 3, mr = m & 7;
-        double* rb = s.rowbuf + (m & 1) * LB;
-        if (ty == mb && tx >= mb) {
-            const double inv = 1.0 / s.U[m + m * LB];
 #pragma unroll
-            for (int r = 0; r < 8; ++r)
-                if (r == mr) {
+    for (int mr = 7; mr >= 0; --mr) {
+#pragma unroll 1
+        for (int mo = 15; mo >= 0; --mo) {
+            const int m = mr * 16 + mo;
+            double* rb = s.rowbuf + (m & 1) * LB;
+            if (ty == mo) {
+                const double inv = s.dinv[m];
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) { v[r][c] *= inv; rb[8 * tx + c] = v[r][c]; }
+                for (int c = mr; c < 8; ++c) {
+                    v[mr][c] *= inv;
+                    rb[tx + 16 * c] = v[mr][c];
                 }
-        }
-        __syncthreads();
-        if (ty <= mb && tx >= mb && tx >= ty) {
-            double rc[8], uk[8];
+            }
+            __syncthreads();
 #pragma unroll
-            for (int c = 0; c < 8; ++c) rc[c] = rb[8 * tx + c];
+            for (int r = 0; r <= mr; ++r) {
+                const bool rowact = (r < mr) || (ty < mo);
+                const double uk = s.U[ty + 16 * r + m * LP];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) uk[r] = (8 * ty + r < m) ? s.U[8 * ty + r + m * LB] : 0.0;
-#pragma unroll
-            for (int r = 0; r < 8; ++r)
-#pragma unroll
-                for (int c = 0; c < 8; ++c) v[r][c] = fma(-uk[r], rc[c], v[r][c]);
+                for (int c = mr; c < 8; ++c) {
+                    const bool colact = (c > mr) || (tx >= mo);
+                    if (rowact && colact) v[r][c] = fma(-uk, rb[tx + 16 * c], v[r][c]);
+                }
+            }
         }
     }
+    __syncthreads();   // every thread is done reading U before it is overwritten
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            s.U[row + col * LP] = (row <= col) ? v[r][c] : 0.0;
+        }
+    __syncthreads();
 }
 
 // S: N x N column-major (ld), block starts at (j0, j0), order nb = min(LB, N - j0).
@@ -85,79 +125,66 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
     const int nb = min(LB, N - j0);
     double* blk = S + j0 + (long long)j0 * ld;
 
-    double a[8][8];
-    if (ty <= tx) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c)
-#pragma unroll
-            for (int r = 0; r < 8; ++r) {
-                const int row = 8 * ty + r, col = 8 * tx + c;
-                a[r][c] = (row < nb && col < nb) ? blk[row + (long long)col * ld] : (row == col ? 1.0 : 0.0);
-            }
-    }
-    if (t == 0) *s.flag = 0;
+    leaf_load_upper(s, blk, ld, nb, t);
     __syncthreads();
+    double a[8][8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) a[r][c] = s.U[ty + 16 * r + (tx + 16 * c) * LP];
 
     // right-looking factorisation without square roots inside the sweep:
     //   step j: d_j = a(j,j);  a(i,c) -= a(j,i) a(j,c) / d_j  (j < i <= c);  U(j,c) = a(j,c) / sqrt(d_j) afterwards
-    for (int j = 0; j < LB; ++j) {
-        const int jb = j >> 3, jr = j & 7;
-        double* rb = s.rowbuf + (j & 1) * LB;
-        if (ty == jb && tx >= jb) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r)
-                if (r == jr) {
+    for (int jr = 0; jr < 8; ++jr) {
+#pragma unroll 1
+        for (int jo = 0; jo < 16; ++jo) {
+            const int j = jr * 16 + jo;
+            double* rb = s.rowbuf + (j & 1) * LB;
+            if (ty == jo) {
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) rb[8 * tx + c] = a[r][c];
-                }
-        }
-        __syncthreads();
-        const double d = rb[j];
-        if (!(d > 0.0)) {   // uniform: every thread reads the same value
-            if (t == 0) atomicCAS(info, 0, j0 + j + 1);
-            return;
-        }
-        if (t == 0) s.dvec[j] = d;
-        if (ty >= jb && tx >= ty) {
+                for (int c = jr; c < 8; ++c) rb[tx + 16 * c] = a[jr][c];
+            }
+            __syncthreads();
+            const double d = rb[j];
+            if (!(d > 0.0)) {   // uniform: every thread reads the same value
+                if (t == 0) atomicCAS(info, 0, j0 + j + 1);
+                return;
+            }
+            if (t == 0) s.dvec[j] = d;
             const double invd = 1.0 / d;
-            double rc[8], ri[8];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) rc[c] = rb[8 * tx + c];
+            for (int r = jr; r < 8; ++r) {
+                const bool rowact = (r > jr) || (ty > jo);
+                const double ri = rb[ty + 16 * r] * invd;
 #pragma unroll
-            for (int r = 0; r < 8; ++r) ri[r] = (8 * ty + r > j) ? rb[8 * ty + r] * invd : 0.0;
-#pragma unroll
-            for (int r = 0; r < 8; ++r)
-#pragma unroll
-                for (int c = 0; c < 8; ++c) a[r][c] = fma(-ri[r], rc[c], a[r][c]);
+                for (int c = r; c < 8; ++c) {
+                    const bool colact = (c > r) || (tx >= ty);
+                    if (rowact && colact) a[r][c] = fma(-ri, rb[tx + 16 * c], a[r][c]);
+                }
+            }
         }
     }
     __syncthreads();
-
-    // scale rows, write U to global (whole block: upper = U, strictly lower = 0) and to shared memory
-#pragma unroll
-    for (int c = 0; c < 8; ++c)
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int row = 8 * ty + r, col = 8 * tx + c;
-            double u = 0.0;
-            if (ty <= tx && row <= col) {
-                const double sd = sqrt(s.dvec[row]);
-                u = (row == col) ? sd : a[r][c] / sd;
-            }
-            s.U[row + col * LB] = u;
-            if (row < nb && col < nb) blk[row + (long long)col * ld] = u;
-        }
+    if (t < LB) s.dinv[t] = 1.0 / sqrt(s.dvec[t]);
     __syncthreads();
 
-    double v[8][8];
-    invert_upper_from_smem(s, v, tx, ty);
+    // scale rows; shared image = U (upper) with zeros below; write it out
 #pragma unroll
-    for (int c = 0; c < 8; ++c)
+    for (int r = 0; r < 8; ++r)
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int row = 8 * ty + r, col = 8 * tx + c;
-            Winv[row + col * LB] = (ty <= tx && row <= col) ? v[r][c] : 0.0;
+        for (int c = 0; c < 8; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            double u = 0.0;
+            if (row == col) u = sqrt(s.dvec[row]);
+            else if (row < col) u = a[r][c] * s.dinv[row];
+            s.U[row + col * LP] = u;
         }
+    __syncthreads();
+    leaf_store_all(s, blk, ld, nb, t);
+
+    leaf_invert_upper(s, tx, ty);
+    leaf_store_all(s, Winv, LB, LB, t);
 }
 
 // One CTA per diagonal block b: V_bb = U_bb^-1.  Reads only the upper triangle of U_bb; writes the
@@ -175,31 +202,25 @@ trtri_leaf_kernel(const double* __restrict__ U, double* __restrict__ V, long lon
     const double* ub = U + j0 + (long long)j0 * ld;
     double* vb = V + j0 + (long long)j0 * ld;
     if (t == 0) *s.flag = 0;
+    leaf_load_upper(s, ub, ld, nb, t);
     __syncthreads();
-#pragma unroll
-    for (int c = 0; c < 8; ++c)
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int row = 8 * ty + r, col = 8 * tx + c;
-            double u = (row == col) ? 1.0 : 0.0;
-            if (row <= col && col < nb) u = ub[row + (long long)col * ld];
-            if (row == col && u == 0.0) *s.flag = row + 1;
-            s.U[row + col * LB] = u;
-        }
+    if (t < LB) {
+        const double u = s.U[t + t * LP];
+        if (u == 0.0) atomicMax(s.flag, t + 1);
+        s.dinv[t] = 1.0 / u;
+    }
     __syncthreads();
     if (*s.flag != 0) {
-        if (t == 0) atomicCAS(info, 0, -(j0 + *s.flag));
+        if (t == 0) {
+            int first = LB;   // report the FIRST zero diagonal entry
+            for (int i = LB - 1; i >= 0; --i)
+                if (s.U[i + i * LP] == 0.0) first = i;
+            atomicCAS(info, 0, -(j0 + first + 1));
+        }
         return;
     }
-    double v[8][8];
-    invert_upper_from_smem(s, v, tx, ty);
-#pragma unroll
-    for (int c = 0; c < 8; ++c)
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int row = 8 * ty + r, col = 8 * tx + c;
-            if (row < nb && col < nb) vb[row + (long long)col * ld] = (ty <= tx && row <= col) ? v[r][c] : 0.0;
-        }
+    leaf_invert_upper(s, tx, ty);
+    leaf_store_all(s, vb, ld, nb, t);
 }
 
 // Zero the strictly-lower part of an N x N column-major matrix outside its 128 x 128 diagonal

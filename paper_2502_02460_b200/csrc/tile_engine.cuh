@@ -57,6 +57,7 @@ enum : int {
     ORDER_COL_REV = 3,    // full grid, I fastest, J descending
     ORDER_TRI_ROW_DESC = 4,   // upper triangle I <= J, rows I descending (cost ~ I+1)
     ORDER_TRI_DIAG_DESC = 5,  // upper triangle, diagonals d = J-I descending (cost ~ d+1)
+    ORDER_TRAPEZOID = 6,      // tiles_m rows of a tiles_n-wide upper trapezoid: row I holds J = I .. tiles_n-1
 };
 
 struct OperandCoord {
@@ -112,6 +113,13 @@ __device__ __forceinline__ void decode_tile(const EngineParams& p, int id, int& 
             const int per = tm * tn;
             b = id / per; const int r = id - b * per;
             I = r / tn; J = r - I * tn; I = tm - 1 - I;
+        } break;
+        case ORDER_TRAPEZOID: {
+            const int per = tm * tn - tm * (tm - 1) / 2;
+            b = id / per; int r = id - b * per;
+            I = 0;
+            while (r >= tn - I) { r -= tn - I; ++I; }
+            J = I + r;
         } break;
         default: {
             // triangular enumerations over an n x n tile grid (n = tiles_n = tiles_m): group u has u+1 tiles
