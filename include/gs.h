@@ -131,6 +131,17 @@ typedef struct {
 gs_status_t gs_plan_set_timing(gs_plan_t* plan, int mode);
 gs_status_t gs_plan_launch_times(gs_plan_t* plan, gs_launch_time_t* out, int cap, int* count);
 
+/* The same events as a timeline (does not clear them; call before gs_plan_launch_times): entry i =
+ * launch i since gs_plan_set_timing(…, 1), start / end in milliseconds after the start of launch 0,
+ * side_stream = 1 if it ran on the plan's look-ahead stream.  *count = number of launches recorded
+ * (may exceed cap; only cap entries are written).  Call after the stream has been synchronised. */
+typedef struct {
+    char label[32];
+    int32_t side_stream;
+    double t0_ms, t1_ms;
+} gs_launch_trace_t;
+gs_status_t gs_plan_launch_trace(gs_plan_t* plan, gs_launch_trace_t* out, int cap, int* count);
+
 /* Number of kernels the library has launched on behalf of this plan since creation. */
 gs_status_t gs_plan_launch_count(const gs_plan_t* plan, int64_t* launches);
 

@@ -34,6 +34,7 @@ static const char* const kLabelNames[L_COUNT] = {
 
 struct TimedLaunch {
     int label;
+    int side;           // 1 = launched on the plan's side stream
     cudaEvent_t e0, e1;
 };
 
@@ -50,8 +51,10 @@ struct gs_plan {
     // look-ahead of the blocked factorisation: a high-priority side stream owned by the plan, forked
     // from and joined back into the caller's stream with events inside every call that uses it
     cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_rows = nullptr, ev_join = nullptr;
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
+    int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
+    int potrf_tail = 40;
     char cuda_error[256] = {0};
 };
 
@@ -59,12 +62,14 @@ namespace {
 
 constexpr size_t kInfoBytes = 256;
 
-size_t winv_bytes(const gs_plan* p) { return size_t(p->nblk) * LB * LB * sizeof(double); }
-size_t big_offset(const gs_plan* p) { return kInfoBytes + ((winv_bytes(p) + 255) / 256) * 256; }
+// Workspace layout: [info flag | 2 panel-inverse buffers Wp (ldw x ldw each) | one N x N matrix]
+int wp_ld(const gs_plan* p) { return LB * (p->nblk < p->potrf_nb ? p->nblk : p->potrf_nb); }
+size_t wp_bytes(const gs_plan* p) { return size_t(wp_ld(p)) * size_t(wp_ld(p)) * sizeof(double); }
+size_t big_offset(const gs_plan* p) { return kInfoBytes + ((2 * wp_bytes(p) + 255) / 256) * 256; }
 size_t workspace_bytes(const gs_plan* p) { return big_offset(p) + size_t(p->N) * size_t(p->N) * sizeof(double); }
 
 int* info_ptr(const gs_plan* p) { return reinterpret_cast<int*>(p->ws); }
-double* winv_ptr(const gs_plan* p) { return reinterpret_cast<double*>(p->ws + kInfoBytes); }
+double* wp_ptr(const gs_plan* p, int which) { return reinterpret_cast<double*>(p->ws + kInfoBytes + size_t(which & 1) * wp_bytes(p)); }
 double* big_ptr(const gs_plan* p) { return reinterpret_cast<double*>(p->ws + big_offset(p)); }
 
 gs_status_t cuda_fail(gs_plan* p, cudaError_t e)
@@ -83,6 +88,7 @@ struct LaunchTimer {
     {
         if (p->timing_mode == 1 || (p->timing_mode == 2 && label == L_TOSTD_SYR2K)) {
             t.label = label;
+            t.side = (p->side != nullptr && s == p->side) ? 1 : 0;
             if (cudaEventCreate(&t.e0) == cudaSuccess && cudaEventCreate(&t.e1) == cudaSuccess) {
                 on = true;
                 cudaEventRecord(t.e0, stream);
@@ -181,8 +187,66 @@ gs_status_t zero_lower(Stage& st, double* X)
 }
 
 // ------------------------------------------------------------------------------------------------
-// gs_cholesky: recursive blocked POTRF on 128-blocks.
-//   potrf(b0,b1): potrf(b0,mid); S12 = U11^-T S12 (trsm); S22 -= S12^T S12 (syrk, upper tiles); potrf(mid,b1)
+// Block-recursive inversion by doubling of an nb-block upper triangular matrix whose diagonal
+// 128-blocks are already inverted in the destination.  With U = [A B; 0 D],
+// U^-1 = [A^-1, -A^-1 B D^-1; 0, D^-1].  Level s (in 128-blocks): all pairs (A = blocks
+// [2is, 2is+s), D = the next s blocks) at once:
+//   W = B * D^-1   (k <= J: D^-1 upper)      -> temp T, at the position of the target block
+//   X = -A^-1 * W  (k >= I: A^-1 upper)      -> V
+// The triangular matrix is the diagonal sub-block of vU starting at element offset uo; likewise vo
+// (destination V) and to (temp T).
+// ------------------------------------------------------------------------------------------------
+gs_status_t invert_levels(Stage& st, const MatView& vU, int uo, const MatView& vV, int vo, const MatView& vT, int to,
+                          int nb, int label_w, int label_x)
+{
+    gs_plan* plan = st.plan;
+    double* V = const_cast<double*>(vV.ptr);
+    double* T = const_cast<double*>(vT.ptr);
+    for (int s = 1; s < nb; s *= 2) {
+        const int npairs = (nb - s + 2 * s - 1) / (2 * s);
+        const int stride = 2 * s * LB;   // elements between consecutive pairs
+        {   // W = B * Dinv
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vU, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
+            p.C = T; p.ldc = vT.ld;
+            p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_COL_REV;
+            p.c_row0 = to; p.c_col0 = to + s * LB; p.c_brow = stride; p.c_bcol = stride;
+            p.c_rows = int(vT.rows); p.c_cols = int(vT.cols);
+            p.khi_c = LB / BK; p.khi_j = LB / BK; p.kmax = s * (LB / BK);
+            p.a.x0 = uo; p.a.bx = stride; p.a.k0 = uo + s * LB; p.a.bk = stride;
+            p.b.k0 = vo + s * LB; p.b.bk = stride; p.b.x0 = vo + s * LB; p.b.bx = stride;
+            GS_TRY(launch(st, p, true, label_w));
+        }
+        {   // X = -Ainv * W
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vT, false)) return GS_ERR_CUDA;
+            p.C = V; p.ldc = vV.ld;
+            p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_ROW;
+            p.c_row0 = vo; p.c_col0 = vo + s * LB; p.c_brow = stride; p.c_bcol = stride;
+            p.c_rows = int(vV.rows); p.c_cols = int(vV.cols);
+            p.klo_i = LB / BK; p.khi_c = s * (LB / BK); p.kmax = s * (LB / BK);
+            p.a.x0 = vo; p.a.bx = stride; p.a.k0 = vo; p.a.bk = stride;
+            p.b.k0 = to; p.b.bk = stride; p.b.x0 = to + s * LB; p.b.bx = stride;
+            p.alpha = -1.0;
+            GS_TRY(launch(st, p, true, label_x));
+        }
+    }
+    return GS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// gs_cholesky: right-looking over panels of NB 128-blocks with one panel of look-ahead.
+//
+//   panel p = block rows [b1, b2).  Given the finished row panel p-1 = U[b0:b1, b1:n]:
+//     side stream : A  S[b1:b2, b1:b2] -= U[b0:b1, b1:b2]^T U[b0:b1, b1:b2]     (diagonal block, upper tiles)
+//                   B  recursive POTRF of the diagonal block (leaf kernels emit the inverted 128-blocks)
+//                   C  Wp = U_pp^-1 by doubling
+//     main stream : D  S[b1:b2, b2:n] -= U[b0:b1, b1:b2]^T U[b0:b1, b2:n]       (rest of the panel's rows)
+//                   E  S[b2:n, b2:n] -= U[b0:b1, b2:n]^T U[b0:b1, b2:n]         (trailing matrix, upper tiles)
+//     side stream : F  U[b1:b2, b2:n] = Wp^T S[b1:b2, b2:n]  (after D; one launch; out of place + copy back)
+//   so the latency-bound chain A-B-C runs beside the large updates D, E, and the panel solve is a
+//   single tensor-core launch instead of a chain of 128-row solves.
+//   potrf(b0,b1): potrf(b0,mid); S12 = U11^-T S12 (trsm); S22 -= S12^T S12 (syrk); potrf(mid,b1)
 //   trsm(r0,r1 | c0,c1): recursive on the triangular block; leaves multiply by the inverted
 //   diagonal block W = U_kk^-1 produced by the leaf factorisation.
 // ------------------------------------------------------------------------------------------------
@@ -190,14 +254,16 @@ struct Potrf {
     Stage st;
     double* S;
     MatView vS;
-    MatView vW;   // one Winv slot viewed as 128 x (128*nblk) matrix, ld 128
+    MatView vT;   // the N x N workspace matrix
+    MatView vW;   // inverse of the current panel's diagonal block (ldw x ldw), diagonal 128-blocks first
+    int pb;       // first block of the current panel
 
     gs_status_t leaf(int b)
     {
         gs_plan* plan = st.plan;
         LaunchTimer timer(plan, L_POTRF_LEAF, st.stream);
-        potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(S, plan->N, int(plan->N), b * LB,
-                                                                          winv_ptr(plan) + size_t(b) * LB * LB, info_ptr(plan));
+        double* w = const_cast<double*>(vW.ptr) + size_t(b - pb) * LB * (vW.ld + 1);
+        potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(S, plan->N, int(plan->N), b * LB, w, vW.ld, info_ptr(plan));
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
@@ -213,7 +279,7 @@ struct Potrf {
         p.tiles_m = 1; p.tiles_n = c1 - c0; p.order = ORDER_COL;
         p.c_row0 = r0 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
         p.khi_c = LB / BK; p.kmax = LB / BK;
-        p.a.k0 = 0; p.a.x0 = r0 * LB;          // W slot r0 = columns [128 r0, 128 r0 + 128) of vW
+        p.a.k0 = (r0 - pb) * LB; p.a.x0 = (r0 - pb) * LB;
         p.b.k0 = r0 * LB; p.b.x0 = c0 * LB;
         return launch(st, p, false, L_POTRF_TRSM);
     }
@@ -259,23 +325,6 @@ struct Potrf {
         return launch(st, p, false, L_POTRF_SYRK);
     }
 
-    // Block rows [r0, r1) of the trailing update (the next panel's rows), upper trapezoid:
-    // S[r0:r1, r0:n] -= S[k0:k1, r0:r1]^T S[k0:k1, r0:n]
-    gs_status_t update_rows(int k0, int k1, int r0, int r1, int n)
-    {
-        EngineParams p = blank_params(st.plan);
-        if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
-        p.C = S; p.ldc = vS.ld;
-        p.tiles_m = r1 - r0; p.tiles_n = n - r0; p.order = ORDER_TRAPEZOID;
-        p.c_row0 = r0 * LB; p.c_col0 = r0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
-        p.khi_c = (k1 - k0) * (LB / BK); p.kmax = p.khi_c;
-        p.a.k0 = k0 * LB; p.a.x0 = r0 * LB;
-        p.b.k0 = k0 * LB; p.b.x0 = r0 * LB;
-        p.alpha = -1.0; p.beta = 1.0;
-        p.flags = F_STORE_UPPER;
-        return launch(st, p, false, L_POTRF_SYRK);
-    }
-
     // recursive factorisation of the diagonal block [b0, b1) (touches nothing outside it)
     gs_status_t potrf(int b0, int b1)
     {
@@ -287,38 +336,106 @@ struct Potrf {
         return potrf(mid, b1);
     }
 
-    // panel = block rows [b0, b1): factor the diagonal block, then solve the row panel to its right
-    gs_status_t panel(int b0, int b1, int n)
+    // B + C: factor the diagonal block of panel [b1, b2) and, if a row panel follows, invert it
+    gs_status_t panel_diag(int b1, int b2, int n)
     {
-        GS_TRY(potrf(b0, b1));
-        return trsm(b0, b1, b1, n);
+        pb = b1;
+        GS_TRY(potrf(b1, b2));
+        if (b2 < n) GS_TRY(invert_levels(st, vS, b1 * LB, vW, 0, vT, b1 * LB, b2 - b1, L_POTRF_GEMM, L_POTRF_GEMM));
+        return GS_OK;
     }
 
-    // Right-looking over panels of NB blocks with one panel of look-ahead: while the caller's
-    // stream applies panel p to the trailing matrix beyond panel p+1, the plan's high-priority
-    // side stream applies it to the rows of panel p+1 and factors that panel.
-    gs_status_t factor(int n, int NB, cudaStream_t main_stream, cudaStream_t side, cudaEvent_t ev_fork, cudaEvent_t ev_join)
+    // F: U[b1:b2, c0:c1] = Wp^T S[b1:b2, c0:c1], through the workspace matrix (W = vW of that panel)
+    gs_status_t panel_solve(const MatView& W, int b1, int b2, int c0, int c1)
+    {
+        if (c1 <= c0) return GS_OK;
+        gs_plan* plan = st.plan;
+        EngineParams p = blank_params(plan);
+        if (!set_operand(st, p, 0, W, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
+        p.C = const_cast<double*>(vT.ptr); p.ldc = vT.ld;
+        p.tiles_m = b2 - b1; p.tiles_n = c1 - c0; p.order = ORDER_ROW_REV;
+        p.c_row0 = b1 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vT.rows); p.c_cols = int(vT.cols);
+        p.khi_c = LB / BK; p.khi_i = LB / BK; p.kmax = (b2 - b1) * (LB / BK);
+        p.a.k0 = 0; p.a.x0 = 0;
+        p.b.k0 = b1 * LB; p.b.x0 = c0 * LB;
+        GS_TRY(launch(st, p, false, L_POTRF_TRSM));
+        const int N = int(plan->N);
+        const int rows = (b2 * LB < N ? b2 * LB : N) - b1 * LB;
+        const int cols = (c1 * LB < N ? c1 * LB : N) - c0 * LB;
+        dim3 grid((rows + 255) / 256, cols);
+        LaunchTimer timer(plan, L_POTRF_TRSM, st.stream);
+        copy_block_kernel<<<grid, 256, 0, st.stream>>>(vT.ptr, S, plan->N, b1 * LB, rows, c0 * LB, info_ptr(plan));
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+        plan->launches += 1;
+        return GS_OK;
+    }
+
+    // D: S[b1:b2, b2:n] -= U[b0:b1, b1:b2]^T U[b0:b1, b2:n]
+    gs_status_t update_rows(int b0, int b1, int b2, int n) { return gemm_update(b0, b1, b2, b2, n); }
+
+    // Panel boundaries: wide panels while the trailing matrix is large (the trailing update hides the
+    // panel chain), narrow ones in the tail (the chain is exposed there, and it is shorter per row).
+    static std::vector<int> panel_starts(int n, int nb_big, int nb_tail, int tail)
+    {
+        std::vector<int> s;
+        int b = 0;
+        while (b < n) {
+            s.push_back(b);
+            b += (n - b > tail) ? nb_big : nb_tail;
+        }
+        s.push_back(n);
+        return s;
+    }
+
+    // Iteration i applies row panel i-1 = U[s0:s1, s1:n] and factors panel i = [s1, s2); s3 = end of panel i+1.
+    //   side : A_i  S[s1:s2, s1:s2] -= U[s0:s1, s1:s2]^T U[s0:s1, s1:s2]
+    //          B_i, C_i  factor the diagonal block, invert it (Wp_i)
+    //          F1_i U[s1:s2, s2:s3] = Wp_i^T S[s1:s2, s2:s3]     (after D_i; the columns panel i+1 needs first)
+    //   main : F2_{i-1}  the remaining columns [s2, n) of row panel i-1
+    //          D_i  S[s1:s2, s2:n] -= U[s0:s1, s1:s2]^T U[s0:s1, s2:n]
+    //          E_i  S[s2:n, s2:n] -= U[s0:s1, s2:n]^T U[s0:s1, s2:n]
+    gs_status_t factor(int n, cudaStream_t main_stream)
     {
         gs_plan* plan = st.plan;
+        cudaStream_t side = plan->side;
+        const std::vector<int> ps = panel_starts(n, plan->potrf_nb, plan->potrf_nb_tail, plan->potrf_tail);
+        const int np = int(ps.size()) - 1;
+        const int ldw = wp_ld(plan);
+        auto W = [&](int i) { return MatView{wp_ptr(plan, i), ldw, ldw, ldw}; };
         st.stream = main_stream;
-        GS_TRY(panel(0, NB < n ? NB : n, n));
-        for (int b0 = 0; b0 + NB < n; b0 += NB) {
-            const int b1 = b0 + NB;
-            const int b2 = b1 + NB < n ? b1 + NB : n;
-            GS_CUDA(plan, cudaEventRecord(ev_fork, main_stream));
-            GS_CUDA(plan, cudaStreamWaitEvent(side, ev_fork, 0));
+        vW = W(0);
+        GS_TRY(panel_diag(ps[0], ps[1], n));
+        if (np == 1) return GS_OK;
+        GS_TRY(panel_solve(W(0), ps[0], ps[1], ps[1], ps[2]));            // F1_0
+        gs_status_t rc = GS_OK;
+        cudaError_t ce = cudaSuccess;
+        auto cu = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
+        for (int i = 1; i < np && rc == GS_OK && ce == cudaSuccess; ++i) {
+            const int s0 = ps[i - 1], s1 = ps[i], s2 = ps[i + 1], s3 = (i + 1 < np) ? ps[i + 2] : n;
+            cu(cudaEventRecord(plan->ev_fork, main_stream));
+            cu(cudaStreamWaitEvent(side, plan->ev_fork, 0));
             st.stream = side;
-            gs_status_t rc = update_rows(b0, b1, b1, b2, n);
-            if (rc == GS_OK) rc = panel(b1, b2, n);
+            vW = W(i);
+            rc = syrk(s0, s1, s1, s2);                                           // A_i
+            if (rc == GS_OK) rc = panel_diag(s1, s2, n);                          // B_i, C_i
             st.stream = main_stream;
-            if (rc == GS_OK && b2 < n) rc = syrk(b0, b1, b2, n);
-            // always join the side stream back, also on failure
-            const cudaError_t e1 = cudaEventRecord(ev_join, side);
-            const cudaError_t e2 = cudaStreamWaitEvent(main_stream, ev_join, 0);
-            GS_TRY(rc);
-            GS_CUDA(plan, e1);
-            GS_CUDA(plan, e2);
+            if (rc == GS_OK) rc = panel_solve(W(i - 1), s0, s1, s2, n);           // F2_{i-1}
+            if (s2 < n) {
+                if (rc == GS_OK) rc = update_rows(s0, s1, s2, n);                 // D_i
+                cu(cudaEventRecord(plan->ev_rows, main_stream));
+                if (rc == GS_OK) rc = syrk(s0, s1, s2, n);                        // E_i
+                cu(cudaStreamWaitEvent(side, plan->ev_rows, 0));
+                st.stream = side;
+                if (rc == GS_OK) rc = panel_solve(W(i), s1, s2, s2, s3);          // F1_i
+                st.stream = main_stream;
+            }
+            // main continues only when the side chain of this iteration is done (also on failure)
+            cu(cudaEventRecord(plan->ev_join, side));
+            cu(cudaStreamWaitEvent(main_stream, plan->ev_join, 0));
         }
+        GS_TRY(rc);
+        GS_CUDA(plan, ce);
         return GS_OK;
     }
 };
@@ -330,6 +447,7 @@ gs_status_t ensure_side_stream(gs_plan* plan)
     GS_CUDA(plan, cudaDeviceGetStreamPriorityRange(&lo, &hi));
     GS_CUDA(plan, cudaStreamCreateWithPriority(&plan->side, cudaStreamNonBlocking, hi));
     GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_fork, cudaEventDisableTiming));
+    GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_rows, cudaEventDisableTiming));
     GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_join, cudaEventDisableTiming));
     return GS_OK;
 }
@@ -365,10 +483,17 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     p->nev = nev;
     p->dtype = dtype;
     p->nblk = int((N + LB - 1) / LB);
-    if (const char* e = std::getenv("GS_POTRF_NB")) {
-        const int v = std::atoi(e);
-        if (v >= 1 && v <= 64) p->potrf_nb = v;
-    }
+    // tuning knobs of the POTRF schedule
+    auto knob = [](const char* name, int lo, int hi, int* out) {
+        if (const char* e = std::getenv(name)) {
+            const int v = std::atoi(e);
+            if (v >= lo && v <= hi) *out = v;
+        }
+    };
+    knob("GS_POTRF_NB", 1, 32, &p->potrf_nb);
+    knob("GS_POTRF_NB_TAIL", 1, 32, &p->potrf_nb_tail);
+    knob("GS_POTRF_TAIL", 0, 1 << 20, &p->potrf_tail);
+    if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
     *plan = p;
     return GS_OK;
 }
@@ -378,6 +503,7 @@ gs_status_t gs_plan_destroy(gs_plan_t* plan)
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
     clear_timed(plan);
     if (plan->ev_fork != nullptr) cudaEventDestroy(plan->ev_fork);
+    if (plan->ev_rows != nullptr) cudaEventDestroy(plan->ev_rows);
     if (plan->ev_join != nullptr) cudaEventDestroy(plan->ev_join);
     if (plan->side != nullptr) cudaStreamDestroy(plan->side);
     delete plan;
@@ -416,16 +542,14 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     f.st = Stage{plan, stream, plan->N % 2 == 0};
     f.S = S;
     f.vS = MatView{S, plan->N, plan->N, plan->N};
-    f.vW = MatView{winv_ptr(plan), LB, (long long)LB * plan->nblk, LB};
-    if (plan->nblk > plan->potrf_nb) GS_TRY(ensure_side_stream(plan));
+    f.vT = MatView{big_ptr(plan), plan->N, plan->N, plan->N};
+    f.pb = 0;
+    if (plan->nblk > 1) GS_TRY(ensure_side_stream(plan));
     GS_TRY(zero_lower(f.st, S));   // off-diagonal lower blocks: never touched by the factorisation
-    return f.factor(plan->nblk, plan->potrf_nb, stream, plan->side, plan->ev_fork, plan->ev_join);
+    return f.factor(plan->nblk, stream);
 }
 
-// Block-recursive inversion by doubling: with U = [A B; 0 D],  U^-1 = [A^-1, -A^-1 B D^-1; 0, D^-1].
-// Level s (in 128-blocks): all pairs (A = blocks [2is, 2is+s), D = the next s blocks) at once:
-//   W = B * D^-1   (k <= J: D^-1 upper)      -> workspace, at the position of the target block
-//   X = -A^-1 * W  (k >= I: A^-1 upper)      -> V
+// V = U^-1: every diagonal 128-block inverted by the leaf kernel, then block-recursive doubling.
 gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
@@ -434,7 +558,6 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
     GS_TRY(configure_leaf(plan));
     const double* U = static_cast<const double*>(U_);
     double* V = static_cast<double*>(Uinv_);
-    double* W = big_ptr(plan);
     const int N = int(plan->N), nblk = plan->nblk;
     Stage st{plan, stream, plan->N % 2 == 0};
 
@@ -446,35 +569,8 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
     plan->launches += 1;
     GS_TRY(zero_lower(st, V));
 
-    const MatView vU{U, N, N, N}, vV{V, N, N, N}, vWs{W, N, N, N};
-    for (int s = 1; s < nblk; s *= 2) {
-        const int npairs = (nblk - s + 2 * s - 1) / (2 * s);
-        const int stride = 2 * s * LB;   // elements between consecutive pairs
-        {   // W = B * Dinv
-            EngineParams p = blank_params(plan);
-            if (!set_operand(st, p, 0, vU, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
-            p.C = W; p.ldc = N;
-            p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_COL_REV;
-            p.c_row0 = 0; p.c_col0 = s * LB; p.c_brow = stride; p.c_bcol = stride; p.c_rows = N; p.c_cols = N;
-            p.khi_c = LB / BK; p.khi_j = LB / BK; p.kmax = s * (LB / BK);
-            p.a.x0 = 0; p.a.bx = stride; p.a.k0 = s * LB; p.a.bk = stride;
-            p.b.k0 = s * LB; p.b.bk = stride; p.b.x0 = s * LB; p.b.bx = stride;
-            GS_TRY(launch(st, p, true, L_TRTRI_W));
-        }
-        {   // X = -Ainv * W
-            EngineParams p = blank_params(plan);
-            if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vWs, false)) return GS_ERR_CUDA;
-            p.C = V; p.ldc = N;
-            p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_ROW;
-            p.c_row0 = 0; p.c_col0 = s * LB; p.c_brow = stride; p.c_bcol = stride; p.c_rows = N; p.c_cols = N;
-            p.klo_i = LB / BK; p.khi_c = s * (LB / BK); p.kmax = s * (LB / BK);
-            p.a.x0 = 0; p.a.bx = stride; p.a.k0 = 0; p.a.bk = stride;
-            p.b.k0 = 0; p.b.bk = stride; p.b.x0 = s * LB; p.b.bx = stride;
-            p.alpha = -1.0;
-            GS_TRY(launch(st, p, true, L_TRTRI_X));
-        }
-    }
-    return GS_OK;
+    const MatView vU{U, N, N, N}, vV{V, N, N, N}, vT{big_ptr(plan), N, N, N};
+    return invert_levels(st, vU, 0, vV, 0, vT, 0, nblk, L_TRTRI_W, L_TRTRI_X);
 }
 
 // H~ = V^T H V with H = T + T^T, T = triu(H,1) + diag(H)/2:
@@ -643,6 +739,25 @@ gs_status_t gs_plan_launch_times(gs_plan_t* plan, gs_launch_time_t* out, int cap
         ++k;
     }
     *count = k;
+    return GS_OK;
+}
+
+gs_status_t gs_plan_launch_trace(gs_plan_t* plan, gs_launch_trace_t* out, int cap, int* count)
+{
+    if (plan == nullptr || count == nullptr || (out == nullptr && cap > 0)) return GS_ERR_INVALID_ARG;
+    const int n = int(plan->timed.size());
+    for (int i = 0; i < n && i < cap; ++i) {
+        const TimedLaunch& t = plan->timed[i];
+        float a = 0.f, b = 0.f;
+        cudaError_t e = cudaEventElapsedTime(&a, plan->timed[0].e0, t.e0);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&b, plan->timed[0].e0, t.e1);
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+        std::snprintf(out[i].label, sizeof(out[i].label), "%s", kLabelNames[t.label]);
+        out[i].side_stream = t.side;
+        out[i].t0_ms = a;
+        out[i].t1_ms = b;
+    }
+    *count = n;
     return GS_OK;
 }
 

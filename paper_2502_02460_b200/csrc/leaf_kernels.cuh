@@ -113,10 +113,10 @@ __device__ __forceinline__ void leaf_invert_upper(const LeafSmem& s, int tx, int
 }
 
 // S: N x N column-major (ld), block starts at (j0, j0), order nb = min(LB, N - j0).
-// Winv: dense LB x LB column-major slot receiving U_kk^-1 (identity-padded).
+// Winv: LB x LB column-major block (leading dimension ldw) receiving U_kk^-1 (identity-padded).
 // info: device flag; set (if still 0) to j0 + j + 1 when pivot j is not > 0.
 __global__ void __launch_bounds__(kLeafThreads, 1)
-potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* __restrict__ Winv, int* info)
+potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* __restrict__ Winv, long long ldw, int* info)
 {
     if (*info != 0) return;
     extern __shared__ __align__(16) unsigned char leaf_raw[];
@@ -184,7 +184,7 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
     leaf_store_all(s, blk, ld, nb, t);
 
     leaf_invert_upper(s, tx, ty);
-    leaf_store_all(s, Winv, LB, LB, t);
+    leaf_store_all(s, Winv, ldw, LB, t);
 }
 
 // One CTA per diagonal block b: V_bb = U_bb^-1.  Reads only the upper triangle of U_bb; writes the
@@ -233,6 +233,18 @@ __global__ void zero_lower_blocks_kernel(double* __restrict__ X, long long ld, i
     const int first = (col / LB + 1) * LB;   // first row below the diagonal block of this column
     const int row = first + blockIdx.x * blockDim.x + threadIdx.x;
     if (row < N) X[row + (long long)col * ld] = 0.0;
+}
+
+// dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid row (blockIdx.y) per column c.
+__global__ void copy_block_kernel(const double* __restrict__ src, double* __restrict__ dst, long long ld, int row0, int rows,
+                                  int col0, const int* info)
+{
+    if (*info != 0) return;
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < rows) {
+        const long long off = row0 + r + (long long)(col0 + blockIdx.y) * ld;
+        dst[off] = src[off];
+    }
 }
 
 }  // namespace gs

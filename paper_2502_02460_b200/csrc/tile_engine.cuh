@@ -293,11 +293,43 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
     const int g = lane >> 2, q = lane & 3;
     const int rho = (g >> 1) + 4 * (g & 1);   // logical row within an 8-row group for k-contiguous operands
 
+    // C tile coordinates of this thread's accumulators (fragment row g of m-group mg, fragment
+    // columns 2q+e of n-group ng; the column was supplied by the B-lane with g' = 2q+e -> n = rho(g'))
+    const long long crow0 = p.c_row0 + (long long)b * p.c_brow + (long long)BM * I + wm * 32;
+    const long long ccol0 = p.c_col0 + (long long)b * p.c_bcol + (long long)BN * J + wn * 64;
+    const bool upper_only = (p.flags & F_STORE_UPPER) != 0;
+    const double alpha = p.alpha, beta = p.beta;
+    auto c_row = [&](int mg) -> long long {
+        return crow0 + (kANN ? ((mg >> 1) * 16 + 2 * g + (mg & 1)) : (mg * 8 + rho));
+    };
+    auto c_col = [&](int ng, int e) -> long long {
+        const int gp = 2 * q + e;
+        return ccol0 + ng * 8 + ((gp >> 1) + 4 * (gp & 1));
+    };
+
+    // beta != 0: the accumulators start from (beta/alpha) * C, so the loads of the C tile overlap
+    // the pipeline fill instead of forming a dependent load-FMA-store chain in the epilogue.
     double acc[4][8][2];
+    if (beta != 0.0) {
+        const double sc = beta / alpha;
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+        for (int mg = 0; mg < 4; ++mg) {
+            const long long row = c_row(mg);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+            for (int ng = 0; ng < 8; ++ng)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const long long col = c_col(ng, e);
+                    const bool ok = row < p.c_rows && col < p.c_cols && (!upper_only || row <= col);
+                    acc[mg][ng][e] = ok ? sc * __ldg(p.C + row + col * p.ldc) : 0.0;
+                }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+    }
 
     // per-thread byte offsets inside a stage (k8-step h = 0); h = 1 is offset ^ 64 (k-contig) / + 1024 (m-contig)
     const uint32_t offB = kTileBytes + (wn * 64 + rho) * 128 + ((q ^ rho) * 16);
@@ -383,32 +415,17 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
         if (lane == 0) mbar_arrive(empty0 + 8 * stage);
     }
 
-    // ===================== epilogue: C = alpha*acc + beta*C (predicated, direct to global) =====================
-    const long long crow0 = p.c_row0 + (long long)b * p.c_brow + (long long)BM * I + wm * 32;
-    const long long ccol0 = p.c_col0 + (long long)b * p.c_bcol + (long long)BN * J + wn * 64;
-    const bool upper_only = (p.flags & F_STORE_UPPER) != 0;
-    const double alpha = p.alpha, beta = p.beta;
+    // ===================== epilogue: C = alpha * acc (predicated, direct to global) =====================
 #pragma unroll
     for (int mg = 0; mg < 4; ++mg) {
-        // logical row of fragment row g in m-group mg
-        int mrow;
-        if (kANN) mrow = (mg >> 1) * 16 + 2 * g + (mg & 1);
-        else mrow = mg * 8 + rho;
-        const long long row = crow0 + mrow;
+        const long long row = c_row(mg);
 #pragma unroll
         for (int ng = 0; ng < 8; ++ng) {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                // fragment column c = 2q+e was supplied by the B-lane with g' = 2q+e -> logical n = rho(g')
-                const int gp = 2 * q + e;
-                const int ncol = ng * 8 + ((gp >> 1) + 4 * (gp & 1));
-                const long long col = ccol0 + ncol;
-                if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col)) {
-                    double* dst = p.C + row + col * p.ldc;
-                    double v = alpha * acc[mg][ng][e];
-                    if (beta != 0.0) v += beta * (*dst);
-                    *dst = v;
-                }
+                const long long col = c_col(ng, e);
+                if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col))
+                    p.C[row + col * p.ldc] = alpha * acc[mg][ng][e];
             }
         }
     }

@@ -30,12 +30,17 @@ EXPORTS = (
     "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_last_info",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
-    "gs_plan_set_timing", "gs_plan_launch_times",
+    "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
 )
 
 
 class LaunchTime(ctypes.Structure):
     _fields_ = [("label", ctypes.c_char * 32), ("launches", ctypes.c_int64), ("ms", ctypes.c_double)]
+
+class LaunchTrace(ctypes.Structure):
+    _fields_ = [("label", ctypes.c_char * 32), ("side_stream", ctypes.c_int32),
+                ("t0_ms", ctypes.c_double), ("t1_ms", ctypes.c_double)]
+
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgs.so")
@@ -76,6 +81,7 @@ def lib() -> ctypes.CDLL:
         L.gs_backtransform_host.argtypes = [vp, vp, vp, vp, sz, vp]
         L.gs_plan_set_timing.argtypes = [vp, ctypes.c_int]
         L.gs_plan_launch_times.argtypes = [vp, ctypes.POINTER(LaunchTime), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
+        L.gs_plan_launch_trace.argtypes = [vp, ctypes.POINTER(LaunchTrace), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.gs_plan_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
         L.gs_status_string.argtypes = [ctypes.c_int]
         L.gs_status_string.restype = ctypes.c_char_p
@@ -215,6 +221,14 @@ class Plan:
     # ---- optional per-launch timing (roofline reports) ----
     def set_timing(self, mode: int):
         self._check(lib().gs_plan_set_timing(self._h, mode))
+
+    def launch_trace(self, cap: int = 8192) -> list:
+        """[(label, side_stream, t0_ms, t1_ms)] per launch since set_timing(1); call before launch_times()."""
+        buf = (LaunchTrace * cap)()
+        n = ctypes.c_int(0)
+        self._check(lib().gs_plan_launch_trace(self._h, buf, cap, ctypes.byref(n)))
+        return [(buf[i].label.decode(), int(buf[i].side_stream), float(buf[i].t0_ms), float(buf[i].t1_ms))
+                for i in range(min(n.value, cap))]
 
     def launch_times(self) -> dict:
         """{label: (launches, total_ms)} since the last set_timing; call after a stream synchronise."""
