@@ -201,31 +201,25 @@ def _nvml_index(local_rank: int) -> int:
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
 
     from paper_2502_02460_b200 import gs
     from paper_2502_02460_b200 import workloads as wl
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2502_02460_b200 import replicas
+
+    info = replicas.rank_info()
+    rank, world, local_rank = info.rank, info.world, info.local_rank
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    replicas.init(info, "nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier(info)
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(info, x, dev)
 
     cfg = wl.CONFIGS[args.config]
     if cfg.complex:
@@ -234,7 +228,7 @@ def run_ours(args):
     flops = wl.nominal_flops(N, nev)
 
     # every rank reduces its own independent pencil (replicas; different seed per rank)
-    pencil = wl.make_pencil(N, cfg.box, cfg.seed + 100 * rank, device=dev)
+    pencil = wl.make_pencil(N, cfg.box, replicas.replica_seed(cfg.seed, rank), device=dev)
     H, S0 = pencil.H, pencil.S
     U = wl.colmajor_empty(N, N, device=dev)
     V = wl.colmajor_empty(N, N, device=dev)
@@ -290,7 +284,7 @@ def run_ours(args):
 
     stage_ms = [sum(e[i].elapsed_time(e[i + 1]) for e in events) / args.steps for i in range(4)]
     step_ms = max_over_ranks(sum(stage_ms))
-    value = world * flops["total"] / (step_ms * 1e-3) / 1e12
+    value = replicas.aggregate_throughput(info, flops["total"], step_ms)
 
     # per-kernel device times: one extra (untimed) step with events around every launch
     plan.set_timing(1)
@@ -410,8 +404,7 @@ def run_ours(args):
             "paper_context": "PAPER.md:133 Table 1 (ELPA 2024.05, NCCL, 4x A100-40GB, N=40960, nev=N): Cholesky 2.3 s, "
                              "Invert 1.8 s, Multiply 18.8 s, Backtr. 6.8 s = 29.7 s, i.e. ~6.2 TFLOP/s on 4 GPUs (context only)",
         }))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finalize(info)
 
 
 def main():

@@ -54,7 +54,7 @@ struct gs_plan {
     cudaEvent_t ev_fork = nullptr, ev_rows = nullptr, ev_join = nullptr;
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
-    int potrf_tail = 40;
+    int potrf_tail = 64;
     char cuda_error[256] = {0};
 };
 
