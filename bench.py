@@ -222,20 +222,20 @@ def run_ours(args):
         return replicas.max_over_ranks(info, x, dev)
 
     cfg = wl.CONFIGS[args.config]
-    if cfg.complex:
-        raise SystemExit("bench.py: the complex (Hermitian) path is not built yet (DESIGN.md, out of scope this round)")
     N, nev = cfg.N, cfg.nev
-    flops = wl.nominal_flops(N, nev)
+    cplx = cfg.complex
+    tdt = torch.complex128 if cplx else torch.float64
+    flops = wl.nominal_flops(N, nev, cplx)     # complex: real-equivalent = 4x the real formulas
 
     # every rank reduces its own independent pencil (replicas; different seed per rank)
-    pencil = wl.make_pencil(N, cfg.box, replicas.replica_seed(cfg.seed, rank), device=dev)
+    pencil = wl.make_pencil(N, cfg.box, replicas.replica_seed(cfg.seed, rank), complex=cplx, device=dev)
     H, S0 = pencil.H, pencil.S
-    U = wl.colmajor_empty(N, N, device=dev)
-    V = wl.colmajor_empty(N, N, device=dev)
-    Ht = wl.colmajor_zeros(N, N, device=dev)
-    Ct = wl.dense_rhs(N, nev, seed=rank, device=dev)
-    C = wl.colmajor_empty(N, nev, device=dev)
-    plan = gs.Plan(N, nev, device=dev)
+    U = wl.colmajor_empty(N, N, dtype=tdt, device=dev)
+    V = wl.colmajor_empty(N, N, dtype=tdt, device=dev)
+    Ht = wl.colmajor_zeros(N, N, dtype=tdt, device=dev)
+    Ct = wl.dense_rhs(N, nev, seed=rank, complex=cplx, device=dev)
+    C = wl.colmajor_empty(N, nev, dtype=tdt, device=dev)
+    plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64, device=dev)
 
     # FP64 roofline denominator, measured on this device right now (MEASURED_PEAKS.json has no FP64 entry)
     dmma_sus, dmma_burst = gs.measure_fp64_peak(0, 1.0)
@@ -295,12 +295,12 @@ def run_ours(args):
 
     # roofline of the dominant kernel: the SYR2K-shaped launch of gs_to_standard (2N^3/3 flop of the
     # nominal 2.67 N^3-ish path: the largest single launch), timed live with CUDA events above
-    dom_flop = 2.0 * float(N) ** 3 / 3.0
+    dom_flop = (4.0 if cplx else 1.0) * 2.0 * float(N) ** 3 / 3.0
     dom_ms = dom[1] / max(dom[0], 1)
     achieved = dom_flop / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else None
     mp = _measured_peaks()
     roofline = {
-        "bound": "tensor", "kernel": "tile_engine_kernel<TN,TMA> as to_standard.syr2k (FP64 DMMA)",
+        "bound": "tensor", "kernel": ("ctile_engine_kernel<TN>" if cplx else "tile_engine_kernel<TN,TMA>") + " as to_standard.syr2k (FP64 DMMA)",
         "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
         "frac": (achieved / fp64_peak) if achieved else None,
         "traffic": _ncu_traffic("to_standard.syr2k"),
@@ -323,7 +323,7 @@ def run_ours(args):
     if not args.no_checks and rank == 0:
         Ut = torch.triu(U)
         checks = {
-            "chol_resid_fro": ((Ut.t() @ Ut - S0).norm() / S0.norm()).item(),
+            "chol_resid_fro": ((Ut.conj().t() @ Ut - S0).norm() / S0.norm()).item(),
             "lower_U_max": torch.tril(U, -1).abs().max().item(),
             "lower_Uinv_max": torch.tril(V, -1).abs().max().item(),
         }
@@ -331,7 +331,7 @@ def run_ours(args):
         R.diagonal().sub_(1.0)
         checks["U_Uinv_minus_I_fro_over_sqrtN"] = R.norm().item() / N ** 0.5
         del R
-        Href = V.t() @ (H @ V)
+        Href = V.conj().t() @ (H @ V)
         checks["Htilde_rel_fro_vs_torch"] = (torch.triu(Ht - Href).norm() / torch.triu(Href).norm()).item()
         del Href
         Cref = V @ Ct
@@ -346,11 +346,11 @@ def run_ours(args):
     if not args.no_e2e:
         del U, Ht, C
         torch.cuda.empty_cache()
-        hH = torch.empty((N, N), dtype=torch.float64).pin_memory()
-        hS = torch.empty((N, N), dtype=torch.float64).pin_memory()
-        hHt = torch.empty((N, N), dtype=torch.float64).pin_memory()
-        hCt = torch.empty((nev, N), dtype=torch.float64).pin_memory()
-        hC = torch.empty((nev, N), dtype=torch.float64).pin_memory()
+        hH = torch.empty((N, N), dtype=tdt).pin_memory()
+        hS = torch.empty((N, N), dtype=tdt).pin_memory()
+        hHt = torch.empty((N, N), dtype=tdt).pin_memory()
+        hCt = torch.empty((nev, N), dtype=tdt).pin_memory()
+        hC = torch.empty((nev, N), dtype=tdt).pin_memory()
         hH.copy_(H.t())           # buffers hold the column-major images
         hS.copy_(S0.t())
         hCt.copy_(Ct.t())
@@ -371,13 +371,14 @@ def run_ours(args):
         t1 = time.perf_counter()
         barrier()
         e2e_sec = max_over_ranks((t1 - t0) / e2e_steps)
+        esz = 16 if cplx else 8
         e2e = {"value": world * flops["total"] / e2e_sec / 1e12, "unit": UNIT,
-               "h2d_bytes_per_step": 2 * N * N * 8 + N * nev * 8, "d2h_bytes_per_step": N * N * 8 + N * nev * 8,
+               "h2d_bytes_per_step": (2 * N * N + N * nev) * esz, "d2h_bytes_per_step": (N * N + N * nev) * esz,
                "ms_per_step": e2e_sec * 1e3, "steps": e2e_steps,
                "api": "gs_reduce_host + gs_backtransform_host (pinned host buffers in, H~ and C out)"}
         if checks is not None:
             # the host-buffer path must reproduce the device-buffer path bit for bit (same kernels, same order)
-            plan.to_standard(H, V, Ht2 := wl.colmajor_zeros(N, N, device=dev))
+            plan.to_standard(H, V, Ht2 := wl.colmajor_zeros(N, N, dtype=tdt, device=dev))
             plan.last_info()
             checks["e2e_Htilde_equals_device_path"] = bool(torch.equal(torch.triu(hHt.t().to(dev)), torch.triu(Ht2)))
             del Ht2
@@ -391,11 +392,11 @@ def run_ours(args):
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": "c128 (FP64 arithmetic)" if cplx else "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
                        "recipe": "BASELINE.json configs[%d]: Gaussian-overlap S, H = -S(1+0.1g)+diag" % cfg.index,
                        "parallelism": "replicas x%d (one independent pencil per GPU)" % world,
-                       "cache": "inputs_larger_than_L2 (each matrix %.1f GiB vs 126 MB L2)" % (N * N * 8 / 2 ** 30),
+                       "cache": "inputs_larger_than_L2 (each matrix %.1f GiB vs 126 MB L2)" % (N * N * (16 if cplx else 8) / 2 ** 30),
                        "timing": "CUDA events per step on the launching stream; S restored between steps outside the events"},
             "frac_of_fp64_peak": value / world / fp64_peak, "fp64_peak_tflops": fp64_peak,
             "stages": stages, "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e,

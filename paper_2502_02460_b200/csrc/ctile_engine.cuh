@@ -1,0 +1,256 @@
+// ctile_engine.cuh -- the complex128 (Hermitian path) variant of the tile engine.
+//
+// Same contract as tile_engine.cuh (one launch = a set of output tiles with affine k-ranges, the
+// same EngineParams, flags and tile orders), for interleaved complex matrices (re, im doubles):
+//     C[I,J] = alpha * sum_kt ( opA(kt,I) * B(kt,J) [+ opA2(kt,I) * B2(kt,J)] ) + beta * C[I,J]
+// opA is A^H for the k-contiguous ("TN") layout -- "A^T corresponds to the ... conjugate-transpose
+// of a ... complex-valued matrix" -- and plain A for the m-contiguous ("NN") layout.
+// Coordinates in EngineParams are in COMPLEX elements.
+//
+// Hardware mapping (sm_100a): one complex multiply-accumulate = 4 real FP64 tensor-core MMAs
+// (mma.sync.m8n8k4.f64):  re += ar*br + (-+ai)*bi,  im += ar*bi + (+-ai)*br.  No 3-multiply trick
+// (reading Q10).  A 16-byte shared-memory chunk is exactly one complex number, so one
+// conflict-free LDS.128 yields the (re, im) fragment of one DMMA operand element.
+//   * C tile 64 x 64 complex, 4 consumer warps (2 x 2, warp tile 32 x 32 complex = 64 FP64
+//     accumulators per thread) + 1 TMA producer warp; 2 CTAs per SM, so one CTA's epilogue and
+//     pipeline fill overlap the other's main loop.
+//   * Operand tiles 64 x 8 complex (8 KB) staged by TMA (FP64 tensor map over the interleaved
+//     matrix viewed as 2*rows x cols doubles, 128-byte swizzle) into a 6-stage ring.
+#pragma once
+#include "tile_engine.cuh"
+
+namespace gs {
+
+constexpr int CT = 64;        // complex C tile rows = cols
+constexpr int CBK = 8;        // complex k-slab per pipeline stage (8 x 16 B = one 128-byte swizzle row)
+constexpr int kCStages = 6;
+constexpr int kCConsumerWarps = 4;
+constexpr int kCThreads = (kCConsumerWarps + 1) * 32;
+constexpr int kCTileBytes = CT * CBK * 16;                  // 8 KB per operand tile
+constexpr int kCStageBytes = 2 * kCTileBytes;               // A + B
+constexpr int kCSmemBytes = kCStages * kCStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+
+// Zero / halve the part of a complex operand tile that lies below / on the global diagonal.
+// k-contiguous tile: 64 rows (free index x) of 8 complex (k): element (row = k0 + k, col = x0 + x).
+// m-contiguous tile: 8 boxes [mb][k][8 m]: element (row = x0 + 8*mb + m_in, col = k0 + k).
+template <bool kMContig>
+__device__ __forceinline__ void mask_ctile(unsigned char* tile, int k0, int x0, bool half_diag, int ctid)
+{
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        const int chunk_lin = ctid + it * 128;          // 0..511 : complex element index in the tile
+        const int row128 = chunk_lin >> 3;              // 128-byte row
+        const int ch = chunk_lin & 7;                   // logical chunk within the row
+        const int phys = ch ^ (row128 & 7);
+        double2* ptr = reinterpret_cast<double2*>(tile + row128 * 128 + phys * 16);
+        int grow, gcol;
+        if (!kMContig) { gcol = x0 + row128; grow = k0 + ch; }
+        else { const int mb = row128 >> 3, k = row128 & 7; grow = x0 + mb * 8 + ch; gcol = k0 + k; }
+        if (grow > gcol) *ptr = make_double2(0.0, 0.0);
+        else if (half_diag && grow == gcol) { double2 v = *ptr; v.x *= 0.5; v.y *= 0.5; *ptr = v; }
+    }
+}
+
+template <bool kANN>
+__global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid_constant__ EngineParams p)
+{
+    if (p.info != nullptr && *p.info != 0) return;
+
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kCStages * kCStageBytes);
+    const uint32_t full0 = smem_u32(bars);
+    const uint32_t empty0 = smem_u32(bars + kCStages);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    int b, I, J;
+    decode_tile(p, blockIdx.x, b, I, J);
+    int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
+    int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
+    if (k_lo < 0) k_lo = 0;
+    if (k_hi > p.kmax) k_hi = p.kmax;
+    const int nk = k_hi > k_lo ? k_hi - k_lo : 0;
+    const bool dual = (p.flags & F_DUAL) != 0;
+    const int nsteps = dual ? 2 * nk : nk;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kCStages; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, kCConsumerWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // element coordinates (complex elements) of the operand tiles at k-step 0
+    const int a_x = p.a.x0 + b * p.a.bx + CT * I, a_k = p.a.k0 + b * p.a.bk;
+    const int b_x = p.b.x0 + b * p.b.bx + CT * J, b_k = p.b.k0 + b * p.b.bk;
+    const int a2_x = p.a2.x0 + b * p.a2.bx + CT * I, a2_k = p.a2.k0 + b * p.a2.bk;
+    const int b2_x = p.b2.x0 + b * p.b2.bx + CT * J, b2_k = p.b2.k0 + b * p.b2.bk;
+
+    if (warp == kCConsumerWarps) {
+        // ===================== TMA producer (one elected lane) =====================
+        if (lane == 0) {
+            tma_prefetch_desc(&p.mapA);
+            tma_prefetch_desc(&p.mapB);
+            if (dual) { tma_prefetch_desc(&p.mapA2); tma_prefetch_desc(&p.mapB2); }
+            for (int s = 0; s < nsteps; ++s) {
+                const int stage = s % kCStages;
+                const uint32_t ph = (s / kCStages) & 1;
+                mbar_wait(empty0 + 8 * stage, ph ^ 1);
+                const uint32_t full = full0 + 8 * stage;
+                mbar_arrive_expect_tx(full, kCStageBytes);
+                const uint32_t dstA = smem_u32(smem + stage * kCStageBytes);
+                const uint32_t dstB = dstA + kCTileBytes;
+                const bool second = dual && (s & 1);
+                const int kt = k_lo + (dual ? (s >> 1) : s);
+                const CUtensorMap* mA = second ? &p.mapA2 : &p.mapA;
+                const CUtensorMap* mB = second ? &p.mapB2 : &p.mapB;
+                const int ax = second ? a2_x : a_x, ak = (second ? a2_k : a_k) + kt * CBK;
+                const int bx = second ? b2_x : b_x, bk = (second ? b2_k : b_k) + kt * CBK;
+                // the tensor maps see the matrix as doubles: contiguous coordinate = 2 x complex index
+                if (kANN) {
+#pragma unroll
+                    for (int mb = 0; mb < CT / 8; ++mb)
+                        tma_load_2d(dstA + mb * 1024, mA, 2 * (ax + mb * 8), ak, full);
+                } else {
+                    tma_load_2d(dstA, mA, 2 * ak, ax, full);
+                }
+                tma_load_2d(dstB, mB, 2 * bk, bx, full);
+            }
+        }
+        return;
+    }
+
+    // ===================== consumers: 4 warps, 2 (m) x 2 (n), warp tile 32 x 32 complex =====================
+    const int wm = warp & 1, wn = warp >> 1;
+    const int g = lane >> 2, q = lane & 3;
+    const int rho = (g >> 1) + 4 * (g & 1);   // logical row within an 8-row group (conflict-free LDS.128)
+
+    const long long crow0 = p.c_row0 + (long long)b * p.c_brow + (long long)CT * I + wm * 32;
+    const long long ccol0 = p.c_col0 + (long long)b * p.c_bcol + (long long)CT * J + wn * 32;
+    const bool upper_only = (p.flags & F_STORE_UPPER) != 0;
+    const bool real_diag = (p.flags & F_REAL_DIAG) != 0;
+    const double alpha = p.alpha, beta = p.beta;
+    double2* Cz = reinterpret_cast<double2*>(p.C);
+    auto c_row = [&](int mg) -> long long { return crow0 + mg * 8 + rho; };
+    auto c_col = [&](int ng, int e) -> long long {
+        const int gp = 2 * q + e;
+        return ccol0 + ng * 8 + ((gp >> 1) + 4 * (gp & 1));
+    };
+
+    double acc[4][4][2][2];   // [mg][ng][fragment column e][re, im]
+    if (beta != 0.0) {
+        const double sc = beta / alpha;
+#pragma unroll
+        for (int mg = 0; mg < 4; ++mg) {
+            const long long row = c_row(mg);
+#pragma unroll
+            for (int ng = 0; ng < 4; ++ng)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const long long col = c_col(ng, e);
+                    const bool ok = row < p.c_rows && col < p.c_cols && (!upper_only || row <= col);
+                    double2 v = make_double2(0.0, 0.0);
+                    if (ok) v = __ldcg(Cz + row + col * p.ldc);
+                    acc[mg][ng][e][0] = sc * v.x;
+                    acc[mg][ng][e][1] = sc * v.y;
+                }
+        }
+    } else {
+#pragma unroll
+        for (int mg = 0; mg < 4; ++mg)
+#pragma unroll
+            for (int ng = 0; ng < 4; ++ng)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) { acc[mg][ng][e][0] = 0.0; acc[mg][ng][e][1] = 0.0; }
+    }
+
+    // per-thread byte offsets inside a stage at k4-step h = 0
+    const uint32_t offB = kCTileBytes + (wn * 32 + rho) * 128 + ((q ^ rho) * 16);
+    uint32_t offA;
+    if (kANN) offA = (wm * 4) * 1024 + q * 128 + ((rho ^ q) * 16);   // box wm*4+mg, row k = q (+4h), chunk rho ^ k
+    else offA = (wm * 32 + rho) * 128 + ((q ^ rho) * 16);            // row x = wm*32 + mg*8 + rho, chunk k ^ rho
+    const uint32_t mask_any = p.flags & (F_MASK_A | F_MASK_B | F_MASK_A2 | F_MASK_B2);
+    const int ctid = threadIdx.x;   // 0..127 for consumers
+
+    for (int s = 0; s < nsteps; ++s) {
+        const int stage = s % kCStages;
+        const uint32_t ph = (s / kCStages) & 1;
+        mbar_wait(full0 + 8 * stage, ph);
+        release_previous_stage(s, kCStages, empty0, lane);
+        unsigned char* st = smem + stage * kCStageBytes;
+
+        if (mask_any) {
+            const bool second = dual && (s & 1);
+            const int kt = k_lo + (dual ? (s >> 1) : s);
+            const bool mA = (p.flags & (second ? F_MASK_A2 : F_MASK_A)) != 0;
+            const bool mB = (p.flags & (second ? F_MASK_B2 : F_MASK_B)) != 0;
+            const int ax = second ? a2_x : a_x, ak = (second ? a2_k : a_k) + kt * CBK;
+            const int bx = second ? b2_x : b_x, bk = (second ? b2_k : b_k) + kt * CBK;
+            bool did = false;
+            if (mA) {
+                const bool straddle = kANN ? (ax + CT - 1 >= ak) : (ak + CBK - 1 >= ax);
+                if (straddle) {
+                    mask_ctile<kANN>(st, ak, ax, !second && (p.flags & F_HALF_DIAG_A), ctid);
+                    did = true;
+                }
+            }
+            if (mB) {
+                if (bk + CBK - 1 >= bx) { mask_ctile<false>(st + kCTileBytes, bk, bx, false, ctid); did = true; }
+            }
+            if (did) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                named_bar_sync(1, kCConsumerWarps * 32);
+            }
+        }
+
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            double ar[4], a2[4], a3[4];
+#pragma unroll
+            for (int mg = 0; mg < 4; ++mg) {
+                const uint32_t off = kANN ? ((offA + mg * 1024 + h * 512) ^ (h * 64)) : ((offA + mg * 1024) ^ (h * 64));
+                const double2 v = *reinterpret_cast<const double2*>(st + off);
+                ar[mg] = v.x;
+                // TN = conjugate transpose: (ar - i ai)(br + i bi) = (ar br + ai bi) + i (ar bi - ai br)
+                a2[mg] = kANN ? -v.y : v.y;    // multiplies bi into the real part
+                a3[mg] = kANN ? v.y : -v.y;    // multiplies br into the imaginary part
+            }
+            double2 bf[4];
+#pragma unroll
+            for (int ng = 0; ng < 4; ++ng)
+                bf[ng] = *reinterpret_cast<const double2*>(st + ((offB + ng * 1024) ^ (h * 64)));
+#pragma unroll
+            for (int mg = 0; mg < 4; ++mg)
+#pragma unroll
+                for (int ng = 0; ng < 4; ++ng) {
+                    dmma_8x8x4(acc[mg][ng][0][0], acc[mg][ng][1][0], ar[mg], bf[ng].x);
+                    dmma_8x8x4(acc[mg][ng][0][1], acc[mg][ng][1][1], ar[mg], bf[ng].y);
+                    dmma_8x8x4(acc[mg][ng][0][0], acc[mg][ng][1][0], a2[mg], bf[ng].y);
+                    dmma_8x8x4(acc[mg][ng][0][1], acc[mg][ng][1][1], a3[mg], bf[ng].x);
+                }
+        }
+    }
+
+    // ===================== epilogue: C = alpha * acc (predicated 16-byte stores) =====================
+#pragma unroll
+    for (int mg = 0; mg < 4; ++mg) {
+        const long long row = c_row(mg);
+#pragma unroll
+        for (int ng = 0; ng < 4; ++ng)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const long long col = c_col(ng, e);
+                if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col)) {
+                    double2 v = make_double2(alpha * acc[mg][ng][e][0], alpha * acc[mg][ng][e][1]);
+                    if (real_diag && row == col) v.y = 0.0;
+                    Cz[row + col * p.ldc] = v;
+                }
+            }
+    }
+}
+
+}  // namespace gs

@@ -6,6 +6,7 @@
 
 #include <cstring>
 
+#include "ctile_engine.cuh"
 #include "tile_engine.cuh"
 
 namespace gs {
@@ -27,8 +28,9 @@ inline PFN_cuTensorMapEncodeTiled tensor_map_encoder()
 
 // Column-major FP64 matrix view: rows x cols, leading dimension ld (elements).  TMA needs a
 // 16-byte aligned base and a row pitch that is a multiple of 16 bytes (even ld).
+// (complex128: interleaved (re, im); rows, cols, ld count complex elements.)
 struct MatView {
-    const double* ptr;
+    const void* ptr;
     long long rows, cols, ld;
 };
 
@@ -38,15 +40,17 @@ inline bool tma_compatible(const MatView& m)
 }
 
 // box = box_rows (contiguous dim, always 16 doubles = 128 B) x box_cols
-inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols)
+// A complex matrix is described to TMA as a 2*rows x cols FP64 matrix.
+inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols, bool cplx)
 {
     PFN_cuTensorMapEncodeTiled enc = tensor_map_encoder();
     if (enc == nullptr) return false;
-    cuuint64_t dims[2] = {static_cast<cuuint64_t>(m.rows), static_cast<cuuint64_t>(m.cols)};
-    cuuint64_t strides[1] = {static_cast<cuuint64_t>(m.ld) * 8};
+    const int w = cplx ? 2 : 1;
+    cuuint64_t dims[2] = {static_cast<cuuint64_t>(m.rows) * w, static_cast<cuuint64_t>(m.cols)};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(m.ld) * 8 * w};
     cuuint32_t box[2] = {static_cast<cuuint32_t>(BK), static_cast<cuuint32_t>(box_cols)};
     cuuint32_t estr[2] = {1, 1};
-    const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(m.ptr), dims, strides, box, estr,
+    const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(m.ptr), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
@@ -72,6 +76,10 @@ inline cudaError_t engine_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(tile_engine_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ctile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ctile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
+    if (e != cudaSuccess) return e;
     done = true;
     return cudaSuccess;
 }
@@ -92,6 +100,18 @@ inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, bool use_tma,
         if (a_nn) tile_engine_kernel<true, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
         else tile_engine_kernel<false, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
     }
+    return cudaGetLastError();
+}
+
+// complex128 engine: operands always go through TMA (a complex row pitch is a multiple of 16 bytes)
+inline cudaError_t cengine_launch(const EngineParams& p, bool a_nn, cudaStream_t stream)
+{
+    const int grid = num_tiles(p);
+    if (grid <= 0) return cudaSuccess;
+    cudaError_t e = engine_configure();
+    if (e != cudaSuccess) return e;
+    if (a_nn) ctile_engine_kernel<true><<<grid, kCThreads, kCSmemBytes, stream>>>(p);
+    else ctile_engine_kernel<false><<<grid, kCThreads, kCSmemBytes, stream>>>(p);
     return cudaGetLastError();
 }
 

@@ -20,6 +20,7 @@
 
 #include "engine_host.cuh"
 #include "leaf_kernels.cuh"
+#include "cleaf_kernels.cuh"
 
 using namespace gs;
 
@@ -42,7 +43,11 @@ struct gs_plan {
     int64_t N = 0;
     int64_t nev = 0;
     gs_dtype_t dtype = GS_REAL64;
-    int nblk = 0;                    // ceil(N / 128)
+    bool z = false;                  // GS_COMPLEX128
+    int lb = LB;                     // leaf / tile block order in elements: 128 (real) or 64 (complex)
+    int bk = BK;                     // k-slab of one pipeline stage in elements: 16 (real) or 8 (complex)
+    size_t es = sizeof(double);      // bytes per element
+    int nblk = 0;                    // ceil(N / lb)
     unsigned char* ws = nullptr;     // caller-owned device workspace
     size_t ws_bytes = 0;
     int64_t launches = 0;
@@ -61,16 +66,18 @@ struct gs_plan {
 namespace {
 
 constexpr size_t kInfoBytes = 256;
+constexpr int KPB = 8;   // pipeline k-steps per block: 128 / 16 (real) = 64 / 8 (complex)
+static_assert(LB / BK == KPB && CLB / CBK == KPB && CT == CLB, "block / k-slab ratio");
 
 // Workspace layout: [info flag | 2 panel-inverse buffers Wp (ldw x ldw each) | one N x N matrix]
-int wp_ld(const gs_plan* p) { return LB * (p->nblk < p->potrf_nb ? p->nblk : p->potrf_nb); }
-size_t wp_bytes(const gs_plan* p) { return size_t(wp_ld(p)) * size_t(wp_ld(p)) * sizeof(double); }
+int wp_ld(const gs_plan* p) { return p->lb * (p->nblk < p->potrf_nb ? p->nblk : p->potrf_nb); }
+size_t wp_bytes(const gs_plan* p) { return size_t(wp_ld(p)) * size_t(wp_ld(p)) * p->es; }
 size_t big_offset(const gs_plan* p) { return kInfoBytes + ((2 * wp_bytes(p) + 255) / 256) * 256; }
-size_t workspace_bytes(const gs_plan* p) { return big_offset(p) + size_t(p->N) * size_t(p->N) * sizeof(double); }
+size_t workspace_bytes(const gs_plan* p) { return big_offset(p) + size_t(p->N) * size_t(p->N) * p->es; }
 
 int* info_ptr(const gs_plan* p) { return reinterpret_cast<int*>(p->ws); }
-double* wp_ptr(const gs_plan* p, int which) { return reinterpret_cast<double*>(p->ws + kInfoBytes + size_t(which & 1) * wp_bytes(p)); }
-double* big_ptr(const gs_plan* p) { return reinterpret_cast<double*>(p->ws + big_offset(p)); }
+void* wp_ptr(const gs_plan* p, int which) { return p->ws + kInfoBytes + size_t(which & 1) * wp_bytes(p); }
+void* big_ptr(const gs_plan* p) { return p->ws + big_offset(p); }
 
 gs_status_t cuda_fail(gs_plan* p, cudaError_t e)
 {
@@ -126,7 +133,15 @@ struct Stage {
     gs_plan* plan;
     cudaStream_t stream;
     bool tma;
+    bool z;       // complex128
+    int lb, bk;   // block order and k-slab in elements (plan->lb, plan->bk)
 };
+
+Stage make_stage(gs_plan* plan, cudaStream_t stream)
+{
+    // a real matrix with odd N has a row pitch that is not a multiple of 16 bytes: no tensor map
+    return Stage{plan, stream, plan->z || plan->N % 2 == 0, plan->z, plan->lb, plan->bk};
+}
 
 EngineParams blank_params(const gs_plan* plan)
 {
@@ -142,17 +157,18 @@ EngineParams blank_params(const gs_plan* plan)
 // which: 0 = A, 1 = B, 2 = A2, 3 = B2.  mcontig selects the 16 x 16 box of the m-contiguous A operand.
 bool set_operand(const Stage& st, EngineParams& p, int which, const MatView& m, bool mcontig)
 {
-    RawOperand r{m.ptr, m.ld, int(m.rows), int(m.cols)};
+    RawOperand r{static_cast<const double*>(m.ptr), m.ld, int(m.rows), int(m.cols)};
     CUtensorMap* map = which == 0 ? &p.mapA : which == 1 ? &p.mapB : which == 2 ? &p.mapA2 : &p.mapB2;
     (which == 0 ? p.rawA : which == 1 ? p.rawB : which == 2 ? p.rawA2 : p.rawB2) = r;
     if (!st.tma) return true;
-    return make_tensor_map(map, m, mcontig ? 16 : BN);
+    if (st.z) return make_tensor_map(map, m, mcontig ? 8 : CT, true);
+    return make_tensor_map(map, m, mcontig ? 16 : BN, false);
 }
 
 gs_status_t launch(Stage& st, const EngineParams& p, bool a_nn, int label)
 {
     LaunchTimer timer(st.plan, label, st.stream);
-    const cudaError_t e = engine_launch(p, a_nn, st.tma, st.stream);
+    const cudaError_t e = st.z ? cengine_launch(p, a_nn, st.stream) : engine_launch(p, a_nn, st.tma, st.stream);
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
     st.plan->launches += 1;
     return GS_OK;
@@ -167,19 +183,19 @@ gs_status_t launch(Stage& st, const EngineParams& p, bool a_nn, int label)
 gs_status_t check_ready(const gs_plan* plan)
 {
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
-    if (plan->dtype != GS_REAL64) return GS_ERR_INVALID_ARG;   // complex path: not built yet
     if (plan->ws == nullptr || plan->ws_bytes < workspace_bytes(plan)) return GS_ERR_WORKSPACE;
     return GS_OK;
 }
 
-gs_status_t zero_lower(Stage& st, double* X)
+gs_status_t zero_lower(Stage& st, void* X)
 {
     const gs_plan* plan = st.plan;
     const int N = int(plan->N);
-    if (N <= LB) return GS_OK;
+    if (N <= st.lb) return GS_OK;
     dim3 grid((N + 255) / 256, N);
     LaunchTimer timer(st.plan, L_ZERO_LOWER, st.stream);
-    zero_lower_blocks_kernel<<<grid, 256, 0, st.stream>>>(X, plan->N, N, info_ptr(plan));
+    if (st.z) zero_lower_blocks_kernel<double2, CLB><<<grid, 256, 0, st.stream>>>(static_cast<double2*>(X), plan->N, N, info_ptr(plan));
+    else zero_lower_blocks_kernel<double, LB><<<grid, 256, 0, st.stream>>>(static_cast<double*>(X), plan->N, N, info_ptr(plan));
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
     st.plan->launches += 1;
@@ -200,21 +216,21 @@ gs_status_t invert_levels(Stage& st, const MatView& vU, int uo, const MatView& v
                           int nb, int label_w, int label_x)
 {
     gs_plan* plan = st.plan;
-    double* V = const_cast<double*>(vV.ptr);
-    double* T = const_cast<double*>(vT.ptr);
+    double* V = static_cast<double*>(const_cast<void*>(vV.ptr));
+    double* T = static_cast<double*>(const_cast<void*>(vT.ptr));
     for (int s = 1; s < nb; s *= 2) {
         const int npairs = (nb - s + 2 * s - 1) / (2 * s);
-        const int stride = 2 * s * LB;   // elements between consecutive pairs
+        const int stride = 2 * s * st.lb;   // elements between consecutive pairs
         {   // W = B * Dinv
             EngineParams p = blank_params(plan);
             if (!set_operand(st, p, 0, vU, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
             p.C = T; p.ldc = vT.ld;
             p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_COL_REV;
-            p.c_row0 = to; p.c_col0 = to + s * LB; p.c_brow = stride; p.c_bcol = stride;
+            p.c_row0 = to; p.c_col0 = to + s * st.lb; p.c_brow = stride; p.c_bcol = stride;
             p.c_rows = int(vT.rows); p.c_cols = int(vT.cols);
-            p.khi_c = LB / BK; p.khi_j = LB / BK; p.kmax = s * (LB / BK);
-            p.a.x0 = uo; p.a.bx = stride; p.a.k0 = uo + s * LB; p.a.bk = stride;
-            p.b.k0 = vo + s * LB; p.b.bk = stride; p.b.x0 = vo + s * LB; p.b.bx = stride;
+            p.khi_c = KPB; p.khi_j = KPB; p.kmax = s * (KPB);
+            p.a.x0 = uo; p.a.bx = stride; p.a.k0 = uo + s * st.lb; p.a.bk = stride;
+            p.b.k0 = vo + s * st.lb; p.b.bk = stride; p.b.x0 = vo + s * st.lb; p.b.bx = stride;
             GS_TRY(launch(st, p, true, label_w));
         }
         {   // X = -Ainv * W
@@ -222,11 +238,11 @@ gs_status_t invert_levels(Stage& st, const MatView& vU, int uo, const MatView& v
             if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vT, false)) return GS_ERR_CUDA;
             p.C = V; p.ldc = vV.ld;
             p.tiles_m = s; p.tiles_n = s; p.batch = npairs; p.order = ORDER_ROW;
-            p.c_row0 = vo; p.c_col0 = vo + s * LB; p.c_brow = stride; p.c_bcol = stride;
+            p.c_row0 = vo; p.c_col0 = vo + s * st.lb; p.c_brow = stride; p.c_bcol = stride;
             p.c_rows = int(vV.rows); p.c_cols = int(vV.cols);
-            p.klo_i = LB / BK; p.khi_c = s * (LB / BK); p.kmax = s * (LB / BK);
+            p.klo_i = KPB; p.khi_c = s * (KPB); p.kmax = s * (KPB);
             p.a.x0 = vo; p.a.bx = stride; p.a.k0 = vo; p.a.bk = stride;
-            p.b.k0 = to; p.b.bk = stride; p.b.x0 = to + s * LB; p.b.bx = stride;
+            p.b.k0 = to; p.b.bk = stride; p.b.x0 = to + s * st.lb; p.b.bx = stride;
             p.alpha = -1.0;
             GS_TRY(launch(st, p, true, label_x));
         }
@@ -252,7 +268,7 @@ gs_status_t invert_levels(Stage& st, const MatView& vU, int uo, const MatView& v
 // ------------------------------------------------------------------------------------------------
 struct Potrf {
     Stage st;
-    double* S;
+    void* S;
     MatView vS;
     MatView vT;   // the N x N workspace matrix
     MatView vW;   // inverse of the current panel's diagonal block (ldw x ldw), diagonal 128-blocks first
@@ -262,8 +278,13 @@ struct Potrf {
     {
         gs_plan* plan = st.plan;
         LaunchTimer timer(plan, L_POTRF_LEAF, st.stream);
-        double* w = const_cast<double*>(vW.ptr) + size_t(b - pb) * LB * (vW.ld + 1);
-        potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(S, plan->N, int(plan->N), b * LB, w, vW.ld, info_ptr(plan));
+        void* w = static_cast<unsigned char*>(const_cast<void*>(vW.ptr)) + size_t(b - pb) * st.lb * (vW.ld + 1) * plan->es;
+        if (st.z)
+            potrf_cleaf_kernel<<<1, kCLeafThreads, kCLeafSmemBytes, st.stream>>>(static_cast<double2*>(S), plan->N, int(plan->N), b * st.lb,
+                                                                                 static_cast<double2*>(w), vW.ld, info_ptr(plan));
+        else
+            potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(static_cast<double*>(S), plan->N, int(plan->N), b * st.lb,
+                                                                              static_cast<double*>(w), vW.ld, info_ptr(plan));
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
@@ -275,12 +296,12 @@ struct Potrf {
     {
         EngineParams p = blank_params(st.plan);
         if (!set_operand(st, p, 0, vW, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
-        p.C = S; p.ldc = vS.ld;
+        p.C = static_cast<double*>(S); p.ldc = vS.ld;
         p.tiles_m = 1; p.tiles_n = c1 - c0; p.order = ORDER_COL;
-        p.c_row0 = r0 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
-        p.khi_c = LB / BK; p.kmax = LB / BK;
-        p.a.k0 = (r0 - pb) * LB; p.a.x0 = (r0 - pb) * LB;
-        p.b.k0 = r0 * LB; p.b.x0 = c0 * LB;
+        p.c_row0 = r0 * st.lb; p.c_col0 = c0 * st.lb; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = KPB; p.kmax = KPB;
+        p.a.k0 = (r0 - pb) * st.lb; p.a.x0 = (r0 - pb) * st.lb;
+        p.b.k0 = r0 * st.lb; p.b.x0 = c0 * st.lb;
         return launch(st, p, false, L_POTRF_TRSM);
     }
 
@@ -289,12 +310,12 @@ struct Potrf {
     {
         EngineParams p = blank_params(st.plan);
         if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
-        p.C = S; p.ldc = vS.ld;
+        p.C = static_cast<double*>(S); p.ldc = vS.ld;
         p.tiles_m = r1 - h; p.tiles_n = c1 - c0; p.order = ORDER_COL;
-        p.c_row0 = h * LB; p.c_col0 = c0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
-        p.khi_c = (h - r0) * (LB / BK); p.kmax = p.khi_c;
-        p.a.k0 = r0 * LB; p.a.x0 = h * LB;
-        p.b.k0 = r0 * LB; p.b.x0 = c0 * LB;
+        p.c_row0 = h * st.lb; p.c_col0 = c0 * st.lb; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = (h - r0) * (KPB); p.kmax = p.khi_c;
+        p.a.k0 = r0 * st.lb; p.a.x0 = h * st.lb;
+        p.b.k0 = r0 * st.lb; p.b.x0 = c0 * st.lb;
         p.alpha = -1.0; p.beta = 1.0;
         return launch(st, p, false, L_POTRF_GEMM);
     }
@@ -314,14 +335,14 @@ struct Potrf {
     {
         EngineParams p = blank_params(st.plan);
         if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
-        p.C = S; p.ldc = vS.ld;
+        p.C = static_cast<double*>(S); p.ldc = vS.ld;
         p.tiles_m = c1 - c0; p.tiles_n = c1 - c0; p.order = ORDER_TRI_ROW_DESC;
-        p.c_row0 = c0 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
-        p.khi_c = (k1 - k0) * (LB / BK); p.kmax = p.khi_c;
-        p.a.k0 = k0 * LB; p.a.x0 = c0 * LB;
-        p.b.k0 = k0 * LB; p.b.x0 = c0 * LB;
+        p.c_row0 = c0 * st.lb; p.c_col0 = c0 * st.lb; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = (k1 - k0) * (KPB); p.kmax = p.khi_c;
+        p.a.k0 = k0 * st.lb; p.a.x0 = c0 * st.lb;
+        p.b.k0 = k0 * st.lb; p.b.x0 = c0 * st.lb;
         p.alpha = -1.0; p.beta = 1.0;
-        p.flags = F_STORE_UPPER;
+        p.flags = F_STORE_UPPER | F_REAL_DIAG;   // HERK: the diagonal of U^H U is real
         return launch(st, p, false, L_POTRF_SYRK);
     }
 
@@ -341,7 +362,7 @@ struct Potrf {
     {
         pb = b1;
         GS_TRY(potrf(b1, b2));
-        if (b2 < n) GS_TRY(invert_levels(st, vS, b1 * LB, vW, 0, vT, b1 * LB, b2 - b1, L_POTRF_GEMM, L_POTRF_GEMM));
+        if (b2 < n) GS_TRY(invert_levels(st, vS, b1 * st.lb, vW, 0, vT, b1 * st.lb, b2 - b1, L_POTRF_GEMM, L_POTRF_GEMM));
         return GS_OK;
     }
 
@@ -352,19 +373,24 @@ struct Potrf {
         gs_plan* plan = st.plan;
         EngineParams p = blank_params(plan);
         if (!set_operand(st, p, 0, W, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
-        p.C = const_cast<double*>(vT.ptr); p.ldc = vT.ld;
+        p.C = static_cast<double*>(const_cast<void*>(vT.ptr)); p.ldc = vT.ld;
         p.tiles_m = b2 - b1; p.tiles_n = c1 - c0; p.order = ORDER_ROW_REV;
-        p.c_row0 = b1 * LB; p.c_col0 = c0 * LB; p.c_rows = int(vT.rows); p.c_cols = int(vT.cols);
-        p.khi_c = LB / BK; p.khi_i = LB / BK; p.kmax = (b2 - b1) * (LB / BK);
+        p.c_row0 = b1 * st.lb; p.c_col0 = c0 * st.lb; p.c_rows = int(vT.rows); p.c_cols = int(vT.cols);
+        p.khi_c = KPB; p.khi_i = KPB; p.kmax = (b2 - b1) * (KPB);
         p.a.k0 = 0; p.a.x0 = 0;
-        p.b.k0 = b1 * LB; p.b.x0 = c0 * LB;
+        p.b.k0 = b1 * st.lb; p.b.x0 = c0 * st.lb;
         GS_TRY(launch(st, p, false, L_POTRF_TRSM));
         const int N = int(plan->N);
-        const int rows = (b2 * LB < N ? b2 * LB : N) - b1 * LB;
-        const int cols = (c1 * LB < N ? c1 * LB : N) - c0 * LB;
+        const int rows = (b2 * st.lb < N ? b2 * st.lb : N) - b1 * st.lb;
+        const int cols = (c1 * st.lb < N ? c1 * st.lb : N) - c0 * st.lb;
         dim3 grid((rows + 255) / 256, cols);
         LaunchTimer timer(plan, L_POTRF_TRSM, st.stream);
-        copy_block_kernel<<<grid, 256, 0, st.stream>>>(vT.ptr, S, plan->N, b1 * LB, rows, c0 * LB, info_ptr(plan));
+        if (st.z)
+            copy_block_kernel<double2><<<grid, 256, 0, st.stream>>>(static_cast<const double2*>(vT.ptr), static_cast<double2*>(S), plan->N,
+                                                                    b1 * st.lb, rows, c0 * st.lb, info_ptr(plan));
+        else
+            copy_block_kernel<double><<<grid, 256, 0, st.stream>>>(static_cast<const double*>(vT.ptr), static_cast<double*>(S), plan->N,
+                                                                   b1 * st.lb, rows, c0 * st.lb, info_ptr(plan));
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
@@ -458,6 +484,8 @@ gs_status_t configure_leaf(gs_plan* plan)
     if (done) return GS_OK;
     GS_CUDA(plan, cudaFuncSetAttribute(potrf_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
     GS_CUDA(plan, cudaFuncSetAttribute(trtri_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
+    GS_CUDA(plan, cudaFuncSetAttribute(potrf_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
+    GS_CUDA(plan, cudaFuncSetAttribute(trtri_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
     done = true;
     return GS_OK;
 }
@@ -482,7 +510,11 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     p->N = N;
     p->nev = nev;
     p->dtype = dtype;
-    p->nblk = int((N + LB - 1) / LB);
+    p->z = dtype == GS_COMPLEX128;
+    p->lb = p->z ? CLB : LB;
+    p->bk = p->z ? CBK : BK;
+    p->es = p->z ? 2 * sizeof(double) : sizeof(double);
+    p->nblk = int((N + p->lb - 1) / p->lb);
     // tuning knobs of the POTRF schedule
     auto knob = [](const char* name, int lo, int hi, int* out) {
         if (const char* e = std::getenv(name)) {
@@ -490,7 +522,7 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
             if (v >= lo && v <= hi) *out = v;
         }
     };
-    knob("GS_POTRF_NB", 1, 32, &p->potrf_nb);
+    knob("GS_POTRF_NB", 1, 256, &p->potrf_nb);
     knob("GS_POTRF_NB_TAIL", 1, 32, &p->potrf_nb_tail);
     knob("GS_POTRF_TAIL", 0, 1 << 20, &p->potrf_tail);
     if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
@@ -537,9 +569,9 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     GS_TRY(configure_leaf(plan));
     GS_CUDA(plan, cudaMemsetAsync(info_ptr(plan), 0, sizeof(int), stream));
-    double* S = static_cast<double*>(S_inout);
+    void* S = S_inout;
     Potrf f;
-    f.st = Stage{plan, stream, plan->N % 2 == 0};
+    f.st = make_stage(plan, stream);
     f.S = S;
     f.vS = MatView{S, plan->N, plan->N, plan->N};
     f.vT = MatView{big_ptr(plan), plan->N, plan->N, plan->N};
@@ -556,14 +588,19 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
     if (U_ == nullptr || Uinv_ == nullptr || U_ == Uinv_ || !aligned16(U_) || !aligned16(Uinv_)) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     GS_TRY(configure_leaf(plan));
-    const double* U = static_cast<const double*>(U_);
-    double* V = static_cast<double*>(Uinv_);
+    const void* U = U_;
+    void* V = Uinv_;
     const int N = int(plan->N), nblk = plan->nblk;
-    Stage st{plan, stream, plan->N % 2 == 0};
+    Stage st = make_stage(plan, stream);
 
     {
         LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
-        trtri_leaf_kernel<<<nblk, kLeafThreads, kLeafSmemBytes, stream>>>(U, V, plan->N, N, info_ptr(plan));
+        if (plan->z)
+            trtri_cleaf_kernel<<<nblk, kCLeafThreads, kCLeafSmemBytes, stream>>>(static_cast<const double2*>(U), static_cast<double2*>(V),
+                                                                                 plan->N, N, info_ptr(plan));
+        else
+            trtri_leaf_kernel<<<nblk, kLeafThreads, kLeafSmemBytes, stream>>>(static_cast<const double*>(U), static_cast<double*>(V),
+                                                                              plan->N, N, info_ptr(plan));
     }
     GS_CUDA(plan, cudaGetLastError());
     plan->launches += 1;
@@ -585,17 +622,17 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const int N = int(plan->N), nblk = plan->nblk;
-    Stage st{plan, stream, plan->N % 2 == 0};
-    double* G = big_ptr(plan);
-    const MatView vH{static_cast<const double*>(H_), N, N, N}, vV{static_cast<const double*>(Uinv_), N, N, N}, vG{G, N, N, N};
-    const int kt = LB / BK;
+    Stage st = make_stage(plan, stream);
+    void* G = big_ptr(plan);
+    const MatView vH{H_, N, N, N}, vV{Uinv_, N, N, N}, vG{G, N, N, N};
+    const int kt = KPB;
     {
         EngineParams p = blank_params(plan);
         if (!set_operand(st, p, 0, vH, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
-        p.C = G; p.ldc = N;
+        p.C = static_cast<double*>(G); p.ldc = N;
         p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_DIAG_DESC;
         p.c_rows = N; p.c_cols = N;
-        p.klo_i = kt; p.khi_c = kt; p.khi_j = kt; p.kmax = (N + BK - 1) / BK;
+        p.klo_i = kt; p.khi_c = kt; p.khi_j = kt; p.kmax = (N + st.bk - 1) / st.bk;
         p.flags = F_MASK_A | F_HALF_DIAG_A | F_MASK_B;
         GS_TRY(launch(st, p, true, L_TOSTD_G));
     }
@@ -607,8 +644,8 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         p.C = static_cast<double*>(Htilde_); p.ldc = N;
         p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_ROW_DESC;
         p.c_rows = N; p.c_cols = N;
-        p.khi_c = kt; p.khi_i = kt; p.kmax = (N + BK - 1) / BK;
-        p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER;
+        p.khi_c = kt; p.khi_i = kt; p.kmax = (N + st.bk - 1) / st.bk;
+        p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;   // Hermitian: Im(diag) = 0 exactly
         GS_TRY(launch(st, p, false, L_TOSTD_SYR2K));
     }
     return GS_OK;
@@ -623,14 +660,14 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
         return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const int N = int(plan->N), nev = int(plan->nev);
-    Stage st{plan, stream, plan->N % 2 == 0};
-    const MatView vV{static_cast<const double*>(Uinv_), N, N, N}, vC{static_cast<const double*>(Ctilde_), N, nev, N};
+    Stage st = make_stage(plan, stream);
+    const MatView vV{Uinv_, N, N, N}, vC{Ctilde_, N, nev, N};
     EngineParams p = blank_params(plan);
     if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
     p.C = static_cast<double*>(C_); p.ldc = N;
-    p.tiles_m = plan->nblk; p.tiles_n = (nev + BN - 1) / BN; p.order = ORDER_ROW;
+    p.tiles_m = plan->nblk; p.tiles_n = (nev + st.lb - 1) / st.lb; p.order = ORDER_ROW;
     p.c_rows = N; p.c_cols = nev;
-    p.klo_i = LB / BK; p.khi_c = (N + BK - 1) / BK; p.kmax = p.khi_c;
+    p.klo_i = KPB; p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
     p.flags = F_MASK_A;
     return launch(st, p, true, L_BACK_TRMM);
 }
@@ -652,7 +689,7 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)
 gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes)
 {
     if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
-    const size_t mat = ((size_t(plan->N) * size_t(plan->N) * sizeof(double) + 255) / 256) * 256;
+    const size_t mat = ((size_t(plan->N) * size_t(plan->N) * plan->es + 255) / 256) * 256;
     *bytes = 4 * mat;   // S->U, H (later C~ and C), Uinv, Htilde
     return GS_OK;
 }
@@ -667,7 +704,7 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
         (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
         return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    const size_t bytes = size_t(plan->N) * size_t(plan->N) * sizeof(double);
+    const size_t bytes = size_t(plan->N) * size_t(plan->N) * plan->es;
     const size_t mat = need / 4;
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
     void *dS = base, *dH = base + mat, *dV = base + 2 * mat, *dHt = base + 3 * mat;
@@ -696,7 +733,7 @@ gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void
     if (host_Ctilde == nullptr || host_C == nullptr) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const size_t mat = need / 4;
-    const size_t cbytes = size_t(plan->N) * size_t(plan->nev) * sizeof(double);
+    const size_t cbytes = size_t(plan->N) * size_t(plan->nev) * plan->es;
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
     // U^-1 was left at base + 2*mat by gs_reduce_host; C~ and C reuse the S and H slots
     void *dV = base + 2 * mat, *dCt = base, *dC = base + mat;

@@ -226,17 +226,19 @@ trtri_leaf_kernel(const double* __restrict__ U, double* __restrict__ V, long lon
 // Zero the strictly-lower part of an N x N column-major matrix outside its 128 x 128 diagonal
 // blocks (those are written whole by the leaf kernels): the "strictly-lower part is zero" contract
 // of U and U^-1 (include/gs.h).
-__global__ void zero_lower_blocks_kernel(double* __restrict__ X, long long ld, int N, const int* info)
+template <typename T, int kLB>
+__global__ void zero_lower_blocks_kernel(T* __restrict__ X, long long ld, int N, const int* info)
 {
     if (*info != 0) return;
     const int col = blockIdx.y;
-    const int first = (col / LB + 1) * LB;   // first row below the diagonal block of this column
+    const int first = (col / kLB + 1) * kLB;   // first row below the diagonal block of this column
     const int row = first + blockIdx.x * blockDim.x + threadIdx.x;
-    if (row < N) X[row + (long long)col * ld] = 0.0;
+    if (row < N) X[row + (long long)col * ld] = T{};
 }
 
 // dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid row (blockIdx.y) per column c.
-__global__ void copy_block_kernel(const double* __restrict__ src, double* __restrict__ dst, long long ld, int row0, int rows,
+template <typename T>
+__global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst, long long ld, int row0, int rows,
                                   int col0, const int* info)
 {
     if (*info != 0) return;

@@ -76,6 +76,21 @@ __device__ __forceinline__ void dmma_8x8x4(double& d0, double& d1, double a, dou
         : "d"(a), "d"(b));
 }
 
+// Consumer release of pipeline stage s-1, performed at the top of iteration s (after the wait on
+// stage s).  It must NOT sit right behind the last fragment loads of the stage it releases: an
+// mbarrier arrive is not held back by LDS instructions that are still in flight (SASS: the last
+// LDS.128 was issued three instructions before SYNCS.ARRIVE, its DMMAs after it), so the producer's
+// next TMA fill could overwrite the stage under a pending load -- seen as sporadic wrong tiles with
+// two CTAs per SM.  One iteration later every DMMA that consumed those loads has been issued
+// (they precede the spin-wait in program order), i.e. the loads have returned.
+__device__ __forceinline__ void release_previous_stage(int s, int nstages, uint32_t empty0, int lane)
+{
+    if (s > 0) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * ((s - 1) % nstages));
+    }
+}
+
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
     double2 v;

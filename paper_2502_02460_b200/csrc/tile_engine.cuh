@@ -47,6 +47,7 @@ enum : uint32_t {
     F_MASK_A2 = 1u << 4,
     F_MASK_B2 = 1u << 5,
     F_STORE_UPPER = 1u << 6,   // store only C elements with global row <= col
+    F_REAL_DIAG = 1u << 7,     // complex engine: store Im = 0 on the global diagonal (Hermitian results)
 };
 
 // tile enumeration orders (heaviest tiles first so the tail of the grid is made of short tiles)
@@ -349,6 +350,7 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
         const int stage = s % kStages;
         const uint32_t ph = (s / kStages) & 1;
         mbar_wait(full0 + 8 * stage, ph);
+        release_previous_stage(s, kStages, empty0, lane);
         unsigned char* st = smem + stage * kStageBytes;
 
         if (mask_any) {
@@ -411,8 +413,6 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
                             dmma_8x8x4(acc[mg][half * 4 + ng][0], acc[mg][half * 4 + ng][1], af[mg][kk], bf[ng][kk]);
             }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty0 + 8 * stage);
     }
 
     // ===================== epilogue: C = alpha * acc (predicated, direct to global) =====================

@@ -242,11 +242,12 @@ def generalized_to_standard(H: torch.Tensor, S: torch.Tensor, nev: int | None = 
     """Convenience: run steps 1-3 on fresh buffers.  Returns (plan, U, Uinv, Htilde); S is not modified."""
     from .workloads import colmajor_empty, colmajor_zeros
     N = H.shape[0]
-    plan = Plan(N, nev)
-    U = colmajor_empty(N, N, device=H.device)
+    cplx = H.dtype == torch.complex128
+    plan = Plan(N, nev, dtype=GS_COMPLEX128 if cplx else GS_REAL64)
+    U = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
     U.copy_(S)
-    Uinv = colmajor_empty(N, N, device=H.device)
-    Ht = colmajor_zeros(N, N, device=H.device)
+    Uinv = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
+    Ht = colmajor_zeros(N, N, dtype=H.dtype, device=H.device)
     plan.cholesky(U)
     plan.invert_triangular(U, Uinv)
     plan.to_standard(H, Uinv, Ht)
