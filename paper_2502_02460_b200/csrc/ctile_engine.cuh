@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid
     const int lane = threadIdx.x & 31;
 
     int b, I, J;
-    decode_tile(p, blockIdx.x, b, I, J);
+    if (!decode_tile(p, blockIdx.x, b, I, J)) return;
     int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
     int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
     if (k_lo < 0) k_lo = 0;

@@ -59,7 +59,11 @@ inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols, bo
 inline int num_tiles(const EngineParams& p)
 {
     int per = p.tiles_m * p.tiles_n;
-    if (p.order == ORDER_TRI_ROW_DESC || p.order == ORDER_TRI_DIAG_DESC) per = p.tiles_n * (p.tiles_n + 1) / 2;
+    if (p.order == ORDER_TRI_ROW_DESC || p.order == ORDER_TRI_DIAG_DESC) {
+        const int G = p.super > 1 ? p.super : 1;
+        const int ns = (p.tiles_n + G - 1) / G;
+        per = ns * (ns + 1) / 2 * G * G;     // padded: CTAs outside the triangle exit at once
+    }
     else if (p.order == ORDER_TRAPEZOID) per = p.tiles_m * p.tiles_n - p.tiles_m * (p.tiles_m - 1) / 2;
     return per * p.batch;
 }

@@ -60,6 +60,7 @@ struct gs_plan {
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
     int potrf_tail = 64;
+    int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
 };
 
@@ -151,6 +152,7 @@ EngineParams blank_params(const gs_plan* plan)
     p.alpha = 1.0;
     p.beta = 0.0;
     p.info = info_ptr(plan);
+    p.super = plan->super_tile;
     return p;
 }
 
@@ -526,6 +528,8 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_POTRF_NB_TAIL", 1, 32, &p->potrf_nb_tail);
     knob("GS_POTRF_TAIL", 0, 1 << 20, &p->potrf_tail);
     if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
+    p->super_tile = p->z ? 16 : 12;
+    knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
     *plan = p;
     return GS_OK;
 }

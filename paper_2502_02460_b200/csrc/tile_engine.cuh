@@ -81,6 +81,7 @@ struct EngineParams {
     long long ldc;
     const int* info;              // device flag: non-zero => the whole launch is a no-op
     int tiles_m, tiles_n, batch, order;
+    int super;                    // triangular orders: edge (in tiles) of the square super-tiles the grid is rasterised in (<= 1: off)
     int c_row0, c_col0, c_brow, c_bcol;   // C tile (b,I,J) starts at (c_row0 + b*c_brow + BM*I, c_col0 + b*c_bcol + BN*J)
     int c_rows, c_cols;                   // stores are predicated on row < c_rows && col < c_cols
     int klo_c, klo_i, klo_j;              // k_lo = klo_c + klo_i*I + klo_j*J   (units of BK), clamped to >= 0
@@ -91,7 +92,8 @@ struct EngineParams {
     double alpha, beta;
 };
 
-__device__ __forceinline__ void decode_tile(const EngineParams& p, int id, int& b, int& I, int& J)
+// Returns false for the padding CTAs of a super-tiled triangular grid (they exit at once).
+__device__ __forceinline__ bool decode_tile(const EngineParams& p, int id, int& b, int& I, int& J)
 {
     const int tm = p.tiles_m, tn = p.tiles_n;
     switch (p.order) {
@@ -123,18 +125,30 @@ __device__ __forceinline__ void decode_tile(const EngineParams& p, int id, int& 
             J = I + r;
         } break;
         default: {
-            // triangular enumerations over an n x n tile grid (n = tiles_n = tiles_m): group u has u+1 tiles
+            // triangular enumerations over an n x n tile grid (n = tiles_n = tiles_m): group u has u+1 members.
+            // With super-tiles the members are G x G squares of tiles: the ~1 wave of CTAs resident at a
+            // time then shares 2G operand panels instead of G*G + 1, which is what keeps the operand
+            // traffic in L2 (profiles/: DRAM bytes per launch).  Heavy tiles still come first.
+            const int G = p.super > 1 ? p.super : 1;
             const int n = tn;
-            const int per = n * (n + 1) / 2;
-            b = id / per; const int r = id - b * per;
+            const int ns = (n + G - 1) / G;
+            const int per = ns * (ns + 1) / 2 * G * G;
+            b = id / per; const int r0 = id - b * per;
+            const int r = r0 / (G * G), t = r0 - r * (G * G);
             int u = static_cast<int>((sqrtf(8.0f * r + 1.0f) - 1.0f) * 0.5f);
             while ((u + 1) * (u + 2) / 2 <= r) ++u;
             while (u * (u + 1) / 2 > r) --u;
             const int v = r - u * (u + 1) / 2;   // 0..u
-            if (p.order == ORDER_TRI_ROW_DESC) { I = n - 1 - u; J = I + v; }
-            else { const int d = n - 1 - u; I = v; J = v + d; }
+            int SI, SJ;
+            if (p.order == ORDER_TRI_ROW_DESC) { SI = ns - 1 - u; SJ = SI + v; }
+            else { const int d = ns - 1 - u; SI = v; SJ = v + d; }
+            const int ti = t / G, tj = t - ti * G;
+            I = SI * G + (p.order == ORDER_TRI_ROW_DESC ? G - 1 - ti : ti);
+            J = SJ * G + (p.order == ORDER_TRI_ROW_DESC ? tj : G - 1 - tj);
+            if (I > J || J >= n || I >= n) return false;
         } break;
     }
+    return true;
 }
 
 // Zero / halve the part of an operand tile that lies below / on the global diagonal.
@@ -211,7 +225,7 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
     const int lane = threadIdx.x & 31;
 
     int b, I, J;
-    decode_tile(p, blockIdx.x, b, I, J);
+    if (!decode_tile(p, blockIdx.x, b, I, J)) return;
     int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
     int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
     if (k_lo < 0) k_lo = 0;
