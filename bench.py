@@ -324,6 +324,24 @@ def run_ours(args):
                   "hbm_gbs_measured": mp.get("hbm_gbs")},
     }
 
+    # NEXT-1 (outside the metric): the density matrix P = sum_l f_l c*_l c_l over the nev columns of C
+    # (PAPER.md:77), a weighted SYRK / HERK on the same tile engine; nominal N^2 nev flop (one triangle)
+    focc = torch.full((nev,), 2.0, dtype=torch.float64, device=dev)
+    plan.density_matrix(C, focc, Ht)
+    ev_d = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev_d[0].record()
+    for _ in range(3):
+        plan.density_matrix(C, focc, Ht)
+    ev_d[1].record()
+    plan.last_info()
+    dens_ms = ev_d[0].elapsed_time(ev_d[1]) / 3.0
+    dens_flop = (4.0 if cplx else 1.0) * float(N) ** 2 * nev
+    next_stages = {"density_matrix": {"ms": round(dens_ms, 3), "tflops": dens_flop / (dens_ms * 1e-3) / 1e12,
+                                      "frac_of_fp64_peak": dens_flop / (dens_ms * 1e-3) / 1e12 / fp64_peak,
+                                      "nominal_flop": dens_flop}}
+    plan.to_standard(H, V, Ht)            # restore H~ for the checks below
+    plan.last_info()
+
     stages = {}
     for name, ms in zip(STAGES, stage_ms):
         stages[name] = {"ms": round(ms, 3), "tflops": flops[name] / (ms * 1e-3) / 1e12,
@@ -410,7 +428,7 @@ def run_ours(args):
                        "cache": "inputs_larger_than_L2 (each matrix %.1f GiB vs 126 MB L2)" % (N * N * (16 if cplx else 8) / 2 ** 30),
                        "timing": "CUDA events per step on the launching stream; S restored between steps outside the events"},
             "frac_of_fp64_peak": value / world / fp64_peak, "fp64_peak_tflops": fp64_peak,
-            "stages": stages, "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e,
+            "stages": stages, "next_stages": next_stages, "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks, "checks": checks,
             "wall_s_timed_region": wall1 - wall0,
             "paper_context": "PAPER.md:133 Table 1 (ELPA 2024.05, NCCL, 4x A100-40GB, N=40960, nev=N): Cholesky 2.3 s, "

@@ -98,6 +98,16 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H, const void* Uinv, voi
 gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C,
                              void* cuda_stream);
 
+/* Density matrix (the step that follows the path; "single-particle density matrix
+ * P_ij = sum_l f_l c*_li c_lj", with c_li = C(i,l), eigenvectors stored as columns):
+ *     P(i,j) = sum_{l < nev} f[l] * conj(C(i,l)) * C(j,l).
+ * C is N x nev (ld N); f is a DEVICE array of nev real occupation numbers, f[l] >= 0 (a negative
+ * occupation gives NaN); P is N x N (ld N): the UPPER triangle (incl. the diagonal, exactly real for
+ * GS_COMPLEX128) is written, the strictly-lower part is left untouched.  nev == 0 writes zeros.
+ * One weighted SYRK / HERK on the tensor-core tile engine over sqrt(f)-scaled, transposed C (held
+ * in the plan's workspace). */
+gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C, const double* f, void* P, void* cuda_stream);
+
 /* Synchronises `cuda_stream`, then reports the plan's numerical status: GS_OK with *info = 0, or
  * GS_ERR_NOT_POSDEF / GS_ERR_SINGULAR with *info = 1-based index of the first bad pivot
  * (LAPACK-style).  GS_ERR_CUDA if the stream reports an asynchronous error. */

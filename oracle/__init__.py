@@ -45,6 +45,8 @@ def _load():
             getattr(lib, f"orc_backtransform_{t}").restype = None
             getattr(lib, f"orc_jacobi_{t}").argtypes = [i64, p, p, p]
             getattr(lib, f"orc_jacobi_{t}").restype = i64
+            getattr(lib, f"orc_density_{t}").argtypes = [i64, i64, p, p, p]
+            getattr(lib, f"orc_density_{t}").restype = None
         lib.orc_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -119,6 +121,17 @@ def backtransform(V, Ct) -> np.ndarray:
     if nev > 0:
         getattr(_load(), f"orc_backtransform_{_sfx(V)}")(N, nev, _ptr(V), _ptr(Ct), _ptr(C))
     return C
+
+
+def density_matrix(C, f) -> np.ndarray:
+    """O7: P_ij = sum_l f_l conj(C_il) C_jl, FULL matrix."""
+    C = _f(C)
+    N, nev = C.shape
+    f = np.ascontiguousarray(np.asarray(f, dtype=np.float64))
+    assert f.shape == (nev,)
+    P = np.zeros((N, N), dtype=C.dtype, order="F")
+    getattr(_load(), f"orc_density_{_sfx(C)}")(N, nev, _ptr(C), f.ctypes.data_as(ctypes.c_void_p), _ptr(P))
+    return P
 
 
 def jacobi(A):

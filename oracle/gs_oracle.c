@@ -31,7 +31,9 @@
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): diagonal pencil closed form, S = I, the
  * tridiag(-1,2,-1) closed forms for U, U^-1, H~ and eps, 2x2 quadratic, Sturm/inertia brute force
- * at tiny N, planted factor, complex = real (x) phase identity, scipy/LAPACK cross-checks.
+ * at tiny N, planted factor, complex = real (x) phase identity, scipy/LAPACK cross-checks; the density
+ * matrix (O7): hand-computed case fixing the conjugate, electron count sum_ij P_ij S_ij = sum_l f_l,
+ * projector identity, numpy einsum (tests/test_oracle_density.py).
  * No function here is "parity unpinned".
  */
 #include <complex.h>
@@ -380,4 +382,31 @@ int orc_num_threads(void)
 #else
     return 1;
 #endif
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O7 (NEXT-1, off the four-step path). Single-particle density matrix:            */
+/*   P_ij = sum_l f_l c*_li c_lj,   c_li = C(i,l) (eigenvectors stored as columns)  */
+/* Plain triple loop over all i, j (both triangles computed independently).                     */
+/* ------------------------------------------------------------------------------------------ */
+void orc_density_d(int64_t N, int64_t nev, const double *C, const double *f, double *P)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < N; ++i) {
+            double s = 0.0;
+            for (int64_t l = 0; l < nev; ++l) s += f[l] * AT(C, i, l) * AT(C, j, l);
+            AT(P, i, j) = s;
+        }
+}
+
+void orc_density_z(int64_t N, int64_t nev, const zdouble *C, const double *f, zdouble *P)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < N; ++i) {
+            zdouble s = 0.0;
+            for (int64_t l = 0; l < nev; ++l) s += f[l] * conj(AT(C, i, l)) * AT(C, j, l);
+            AT(P, i, j) = s;
+        }
 }

@@ -27,11 +27,12 @@ using namespace gs;
 // launch labels for the optional per-launch timing (gs_plan_set_timing)
 enum LaunchLabel : int {
     L_POTRF_LEAF = 0, L_POTRF_TRSM, L_POTRF_GEMM, L_POTRF_SYRK, L_ZERO_LOWER,
-    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_COUNT
+    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_DENS_T, L_DENS_SYRK, L_COUNT
 };
 static const char* const kLabelNames[L_COUNT] = {
     "potrf.leaf", "potrf.trsm_leaf", "potrf.gemm", "potrf.syrk", "zero_lower",
-    "trtri.leaf", "trtri.w", "trtri.x", "to_standard.g", "to_standard.syr2k", "backtransform.trmm"};
+    "trtri.leaf", "trtri.w", "trtri.x", "to_standard.g", "to_standard.syr2k", "backtransform.trmm",
+    "density.transpose", "density.syrk"};
 
 struct TimedLaunch {
     int label;
@@ -74,7 +75,8 @@ static_assert(LB / BK == KPB && CLB / CBK == KPB && CT == CLB, "block / k-slab r
 int wp_ld(const gs_plan* p) { return p->lb * (p->nblk < p->potrf_nb ? p->nblk : p->potrf_nb); }
 size_t wp_bytes(const gs_plan* p) { return size_t(wp_ld(p)) * size_t(wp_ld(p)) * p->es; }
 size_t big_offset(const gs_plan* p) { return kInfoBytes + ((2 * wp_bytes(p) + 255) / 256) * 256; }
-size_t workspace_bytes(const gs_plan* p) { return big_offset(p) + size_t(p->N) * size_t(p->N) * p->es; }
+// (+ 2 columns: gs_density_matrix pads the pitch of the transposed eigenvector block to an even value)
+size_t workspace_bytes(const gs_plan* p) { return big_offset(p) + size_t(p->N) * size_t(p->N + 2) * p->es; }
 
 int* info_ptr(const gs_plan* p) { return reinterpret_cast<int*>(p->ws); }
 void* wp_ptr(const gs_plan* p, int which) { return p->ws + kInfoBytes + size_t(which & 1) * wp_bytes(p); }
@@ -674,6 +676,43 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
     p.klo_i = KPB; p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
     p.flags = F_MASK_A;
     return launch(st, p, true, L_BACK_TRMM);
+}
+
+// P(i,j) = sum_l f_l conj(C(i,l)) C(j,l) = (X^H X)(i,j) with X(l,i) = sqrt(f_l) C(i,l): one transpose-and-scale
+// pass into the workspace, then a SYRK / HERK of k-extent nev on the tile engine (upper tiles only).
+gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C_, const double* f, void* P_, void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (P_ == nullptr || !aligned16(P_)) return GS_ERR_INVALID_ARG;
+    const int N = int(plan->N), nev = int(plan->nev);
+    if (nev > 0 && (C_ == nullptr || f == nullptr || C_ == P_ || !aligned16(C_))) return GS_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Stage st = make_stage(plan, stream);
+    void* X = big_ptr(plan);
+    const long long ldx = nev == 0 ? 2 : (plan->z ? nev : ((nev + 1) & ~1LL));   // real: even pitch so that TMA applies
+    if (nev > 0) {
+        dim3 grid((N + 31) / 32, (nev + 31) / 32), block(32, 8);
+        LaunchTimer timer(plan, L_DENS_T, stream);
+        if (plan->z)
+            transpose_scale_kernel<double2><<<grid, block, 0, stream>>>(static_cast<const double2*>(C_), plan->N, f,
+                                                                       static_cast<double2*>(X), ldx, N, nev, info_ptr(plan));
+        else
+            transpose_scale_kernel<double><<<grid, block, 0, stream>>>(static_cast<const double*>(C_), plan->N, f,
+                                                                     static_cast<double*>(X), ldx, N, nev, info_ptr(plan));
+        GS_CUDA(plan, cudaGetLastError());
+        plan->launches += 1;
+    }
+    // nev == 0: an empty k-range stores zeros; the operand view only has to be a valid tensor
+    const MatView vX{X, nev > 0 ? nev : 1, N, ldx};
+    st.tma = true;   // X has a 16-byte-multiple pitch by construction, also for odd N
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vX, false) || !set_operand(st, p, 1, vX, false)) return GS_ERR_CUDA;
+    p.C = static_cast<double*>(P_); p.ldc = N;
+    p.tiles_m = plan->nblk; p.tiles_n = plan->nblk; p.order = ORDER_TRI_ROW_DESC;
+    p.c_rows = N; p.c_cols = N;
+    p.khi_c = (nev + st.bk - 1) / st.bk; p.kmax = p.khi_c;
+    p.flags = F_STORE_UPPER | F_REAL_DIAG;
+    return launch(st, p, false, L_DENS_SYRK);
 }
 
 gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)

@@ -249,4 +249,30 @@ __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst
     }
 }
 
+// X[l + i * ldx] = sqrt(f[l]) * C[i + l * ldc]  for i < N, l < nev: the occupation-weighted, transposed
+// eigenvector block of gs_density_matrix (P_ij = sum_l f_l c*_li c_lj).  32 x 32 tiles
+// through shared memory so that both the read (along i) and the write (along l) are coalesced.
+template <typename T>
+__global__ void transpose_scale_kernel(const T* __restrict__ C, long long ldc, const double* __restrict__ f, T* __restrict__ X,
+                                       long long ldx, int N, int nev, const int* info)
+{
+    if (*info != 0) return;
+    __shared__ T tile[32][33];
+    const int i0 = blockIdx.x * 32, l0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int i = i0 + threadIdx.x, l = l0 + r;
+        if (i < N && l < nev) tile[r][threadIdx.x] = C[i + (long long)l * ldc];
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int l = l0 + threadIdx.x, i = i0 + r;
+        if (i < N && l < nev) {
+            const double w = sqrt(f[l]);
+            T v = tile[threadIdx.x][r];
+            if constexpr (sizeof(T) == 16) { v.x *= w; v.y *= w; } else { v *= w; }
+            X[l + (long long)i * ldx] = v;
+        }
+    }
+}
+
 }  // namespace gs

@@ -27,7 +27,7 @@ STATUS_NAMES = {
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
-    "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_last_info",
+    "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
@@ -75,6 +75,7 @@ def lib() -> ctypes.CDLL:
         L.gs_invert_triangular.argtypes = [vp, vp, vp, vp]
         L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
         L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_density_matrix.argtypes = [vp, vp, vp, vp, vp]
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
         L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -186,6 +187,16 @@ class Plan:
         self._check(lib().gs_backtransform(self._h, _dev_ptr(Uinv, self.N, self.N, self.tdtype),
                                            _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
                                            _dev_ptr(C, self.N, self.nev, self.tdtype), _stream_ptr(stream)))
+
+    def density_matrix(self, C: torch.Tensor, f: torch.Tensor, P: torch.Tensor, stream=None):
+        """P(i,j) = sum_l f[l] conj(C(i,l)) C(j,l); upper triangle of P is written."""
+        if self.nev == 0:
+            self._check(lib().gs_density_matrix(self._h, None, None, _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+            return
+        if not (f.is_cuda and f.dtype == torch.float64 and f.dim() == 1 and f.numel() == self.nev and f.is_contiguous()):
+            raise ValueError("f: expected a contiguous CUDA float64 vector of length nev")
+        self._check(lib().gs_density_matrix(self._h, _dev_ptr(C, self.N, self.nev, self.tdtype), f.data_ptr(),
+                                            _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
 
     def last_info(self, stream=None, raise_on_failure: bool = True) -> int:
         info = ctypes.c_int64(0)
