@@ -44,6 +44,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-checks", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="NEXT-2: K independent pencils in flight on one GPU (not the headline)")
+    ap.add_argument("--batch-n", type=int, default=2048)
+    ap.add_argument("--batch-complex", action="store_true")
     return ap.parse_args()
 
 
@@ -402,7 +405,7 @@ def run_ours(args):
         e2e_sec = max_over_ranks((t1 - t0) / e2e_steps)
         esz = 16 if cplx else 8
         e2e = {"value": world * flops["total"] / e2e_sec / 1e12, "unit": UNIT,
-               "h2d_bytes_per_step": (2 * N * N + N * nev) * esz, "d2h_bytes_per_step": (N * N + N * nev) * esz,
+               "h2d_bytes_per_step": (2 * N * N + N * nev) * esz, "d2h_bytes_per_step": plan.reduce_host_d2h_bytes() + N * nev * esz,
                "ms_per_step": e2e_sec * 1e3, "steps": e2e_steps,
                "api": "gs_reduce_host + gs_backtransform_host (pinned host buffers in, H~ and C out)"}
         if checks is not None:
@@ -437,8 +440,60 @@ def run_ours(args):
     replicas.finalize(info)
 
 
+def run_batch(args):
+    """NEXT-2: K mid-size pencils concurrently on K streams vs one after the other."""
+    import torch
+
+    from paper_2502_02460_b200 import workloads as wl
+    from paper_2502_02460_b200.batch import Batch
+
+    torch.cuda.set_device(0)
+    K, N, cplx = args.batch, args.batch_n, args.batch_complex
+    nev = N // 4
+    flops = wl.nominal_flops(N, nev, cplx)["total"]
+    pens = [wl.make_pencil(N, wl.scaled_box(N), wl.BASE_SEED + 700 + k, complex=cplx, device="cuda") for k in range(K)]
+    b = Batch(K, N, nev, complex=cplx)
+    U, V, Ht, C = b.alloc(), b.alloc(), b.alloc(zeros=True), b.alloc(cols=nev)
+    Ct = [wl.dense_rhs(N, nev, seed=k, complex=cplx, device="cuda") for k in range(K)]
+    H, S = [p.H for p in pens], [p.S for p in pens]
+
+    def concurrent():
+        b.reduce(H, S, U, V, Ht)
+        b.backtransform(V, Ct, C)
+
+    def sequential():
+        for k in range(K):
+            U[k].copy_(S[k])
+            b.plans[k].cholesky(U[k])
+            b.plans[k].invert_triangular(U[k], V[k])
+            b.plans[k].to_standard(H[k], V[k], Ht[k])
+            b.plans[k].backtransform(V[k], Ct[k], C[k])
+
+    out = {}
+    for name, fn in (("sequential", sequential), ("concurrent", concurrent)):
+        for _ in range(max(1, args.warmup)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        out[name] = {"ms_per_batch": ms, "tflops": K * flops / (ms * 1e-3) / 1e12}
+    assert b.last_info() == [0] * K
+    print(json.dumps({"metric": "FP64 TFLOP/s of K independent reductions in flight (NEXT-2, not the headline)",
+                      "unit": UNIT, "value": out["concurrent"]["tflops"], "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+                      "config": {"workload": f"batch_K{K}_N{N}_{'c128' if cplx else 'f64'}_nev{nev}"}, "dtype": "c128" if cplx else "f64",
+                      "data": "synthetic", "detail": out}))
+
+
 def main():
     args = parse_args()
+    if args.batch > 0:
+        run_batch(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

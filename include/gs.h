@@ -115,13 +115,17 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 
 /* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
  * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
- * inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3 there and copies H~ (the whole
- * N x N buffer; its upper triangle is the result, the strictly-lower part is zero) back to
- * host_Htilde.  host_U / host_Uinv may be NULL (then they are not copied back).  U^-1 stays in the
- * scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in, forms
- * C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report numerical
- * failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte aligned. */
+ * inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3 there and copies the UPPER
+ * triangle of H~ back to host_Htilde (N x N, ld N; it is copied as 1024-column trapezoids, so host
+ * entries below the diagonal block of their column panel are left untouched -- callers read the
+ * upper triangle only).  The H2D copy of H runs on a plan-owned copy stream beside steps 1-2 and is
+ * joined before step 3.  host_U / host_Uinv may be NULL (then they are not copied back).  U^-1 stays
+ * in the scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in,
+ * forms C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report
+ * numerical failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte
+ * aligned.  gs_reduce_host_d2h_bytes reports the bytes gs_reduce_host copies back for H~. */
 gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_reduce_host_d2h_bytes(const gs_plan_t* plan, size_t* bytes);
 gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host_S,
                            void* host_U, void* host_Uinv, void* host_Htilde,
                            void* dev_scratch, size_t scratch_bytes, void* cuda_stream);

@@ -58,6 +58,8 @@ struct gs_plan {
     // from and joined back into the caller's stream with events inside every call that uses it
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_rows = nullptr, ev_join = nullptr;
+    cudaStream_t copy = nullptr;     // host-buffer entry points: H2D of H overlaps the factorisation of S
+    cudaEvent_t ev_copy = nullptr;
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
     int potrf_tail = 64;
@@ -68,6 +70,7 @@ struct gs_plan {
 namespace {
 
 constexpr size_t kInfoBytes = 256;
+constexpr int64_t kHostPanel = 1024;   // column-block width of the trapezoidal D2H copy of H~ (gs_reduce_host)
 constexpr int KPB = 8;   // pipeline k-steps per block: 128 / 16 (real) = 64 / 8 (complex)
 static_assert(LB / BK == KPB && CLB / CBK == KPB && CT == CLB, "block / k-slab ratio");
 
@@ -544,6 +547,8 @@ gs_status_t gs_plan_destroy(gs_plan_t* plan)
     if (plan->ev_rows != nullptr) cudaEventDestroy(plan->ev_rows);
     if (plan->ev_join != nullptr) cudaEventDestroy(plan->ev_join);
     if (plan->side != nullptr) cudaStreamDestroy(plan->side);
+    if (plan->ev_copy != nullptr) cudaEventDestroy(plan->ev_copy);
+    if (plan->copy != nullptr) cudaStreamDestroy(plan->copy);
     delete plan;
     return GS_OK;
 }
@@ -737,6 +742,18 @@ gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes)
     return GS_OK;
 }
 
+gs_status_t gs_reduce_host_d2h_bytes(const gs_plan_t* plan, size_t* bytes)
+{
+    if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
+    size_t b = 0;
+    for (int64_t c0 = 0; c0 < plan->N; c0 += kHostPanel) {
+        const int64_t cols = plan->N - c0 < kHostPanel ? plan->N - c0 : kHostPanel;
+        b += size_t(c0 + cols) * size_t(cols) * plan->es;
+    }
+    *bytes = b;
+    return GS_OK;
+}
+
 gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host_S, void* host_U, void* host_Uinv,
                            void* host_Htilde, void* dev_scratch, size_t scratch_bytes, void* cuda_stream)
 {
@@ -751,15 +768,32 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     const size_t mat = need / 4;
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
     void *dS = base, *dH = base + mat, *dV = base + 2 * mat, *dHt = base + 3 * mat;
+    if (plan->copy == nullptr) {
+        GS_CUDA(plan, cudaStreamCreateWithFlags(&plan->copy, cudaStreamNonBlocking));
+        GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_copy, cudaEventDisableTiming));
+    }
+    // S first on the caller's stream; H (not needed before step 3) and the clearing of the H~ buffer go
+    // on the plan's copy stream and overlap steps 1-2; the copy stream is forked from / joined into `stream`
     GS_CUDA(plan, cudaMemcpyAsync(dS, host_S, bytes, cudaMemcpyHostToDevice, stream));
-    GS_CUDA(plan, cudaMemcpyAsync(dH, host_H, bytes, cudaMemcpyHostToDevice, stream));
-    GS_CUDA(plan, cudaMemsetAsync(dHt, 0, bytes, stream));
-    GS_TRY(gs_cholesky(plan, dS, stream));
-    GS_TRY(gs_invert_triangular(plan, dS, dV, stream));
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));          // H follows S on the link, not beside it
+    GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
+    GS_CUDA(plan, cudaMemcpyAsync(dH, host_H, bytes, cudaMemcpyHostToDevice, plan->copy));
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy));
+    gs_status_t rc = gs_cholesky(plan, dS, stream);
+    if (rc == GS_OK) rc = gs_invert_triangular(plan, dS, dV, stream);
+    GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_copy, 0));   // join, also on failure
+    GS_TRY(rc);
     GS_TRY(gs_to_standard(plan, dH, dV, dHt, stream));
     if (host_U) GS_CUDA(plan, cudaMemcpyAsync(host_U, dS, bytes, cudaMemcpyDeviceToHost, stream));
     if (host_Uinv) GS_CUDA(plan, cudaMemcpyAsync(host_Uinv, dV, bytes, cudaMemcpyDeviceToHost, stream));
-    GS_CUDA(plan, cudaMemcpyAsync(host_Htilde, dHt, bytes, cudaMemcpyDeviceToHost, stream));
+    // H~: only the upper triangle exists; copy it as column-block trapezoids (kHostPanel columns each)
+    for (int64_t c0 = 0; c0 < plan->N; c0 += kHostPanel) {
+        const int64_t cols = plan->N - c0 < kHostPanel ? plan->N - c0 : kHostPanel;
+        const int64_t rows = c0 + cols;   // rows 0 .. last column of the block
+        const size_t off = size_t(c0) * size_t(plan->N) * plan->es, pitch = size_t(plan->N) * plan->es;
+        GS_CUDA(plan, cudaMemcpy2DAsync(static_cast<unsigned char*>(host_Htilde) + off, pitch, static_cast<unsigned char*>(dHt) + off,
+                                        pitch, size_t(rows) * plan->es, size_t(cols), cudaMemcpyDeviceToHost, stream));
+    }
     int64_t info = 0;
     return gs_last_info(plan, stream, &info);
 }

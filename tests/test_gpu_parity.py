@@ -167,3 +167,37 @@ def test_argument_errors():
         plan.cholesky(torch.empty((64, 64), dtype=torch.float64, device="cuda"))   # row-major
     plan.backtransform(None, None, None)    # nev == 0: no-op
     plan.close()
+
+
+@pytest.mark.parametrize("N,cplx", [(300, False), (2500, False), (1100, True)])
+def test_host_buffer_entry_points_match_the_device_path(N, cplx):
+    """gs_reduce_host / gs_backtransform_host (pinned host buffers, copies inside) give bit for bit what
+    the device-pointer calls give: same kernels, same order.  N = 2500 spans three 1024-column D2H panels."""
+    gs = _gs()
+    nev = N // 3
+    dt = torch.complex128 if cplx else torch.float64
+    p = wl.small_pencil(N, seed=77, complex=cplx, device="cuda")
+    plan, U, V, Ht = gs.generalized_to_standard(p.H, p.S, nev)
+    Ct = wl.dense_rhs(N, nev, seed=5, complex=cplx, device="cuda")
+    C = wl.colmajor_empty(N, nev, dtype=dt, device="cuda")
+    plan.backtransform(V, Ct, C)
+    plan.last_info()
+
+    def host(rows, cols, src=None):
+        h = torch.empty((cols, rows), dtype=dt).pin_memory()      # column-major image of a rows x cols matrix
+        if src is not None:
+            h.copy_(src.t())
+        return h
+
+    hH, hS, hCt = host(N, N, p.H), host(N, N, p.S), host(N, nev, Ct)
+    hU, hV, hHt, hC = host(N, N), host(N, N), host(N, N), host(N, nev)
+    hHt.fill_(-9.0)
+    scratch = torch.empty(plan.host_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    plan.reduce_host(hH, hS, hU, hV, hHt, scratch)
+    plan.backtransform_host(hCt, hC, scratch)
+    assert torch.equal(torch.triu(hU.t()), torch.triu(U.cpu()))
+    assert torch.equal(torch.triu(hV.t()), torch.triu(V.cpu()))
+    assert torch.equal(torch.triu(hHt.t()), torch.triu(Ht.cpu()))
+    assert torch.equal(hC.t(), C.cpu())
+    assert 0 < plan.reduce_host_d2h_bytes() <= N * N * (16 if cplx else 8)
+    plan.close()
