@@ -199,7 +199,7 @@ gs_status_t zero_lower(Stage& st, void* X)
     const gs_plan* plan = st.plan;
     const int N = int(plan->N);
     if (N <= st.lb) return GS_OK;
-    dim3 grid((N + 255) / 256, N);
+    dim3 grid(N > 2048 ? 8 : (N + 255) / 256, N);
     LaunchTimer timer(st.plan, L_ZERO_LOWER, st.stream);
     if (st.z) zero_lower_blocks_kernel<double2, CLB><<<grid, 256, 0, st.stream>>>(static_cast<double2*>(X), plan->N, N, info_ptr(plan));
     else zero_lower_blocks_kernel<double, LB><<<grid, 256, 0, st.stream>>>(static_cast<double*>(X), plan->N, N, info_ptr(plan));
@@ -587,9 +587,23 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     f.vS = MatView{S, plan->N, plan->N, plan->N};
     f.vT = MatView{big_ptr(plan), plan->N, plan->N, plan->N};
     f.pb = 0;
-    if (plan->nblk > 1) GS_TRY(ensure_side_stream(plan));
-    GS_TRY(zero_lower(f.st, S));   // off-diagonal lower blocks: never touched by the factorisation
-    return f.factor(plan->nblk, stream);
+    if (plan->nblk <= 1) return f.factor(plan->nblk, stream);
+    GS_TRY(ensure_side_stream(plan));
+    // the off-diagonal lower blocks are never touched by the factorisation: zero them on the side
+    // stream, beside the first panel (its own fork/join events; factor() forks after this work)
+    GS_CUDA(plan, cudaEventRecord(plan->ev_fork, stream));
+    GS_CUDA(plan, cudaStreamWaitEvent(plan->side, plan->ev_fork, 0));
+    f.st.stream = plan->side;
+    const gs_status_t zs = zero_lower(f.st, S);
+    f.st.stream = stream;
+    const gs_status_t fs = zs == GS_OK ? f.factor(plan->nblk, stream) : zs;
+    // factor() joins the side stream after every panel; a single-panel factorisation has no join of its own
+    const cudaError_t e1 = cudaEventRecord(plan->ev_join, plan->side);
+    const cudaError_t e2 = cudaStreamWaitEvent(stream, plan->ev_join, 0);
+    GS_TRY(fs);
+    GS_CUDA(plan, e1);
+    GS_CUDA(plan, e2);
+    return GS_OK;
 }
 
 // V = U^-1: every diagonal 128-block inverted by the leaf kernel, then block-recursive doubling.

@@ -232,8 +232,8 @@ __global__ void zero_lower_blocks_kernel(T* __restrict__ X, long long ld, int N,
     if (*info != 0) return;
     const int col = blockIdx.y;
     const int first = (col / kLB + 1) * kLB;   // first row below the diagonal block of this column
-    const int row = first + blockIdx.x * blockDim.x + threadIdx.x;
-    if (row < N) X[row + (long long)col * ld] = T{};
+    for (int row = first + blockIdx.x * blockDim.x + threadIdx.x; row < N; row += gridDim.x * blockDim.x)
+        X[row + (long long)col * ld] = T{};
 }
 
 // dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid row (blockIdx.y) per column c.
