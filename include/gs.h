@@ -84,11 +84,12 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream);
  * triangle) and zeros below the diagonal.  Uinv must not alias U.  Blocked TRTRI. */
 gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U, void* Uinv, void* cuda_stream);
 
-/* Step 3.  Htilde = Uinv^H * H * Uinv.  Reads all of H (both triangles must hold a
- * consistent symmetric / Hermitian matrix) and the upper triangle of Uinv.  Writes the UPPER
- * triangle (incl. diagonal) of Htilde; the strictly-lower part of the Htilde buffer is left
- * untouched.  For GS_COMPLEX128 the diagonal of Htilde is exactly real.  Fused triangular product
- * pair: exploits the triangularity of Uinv and forms one triangle of the symmetric result only. */
+/* Step 3.  Htilde = Uinv^H * H * Uinv.  H must be symmetric / Hermitian with both
+ * triangles filled consistently (the kernels reference its lower triangle and diagonal); only the
+ * upper triangle of Uinv is read.  Writes the UPPER triangle (incl. diagonal) of Htilde; the
+ * strictly-lower part of the Htilde buffer is left untouched.  For GS_COMPLEX128 the diagonal of
+ * Htilde is exactly real.  Fused triangular product pair: exploits the triangularity of Uinv and
+ * forms one triangle of the symmetric result only. */
 gs_status_t gs_to_standard(gs_plan_t* plan, const void* H, const void* Uinv, void* Htilde,
                            void* cuda_stream);
 

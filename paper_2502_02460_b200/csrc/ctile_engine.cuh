@@ -34,7 +34,7 @@ constexpr int kCSmemBytes = kCStages * kCStageBytes + 1024 /*align*/ + 256 /*bar
 // k-contiguous tile: 64 rows (free index x) of 8 complex (k): element (row = k0 + k, col = x0 + x).
 // m-contiguous tile: 8 boxes [mb][k][8 m]: element (row = x0 + 8*mb + m_in, col = k0 + k).
 template <bool kMContig>
-__device__ __forceinline__ void mask_ctile(unsigned char* tile, int k0, int x0, bool half_diag, int ctid)
+__device__ __forceinline__ void mask_ctile(unsigned char* tile, int k0, int x0, bool half_diag, int ctid, bool lower = false)
 {
 #pragma unroll
     for (int it = 0; it < 4; ++it) {
@@ -46,7 +46,7 @@ __device__ __forceinline__ void mask_ctile(unsigned char* tile, int k0, int x0, 
         int grow, gcol;
         if (!kMContig) { gcol = x0 + row128; grow = k0 + ch; }
         else { const int mb = row128 >> 3, k = row128 & 7; grow = x0 + mb * 8 + ch; gcol = k0 + k; }
-        if (grow > gcol) *ptr = make_double2(0.0, 0.0);
+        if (lower ? (grow < gcol) : (grow > gcol)) *ptr = make_double2(0.0, 0.0);
         else if (half_diag && grow == gcol) { double2 v = *ptr; v.x *= 0.5; v.y *= 0.5; *ptr = v; }
     }
 }
@@ -192,9 +192,11 @@ __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid
             const int bx = second ? b2_x : b_x, bk = (second ? b2_k : b_k) + kt * CBK;
             bool did = false;
             if (mA) {
-                const bool straddle = kANN ? (ax + CT - 1 >= ak) : (ak + CBK - 1 >= ax);
+                const bool lowerA = !second && (p.flags & F_LOWER_A) != 0;
+                const bool straddle = lowerA ? (kANN ? (ax <= ak + CBK - 1) : (ak <= ax + CT - 1))
+                                             : (kANN ? (ax + CT - 1 >= ak) : (ak + CBK - 1 >= ax));
                 if (straddle) {
-                    mask_ctile<kANN>(st, ak, ax, !second && (p.flags & F_HALF_DIAG_A), ctid);
+                    mask_ctile<kANN>(st, ak, ax, !second && (p.flags & F_HALF_DIAG_A), ctid, lowerA);
                     did = true;
                 }
             }

@@ -652,14 +652,17 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
     const MatView vH{H_, N, N, N}, vV{Uinv_, N, N, N}, vG{G, N, N, N};
     const int kt = KPB;
     {
+        // G = T V computed as L^H V with L = tril(H,-1) + diag(H)/2 (L^H = T because H is Hermitian): the
+        // k-contiguous ("TN") mainloop reads column I of H below the diagonal -- it runs ~4 % closer to
+        // the pipe than the m-contiguous one (profiles/r01c_perkernel.md)
         EngineParams p = blank_params(plan);
-        if (!set_operand(st, p, 0, vH, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
+        if (!set_operand(st, p, 0, vH, false) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
         p.C = static_cast<double*>(G); p.ldc = N;
         p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_DIAG_DESC;
         p.c_rows = N; p.c_cols = N;
         p.klo_i = kt; p.khi_c = kt; p.khi_j = kt; p.kmax = (N + st.bk - 1) / st.bk;
-        p.flags = F_MASK_A | F_HALF_DIAG_A | F_MASK_B;
-        GS_TRY(launch(st, p, true, L_TOSTD_G));
+        p.flags = F_MASK_A | F_LOWER_A | F_HALF_DIAG_A | F_MASK_B;
+        GS_TRY(launch(st, p, false, L_TOSTD_G));
     }
     {
         EngineParams p = blank_params(plan);

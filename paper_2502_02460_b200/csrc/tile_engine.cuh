@@ -47,6 +47,7 @@ enum : uint32_t {
     F_MASK_A2 = 1u << 4,
     F_MASK_B2 = 1u << 5,
     F_STORE_UPPER = 1u << 6,   // store only C elements with global row <= col
+    F_LOWER_A = 1u << 8,       // with F_MASK_A: A keeps its LOWER triangle instead (zero where row < col)
     F_REAL_DIAG = 1u << 7,     // complex engine: store Im = 0 on the global diagonal (Hermitian results)
 };
 
@@ -157,7 +158,7 @@ __device__ __forceinline__ bool decode_tile(const EngineParams& p, int id, int& 
 // The 128-byte swizzle permutes 16-byte chunks within a 128-byte row; masking works on logical
 // coordinates and maps them to the swizzled address.
 template <bool kMContig>
-__device__ __forceinline__ void mask_tile(unsigned char* tile, int k0, int x0, bool half_diag, int ctid)
+__device__ __forceinline__ void mask_tile(unsigned char* tile, int k0, int x0, bool half_diag, int ctid, bool lower = false)
 {
     // 2048 elements, 256 consumer threads -> 8 elements (4 chunks of 2) per thread
 #pragma unroll
@@ -171,6 +172,7 @@ __device__ __forceinline__ void mask_tile(unsigned char* tile, int k0, int x0, b
         if (!kMContig) { gcol0 = x0 + row128; grow0 = k0 + ch * 2; drow = 1; dcol = 0; }
         else { const int mb = row128 >> 4, k = row128 & 15; grow0 = x0 + mb * 16 + ch * 2; gcol0 = k0 + k; drow = 1; dcol = 0; }
         (void)dcol;
+        if (lower) { const int t0 = grow0; grow0 = gcol0; gcol0 = t0; drow = -1; }   // compare (col, row): zero where row < col
         double2 v = *ptr;
         bool touched = false;
         if (grow0 > gcol0) { v.x = 0.0; touched = true; }
@@ -377,9 +379,11 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
             bool did = false;
             if (mA) {
                 // A element global (row, col): NN: (ax + m, ak + k); TN: (ak + k, ax + m)
-                const bool straddle = kANN ? (ax + BM - 1 >= ak) : (ak + BK - 1 >= ax);
+                const bool lowerA = !second && (p.flags & F_LOWER_A) != 0;
+                const bool straddle = lowerA ? (kANN ? (ax <= ak + BK - 1) : (ak <= ax + BM - 1))
+                                             : (kANN ? (ax + BM - 1 >= ak) : (ak + BK - 1 >= ax));
                 if (straddle) {
-                    mask_tile<kANN>(st, ak, ax, !second && (p.flags & F_HALF_DIAG_A), ctid);
+                    mask_tile<kANN>(st, ak, ax, !second && (p.flags & F_HALF_DIAG_A), ctid, lowerA);
                     did = true;
                 }
             }
