@@ -11,6 +11,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "ptx.cuh"
+
 namespace gs {
 
 constexpr int CLB = 64;                  // complex leaf block order
@@ -119,6 +121,8 @@ __device__ __forceinline__ void cleaf_invert_upper(const CLeafSmem& s, int tx, i
 __global__ void __launch_bounds__(kCLeafThreads, 1)
 potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2* __restrict__ Winv, long long ldw, int* info)
 {
+    grid_dep_launch();
+    grid_dep_wait();
     if (*info != 0) return;
     extern __shared__ __align__(16) unsigned char leaf_raw[];
     const CLeafSmem s = cleaf_smem(leaf_raw);

@@ -54,8 +54,6 @@ __device__ __forceinline__ void mask_ctile(unsigned char* tile, int k0, int x0, 
 template <bool kANN>
 __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid_constant__ EngineParams p)
 {
-    if (p.info != nullptr && *p.info != 0) return;
-
     extern __shared__ unsigned char smem_raw[];
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kCStages * kCStageBytes);
@@ -83,6 +81,10 @@ __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid
         mbar_fence_init();
     }
     __syncthreads();
+    // everything above touched only parameters and shared memory (ptx.cuh: programmatic dependent launch)
+    grid_dep_launch();
+    grid_dep_wait();
+    if (p.info != nullptr && *p.info != 0) return;
 
     // element coordinates (complex elements) of the operand tiles at k-step 0
     const int a_x = p.a.x0 + b * p.a.bx + CT * I, a_k = p.a.k0 + b * p.a.bk;

@@ -56,6 +56,20 @@ inline bool make_tensor_map(CUtensorMap* out, const MatView& m, int box_cols, bo
     return r == CUDA_SUCCESS;
 }
 
+// Launch with the programmatic-stream-serialization attribute (ptx.cuh: grid_dep_wait): only for
+// kernels that call grid_dep_wait() before their first global-memory access.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 inline int num_tiles(const EngineParams& p)
 {
     int per = p.tiles_m * p.tiles_n;
@@ -98,13 +112,11 @@ inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, bool use_tma,
     cudaError_t e = engine_configure();
     if (e != cudaSuccess) return e;
     if (use_tma) {
-        if (a_nn) tile_engine_kernel<true, true><<<grid, kThreads, kSmemBytes, stream>>>(p);
-        else tile_engine_kernel<false, true><<<grid, kThreads, kSmemBytes, stream>>>(p);
-    } else {
-        if (a_nn) tile_engine_kernel<true, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
-        else tile_engine_kernel<false, false><<<grid, kThreads, kSmemBytes, stream>>>(p);
+        if (a_nn) return launch_pdl(tile_engine_kernel<true, true>, grid, kThreads, kSmemBytes, stream, p);
+        return launch_pdl(tile_engine_kernel<false, true>, grid, kThreads, kSmemBytes, stream, p);
     }
-    return cudaGetLastError();
+    if (a_nn) return launch_pdl(tile_engine_kernel<true, false>, grid, kThreads, kSmemBytes, stream, p);
+    return launch_pdl(tile_engine_kernel<false, false>, grid, kThreads, kSmemBytes, stream, p);
 }
 
 // complex128 engine: operands always go through TMA (a complex row pitch is a multiple of 16 bytes)
@@ -114,9 +126,8 @@ inline cudaError_t cengine_launch(const EngineParams& p, bool a_nn, cudaStream_t
     if (grid <= 0) return cudaSuccess;
     cudaError_t e = engine_configure();
     if (e != cudaSuccess) return e;
-    if (a_nn) ctile_engine_kernel<true><<<grid, kCThreads, kCSmemBytes, stream>>>(p);
-    else ctile_engine_kernel<false><<<grid, kCThreads, kCSmemBytes, stream>>>(p);
-    return cudaGetLastError();
+    if (a_nn) return launch_pdl(ctile_engine_kernel<true>, grid, kCThreads, kCSmemBytes, stream, p);
+    return launch_pdl(ctile_engine_kernel<false>, grid, kCThreads, kCSmemBytes, stream, p);
 }
 
 }  // namespace gs

@@ -286,13 +286,13 @@ struct Potrf {
         gs_plan* plan = st.plan;
         LaunchTimer timer(plan, L_POTRF_LEAF, st.stream);
         void* w = static_cast<unsigned char*>(const_cast<void*>(vW.ptr)) + size_t(b - pb) * st.lb * (vW.ld + 1) * plan->es;
+        cudaError_t e;
         if (st.z)
-            potrf_cleaf_kernel<<<1, kCLeafThreads, kCLeafSmemBytes, st.stream>>>(static_cast<double2*>(S), plan->N, int(plan->N), b * st.lb,
-                                                                                 static_cast<double2*>(w), vW.ld, info_ptr(plan));
+            e = launch_pdl(potrf_cleaf_kernel, 1, kCLeafThreads, kCLeafSmemBytes, st.stream, static_cast<double2*>(S), plan->N, int(plan->N),
+                           b * st.lb, static_cast<double2*>(w), vW.ld, info_ptr(plan));
         else
-            potrf_leaf_kernel<<<1, kLeafThreads, kLeafSmemBytes, st.stream>>>(static_cast<double*>(S), plan->N, int(plan->N), b * st.lb,
-                                                                              static_cast<double*>(w), vW.ld, info_ptr(plan));
-        const cudaError_t e = cudaGetLastError();
+            e = launch_pdl(potrf_leaf_kernel, 1, kLeafThreads, kLeafSmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
+                           b * st.lb, static_cast<double*>(w), vW.ld, info_ptr(plan));
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
         return GS_OK;
@@ -392,13 +392,13 @@ struct Potrf {
         const int cols = (c1 * st.lb < N ? c1 * st.lb : N) - c0 * st.lb;
         dim3 grid((rows + 255) / 256, cols);
         LaunchTimer timer(plan, L_POTRF_TRSM, st.stream);
+        cudaError_t e;
         if (st.z)
-            copy_block_kernel<double2><<<grid, 256, 0, st.stream>>>(static_cast<const double2*>(vT.ptr), static_cast<double2*>(S), plan->N,
-                                                                    b1 * st.lb, rows, c0 * st.lb, info_ptr(plan));
+            e = launch_pdl(copy_block_kernel<double2>, grid, 256, 0, st.stream, static_cast<const double2*>(vT.ptr), static_cast<double2*>(S),
+                           plan->N, b1 * st.lb, rows, c0 * st.lb, static_cast<const int*>(info_ptr(plan)));
         else
-            copy_block_kernel<double><<<grid, 256, 0, st.stream>>>(static_cast<const double*>(vT.ptr), static_cast<double*>(S), plan->N,
-                                                                   b1 * st.lb, rows, c0 * st.lb, info_ptr(plan));
-        const cudaError_t e = cudaGetLastError();
+            e = launch_pdl(copy_block_kernel<double>, grid, 256, 0, st.stream, static_cast<const double*>(vT.ptr), static_cast<double*>(S),
+                           plan->N, b1 * st.lb, rows, c0 * st.lb, static_cast<const int*>(info_ptr(plan)));
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
         return GS_OK;

@@ -16,6 +16,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "ptx.cuh"
+
 namespace gs {
 
 constexpr int LB = 128;                 // leaf block order
@@ -118,6 +120,8 @@ __device__ __forceinline__ void leaf_invert_upper(const LeafSmem& s, int tx, int
 __global__ void __launch_bounds__(kLeafThreads, 1)
 potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* __restrict__ Winv, long long ldw, int* info)
 {
+    grid_dep_launch();
+    grid_dep_wait();
     if (*info != 0) return;
     extern __shared__ __align__(16) unsigned char leaf_raw[];
     const LeafSmem s = leaf_smem(leaf_raw);
@@ -241,6 +245,8 @@ template <typename T>
 __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst, long long ld, int row0, int rows,
                                   int col0, const int* info)
 {
+    grid_dep_launch();
+    grid_dep_wait();
     if (*info != 0) return;
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r < rows) {

@@ -91,6 +91,14 @@ __device__ __forceinline__ void release_previous_stage(int s, int nstages, uint3
     }
 }
 
+// Programmatic dependent launch: a kernel launched with the programmatic-stream-serialization
+// attribute may start while its predecessor in the stream is still running; it must not touch
+// global memory before grid_dep_wait() (which returns once the predecessor has completed and its
+// writes are visible).  grid_dep_launch() lets the successor's CTAs be scheduled early, so launch
+// latency and the prologue (barrier init, descriptor prefetch) hide behind this kernel's tail.
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
     double2 v;

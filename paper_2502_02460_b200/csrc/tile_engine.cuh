@@ -214,8 +214,6 @@ __device__ __forceinline__ void load_tile_mcontig(unsigned char* tile, const Raw
 template <bool kANN, bool kTMA>
 __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_constant__ EngineParams p)
 {
-    if (p.info != nullptr && *p.info != 0) return;
-
     extern __shared__ unsigned char smem_raw[];
     // 1024-byte alignment (128-byte swizzle atom = 8 rows x 128 B) without losing the shared address space
     unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -244,6 +242,10 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
         mbar_fence_init();
     }
     __syncthreads();
+    // everything above touched only parameters and shared memory (ptx.cuh: programmatic dependent launch)
+    grid_dep_launch();
+    grid_dep_wait();
+    if (p.info != nullptr && *p.info != 0) return;
 
     // global element coordinates of the operand tiles at k-step 0
     const int a_x = p.a.x0 + b * p.a.bx + BM * I, a_k = p.a.k0 + b * p.a.bk;
