@@ -63,6 +63,8 @@ struct gs_plan {
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
     int potrf_tail = 64;
+    int potrf_nb_end = 1;            // panel width once at most potrf_end blocks remain
+    int potrf_end = 32;
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
 };
@@ -408,14 +410,16 @@ struct Potrf {
     gs_status_t update_rows(int b0, int b1, int b2, int n) { return gemm_update(b0, b1, b2, b2, n); }
 
     // Panel boundaries: wide panels while the trailing matrix is large (the trailing update hides the
-    // panel chain), narrow ones in the tail (the chain is exposed there, and it is shorter per row).
-    static std::vector<int> panel_starts(int n, int nb_big, int nb_tail, int tail)
+    // panel chain), narrower ones in the tail (the chain is exposed there, and it is shorter per row),
+    // single blocks at the very end (the leaf's inverse IS the panel inverse: no doubling, no recursion).
+    static std::vector<int> panel_starts(int n, const gs_plan* plan)
     {
         std::vector<int> s;
         int b = 0;
         while (b < n) {
             s.push_back(b);
-            b += (n - b > tail) ? nb_big : nb_tail;
+            const int left = n - b;
+            b += left > plan->potrf_tail ? plan->potrf_nb : left > plan->potrf_end ? plan->potrf_nb_tail : plan->potrf_nb_end;
         }
         s.push_back(n);
         return s;
@@ -432,7 +436,7 @@ struct Potrf {
     {
         gs_plan* plan = st.plan;
         cudaStream_t side = plan->side;
-        const std::vector<int> ps = panel_starts(n, plan->potrf_nb, plan->potrf_nb_tail, plan->potrf_tail);
+        const std::vector<int> ps = panel_starts(n, plan);
         const int np = int(ps.size()) - 1;
         const int ldw = wp_ld(plan);
         auto W = [&](int i) { return MatView{wp_ptr(plan, i), ldw, ldw, ldw}; };
@@ -532,6 +536,9 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_POTRF_NB", 1, 256, &p->potrf_nb);
     knob("GS_POTRF_NB_TAIL", 1, 32, &p->potrf_nb_tail);
     knob("GS_POTRF_TAIL", 0, 1 << 20, &p->potrf_tail);
+    knob("GS_POTRF_NB_END", 1, 32, &p->potrf_nb_end);
+    knob("GS_POTRF_END", 0, 1 << 20, &p->potrf_end);
+    if (p->potrf_nb_end > p->potrf_nb_tail) p->potrf_nb_end = p->potrf_nb_tail;
     if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
     p->super_tile = p->z ? 16 : 12;
     knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
