@@ -7,6 +7,7 @@
 #include <cstring>
 
 #include "ctile_engine.cuh"
+#include "tile64_engine.cuh"
 #include "tile_engine.cuh"
 
 namespace gs {
@@ -94,6 +95,10 @@ inline cudaError_t engine_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(tile_engine_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tile64_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, k64SmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tile64_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, k64SmemBytes);
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ctile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ctile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
@@ -117,6 +122,17 @@ inline cudaError_t engine_launch(const EngineParams& p, bool a_nn, bool use_tma,
     }
     if (a_nn) return launch_pdl(tile_engine_kernel<true, false>, grid, kThreads, kSmemBytes, stream, p);
     return launch_pdl(tile_engine_kernel<false, false>, grid, kThreads, kSmemBytes, stream, p);
+}
+
+// real engine with 64 x 64 CTA tiles (tile64_engine.cuh): four CTAs per logical 128-tile; TMA only
+inline cudaError_t engine64_launch(const EngineParams& p, bool a_nn, cudaStream_t stream)
+{
+    const int grid = 4 * num_tiles(p);
+    if (grid <= 0) return cudaSuccess;
+    cudaError_t e = engine_configure();
+    if (e != cudaSuccess) return e;
+    if (a_nn) return launch_pdl(tile64_engine_kernel<true>, grid, k64Threads, k64SmemBytes, stream, p);
+    return launch_pdl(tile64_engine_kernel<false>, grid, k64Threads, k64SmemBytes, stream, p);
 }
 
 // complex128 engine: operands always go through TMA (a complex row pitch is a multiple of 16 bytes)

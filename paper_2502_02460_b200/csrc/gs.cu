@@ -65,6 +65,7 @@ struct gs_plan {
     int potrf_tail = 64;
     int potrf_nb_end = 1;            // panel width once at most potrf_end blocks remain
     int potrf_end = 32;
+    int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
 };
@@ -143,12 +144,19 @@ struct Stage {
     bool tma;
     bool z;       // complex128
     int lb, bk;   // block order and k-slab in elements (plan->lb, plan->bk)
+    // operands of the launch under construction (tensor maps are encoded in launch(), once the tile
+    // size of the kernel is known)
+    MatView opv[4];
+    bool opm[4];
+    bool opset[4];
 };
 
 Stage make_stage(gs_plan* plan, cudaStream_t stream)
 {
     // a real matrix with odd N has a row pitch that is not a multiple of 16 bytes: no tensor map
-    return Stage{plan, stream, plan->z || plan->N % 2 == 0, plan->z, plan->lb, plan->bk};
+    Stage st{};
+    st.plan = plan; st.stream = stream; st.tma = plan->z || plan->N % 2 == 0; st.z = plan->z; st.lb = plan->lb; st.bk = plan->bk;
+    return st;
 }
 
 EngineParams blank_params(const gs_plan* plan)
@@ -163,21 +171,37 @@ EngineParams blank_params(const gs_plan* plan)
     return p;
 }
 
-// which: 0 = A, 1 = B, 2 = A2, 3 = B2.  mcontig selects the 16 x 16 box of the m-contiguous A operand.
-bool set_operand(const Stage& st, EngineParams& p, int which, const MatView& m, bool mcontig)
+// which: 0 = A, 1 = B, 2 = A2, 3 = B2.  mcontig selects the m-contiguous box of the A operand.
+bool set_operand(Stage& st, EngineParams& p, int which, const MatView& m, bool mcontig)
 {
     RawOperand r{static_cast<const double*>(m.ptr), m.ld, int(m.rows), int(m.cols)};
-    CUtensorMap* map = which == 0 ? &p.mapA : which == 1 ? &p.mapB : which == 2 ? &p.mapA2 : &p.mapB2;
     (which == 0 ? p.rawA : which == 1 ? p.rawB : which == 2 ? p.rawA2 : p.rawB2) = r;
-    if (!st.tma) return true;
-    if (st.z) return make_tensor_map(map, m, mcontig ? 8 : CT, true);
-    return make_tensor_map(map, m, mcontig ? 16 : BN, false);
+    st.opv[which] = m; st.opm[which] = mcontig; st.opset[which] = true;
+    return true;
 }
 
-gs_status_t launch(Stage& st, const EngineParams& p, bool a_nn, int label)
+// Real launches with few logical tiles go to the 64 x 64-tile engine (four CTAs per tile: a quarter of
+// the latency on the panel chain); GS_TILE64 = 0 never, 1 below plan->tile64_below tiles, 2 always.
+bool use_tile64(const Stage& st, const EngineParams& p)
 {
+    if (st.z || !st.tma || st.plan->tile64_mode == 0 || (p.flags & F_NO_SPLIT) != 0) return false;
+    return st.plan->tile64_mode == 2 || num_tiles(p) < st.plan->tile64_below;
+}
+
+gs_status_t launch(Stage& st, EngineParams& p, bool a_nn, int label)
+{
+    const bool t64 = use_tile64(st, p);
+    for (int w = 0; w < 4; ++w) {
+        if (!st.opset[w]) continue;
+        st.opset[w] = false;
+        if (!st.tma) continue;
+        CUtensorMap* map = w == 0 ? &p.mapA : w == 1 ? &p.mapB : w == 2 ? &p.mapA2 : &p.mapB2;
+        const int box = st.z ? (st.opm[w] ? 8 : CT) : (st.opm[w] ? 16 : (t64 ? T64 : BN));
+        if (!make_tensor_map(map, st.opv[w], box, st.z)) return GS_ERR_CUDA;
+    }
     LaunchTimer timer(st.plan, label, st.stream);
-    const cudaError_t e = st.z ? cengine_launch(p, a_nn, st.stream) : engine_launch(p, a_nn, st.tma, st.stream);
+    const cudaError_t e = st.z ? cengine_launch(p, a_nn, st.stream)
+                               : t64 ? engine64_launch(p, a_nn, st.stream) : engine_launch(p, a_nn, st.tma, st.stream);
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
     st.plan->launches += 1;
     return GS_OK;
@@ -311,6 +335,7 @@ struct Potrf {
         p.khi_c = KPB; p.kmax = KPB;
         p.a.k0 = (r0 - pb) * st.lb; p.a.x0 = (r0 - pb) * st.lb;
         p.b.k0 = r0 * st.lb; p.b.x0 = c0 * st.lb;
+        p.flags = F_NO_SPLIT;   // in place: a CTA may only read the tile it overwrites
         return launch(st, p, false, L_POTRF_TRSM);
     }
 
@@ -540,8 +565,10 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_POTRF_END", 0, 1 << 20, &p->potrf_end);
     if (p->potrf_nb_end > p->potrf_nb_tail) p->potrf_nb_end = p->potrf_nb_tail;
     if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
-    p->super_tile = p->z ? 16 : 12;
+    p->super_tile = p->z ? 16 : 8;
     knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
+    knob("GS_TILE64", 0, 2, &p->tile64_mode);
+    knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
     *plan = p;
     return GS_OK;
 }

@@ -47,6 +47,7 @@ enum : uint32_t {
     F_MASK_A2 = 1u << 4,
     F_MASK_B2 = 1u << 5,
     F_STORE_UPPER = 1u << 6,   // store only C elements with global row <= col
+    F_NO_SPLIT = 1u << 9,      // host only: C aliases the B operand tile by tile (in-place solve): one CTA per logical tile
     F_LOWER_A = 1u << 8,       // with F_MASK_A: A keeps its LOWER triangle instead (zero where row < col)
     F_REAL_DIAG = 1u << 7,     // complex engine: store Im = 0 on the global diagonal (Hermitian results)
 };
