@@ -314,7 +314,7 @@ def run_ours(args):
     achieved = dom_flop / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else None
     mp = _measured_peaks()
     roofline = {
-        "bound": "tensor", "kernel": ("ctile_engine_kernel<TN>" if cplx else "tile_engine_kernel<TN,TMA>") + " as to_standard.syr2k (FP64 DMMA)",
+        "bound": "tensor", "kernel": ("ctile_engine_kernel<TN>" if cplx else "tile64_engine_kernel<TN> (64x64 CTA tiles, 4 per logical tile)") + " as to_standard.syr2k (FP64 DMMA)",
         "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
         "frac": (achieved / fp64_peak) if achieved else None,
         "traffic": _ncu_traffic("to_standard.syr2k.complex" if cplx else "to_standard.syr2k") if N == (8192 if cplx else 16384) else None,

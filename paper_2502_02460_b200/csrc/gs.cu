@@ -708,6 +708,7 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         p.c_rows = N; p.c_cols = N;
         p.khi_c = kt; p.khi_i = kt; p.kmax = (N + st.bk - 1) / st.bk;
         p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;   // Hermitian: Im(diag) = 0 exactly
+        if (!plan->z && plan->super_tile > 4) p.super = 4;   // four operand panels per tile: smaller super-tiles keep them in L2 (profiles/)
         GS_TRY(launch(st, p, false, L_TOSTD_SYR2K));
     }
     return GS_OK;
