@@ -7,6 +7,7 @@
 #include <cstring>
 
 #include "ctile_engine.cuh"
+#include "ctile_half_engine.cuh"
 #include "tile64_engine.cuh"
 #include "tile_engine.cuh"
 
@@ -99,6 +100,10 @@ inline cudaError_t engine_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(tile64_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, k64SmemBytes);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ctile_half_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kHSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ctile_half_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kHSmemBytes);
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ctile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ctile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
@@ -136,8 +141,16 @@ inline cudaError_t engine64_launch(const EngineParams& p, bool a_nn, cudaStream_
 }
 
 // complex128 engine: operands always go through TMA (a complex row pitch is a multiple of 16 bytes)
-inline cudaError_t cengine_launch(const EngineParams& p, bool a_nn, cudaStream_t stream)
+inline cudaError_t cengine_launch(const EngineParams& p, bool a_nn, bool half, cudaStream_t stream)
 {
+    if (half) {   // two 64 x 32 CTAs per logical tile (ctile_half_engine.cuh)
+        const int g2 = 2 * num_tiles(p);
+        if (g2 <= 0) return cudaSuccess;
+        const cudaError_t e2 = engine_configure();
+        if (e2 != cudaSuccess) return e2;
+        if (a_nn) return launch_pdl(ctile_half_engine_kernel<true>, g2, kCThreads, kHSmemBytes, stream, p);
+        return launch_pdl(ctile_half_engine_kernel<false>, g2, kCThreads, kHSmemBytes, stream, p);
+    }
     const int grid = num_tiles(p);
     if (grid <= 0) return cudaSuccess;
     cudaError_t e = engine_configure();

@@ -65,6 +65,7 @@ struct gs_plan {
     int potrf_tail = 64;
     int potrf_nb_end = 1;            // panel width once at most potrf_end blocks remain
     int potrf_end = 32;
+    int ctile_half = 1;              // complex: two 64 x 32 CTAs per logical tile (3 CTAs/SM) instead of one 64 x 64
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
@@ -196,11 +197,12 @@ gs_status_t launch(Stage& st, EngineParams& p, bool a_nn, int label)
         st.opset[w] = false;
         if (!st.tma) continue;
         CUtensorMap* map = w == 0 ? &p.mapA : w == 1 ? &p.mapB : w == 2 ? &p.mapA2 : &p.mapB2;
-        const int box = st.z ? (st.opm[w] ? 8 : CT) : (st.opm[w] ? 16 : (t64 ? T64 : BN));
+        const bool zhalf = st.z && st.plan->ctile_half != 0;
+        const int box = st.z ? (st.opm[w] ? 8 : ((zhalf && (w & 1)) ? 32 : CT)) : (st.opm[w] ? 16 : (t64 ? T64 : BN));
         if (!make_tensor_map(map, st.opv[w], box, st.z)) return GS_ERR_CUDA;
     }
     LaunchTimer timer(st.plan, label, st.stream);
-    const cudaError_t e = st.z ? cengine_launch(p, a_nn, st.stream)
+    const cudaError_t e = st.z ? cengine_launch(p, a_nn, st.plan->ctile_half != 0, st.stream)
                                : t64 ? engine64_launch(p, a_nn, st.stream) : engine_launch(p, a_nn, st.tma, st.stream);
     if (e != cudaSuccess) return cuda_fail(st.plan, e);
     st.plan->launches += 1;
@@ -568,6 +570,7 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     p->super_tile = p->z ? 16 : 8;
     knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
     knob("GS_TILE64", 0, 2, &p->tile64_mode);
+    knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
     *plan = p;
     return GS_OK;
