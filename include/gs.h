@@ -117,10 +117,10 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 /* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
  * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
  * inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3 there and copies the UPPER
- * triangle of H~ back to host_Htilde (N x N, ld N; it is copied as 1024-column trapezoids, so host
- * entries below the diagonal block of their column panel are left untouched -- callers read the
- * upper triangle only).  The H2D copy of H runs on a plan-owned copy stream beside steps 1-2 and is
- * joined before step 3.  host_U / host_Uinv may be NULL (then they are not copied back).  U^-1 stays
+ * triangle of H~ back to host_Htilde (N x N, ld N; the strictly-lower part of the host buffer is
+ * unspecified -- callers read the upper triangle only).  Copies overlap compute on plan-owned copy
+ * streams that are joined before return: H goes in beside steps 1-2, step 3 is formed in row ranges
+ * whose finished rows go back beside the next range; gs_backtransform_host pipelines column chunks.  host_U / host_Uinv may be NULL (then they are not copied back).  U^-1 stays
  * in the scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in,
  * forms C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report
  * numerical failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte

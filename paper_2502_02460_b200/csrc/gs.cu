@@ -15,6 +15,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
+#include <functional>
 #include <new>
 #include <vector>
 
@@ -58,8 +60,10 @@ struct gs_plan {
     // from and joined back into the caller's stream with events inside every call that uses it
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_rows = nullptr, ev_join = nullptr;
-    cudaStream_t copy = nullptr;     // host-buffer entry points: H2D of H overlaps the factorisation of S
+    cudaStream_t copy = nullptr;     // host-buffer entry points: H2D copies beside compute
+    cudaStream_t copy_out = nullptr; // host-buffer entry points: D2H copies beside compute
     cudaEvent_t ev_copy = nullptr;
+    std::vector<cudaEvent_t> ev_pool;   // per-chunk events of the host-buffer entry points
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
     int potrf_tail = 64;
@@ -74,7 +78,6 @@ struct gs_plan {
 namespace {
 
 constexpr size_t kInfoBytes = 256;
-constexpr int64_t kHostPanel = 1024;   // column-block width of the trapezoidal D2H copy of H~ (gs_reduce_host)
 constexpr int KPB = 8;   // pipeline k-steps per block: 128 / 16 (real) = 64 / 8 (complex)
 static_assert(LB / BK == KPB && CLB / CBK == KPB && CT == CLB, "block / k-slab ratio");
 
@@ -586,6 +589,8 @@ gs_status_t gs_plan_destroy(gs_plan_t* plan)
     if (plan->side != nullptr) cudaStreamDestroy(plan->side);
     if (plan->ev_copy != nullptr) cudaEventDestroy(plan->ev_copy);
     if (plan->copy != nullptr) cudaStreamDestroy(plan->copy);
+    if (plan->copy_out != nullptr) cudaStreamDestroy(plan->copy_out);
+    for (cudaEvent_t e : plan->ev_pool) cudaEventDestroy(e);
     delete plan;
     return GS_OK;
 }
@@ -676,7 +681,39 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
 //   G  = T V                (upper x upper = upper; N^3/3 flop)   -> workspace
 //   H~ = V^T G + G^T V      (upper triangle only; SYR2K-shaped, operands triangular; 2N^3/3 flop)
 // N^3 flop in total instead of the 4N^3/3 of forming W = H V in full.
-gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, void* Htilde_, void* cuda_stream)
+// Row ranges of the SYR2K-shaped launch for the host-buffer path: splits (in blocks, ascending) and a hook
+// that is called after range r = [splits[r], splits[r+1]) has been enqueued.
+struct RowRanges {
+    std::vector<int> splits;
+    std::function<gs_status_t(int)> after;
+};
+
+// rows [I0, I1) (in blocks) of H~ = V^H G + G^H V, upper tiles; whole = the plain triangular launch
+static gs_status_t to_standard_rows(gs_plan* plan, Stage& st, const MatView& vV, const MatView& vG, void* Htilde_, int I0, int I1, bool whole)
+{
+    const int N = int(plan->N), nblk = plan->nblk, kt = KPB;
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vV, false) || !set_operand(st, p, 1, vG, false) || !set_operand(st, p, 2, vG, false) ||
+        !set_operand(st, p, 3, vV, false))
+        return GS_ERR_CUDA;
+    p.C = static_cast<double*>(Htilde_); p.ldc = N;
+    p.c_rows = N; p.c_cols = N;
+    p.kmax = (N + st.bk - 1) / st.bk;
+    p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;   // Hermitian: Im(diag) = 0 exactly
+    if (whole) {
+        p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_ROW_DESC;
+        p.khi_c = kt; p.khi_i = kt;
+        if (!plan->z && plan->super_tile > 4) p.super = 4;   // four operand panels per tile: smaller super-tiles keep them in L2 (profiles/)
+    } else {
+        p.tiles_m = I1 - I0; p.tiles_n = nblk - I0; p.order = ORDER_TRAPEZOID;
+        p.c_row0 = I0 * st.lb; p.c_col0 = I0 * st.lb;
+        p.a.x0 = p.b.x0 = p.a2.x0 = p.b2.x0 = I0 * st.lb;
+        p.khi_c = kt * (I0 + 1); p.khi_i = kt;
+    }
+    return launch(st, p, false, L_TOSTD_SYR2K);
+}
+
+static gs_status_t to_standard_impl(gs_plan* plan, const void* H_, const void* Uinv_, void* Htilde_, void* cuda_stream, RowRanges* ranges)
 {
     GS_TRY(check_ready(plan));
     if (H_ == nullptr || Uinv_ == nullptr || Htilde_ == nullptr || Htilde_ == H_ || Htilde_ == Uinv_ ||
@@ -701,20 +738,37 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
         p.flags = F_MASK_A | F_LOWER_A | F_HALF_DIAG_A | F_MASK_B;
         GS_TRY(launch(st, p, false, L_TOSTD_G));
     }
-    {
-        EngineParams p = blank_params(plan);
-        if (!set_operand(st, p, 0, vV, false) || !set_operand(st, p, 1, vG, false) || !set_operand(st, p, 2, vG, false) ||
-            !set_operand(st, p, 3, vV, false))
-            return GS_ERR_CUDA;
-        p.C = static_cast<double*>(Htilde_); p.ldc = N;
-        p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_ROW_DESC;
-        p.c_rows = N; p.c_cols = N;
-        p.khi_c = kt; p.khi_i = kt; p.kmax = (N + st.bk - 1) / st.bk;
-        p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;   // Hermitian: Im(diag) = 0 exactly
-        if (!plan->z && plan->super_tile > 4) p.super = 4;   // four operand panels per tile: smaller super-tiles keep them in L2 (profiles/)
-        GS_TRY(launch(st, p, false, L_TOSTD_SYR2K));
+    if (ranges == nullptr) return to_standard_rows(plan, st, vV, vG, Htilde_, 0, nblk, true);
+    // host-buffer path: the triangle is formed in row ranges of about equal work so that the D2H copy of a
+    // finished range runs beside the next one; top rows first -- they are the long ones, the copy that
+    // is left exposed at the end is the short bottom trapezoid
+    for (int r = 0; r + 1 < int(ranges->splits.size()); ++r) {
+        GS_TRY(to_standard_rows(plan, st, vV, vG, Htilde_, ranges->splits[r], ranges->splits[r + 1], false));
+        GS_TRY(ranges->after(r));
     }
     return GS_OK;
+}
+
+gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, void* Htilde_, void* cuda_stream)
+{
+    return to_standard_impl(plan, H_, Uinv_, Htilde_, cuda_stream, nullptr);
+}
+
+// C[:, col0 : col0+ncols] = V * C~[:, col0 : col0+ncols]
+static gs_status_t backtransform_cols(gs_plan* plan, const void* Uinv_, const void* Ctilde_, void* C_, int col0, int ncols, cudaStream_t stream)
+{
+    const int N = int(plan->N);
+    Stage st = make_stage(plan, stream);
+    const size_t off = size_t(col0) * size_t(N) * plan->es;
+    const MatView vV{Uinv_, N, N, N}, vC{static_cast<const unsigned char*>(Ctilde_) + off, N, ncols, N};
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
+    p.C = reinterpret_cast<double*>(static_cast<unsigned char*>(C_) + off); p.ldc = N;
+    p.tiles_m = plan->nblk; p.tiles_n = (ncols + st.lb - 1) / st.lb; p.order = ORDER_ROW;
+    p.c_rows = N; p.c_cols = ncols;
+    p.klo_i = KPB; p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
+    p.flags = F_MASK_A;
+    return launch(st, p, true, L_BACK_TRMM);
 }
 
 gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Ctilde_, void* C_, void* cuda_stream)
@@ -724,18 +778,7 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
     if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || C_ == Ctilde_ || C_ == Uinv_ || !aligned16(Uinv_) ||
         !aligned16(Ctilde_) || !aligned16(C_))
         return GS_ERR_INVALID_ARG;
-    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    const int N = int(plan->N), nev = int(plan->nev);
-    Stage st = make_stage(plan, stream);
-    const MatView vV{Uinv_, N, N, N}, vC{Ctilde_, N, nev, N};
-    EngineParams p = blank_params(plan);
-    if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
-    p.C = static_cast<double*>(C_); p.ldc = N;
-    p.tiles_m = plan->nblk; p.tiles_n = (nev + st.lb - 1) / st.lb; p.order = ORDER_ROW;
-    p.c_rows = N; p.c_cols = nev;
-    p.klo_i = KPB; p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
-    p.flags = F_MASK_A;
-    return launch(st, p, true, L_BACK_TRMM);
+    return backtransform_cols(plan, Uinv_, Ctilde_, C_, 0, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
 }
 
 // P(i,j) = sum_l f_l conj(C(i,l)) C(j,l) = (X^H X)(i,j) with X(l,i) = sqrt(f_l) C(i,l): one transpose-and-scale
@@ -797,15 +840,48 @@ gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes)
     return GS_OK;
 }
 
+// Row ranges (in blocks) of about equal work for the split SYR2K launch of the host path: row I of the
+// triangle costs (I + 1)(n - I) tile-steps.
+static std::vector<int> host_row_splits(const gs_plan* plan)
+{
+    const int n = plan->nblk, parts = n >= 16 ? 4 : 1;
+    std::vector<int> s{0};
+    double total = 0.0;
+    for (int I = 0; I < n; ++I) total += double(I + 1) * double(n - I);
+    double acc = 0.0;
+    for (int I = 0; I < n; ++I) {
+        acc += double(I + 1) * double(n - I);
+        if (int(s.size()) < parts && acc >= total * double(s.size()) / parts) s.push_back(I + 1);
+    }
+    if (s.back() != n) s.push_back(n);
+    return s;
+}
+
 gs_status_t gs_reduce_host_d2h_bytes(const gs_plan_t* plan, size_t* bytes)
 {
     if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
+    const std::vector<int> sp = host_row_splits(plan);
     size_t b = 0;
-    for (int64_t c0 = 0; c0 < plan->N; c0 += kHostPanel) {
-        const int64_t cols = plan->N - c0 < kHostPanel ? plan->N - c0 : kHostPanel;
-        b += size_t(c0 + cols) * size_t(cols) * plan->es;
+    for (size_t r = 0; r + 1 < sp.size(); ++r) {
+        const int64_t r0 = int64_t(sp[r]) * plan->lb, r1 = std::min<int64_t>(int64_t(sp[r + 1]) * plan->lb, plan->N);
+        b += size_t(r1 - r0) * size_t(plan->N - r0) * plan->es;
     }
     *bytes = b;
+    return GS_OK;
+}
+
+static gs_status_t ensure_copy_streams(gs_plan* plan, size_t events)
+{
+    if (plan->copy == nullptr) {
+        GS_CUDA(plan, cudaStreamCreateWithFlags(&plan->copy, cudaStreamNonBlocking));
+        GS_CUDA(plan, cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking));
+        GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_copy, cudaEventDisableTiming));
+    }
+    while (plan->ev_pool.size() < events) {
+        cudaEvent_t e;
+        GS_CUDA(plan, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        plan->ev_pool.push_back(e);
+    }
     return GS_OK;
 }
 
@@ -823,32 +899,41 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     const size_t mat = need / 4;
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
     void *dS = base, *dH = base + mat, *dV = base + 2 * mat, *dHt = base + 3 * mat;
-    if (plan->copy == nullptr) {
-        GS_CUDA(plan, cudaStreamCreateWithFlags(&plan->copy, cudaStreamNonBlocking));
-        GS_CUDA(plan, cudaEventCreateWithFlags(&plan->ev_copy, cudaEventDisableTiming));
-    }
-    // S first on the caller's stream; H (not needed before step 3) and the clearing of the H~ buffer go
-    // on the plan's copy stream and overlap steps 1-2; the copy stream is forked from / joined into `stream`
+    RowRanges rr;
+    rr.splits = host_row_splits(plan);
+    GS_TRY(ensure_copy_streams(plan, rr.splits.size()));
+    // S first on the caller's stream; H (not needed before step 3) goes on the plan's copy stream and
+    // overlaps steps 1-2; both copy streams are forked from / joined into `stream`
     GS_CUDA(plan, cudaMemcpyAsync(dS, host_S, bytes, cudaMemcpyHostToDevice, stream));
     GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));          // H follows S on the link, not beside it
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
+    GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_copy, 0));
     GS_CUDA(plan, cudaMemcpyAsync(dH, host_H, bytes, cudaMemcpyHostToDevice, plan->copy));
     GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy));
     gs_status_t rc = gs_cholesky(plan, dS, stream);
     if (rc == GS_OK) rc = gs_invert_triangular(plan, dS, dV, stream);
     GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_copy, 0));   // join, also on failure
     GS_TRY(rc);
-    GS_TRY(gs_to_standard(plan, dH, dV, dHt, stream));
-    if (host_U) GS_CUDA(plan, cudaMemcpyAsync(host_U, dS, bytes, cudaMemcpyDeviceToHost, stream));
-    if (host_Uinv) GS_CUDA(plan, cudaMemcpyAsync(host_Uinv, dV, bytes, cudaMemcpyDeviceToHost, stream));
-    // H~: only the upper triangle exists; copy it as column-block trapezoids (kHostPanel columns each)
-    for (int64_t c0 = 0; c0 < plan->N; c0 += kHostPanel) {
-        const int64_t cols = plan->N - c0 < kHostPanel ? plan->N - c0 : kHostPanel;
-        const int64_t rows = c0 + cols;   // rows 0 .. last column of the block
-        const size_t off = size_t(c0) * size_t(plan->N) * plan->es, pitch = size_t(plan->N) * plan->es;
-        GS_CUDA(plan, cudaMemcpy2DAsync(static_cast<unsigned char*>(host_Htilde) + off, pitch, static_cast<unsigned char*>(dHt) + off,
-                                        pitch, size_t(rows) * plan->es, size_t(cols), cudaMemcpyDeviceToHost, stream));
+    if (host_U || host_Uinv) {   // U, U^-1 are final once steps 1-2 are done: they go back beside step 3
+        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[rr.splits.size() - 1], stream));
+        GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_pool[rr.splits.size() - 1], 0));
+        if (host_U) GS_CUDA(plan, cudaMemcpyAsync(host_U, dS, bytes, cudaMemcpyDeviceToHost, plan->copy_out));
+        if (host_Uinv) GS_CUDA(plan, cudaMemcpyAsync(host_Uinv, dV, bytes, cudaMemcpyDeviceToHost, plan->copy_out));
     }
+    // step 3 in row ranges; the finished rows of H~ (upper trapezoid of each range) go back on the D2H stream
+    rr.after = [&](int r) -> gs_status_t {
+        const int64_t r0 = int64_t(rr.splits[r]) * plan->lb, r1 = std::min<int64_t>(int64_t(rr.splits[r + 1]) * plan->lb, plan->N);
+        const size_t off = (size_t(r0) + size_t(r0) * size_t(plan->N)) * plan->es, pitch = size_t(plan->N) * plan->es;
+        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[r], stream));
+        GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_pool[r], 0));
+        GS_CUDA(plan, cudaMemcpy2DAsync(static_cast<unsigned char*>(host_Htilde) + off, pitch, static_cast<unsigned char*>(dHt) + off,
+                                        pitch, size_t(r1 - r0) * plan->es, size_t(plan->N - r0), cudaMemcpyDeviceToHost, plan->copy_out));
+        return GS_OK;
+    };
+    rc = to_standard_impl(plan, dH, dV, dHt, stream, &rr);
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy_out));
+    GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_copy, 0));   // join the D2H stream
+    GS_TRY(rc);
     int64_t info = 0;
     return gs_last_info(plan, stream, &info);
 }
@@ -865,13 +950,33 @@ gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void
     if (host_Ctilde == nullptr || host_C == nullptr) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const size_t mat = need / 4;
-    const size_t cbytes = size_t(plan->N) * size_t(plan->nev) * plan->es;
     unsigned char* base = static_cast<unsigned char*>(dev_scratch);
     // U^-1 was left at base + 2*mat by gs_reduce_host; C~ and C reuse the S and H slots
-    void *dV = base + 2 * mat, *dCt = base, *dC = base + mat;
-    GS_CUDA(plan, cudaMemcpyAsync(dCt, host_Ctilde, cbytes, cudaMemcpyHostToDevice, stream));
-    GS_TRY(gs_backtransform(plan, dV, dCt, dC, stream));
-    GS_CUDA(plan, cudaMemcpyAsync(host_C, dC, cbytes, cudaMemcpyDeviceToHost, stream));
+    unsigned char *dV = base + 2 * mat, *dCt = base, *dC = base + mat;
+    // column chunks: H2D of chunk c+1, the product of chunk c and the D2H of chunk c-1 run side by side
+    const int nev = int(plan->nev);
+    int chunk = ((nev + 3) / 4 + plan->lb - 1) / plan->lb * plan->lb;
+    if (chunk < 4 * plan->lb) chunk = nev;
+    const int nchunks = (nev + chunk - 1) / chunk;
+    GS_TRY(ensure_copy_streams(plan, size_t(2 * nchunks)));
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));
+    GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
+    GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_copy, 0));
+    gs_status_t rc = GS_OK;
+    for (int c = 0; c < nchunks && rc == GS_OK; ++c) {
+        const int col0 = c * chunk, ncols = std::min(chunk, nev - col0);
+        const size_t off = size_t(col0) * size_t(plan->N) * plan->es, cb = size_t(ncols) * size_t(plan->N) * plan->es;
+        GS_CUDA(plan, cudaMemcpyAsync(dCt + off, static_cast<const unsigned char*>(host_Ctilde) + off, cb, cudaMemcpyHostToDevice, plan->copy));
+        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[2 * c], plan->copy));
+        GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_pool[2 * c], 0));
+        rc = backtransform_cols(plan, dV, dCt, dC, col0, ncols, stream);
+        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[2 * c + 1], stream));
+        GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_pool[2 * c + 1], 0));
+        GS_CUDA(plan, cudaMemcpyAsync(static_cast<unsigned char*>(host_C) + off, dC + off, cb, cudaMemcpyDeviceToHost, plan->copy_out));
+    }
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy_out));
+    GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_copy, 0));   // join (the H2D stream was joined chunk by chunk)
+    GS_TRY(rc);
     int64_t info = 0;
     return gs_last_info(plan, stream, &info);
 }
