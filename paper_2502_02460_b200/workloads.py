@@ -96,10 +96,28 @@ def points(N: int, box: float, gen: torch.Generator, device="cpu") -> torch.Tens
     return torch.rand((N, 3), dtype=torch.float64, device=device, generator=gen) * box
 
 
+def mirror_upper_(A: torch.Tensor, chunk: int = 4096) -> torch.Tensor:
+    """In place: the strictly-lower triangle becomes the (conjugate) transpose of the strictly-upper one;
+    a complex diagonal is made exactly real.  Block by block, to bound temporaries."""
+    N = A.shape[0]
+    for i0 in range(0, N, chunk):
+        i1 = min(N, i0 + chunk)
+        blk = A[i0:i1, i0:i1]
+        up = torch.triu(blk, 1)
+        dg = torch.diag(torch.diagonal(blk).real.to(A.dtype))
+        blk.copy_(up + up.conj().t() + dg)
+        if i1 < N:
+            A[i1:, i0:i1] = A[i0:i1, i1:].conj().t()
+    return A
+
+
 def overlap(r: torch.Tensor, jitter: float = 1e-3, chunk: int = 2048) -> torch.Tensor:
     """S_ij = exp(-0.5 |r_i - r_j|^2) + jitter * delta_ij, column-major, exactly symmetric.
 
-    Differences are formed explicitly (not via |a|^2+|b|^2-2ab) so S_ij == S_ji bit for bit.
+    The squared distances are bitwise symmetric (explicit differences, not |a|^2+|b|^2-2ab), but a
+    vectorised exp need not return the same bits for the same argument at two places of a tensor
+    (seen on the GPU box's host CPU: S_ij and S_ji a few 1e-10 apart in the first call of a fresh
+    process), so the lower triangle is mirrored from the upper one explicitly.
     """
     N = r.shape[0]
     S = colmajor_empty(N, N, device=r.device)
@@ -110,6 +128,7 @@ def overlap(r: torch.Tensor, jitter: float = 1e-3, chunk: int = 2048) -> torch.T
             diff = r[i0:i1, c].unsqueeze(1) - r[:, c].unsqueeze(0)
             d2 += diff * diff
         S[i0:i1, :] = torch.exp(-0.5 * d2)
+    mirror_upper_(S)
     S.diagonal().add_(jitter)
     return S
 
@@ -134,7 +153,8 @@ def hamiltonian(S: torch.Tensor, gen: torch.Generator, chunk: int = 4096) -> tor
             H[i1:, i0:i1] = H[i0:i1, i1:].t()
     H.mul_(0.1).add_(1.0).mul_(S).neg_()
     H.diagonal().add_(d)
-    return H
+    # step 3 reads one triangle of H, the oracle the whole matrix: the two must agree bit for bit
+    return mirror_upper_(H)
 
 
 def phase_factor(x: torch.Tensor, k: float = PHASE_K) -> torch.Tensor:
@@ -168,6 +188,10 @@ def make_pencil(N: int, box: float, seed: int, complex: bool = False, device="cp
         S = to_colmajor(S.to(torch.complex128) * P)
         H = to_colmajor(H.to(torch.complex128) * P)
         # diagonals are exactly real by construction (P_ii = 1)
+        mirror_upper_(S)
+        mirror_upper_(H)
+    if N <= 4096 and not (torch.equal(H, H.conj().t()) and torch.equal(S, S.conj().t())):
+        raise RuntimeError("workloads.make_pencil: H or S is not exactly Hermitian")
     return Pencil(N, complex, H, S, r)
 
 
