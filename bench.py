@@ -405,7 +405,7 @@ def run_ours(args):
         e2e_sec = max_over_ranks((t1 - t0) / e2e_steps)
         esz = 16 if cplx else 8
         e2e = {"value": world * flops["total"] / e2e_sec / 1e12, "unit": UNIT,
-               "h2d_bytes_per_step": (2 * N * N + N * nev) * esz, "d2h_bytes_per_step": plan.reduce_host_d2h_bytes() + N * nev * esz,
+               "h2d_bytes_per_step": plan.reduce_host_h2d_bytes() + N * nev * esz, "d2h_bytes_per_step": plan.reduce_host_d2h_bytes() + N * nev * esz,
                "ms_per_step": e2e_sec * 1e3, "steps": e2e_steps,
                "api": "gs_reduce_host + gs_backtransform_host (pinned host buffers in, H~ and C out)"}
         if checks is not None:

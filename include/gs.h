@@ -116,7 +116,9 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 
 /* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
  * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
- * inside [dev_scratch, dev_scratch + scratch_bytes), runs steps 1-3 there and copies the UPPER
+ * inside [dev_scratch, dev_scratch + scratch_bytes) -- only the triangles the steps reference: the
+ * UPPER triangle of host_S and the LOWER triangle of host_H (both with the diagonal, in column
+ * chunks; the other triangle of either host buffer is never read) --, runs steps 1-3 there and copies the UPPER
  * triangle of H~ back to host_Htilde (N x N, ld N; the strictly-lower part of the host buffer is
  * unspecified -- callers read the upper triangle only).  Copies overlap compute on plan-owned copy
  * streams that are joined before return: H goes in beside steps 1-2, step 3 is formed in row ranges
@@ -124,8 +126,10 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
  * in the scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in,
  * forms C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report
  * numerical failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte
- * aligned.  gs_reduce_host_d2h_bytes reports the bytes gs_reduce_host copies back for H~. */
+ * aligned.  gs_reduce_host_h2d_bytes / gs_reduce_host_d2h_bytes report the bytes gs_reduce_host
+ * copies in for S and H / back for H~. */
 gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_reduce_host_h2d_bytes(const gs_plan_t* plan, size_t* bytes);
 gs_status_t gs_reduce_host_d2h_bytes(const gs_plan_t* plan, size_t* bytes);
 gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host_S,
                            void* host_U, void* host_Uinv, void* host_Htilde,

@@ -854,6 +854,13 @@ static std::vector<int> host_row_splits(const gs_plan* plan)
         if (int(s.size()) < parts && acc >= total * double(s.size()) / parts) s.push_back(I + 1);
     }
     if (s.back() != n) s.push_back(n);
+    // the copy of the last range is the one left exposed: keep halving that range until it is a few block
+    // rows (its trapezoid is then a few MB)
+    if (parts > 1) {
+        s.pop_back();
+        while (n - s.back() > 8) s.push_back(s.back() + (n - s.back() + 1) / 2);
+        s.push_back(n);
+    }
     return s;
 }
 
@@ -867,6 +874,40 @@ gs_status_t gs_reduce_host_d2h_bytes(const gs_plan_t* plan, size_t* bytes)
         b += size_t(r1 - r0) * size_t(plan->N - r0) * plan->es;
     }
     *bytes = b;
+    return GS_OK;
+}
+
+// Host -> device copy of one triangle (diagonal included) of an N x N column-major matrix in column
+// chunks: chunk [c0, c1) moves rows [0, c1) (upper) or [c0, N) (lower) of its columns.
+constexpr int64_t kTriangleChunkCols = 512;
+
+static size_t triangle_h2d_bytes(const gs_plan* plan)
+{
+    size_t b = 0;
+    for (int64_t c0 = 0; c0 < plan->N; c0 += kTriangleChunkCols) {
+        const int64_t c1 = std::min<int64_t>(c0 + kTriangleChunkCols, plan->N);
+        b += size_t(c1) * size_t(c1 - c0) * plan->es;   // the lower trapezoids have the same sizes, mirrored
+    }
+    return b;
+}
+
+static gs_status_t copy_triangle_h2d(gs_plan* plan, void* dev, const void* host, bool upper, cudaStream_t stream)
+{
+    const size_t pitch = size_t(plan->N) * plan->es;
+    for (int64_t c0 = 0; c0 < plan->N; c0 += kTriangleChunkCols) {
+        const int64_t c1 = std::min<int64_t>(c0 + kTriangleChunkCols, plan->N);
+        const int64_t r0 = upper ? 0 : c0, r1 = upper ? c1 : plan->N;
+        const size_t off = size_t(r0) * plan->es + size_t(c0) * pitch;
+        GS_CUDA(plan, cudaMemcpy2DAsync(static_cast<unsigned char*>(dev) + off, pitch, static_cast<const unsigned char*>(host) + off, pitch,
+                                        size_t(r1 - r0) * plan->es, size_t(c1 - c0), cudaMemcpyHostToDevice, stream));
+    }
+    return GS_OK;
+}
+
+gs_status_t gs_reduce_host_h2d_bytes(const gs_plan_t* plan, size_t* bytes)
+{
+    if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
+    *bytes = 2 * triangle_h2d_bytes(plan);   // S upper + H lower
     return GS_OK;
 }
 
@@ -904,11 +945,14 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     GS_TRY(ensure_copy_streams(plan, rr.splits.size()));
     // S first on the caller's stream; H (not needed before step 3) goes on the plan's copy stream and
     // overlaps steps 1-2; both copy streams are forked from / joined into `stream`
-    GS_CUDA(plan, cudaMemcpyAsync(dS, host_S, bytes, cudaMemcpyHostToDevice, stream));
+    // Only the triangles the steps reference cross the link (column chunks, trapezoids): the upper one of
+    // S (step 1) and the lower one of H (step 3) -- about half of each matrix.  What stays unwritten in
+    // the scratch is never read.
+    GS_TRY(copy_triangle_h2d(plan, dS, host_S, true, stream));
     GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));          // H follows S on the link, not beside it
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_copy, 0));
-    GS_CUDA(plan, cudaMemcpyAsync(dH, host_H, bytes, cudaMemcpyHostToDevice, plan->copy));
+    GS_TRY(copy_triangle_h2d(plan, dH, host_H, false, plan->copy));
     GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy));
     gs_status_t rc = gs_cholesky(plan, dS, stream);
     if (rc == GS_OK) rc = gs_invert_triangular(plan, dS, dV, stream);
@@ -954,17 +998,24 @@ gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void
     // U^-1 was left at base + 2*mat by gs_reduce_host; C~ and C reuse the S and H slots
     unsigned char *dV = base + 2 * mat, *dCt = base, *dC = base + mat;
     // column chunks: H2D of chunk c+1, the product of chunk c and the D2H of chunk c-1 run side by side
-    const int nev = int(plan->nev);
-    int chunk = ((nev + 3) / 4 + plan->lb - 1) / plan->lb * plan->lb;
-    if (chunk < 4 * plan->lb) chunk = nev;
-    const int nchunks = (nev + chunk - 1) / chunk;
+    // the first H2D and the last D2H are the exposed ones: those two chunks are narrow (two block columns)
+    const int nev = int(plan->nev), lb = plan->lb;
+    const int chunk = ((nev + 3) / 4 + lb - 1) / lb * lb;
+    std::vector<int> cuts{0};
+    if (nev >= 16 * lb) {
+        cuts.push_back(2 * lb);
+        while (nev - 2 * lb - cuts.back() > chunk) cuts.push_back(cuts.back() + chunk);
+        if (cuts.back() < nev - 2 * lb) cuts.push_back(nev - 2 * lb);
+    }
+    cuts.push_back(nev);
+    const int nchunks = int(cuts.size()) - 1;
     GS_TRY(ensure_copy_streams(plan, size_t(2 * nchunks)));
     GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_copy, 0));
     gs_status_t rc = GS_OK;
     for (int c = 0; c < nchunks && rc == GS_OK; ++c) {
-        const int col0 = c * chunk, ncols = std::min(chunk, nev - col0);
+        const int col0 = cuts[c], ncols = cuts[c + 1] - cuts[c];
         const size_t off = size_t(col0) * size_t(plan->N) * plan->es, cb = size_t(ncols) * size_t(plan->N) * plan->es;
         GS_CUDA(plan, cudaMemcpyAsync(dCt + off, static_cast<const unsigned char*>(host_Ctilde) + off, cb, cudaMemcpyHostToDevice, plan->copy));
         GS_CUDA(plan, cudaEventRecord(plan->ev_pool[2 * c], plan->copy));

@@ -28,7 +28,7 @@ STATUS_NAMES = {
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
     "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
-    "gs_reduce_host_scratch_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
+    "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
 )
@@ -78,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.gs_density_matrix.argtypes = [vp, vp, vp, vp, vp]
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
         L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        L.gs_reduce_host_h2d_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host_d2h_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
         L.gs_backtransform_host.argtypes = [vp, vp, vp, vp, sz, vp]
@@ -215,6 +216,11 @@ class Plan:
     def host_scratch_bytes(self) -> int:
         n = ctypes.c_size_t(0)
         self._check(lib().gs_reduce_host_scratch_bytes(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    def reduce_host_h2d_bytes(self) -> int:
+        n = ctypes.c_size_t(0)
+        self._check(lib().gs_reduce_host_h2d_bytes(self._h, ctypes.byref(n)))
         return int(n.value)
 
     def reduce_host_d2h_bytes(self) -> int:

@@ -172,9 +172,9 @@ def test_argument_errors():
 @pytest.mark.parametrize("N,cplx", [(300, False), (2500, False), (1100, True)])
 def test_host_buffer_entry_points_match_the_device_path(N, cplx):
     """gs_reduce_host / gs_backtransform_host (pinned host buffers, copies inside) give bit for bit what
-    the device-pointer calls give: same kernels, same order.  N = 2500 spans three 1024-column D2H panels."""
+    the device-pointer calls give: same kernels, same order.  N = 2500 spans five 512-column H2D chunks."""
     gs = _gs()
-    nev = N // 3
+    nev = N // 3 if N != 2500 else 2200      # 2200 columns: the back-transform runs in six column chunks
     dt = torch.complex128 if cplx else torch.float64
     p = wl.small_pencil(N, seed=77, complex=cplx, device="cuda")
     plan, U, V, Ht = gs.generalized_to_standard(p.H, p.S, nev)
@@ -192,12 +192,20 @@ def test_host_buffer_entry_points_match_the_device_path(N, cplx):
     hH, hS, hCt = host(N, N, p.H), host(N, N, p.S), host(N, nev, Ct)
     hU, hV, hHt, hC = host(N, N), host(N, N), host(N, N), host(N, nev)
     hHt.fill_(-9.0)
-    scratch = torch.empty(plan.host_scratch_bytes(), dtype=torch.uint8, device="cuda")
+    # only the upper triangle of S and the lower triangle of H cross the link: the other triangles of the
+    # host buffers and whatever the scratch held before must never be read (NaN would spread)
+    nan = float("nan")
+    hS.t()[torch.tril(torch.ones(N, N, dtype=torch.bool), -1)] = nan
+    hH.t()[torch.triu(torch.ones(N, N, dtype=torch.bool), 1)] = nan
+    scratch = torch.full((plan.host_scratch_bytes(),), 0xFF, dtype=torch.uint8, device="cuda")   # all-ones bytes = NaN
     plan.reduce_host(hH, hS, hU, hV, hHt, scratch)
     plan.backtransform_host(hCt, hC, scratch)
     assert torch.equal(torch.triu(hU.t()), torch.triu(U.cpu()))
     assert torch.equal(torch.triu(hV.t()), torch.triu(V.cpu()))
     assert torch.equal(torch.triu(hHt.t()), torch.triu(Ht.cpu()))
     assert torch.equal(hC.t(), C.cpu())
-    assert 0 < plan.reduce_host_d2h_bytes() <= N * N * (16 if cplx else 8)
+    assert torch.count_nonzero(torch.tril(hU.t(), -1)) == 0 and torch.count_nonzero(torch.tril(hV.t(), -1)) == 0
+    esz = 16 if cplx else 8
+    assert 0 < plan.reduce_host_d2h_bytes() <= N * N * esz
+    assert N * (N + 1) * esz <= plan.reduce_host_h2d_bytes() <= (N * N + 512 * N) * esz
     plan.close()
