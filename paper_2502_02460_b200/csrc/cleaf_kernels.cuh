@@ -118,6 +118,24 @@ __device__ __forceinline__ void cleaf_invert_upper(const CLeafSmem& s, int tx, i
     __syncthreads();
 }
 
+// One register row group of the fused factor-and-invert step (see leaf_update_row in leaf_kernels.cuh);
+// rr = a(j,row) as published, the multiplier is conj(rr) / d.
+__device__ __forceinline__ void cleaf_update_row(double2 (&a)[4][4], int jr, int r, const double2* rb, double2 rr, double invd,
+                                                 double2 pj, bool rowact, int tx, int ty, int jo)
+{
+    const double2 ri = make_double2(rr.x * invd, -rr.y * invd);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        if (c < jr) {
+            if (rowact) cfnma(a[r][c], ri, rb[tx + 16 * c]);
+        } else if (c == jr) {
+            if (rowact && ((tx <= jo) || (r == jr && tx >= ty))) cfnma(a[r][c], ri, pj);
+        } else if (c >= r) {
+            if (rowact && ((c > r) || (tx >= ty))) cfnma(a[r][c], ri, rb[tx + 16 * c]);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(kCLeafThreads, 1)
 potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2* __restrict__ Winv, long long ldw, int* info)
 {
@@ -138,7 +156,10 @@ potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2
 #pragma unroll
         for (int c = 0; c < 4; ++c) a[r][c] = s.U[ty + 16 * r + (tx + 16 * c) * CLP];
 
-    // step j: d_j = Re a(j,j);  a(i,c) -= conj(a(j,i)) a(j,c) / d_j  (j < i <= c);  U(j,c) = a(j,c) / sqrt(d_j)
+    // One sweep forms U_kk and U_kk^-1 (leaf_kernels.cuh, potrf_leaf_kernel): S = L D L^H, U = D^1/2 L^H,
+    // Y = L^-1 (unit lower, kept in the strictly-lower register positions), U^-1 = Y^H D^-1/2.
+    //   step j: d_j = Re a(j,j), l_i = conj(a(j,i)) / d_j for i > j;
+    //           a(i,c) -= l_i a(j,c) (c >= i);  Y(i,c) -= l_i Y(j,c) (c < j);  Y(i,j) = -l_i.
 #pragma unroll
     for (int jr = 0; jr < 4; ++jr) {
 #pragma unroll 1
@@ -147,7 +168,7 @@ potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2
             double2* rb = s.rowbuf + (j & 1) * CLB;
             if (ty == jo) {
 #pragma unroll
-                for (int c = jr; c < 4; ++c) rb[tx + 16 * c] = a[jr][c];
+                for (int c = 0; c < 4; ++c) rb[tx + 16 * c] = a[jr][c];
             }
             __syncthreads();
             const double d = rb[j].x;
@@ -157,17 +178,10 @@ potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2
             }
             if (t == 0) s.dvec[j] = d;
             const double invd = 1.0 / d;
+            const double2 pj = (tx == jo) ? make_double2(1.0, 0.0) : rb[tx + 16 * jr];
 #pragma unroll
-            for (int r = jr; r < 4; ++r) {
-                const bool rowact = (r > jr) || (ty > jo);
-                const double2 rr = rb[ty + 16 * r];
-                const double2 ri = make_double2(rr.x * invd, -rr.y * invd);   // conj(a(j,row)) / d
-#pragma unroll
-                for (int c = r; c < 4; ++c) {
-                    const bool colact = (c > r) || (tx >= ty);
-                    if (rowact && colact) cfnma(a[r][c], ri, rb[tx + 16 * c]);
-                }
-            }
+            for (int r = jr; r < 4; ++r)
+                cleaf_update_row(a, jr, r, rb, rb[ty + 16 * r], invd, pj, (r > jr) || (ty > jo), tx, ty, jo);
         }
     }
     __syncthreads();
@@ -188,8 +202,20 @@ potrf_cleaf_kernel(double2* __restrict__ S, long long ld, int N, int j0, double2
         }
     __syncthreads();
     cleaf_store_all(s, blk, ld, nb, t);
+    __syncthreads();   // the image is rewritten next
 
-    cleaf_invert_upper(s, tx, ty);
+    // W = U^-1 = Y^H D^-1/2: the register at (row, col), row > col, is conj(W(col, row)) / dinv[row]
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            double2 w = make_double2(0.0, 0.0);
+            if (row == col) w.x = s.dinv[row].x;
+            else if (row > col) { const double sc = s.dinv[row].x; w = make_double2(a[r][c].x * sc, -a[r][c].y * sc); }
+            s.U[col + row * CLP] = w;
+        }
+    __syncthreads();
     cleaf_store_all(s, Winv, ldw, CLB, t);
 }
 

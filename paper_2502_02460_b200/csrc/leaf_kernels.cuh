@@ -8,9 +8,9 @@
 // One CTA of 256 threads = a 16 x 16 grid of threads.  The block is distributed 2-D CYCLICALLY:
 // thread (ty,tx) keeps the 64 elements (ty + 16 r, tx + 16 c), r,c = 0..7, in registers, so the
 // shrinking active region of a right-looking sweep stays spread over all threads and whole
-// register rows / columns drop out of the (unrolled) update statically: N^3/6 FMAs in total, not
-// N^3/2.  Both factorisation and inversion are rank-1 sweeps: the pivot row is broadcast through a
-// double-buffered shared-memory row (one __syncthreads per step).  Global traffic goes through a
+// register rows / columns drop out of the (unrolled) update statically.  Factorisation and inversion
+// are rank-1 sweeps: the pivot row is broadcast through a double-buffered shared-memory row (one
+// __syncthreads per step); potrf_leaf_kernel forms U_kk and U_kk^-1 in ONE sweep (see there).  Global traffic goes through a
 // padded shared-memory image of the block so that loads and stores are coalesced.  Blocks shorter
 // than 128 (ragged last block) are padded with the identity, which factors / inverts to itself.
 #pragma once
@@ -114,6 +114,24 @@ __device__ __forceinline__ void leaf_invert_upper(const LeafSmem& s, int tx, int
     __syncthreads();
 }
 
+// One register row group r of the fused factor-and-invert step (potrf_leaf_kernel) for pivot j = 16 jr + jo:
+// x(i,c) -= ri * pivot_row(c) for the columns that are live: Y (c <= j) and the Schur complement (c >= i).
+// jr and r are compile-time constants after unrolling, so the register indices are static.
+__device__ __forceinline__ void leaf_update_row(double (&a)[8][8], int jr, int r, const double* rb, double ri, double pj,
+                                                bool rowact, int tx, int ty, int jo)
+{
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        if (c < jr) {                    // Y, columns left of group jr
+            if (rowact) a[r][c] = fma(-ri, rb[tx + 16 * c], a[r][c]);
+        } else if (c == jr) {            // Y for columns <= j; on the diagonal register block also the upper part
+            if (rowact && ((tx <= jo) || (r == jr && tx >= ty))) a[r][c] = fma(-ri, pj, a[r][c]);
+        } else if (c >= r) {             // Schur complement, upper part
+            if (rowact && ((c > r) || (tx >= ty))) a[r][c] = fma(-ri, rb[tx + 16 * c], a[r][c]);
+        }
+    }
+}
+
 // S: N x N column-major (ld), block starts at (j0, j0), order nb = min(LB, N - j0).
 // Winv: LB x LB column-major block (leading dimension ldw) receiving U_kk^-1 (identity-padded).
 // info: device flag; set (if still 0) to j0 + j + 1 when pivot j is not > 0.
@@ -137,17 +155,25 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
 #pragma unroll
         for (int c = 0; c < 8; ++c) a[r][c] = s.U[ty + 16 * r + (tx + 16 * c) * LP];
 
-    // right-looking factorisation without square roots inside the sweep:
-    //   step j: d_j = a(j,j);  a(i,c) -= a(j,i) a(j,c) / d_j  (j < i <= c);  U(j,c) = a(j,c) / sqrt(d_j) afterwards
+    // Right-looking factorisation without square roots inside the sweep, with the inverse formed by the
+    // SAME sweep (elimination applied to the identity):  S = L D L^T, U = D^1/2 L^T, and the row
+    // operations that eliminate column j, applied to I, leave Y = L^-1 (unit lower), so that
+    // U^-1 = Y^T D^-1/2.  The strictly-lower register positions (row > col), unused by the symmetric
+    // factorisation, hold Y; its unit diagonal is implicit.
+    //   step j: d_j = a(j,j), l_i = a(j,i) / d_j for i > j;
+    //           a(i,c) -= l_i a(j,c)  (c >= i: Schur complement),
+    //           Y(i,c) -= l_i Y(j,c)  (c <  j),   Y(i,j) = -l_i.
+    // One pass of 128 dependent steps instead of two (the latency of a step -- barrier, broadcast,
+    // reciprocal -- is paid once).
 #pragma unroll
     for (int jr = 0; jr < 8; ++jr) {
 #pragma unroll 1
         for (int jo = 0; jo < 16; ++jo) {
             const int j = jr * 16 + jo;
             double* rb = s.rowbuf + (j & 1) * LB;
-            if (ty == jo) {
+            if (ty == jo) {   // the whole pivot row: Y(j, <j), d_j, a(j, >j)
 #pragma unroll
-                for (int c = jr; c < 8; ++c) rb[tx + 16 * c] = a[jr][c];
+                for (int c = 0; c < 8; ++c) rb[tx + 16 * c] = a[jr][c];
             }
             __syncthreads();
             const double d = rb[j];
@@ -157,16 +183,10 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
             }
             if (t == 0) s.dvec[j] = d;
             const double invd = 1.0 / d;
+            const double pj = (tx == jo) ? 1.0 : rb[tx + 16 * jr];   // column group jr of the pivot row, Y(j,j) = 1
 #pragma unroll
-            for (int r = jr; r < 8; ++r) {
-                const bool rowact = (r > jr) || (ty > jo);
-                const double ri = rb[ty + 16 * r] * invd;
-#pragma unroll
-                for (int c = r; c < 8; ++c) {
-                    const bool colact = (c > r) || (tx >= ty);
-                    if (rowact && colact) a[r][c] = fma(-ri, rb[tx + 16 * c], a[r][c]);
-                }
-            }
+            for (int r = jr; r < 8; ++r)
+                leaf_update_row(a, jr, r, rb, rb[ty + 16 * r] * invd, pj, (r > jr) || (ty > jo), tx, ty, jo);
         }
     }
     __syncthreads();
@@ -186,8 +206,20 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
         }
     __syncthreads();
     leaf_store_all(s, blk, ld, nb, t);
+    __syncthreads();   // the image is rewritten next
 
-    leaf_invert_upper(s, tx, ty);
+    // W = U^-1 = Y^T D^-1/2: the register at (row, col), row > col, is W(col, row) / dinv[row]
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            double w = 0.0;
+            if (row == col) w = s.dinv[row];
+            else if (row > col) w = a[r][c] * s.dinv[row];
+            s.U[col + row * LP] = w;
+        }
+    __syncthreads();
     leaf_store_all(s, Winv, ldw, LB, t);
 }
 
