@@ -117,8 +117,10 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 /* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
  * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
  * inside [dev_scratch, dev_scratch + scratch_bytes) -- only the triangles the steps reference: the
- * UPPER triangle of host_S and the LOWER triangle of host_H (both with the diagonal, in column
- * chunks; the other triangle of either host buffer is never read) --, runs steps 1-3 there and copies the UPPER
+ * UPPER triangle of host_S and the LOWER triangle of host_H (both with the diagonal, in chunks;
+ * the other triangle of either host buffer is never read; step 1 starts once the rows of S that its
+ * first two panels cover are in, and applies its first trailing update slab by slab as the remaining
+ * rows arrive) --, runs steps 1-3 there and copies the UPPER
  * triangle of H~ back to host_Htilde (N x N, ld N; the strictly-lower part of the host buffer is
  * unspecified -- callers read the upper triangle only).  Copies overlap compute on plan-owned copy
  * streams that are joined before return: H goes in beside steps 1-2, step 3 is formed in row ranges

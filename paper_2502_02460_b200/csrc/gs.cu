@@ -63,6 +63,10 @@ struct gs_plan {
     cudaStream_t copy = nullptr;     // host-buffer entry points: H2D copies beside compute
     cudaStream_t copy_out = nullptr; // host-buffer entry points: D2H copies beside compute
     cudaEvent_t ev_copy = nullptr;
+    // host path (gs_reduce_host): the rows of S below the first two panels arrive in slabs while step 1 is
+    // already running; slab q = block rows [gates[q].first, gates[q+1].first or nblk) is on the device once
+    // gates[q].second fires.  Empty: everything is there.
+    std::vector<std::pair<int, cudaEvent_t>> gates;
     std::vector<cudaEvent_t> ev_pool;   // per-chunk events of the host-buffer entry points
     int potrf_nb = 8;                // panel width of the look-ahead schedule, in 128-blocks
     int potrf_nb_tail = 4;           // panel width once at most potrf_tail blocks remain
@@ -385,6 +389,22 @@ struct Potrf {
         return launch(st, p, false, L_POTRF_SYRK);
     }
 
+    // rows [i0, i1) of the same update of S[.., i0:n]: S[i0:i1, i0:n] -= S[k0:k1, i0:i1]^T S[k0:k1, i0:n], upper tiles
+    gs_status_t syrk_rows(int k0, int k1, int i0, int i1, int n)
+    {
+        EngineParams p = blank_params(st.plan);
+        if (!set_operand(st, p, 0, vS, false) || !set_operand(st, p, 1, vS, false)) return GS_ERR_CUDA;
+        p.C = static_cast<double*>(S); p.ldc = vS.ld;
+        p.tiles_m = i1 - i0; p.tiles_n = n - i0; p.order = ORDER_TRAPEZOID;
+        p.c_row0 = i0 * st.lb; p.c_col0 = i0 * st.lb; p.c_rows = int(vS.rows); p.c_cols = int(vS.cols);
+        p.khi_c = (k1 - k0) * (KPB); p.kmax = p.khi_c;
+        p.a.k0 = k0 * st.lb; p.a.x0 = i0 * st.lb;
+        p.b.k0 = k0 * st.lb; p.b.x0 = i0 * st.lb;
+        p.alpha = -1.0; p.beta = 1.0;
+        p.flags = F_STORE_UPPER | F_REAL_DIAG;
+        return launch(st, p, false, L_POTRF_SYRK);
+    }
+
     // recursive factorisation of the diagonal block [b0, b1) (touches nothing outside it)
     gs_status_t potrf(int b0, int b1)
     {
@@ -491,7 +511,17 @@ struct Potrf {
             if (s2 < n) {
                 if (rc == GS_OK) rc = update_rows(s0, s1, s2, n);                 // D_i
                 cu(cudaEventRecord(plan->ev_rows, main_stream));
-                if (rc == GS_OK) rc = syrk(s0, s1, s2, n);                        // E_i
+                if (i == 1 && !plan->gates.empty()) {
+                    // E_1 is the first launch that touches rows of S below the second panel: slab by slab
+                    // as the rows arrive (gs_reduce_host); the slabs start at s2
+                    for (size_t q = 0; q < plan->gates.size() && rc == GS_OK; ++q) {
+                        const int r0 = plan->gates[q].first, r1 = q + 1 < plan->gates.size() ? plan->gates[q + 1].first : n;
+                        cu(cudaStreamWaitEvent(main_stream, plan->gates[q].second, 0));
+                        rc = syrk_rows(s0, s1, r0, r1, n);
+                    }
+                } else if (rc == GS_OK) {
+                    rc = syrk(s0, s1, s2, n);                                     // E_i
+                }
                 cu(cudaStreamWaitEvent(side, plan->ev_rows, 0));
                 st.stream = side;
                 if (rc == GS_OK) rc = panel_solve(W(i), s1, s2, s2, s3);          // F1_i
@@ -891,6 +921,53 @@ static size_t triangle_h2d_bytes(const gs_plan* plan)
     return b;
 }
 
+// Upload of S's upper triangle in the order step 1 consumes it.  Nothing strictly below a diagonal block is
+// written, so the copies may run beside gs_cholesky's zeroing of the strictly-lower blocks.
+//   top part: rows [0, top) of every block column (chunk [c0, c1) moves rows [0, min(top, c1)));
+//   slab [R0, R1) (block rows, below the top part): for each of its block columns b the rows from the slab
+//   start to the end of the diagonal block, then the rectangle right of the slab's diagonal square.
+static gs_status_t copy_2d_h2d(gs_plan* plan, void* dev, const void* host, int64_t r0, int64_t r1, int64_t c0, int64_t c1, cudaStream_t stream)
+{
+    if (r1 <= r0 || c1 <= c0) return GS_OK;
+    const size_t pitch = size_t(plan->N) * plan->es;
+    const size_t off = size_t(r0) * plan->es + size_t(c0) * pitch;
+    GS_CUDA(plan, cudaMemcpy2DAsync(static_cast<unsigned char*>(dev) + off, pitch, static_cast<const unsigned char*>(host) + off, pitch,
+                                    size_t(r1 - r0) * plan->es, size_t(c1 - c0), cudaMemcpyHostToDevice, stream));
+    return GS_OK;
+}
+
+static gs_status_t copy_upper_top_h2d(gs_plan* plan, void* dev, const void* host, int64_t top, cudaStream_t stream)
+{
+    for (int64_t c0 = 0; c0 < plan->N; c0 += plan->lb) {
+        const int64_t c1 = std::min<int64_t>(c0 + plan->lb, plan->N);
+        GS_TRY(copy_2d_h2d(plan, dev, host, 0, std::min<int64_t>(top, c1), c0, c1, stream));
+        if (c1 >= top) {   // from here on every block column has the same rows: one copy for the rest
+            GS_TRY(copy_2d_h2d(plan, dev, host, 0, top, c1, plan->N, stream));
+            break;
+        }
+    }
+    return GS_OK;
+}
+
+static gs_status_t copy_upper_slab_h2d(gs_plan* plan, void* dev, const void* host, int R0, int R1, cudaStream_t stream)
+{
+    const int64_t lb = plan->lb, N = plan->N;
+    const int64_t r0 = R0 * lb, r1 = std::min<int64_t>(R1 * lb, N);
+    for (int b = R0; b < R1; ++b)
+        GS_TRY(copy_2d_h2d(plan, dev, host, r0, std::min<int64_t>((b + 1) * lb, N), b * lb, std::min<int64_t>((b + 1) * lb, N), stream));
+    return copy_2d_h2d(plan, dev, host, r0, r1, r1, N, stream);
+}
+
+static size_t upper_h2d_bytes(const gs_plan* plan)
+{
+    size_t b = 0;
+    for (int64_t c0 = 0; c0 < plan->N; c0 += plan->lb) {
+        const int64_t c1 = std::min<int64_t>(c0 + plan->lb, plan->N);
+        b += size_t(c1) * size_t(c1 - c0) * plan->es;
+    }
+    return b;
+}
+
 static gs_status_t copy_triangle_h2d(gs_plan* plan, void* dev, const void* host, bool upper, cudaStream_t stream)
 {
     const size_t pitch = size_t(plan->N) * plan->es;
@@ -907,7 +984,7 @@ static gs_status_t copy_triangle_h2d(gs_plan* plan, void* dev, const void* host,
 gs_status_t gs_reduce_host_h2d_bytes(const gs_plan_t* plan, size_t* bytes)
 {
     if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
-    *bytes = 2 * triangle_h2d_bytes(plan);   // S upper + H lower
+    *bytes = upper_h2d_bytes(plan) + triangle_h2d_bytes(plan);   // S upper (block columns) + H lower (512-column chunks)
     return GS_OK;
 }
 
@@ -942,25 +1019,47 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     void *dS = base, *dH = base + mat, *dV = base + 2 * mat, *dHt = base + 3 * mat;
     RowRanges rr;
     rr.splits = host_row_splits(plan);
-    GS_TRY(ensure_copy_streams(plan, rr.splits.size()));
-    // S first on the caller's stream; H (not needed before step 3) goes on the plan's copy stream and
-    // overlaps steps 1-2; both copy streams are forked from / joined into `stream`
-    // Only the triangles the steps reference cross the link (column chunks, trapezoids): the upper one of
-    // S (step 1) and the lower one of H (step 3) -- about half of each matrix.  What stays unwritten in
-    // the scratch is never read.
-    GS_TRY(copy_triangle_h2d(plan, dS, host_S, true, stream));
-    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));          // H follows S on the link, not beside it
+    const size_t nr = rr.splits.size();
+    // Only the triangles the steps reference cross the link: the upper one of S (step 1) and the lower one
+    // of H (step 3) -- about half of each matrix; what stays unwritten in the scratch is never read.  All
+    // uploads go, one after the other, on the plan's copy stream (forked from / joined into `stream`):
+    //   1. the rows of S's triangle that the first two panels cover -- step 1 starts when they are in;
+    //   2. the rest of S in slabs of eight block rows -- needed from the first trailing update on, which is
+    //      applied slab by slab as they arrive (plan->gates), behind the first panel's factorisation, solve
+    //      and row update;
+    //   3. H, not needed before step 3, beside steps 1-2.
+    const std::vector<int> ps = Potrf::panel_starts(plan->nblk, plan);
+    const int top_blk = ps.size() > 2 ? ps[2] : plan->nblk;
+    const int64_t top = std::min<int64_t>(int64_t(top_blk) * plan->lb, plan->N);
+    const int slab = 8;
+    const size_t nslabs = size_t((plan->nblk - top_blk + slab - 1) / slab);
+    GS_TRY(ensure_copy_streams(plan, nr + 1 + nslabs));
+    cudaEvent_t ev_top = plan->ev_pool[nr];
+    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, stream));
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy, plan->ev_copy, 0));
     GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_copy, 0));
-    GS_TRY(copy_triangle_h2d(plan, dH, host_H, false, plan->copy));
-    GS_CUDA(plan, cudaEventRecord(plan->ev_copy, plan->copy));
-    gs_status_t rc = gs_cholesky(plan, dS, stream);
+    GS_TRY(copy_upper_top_h2d(plan, dS, host_S, top, plan->copy));
+    GS_CUDA(plan, cudaEventRecord(ev_top, plan->copy));
+    GS_CUDA(plan, cudaStreamWaitEvent(stream, ev_top, 0));
+    plan->gates.clear();
+    for (size_t q = 0; q < nslabs; ++q) {
+        const int R0 = top_blk + int(q) * slab, R1 = std::min(R0 + slab, plan->nblk);
+        const gs_status_t cs = copy_upper_slab_h2d(plan, dS, host_S, R0, R1, plan->copy);
+        if (cs != GS_OK) { plan->gates.clear(); return cs; }
+        const cudaError_t ce = cudaEventRecord(plan->ev_pool[nr + 1 + q], plan->copy);
+        if (ce != cudaSuccess) { plan->gates.clear(); return cuda_fail(plan, ce); }
+        plan->gates.emplace_back(R0, plan->ev_pool[nr + 1 + q]);
+    }
+    gs_status_t rc = copy_triangle_h2d(plan, dH, host_H, false, plan->copy);
+    if (rc == GS_OK && cudaEventRecord(plan->ev_copy, plan->copy) != cudaSuccess) rc = GS_ERR_CUDA;
+    if (rc == GS_OK) rc = gs_cholesky(plan, dS, stream);
+    plan->gates.clear();
     if (rc == GS_OK) rc = gs_invert_triangular(plan, dS, dV, stream);
     GS_CUDA(plan, cudaStreamWaitEvent(stream, plan->ev_copy, 0));   // join, also on failure
     GS_TRY(rc);
     if (host_U || host_Uinv) {   // U, U^-1 are final once steps 1-2 are done: they go back beside step 3
-        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[rr.splits.size() - 1], stream));
-        GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_pool[rr.splits.size() - 1], 0));
+        GS_CUDA(plan, cudaEventRecord(plan->ev_pool[nr - 1], stream));
+        GS_CUDA(plan, cudaStreamWaitEvent(plan->copy_out, plan->ev_pool[nr - 1], 0));
         if (host_U) GS_CUDA(plan, cudaMemcpyAsync(host_U, dS, bytes, cudaMemcpyDeviceToHost, plan->copy_out));
         if (host_Uinv) GS_CUDA(plan, cudaMemcpyAsync(host_Uinv, dV, bytes, cudaMemcpyDeviceToHost, plan->copy_out));
     }
