@@ -1,13 +1,17 @@
-// gs.cu -- the C ABI of include/gs.h: plan management and the four stage drivers.
+// gs.cu -- the C ABI of include/gs.h: plan management, the four stage drivers, the density matrix and
+// the host-buffer entry points.
 //
-// Every stage is a short host-side schedule of launches of (a) the FP64 tile engine
-// (tile_engine.cuh: TMA-staged DMMA tiles with triangular k-ranges) and (b) the 128 x 128 leaf
-// kernels (leaf_kernels.cuh).  Nothing here calls cuBLAS/cuSOLVER, and there is no CPU fallback.
+// Every stage is a short host-side schedule of launches of (a) the FP64 tile engines -- TMA-staged DMMA
+// tiles with triangular k-ranges: tile64_engine.cuh (real, 64 x 64 CTA tiles, the default),
+// tile_engine.cuh (real, 128 x 128: in-place one-tile solves and odd N), ctile_half_engine.cuh /
+// ctile_engine.cuh (complex128) -- and (b) the diagonal-block kernels (leaf_kernels.cuh, cleaf_kernels.cuh).
+// Nothing here calls cuBLAS/cuSOLVER, and there is no CPU fallback.
 //
-//   gs_cholesky           recursive blocked POTRF  S = U^T U
-//   gs_invert_triangular  block-recursive TRTRI    V = U^-1
-//   gs_to_standard        G = T V (T = triu(H,1) + diag(H)/2), H~ = V^T G + G^T V
-//   gs_backtransform      C = V C~                                                 (PAPER.md:67)
+//   gs_cholesky           blocked POTRF with look-ahead on a side stream  S = U^H U
+//   gs_invert_triangular  block-recursive TRTRI by doubling               V = U^-1
+//   gs_to_standard        G = T V (T = triu(H,1) + diag(H)/2), H~ = V^H G + G^H V
+//   gs_backtransform      C = V C~                                                   (PAPER.md:67)
+//   gs_density_matrix     P = sum_l f_l c*_l c_l (weighted SYRK / HERK)
 #include "../../include/gs.h"
 
 #include <cuda_runtime.h>
