@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--no-checks", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="NEXT-2: K independent pencils in flight on one GPU (not the headline)")
     ap.add_argument("--batch-n", type=int, default=2048)
+    ap.add_argument("--shard-shares", type=int, default=0,
+                    help="NEXT-3: time, on ONE GPU and one after the other, the share each of R ranks would run (not the headline)")
     ap.add_argument("--batch-complex", action="store_true")
     return ap.parse_args()
 
@@ -489,10 +491,83 @@ def run_batch(args):
                       "data": "synthetic", "detail": out}))
 
 
+def run_shard_shares(args):
+    """NEXT-3: the column-range calls of every one of R ranks, timed on ONE GPU one rank
+    after the other.  No multi-GPU hardware is available to this run, so the exchange is not timed: the
+    line reports what each rank would compute (max over ranks = the step's compute time at R GPUs) and
+    the bytes the one exchange step moves."""
+    import torch
+
+    from paper_2502_02460_b200 import gs, sharded
+    from paper_2502_02460_b200 import workloads as wl
+
+    torch.cuda.set_device(0)
+    R = args.shard_shares
+    cfg = wl.CONFIGS[args.config]
+    N, nev, cplx = cfg.N, cfg.nev, cfg.complex
+    pen = wl.make_config(cfg, device="cuda")
+    dt = pen.H.dtype
+    plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
+    U, V, G, Ht = (wl.colmajor_empty(N, N, dtype=dt, device="cuda") for _ in range(4))
+    Ct = wl.dense_rhs(N, nev, seed=3, complex=cplx, device="cuda")
+    C = wl.colmajor_empty(N, nev, dtype=dt, device="cuda")
+    ranges = sharded.column_ranges(N, R, plan.block)
+    eig = sharded.even_ranges(nev, R, 2)
+
+    def timed(fn):
+        for _ in range(max(1, args.warmup)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    def chol():
+        U.copy_(pen.S)
+        plan.cholesky(U)
+    t_copy = timed(lambda: U.copy_(pen.S))
+    t_chol = timed(chol) - t_copy
+    plan.invert_triangular(U, V)           # complete V, G for the step-3 shares
+    for c0, c1 in ranges:
+        plan.to_standard_g_cols(pen.H, V, G, c0, c1 - c0)
+    ranks = []
+    for r, ((c0, c1), (k0, k1)) in enumerate(zip(ranges, eig)):
+        w = c1 - c0
+        Vr = wl.colmajor_empty(N, N, dtype=dt, device="cuda")
+        t = {"cols": [c0, c1], "eig_cols": [k0, k1],
+             "invert": timed(lambda: plan.invert_triangular_cols(U, Vr, c0, w)),
+             "g": timed(lambda: plan.to_standard_g_cols(pen.H, V, G, c0, w)),
+             "syr2k": timed(lambda: plan.to_standard_cols(V, G, Ht, c0, w)),
+             "backtransform": timed(lambda: plan.backtransform_cols(V, Ct, C, k0, k1 - k0))}
+        t["sum_ms"] = t["invert"] + t["g"] + t["syr2k"] + t["backtransform"]
+        ranks.append(t)
+        del Vr
+    plan.last_info()
+    es = 16 if cplx else 8
+    sharded_ms = max(t["sum_ms"] for t in ranks)
+    total_ms = t_chol + sharded_ms
+    flops = wl.nominal_flops(N, nev, cplx)["total"]
+    print(json.dumps({"metric": "FP64 TFLOP/s of the column-sharded path at R ranks, compute only, projected from one GPU (NEXT-3, not the headline)",
+                      "unit": UNIT, "value": flops / (total_ms * 1e-3) / 1e12, "n_gpus": 1, "ranks_projected": R,
+                      "steps": args.steps, "warmup": args.warmup, "dtype": "c128" if cplx else "f64", "data": "synthetic",
+                      "config": {"workload": f"shard_R{R}_{cfg.name}"},
+                      "detail": {"cholesky_replicated_ms": t_chol, "slowest_rank_sharded_ms": sharded_ms, "step_ms": total_ms,
+                                 "sum_over_ranks_sharded_ms": sum(t["sum_ms"] for t in ranks),
+                                 "exchange_bytes_per_rank_received": 2 * N * N * es, "exchange": "not timed (one GPU)",
+                                 "ranks": ranks}}))
+
+
 def main():
     args = parse_args()
     if args.batch > 0:
         run_batch(args)
+        return
+    if args.shard_shares > 0:
+        run_shard_shares(args)
         return
     if args.impl == "reference":
         run_reference(args)

@@ -99,6 +99,35 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H, const void* Uinv, voi
 gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C,
                              void* cuda_stream);
 
+/* Column-range forms of steps 2, 3 and of the back-transformation: the path sharded over the
+ * GPUs of one NVSwitch domain (the paper's multi-GPU direction,
+ * PAPER.md:118).  Every rank holds U (step 1 is replicated) and owns a contiguous
+ * range of block columns J = [col0, col0 + ncols): col0 a multiple of the block order (128 real,
+ * 64 complex), col0 + ncols a multiple of it or equal to the matrix width.  ncols == 0 is a no-op.
+ * All matrices are N x N (C~, C: N x nev), column-major, ld = N, device pointers, caller-owned; a
+ * column range is therefore one contiguous slab of the buffer, which is what the ranks exchange.
+ *
+ * gs_invert_triangular_cols: columns J of Uinv = U^-1, rows 0 .. col0+ncols-1, by
+ *   blocked back substitution of U X = E_J.  Writes zeros below the diagonal of the whole Uinv buffer
+ *   and the inverted diagonal blocks left of J (which it needs and forms itself); the columns right
+ *   of J are left untouched above the diagonal blocks.  Reads only the upper triangle of U.
+ * gs_to_standard_g_cols: columns J of the intermediate G = T Uinv, T = triu(H,1) + diag(H)/2
+ *   (H = T + T^H, so H~ = Uinv^H G + G^H Uinv).  Needs only the columns J of Uinv.
+ *   G is a caller-owned N x N buffer (it is exchanged between ranks).
+ * gs_to_standard_cols: columns J of the UPPER triangle of Htilde (rows 0 .. diagonal).  Reads the
+ *   columns [0, col0 + ncols) of Uinv and of G: the slabs of the lower-numbered ranges and its own.
+ * gs_backtransform_cols: C[:, K] = Uinv C~[:, K] for the eigenvector columns K = [col0, col0+ncols)
+ *   of the plan's nev (any col0 with a 16-byte aligned column start); needs all of Uinv.
+ * Errors and asynchrony as for the whole-matrix calls. */
+gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U, void* Uinv, int64_t col0, int64_t ncols,
+                                      void* cuda_stream);
+gs_status_t gs_to_standard_g_cols(gs_plan_t* plan, const void* H, const void* Uinv, void* G, int64_t col0,
+                                  int64_t ncols, void* cuda_stream);
+gs_status_t gs_to_standard_cols(gs_plan_t* plan, const void* Uinv, const void* G, void* Htilde, int64_t col0,
+                                int64_t ncols, void* cuda_stream);
+gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C, int64_t col0,
+                                  int64_t ncols, void* cuda_stream);
+
 /* Density matrix (the step that follows the path; "single-particle density matrix
  * P_ij = sum_l f_l c*_li c_lj", with c_li = C(i,l), eigenvectors stored as columns):
  *     P(i,j) = sum_{l < nev} f[l] * conj(C(i,l)) * C(j,l).

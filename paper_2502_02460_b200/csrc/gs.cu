@@ -79,6 +79,7 @@ struct gs_plan {
     int potrf_end = 32;
     int ctile_half = 1;              // complex: two 64 x 32 CTAs per logical tile (3 CTAs/SM) instead of one 64 x 64
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
+    int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
 };
@@ -259,12 +260,12 @@ gs_status_t zero_lower(Stage& st, void* X)
 // (destination V) and to (temp T).
 // ------------------------------------------------------------------------------------------------
 gs_status_t invert_levels(Stage& st, const MatView& vU, int uo, const MatView& vV, int vo, const MatView& vT, int to,
-                          int nb, int label_w, int label_x)
+                          int nb, int label_w, int label_x, int s_end = 1 << 30)
 {
     gs_plan* plan = st.plan;
     double* V = static_cast<double*>(const_cast<void*>(vV.ptr));
     double* T = static_cast<double*>(const_cast<void*>(vT.ptr));
-    for (int s = 1; s < nb; s *= 2) {
+    for (int s = 1; s < nb && s < s_end; s *= 2) {   // s_end: stop once the diagonal s_end-blocks are inverted
         const int npairs = (nb - s + 2 * s - 1) / (2 * s);
         const int stride = 2 * s * st.lb;   // elements between consecutive pairs
         {   // W = B * Dinv
@@ -609,6 +610,9 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_TILE64", 0, 2, &p->tile64_mode);
     knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
+    int shard_log2 = p->z ? 4 : 3;   // 1024 rows per panel of the column-range inversion
+    knob("GS_SHARD_PANEL_LOG2", 0, 8, &shard_log2);
+    p->shard_panel = 1 << shard_log2;
     *plan = p;
     return GS_OK;
 }
@@ -813,6 +817,161 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
         !aligned16(Ctilde_) || !aligned16(C_))
         return GS_ERR_INVALID_ARG;
     return backtransform_cols(plan, Uinv_, Ctilde_, C_, 0, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Column-range entry points: every call forms the
+// block columns J = [col0, col0 + ncols) of its result from inputs that do not depend on the other
+// columns of the same result, so R GPUs form disjoint column ranges side by side and exchange the
+// finished slabs once.
+// ------------------------------------------------------------------------------------------------
+static bool col_range_ok(const gs_plan* plan, int64_t col0, int64_t ncols, int64_t width)
+{
+    if (col0 < 0 || ncols < 0 || col0 + ncols > width) return false;
+    if (ncols == 0) return true;                       // an empty range (more ranks than blocks) is a no-op
+    if (col0 % plan->lb != 0) return false;
+    return (col0 + ncols) % plan->lb == 0 || col0 + ncols == width;
+}
+
+// V[:, J] = (U^-1)[:, J] by blocked back substitution over panels of P blocks (U X = E_J):
+//   diagonal P-blocks D_i^-1 by the doubling levels s < P (every rank forms them; N (P lb)^2 / 3 flop),
+//   T[:, J] = 0, then right-looking from the last panel row that reaches into J up to panel 0:
+//     X[i, cols right of panel i] = -D_i^-1 T[i, .]                      (T[i, .] is complete by now)
+//     T[0 : i, cols] += U[0 : i, i] X[i, cols]      for all rows above, cols of J from panel i on
+//   N^3/3 flop over all columns, as the doubling scheme, but no column needs another column range; the
+//   updates are launches of (i P) x |J| tiles, so narrow ranges still fill the machine.
+gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uinv_, int64_t col0, int64_t ncols, void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (U_ == nullptr || Uinv_ == nullptr || U_ == Uinv_ || !aligned16(U_) || !aligned16(Uinv_) ||
+        !col_range_ok(plan, col0, ncols, plan->N))
+        return GS_ERR_INVALID_ARG;
+    if (ncols == 0) return GS_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    GS_TRY(configure_leaf(plan));
+    const int N = int(plan->N), lb = plan->lb;
+    const int jb0 = int(col0 / lb), jb1 = int((col0 + ncols + lb - 1) / lb);
+    const int P = plan->shard_panel;
+    Stage st = make_stage(plan, stream);
+    double* V = static_cast<double*>(Uinv_);
+    {
+        LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
+        if (plan->z)
+            trtri_cleaf_kernel<<<jb1, kCLeafThreads, kCLeafSmemBytes, stream>>>(static_cast<const double2*>(U_), static_cast<double2*>(Uinv_),
+                                                                                plan->N, N, info_ptr(plan));
+        else
+            trtri_leaf_kernel<<<jb1, kLeafThreads, kLeafSmemBytes, stream>>>(static_cast<const double*>(U_), V, plan->N, N, info_ptr(plan));
+    }
+    GS_CUDA(plan, cudaGetLastError());
+    plan->launches += 1;
+    GS_TRY(zero_lower(st, Uinv_));
+    const MatView vU{U_, N, N, N}, vV{Uinv_, N, N, N}, vT{big_ptr(plan), N, N, N};
+    GS_TRY(invert_levels(st, vU, 0, vV, 0, vT, 0, jb1, L_TRTRI_W, L_TRTRI_X, P));
+    const int npan = (jb1 + P - 1) / P;
+    if (npan < 2) return GS_OK;
+    {
+        LaunchTimer timer(plan, L_ZERO_LOWER, stream);
+        GS_CUDA(plan, cudaMemsetAsync(static_cast<unsigned char*>(big_ptr(plan)) + size_t(col0) * size_t(N) * plan->es, 0,
+                                      size_t(ncols) * size_t(N) * plan->es, stream));
+    }
+    for (int i = npan - 1; i >= 0; --i) {
+        const int r0 = i * P, r1 = (r0 + P < jb1) ? r0 + P : jb1;   // panel rows [r0, r1) in blocks
+        const int cb = jb0 > r0 + P ? jb0 : r0 + P;                 // first column block right of the panel
+        if (cb < jb1) {   // X[r0:r1, cb:] = -D_i^-1 T[r0:r1, cb:]   (a panel left of other columns is a full one)
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vV, true) || !set_operand(st, p, 1, vT, false)) return GS_ERR_CUDA;
+            p.C = V; p.ldc = N;
+            p.tiles_m = P; p.tiles_n = jb1 - cb; p.order = ORDER_ROW;
+            p.c_row0 = r0 * lb; p.c_col0 = cb * lb; p.c_rows = N; p.c_cols = N;
+            p.klo_i = KPB; p.khi_c = P * KPB; p.kmax = P * KPB;
+            p.a.x0 = r0 * lb; p.a.k0 = r0 * lb; p.b.k0 = r0 * lb; p.b.x0 = cb * lb;
+            p.alpha = -1.0;
+            GS_TRY(launch(st, p, true, L_TRTRI_X));
+        }
+        if (i == 0) break;
+        const int cu = jb0 > r0 ? jb0 : r0;                         // columns of J from the panel's own block on
+        {   // T[0:r0, cu:] += U[0:r0, r0:r1] X[r0:r1, cu:]; inside the panel X is upper triangular: k up to the column's block
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vU, true) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
+            p.C = static_cast<double*>(big_ptr(plan)); p.ldc = N;
+            p.tiles_m = r0; p.tiles_n = jb1 - cu; p.order = ORDER_COL_REV;
+            p.c_col0 = cu * lb; p.c_rows = N; p.c_cols = N;
+            p.khi_c = KPB * (cu - r0 + 1); p.khi_j = KPB; p.kmax = KPB * (r1 - r0);
+            p.a.k0 = r0 * lb; p.b.k0 = r0 * lb; p.b.x0 = cu * lb;
+            p.beta = 1.0;
+            GS_TRY(launch(st, p, true, L_TRTRI_W));
+        }
+    }
+    return GS_OK;
+}
+
+// G[:, J] = T Uinv[:, J], T = triu(H,1) + diag(H)/2, evaluated as L^H Uinv like the first launch of
+// gs_to_standard; rows below the diagonal blocks of J are written as zeros.
+gs_status_t gs_to_standard_g_cols(gs_plan_t* plan, const void* H_, const void* Uinv_, void* G_, int64_t col0, int64_t ncols,
+                                  void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (H_ == nullptr || Uinv_ == nullptr || G_ == nullptr || G_ == H_ || G_ == Uinv_ || !aligned16(H_) || !aligned16(Uinv_) ||
+        !aligned16(G_) || !col_range_ok(plan, col0, ncols, plan->N))
+        return GS_ERR_INVALID_ARG;
+    if (ncols == 0) return GS_OK;
+    const int N = int(plan->N), lb = plan->lb, kt = KPB;
+    const int jb0 = int(col0 / lb), jb1 = int((col0 + ncols + lb - 1) / lb);
+    Stage st = make_stage(plan, static_cast<cudaStream_t>(cuda_stream));
+    const MatView vH{H_, N, N, N}, vV{Uinv_, N, N, N};
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vH, false) || !set_operand(st, p, 1, vV, false)) return GS_ERR_CUDA;
+    p.C = static_cast<double*>(G_); p.ldc = N;
+    p.tiles_m = jb1; p.tiles_n = jb1 - jb0; p.order = ORDER_COL_REV;
+    p.c_col0 = jb0 * lb; p.b.x0 = jb0 * lb;
+    p.c_rows = N; p.c_cols = int(col0 + ncols);
+    p.klo_i = kt; p.khi_c = kt * (jb0 + 1); p.khi_j = kt; p.kmax = (N + st.bk - 1) / st.bk;
+    p.flags = F_MASK_A | F_LOWER_A | F_HALF_DIAG_A | F_MASK_B;
+    return launch(st, p, false, L_TOSTD_G);
+}
+
+// Htilde[0 : col0+ncols, J] = Uinv^H G + G^H Uinv, upper part: needs the columns [0, col0 + ncols) of
+// Uinv and of G (those of the lower-numbered ranges and its own), nothing to the right of J.
+gs_status_t gs_to_standard_cols(gs_plan_t* plan, const void* Uinv_, const void* G_, void* Htilde_, int64_t col0, int64_t ncols,
+                                void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (Uinv_ == nullptr || G_ == nullptr || Htilde_ == nullptr || Htilde_ == G_ || Htilde_ == Uinv_ || G_ == Uinv_ ||
+        !aligned16(Uinv_) || !aligned16(G_) || !aligned16(Htilde_) || !col_range_ok(plan, col0, ncols, plan->N))
+        return GS_ERR_INVALID_ARG;
+    if (ncols == 0) return GS_OK;
+    const int N = int(plan->N), lb = plan->lb, kt = KPB;
+    const int jb0 = int(col0 / lb), jb1 = int((col0 + ncols + lb - 1) / lb);
+    Stage st = make_stage(plan, static_cast<cudaStream_t>(cuda_stream));
+    const MatView vV{Uinv_, N, N, N}, vG{G_, N, N, N};
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vV, false) || !set_operand(st, p, 1, vG, false) || !set_operand(st, p, 2, vG, false) ||
+        !set_operand(st, p, 3, vV, false))
+        return GS_ERR_CUDA;
+    p.C = static_cast<double*>(Htilde_); p.ldc = N;
+    p.tiles_m = jb1; p.tiles_n = jb1 - jb0; p.order = ORDER_ROW_REV;      // rows descending: long tiles first
+    p.c_col0 = jb0 * lb; p.b.x0 = p.b2.x0 = jb0 * lb;
+    p.c_rows = N; p.c_cols = int(col0 + ncols);
+    p.kmax = (N + st.bk - 1) / st.bk;
+    p.khi_c = kt; p.khi_i = kt;
+    // tiles below the diagonal (I > jb0 + J) get an empty k-range and store nothing: k_lo = kmax (I - jb0 - J)
+    p.klo_c = -p.kmax * jb0; p.klo_i = p.kmax; p.klo_j = -p.kmax;
+    p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;
+    return launch(st, p, false, L_TOSTD_SYR2K);
+}
+
+// C[:, K] = Uinv Ctilde[:, K] for the eigenvector columns K = [col0, col0 + ncols) of the plan's nev.
+gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv_, const void* Ctilde_, void* C_, int64_t col0, int64_t ncols,
+                                  void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (col0 < 0 || ncols < 0 || col0 + ncols > plan->nev) return GS_ERR_INVALID_ARG;
+    if (ncols == 0) return GS_OK;
+    if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || C_ == Ctilde_ || C_ == Uinv_ || !aligned16(Uinv_) ||
+        !aligned16(Ctilde_) || !aligned16(C_))
+        return GS_ERR_INVALID_ARG;
+    if (!plan->z && ((col0 * plan->N) % 2 != 0)) return GS_ERR_INVALID_ARG;   // 16-byte aligned column start
+    return backtransform_cols(plan, Uinv_, Ctilde_, C_, int(col0), int(ncols), static_cast<cudaStream_t>(cuda_stream));
 }
 
 // P(i,j) = sum_l f_l conj(C(i,l)) C(j,l) = (X^H X)(i,j) with X(l,i) = sqrt(f_l) C(i,l): one transpose-and-scale

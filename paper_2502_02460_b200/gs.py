@@ -28,6 +28,7 @@ STATUS_NAMES = {
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
     "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
+    "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
@@ -76,6 +77,10 @@ def lib() -> ctypes.CDLL:
         L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
         L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_density_matrix.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_invert_triangular_cols.argtypes = [vp, vp, vp, i64, i64, vp]
+        L.gs_to_standard_g_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
+        L.gs_to_standard_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
+        L.gs_backtransform_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
         L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host_h2d_bytes.argtypes = [vp, ctypes.POINTER(sz)]
@@ -189,6 +194,32 @@ class Plan:
         self._check(lib().gs_backtransform(self._h, _dev_ptr(Uinv, self.N, self.N, self.tdtype),
                                            _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
                                            _dev_ptr(C, self.N, self.nev, self.tdtype), _stream_ptr(stream)))
+
+    # ---- column-range forms (sharded path, sharded.py) ----
+    @property
+    def block(self) -> int:
+        """Block order the column ranges are aligned to: 128 (real) or 64 (complex)."""
+        return 128 if self.dtype == GS_REAL64 else 64
+
+    def invert_triangular_cols(self, U: torch.Tensor, Uinv: torch.Tensor, col0: int, ncols: int, stream=None):
+        self._check(lib().gs_invert_triangular_cols(self._h, _dev_ptr(U, self.N, self.N, self.tdtype),
+                                                    _dev_ptr(Uinv, self.N, self.N, self.tdtype), col0, ncols,
+                                                    _stream_ptr(stream)))
+
+    def to_standard_g_cols(self, H: torch.Tensor, Uinv: torch.Tensor, G: torch.Tensor, col0: int, ncols: int, stream=None):
+        self._check(lib().gs_to_standard_g_cols(self._h, _dev_ptr(H, self.N, self.N, self.tdtype),
+                                                _dev_ptr(Uinv, self.N, self.N, self.tdtype),
+                                                _dev_ptr(G, self.N, self.N, self.tdtype), col0, ncols, _stream_ptr(stream)))
+
+    def to_standard_cols(self, Uinv: torch.Tensor, G: torch.Tensor, Htilde: torch.Tensor, col0: int, ncols: int, stream=None):
+        self._check(lib().gs_to_standard_cols(self._h, _dev_ptr(Uinv, self.N, self.N, self.tdtype),
+                                              _dev_ptr(G, self.N, self.N, self.tdtype),
+                                              _dev_ptr(Htilde, self.N, self.N, self.tdtype), col0, ncols, _stream_ptr(stream)))
+
+    def backtransform_cols(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, C: torch.Tensor, col0: int, ncols: int, stream=None):
+        self._check(lib().gs_backtransform_cols(self._h, _dev_ptr(Uinv, self.N, self.N, self.tdtype),
+                                                _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
+                                                _dev_ptr(C, self.N, self.nev, self.tdtype), col0, ncols, _stream_ptr(stream)))
 
     def density_matrix(self, C: torch.Tensor, f: torch.Tensor, P: torch.Tensor, stream=None):
         """P(i,j) = sum_l f[l] conj(C(i,l)) C(j,l); upper triangle of P is written."""

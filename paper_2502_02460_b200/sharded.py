@@ -1,0 +1,140 @@
+"""Steps 2, 3 and the back-transformation sharded over the GPUs of one NVSwitch domain
+(the paper's multi-GPU direction, PAPER.md:118, PAPER.md:138;
+DESIGN.md section 9).
+
+One process per GPU.  Every rank holds H, S and forms U itself (step 1 does not shard: each panel
+depends on all earlier trailing updates -- it is replicated, the same kernels give the same bits on
+every rank).  After that the work is split by COLUMN RANGES, which need no exchange while they are
+formed:
+
+    rank r owns the block columns J_r = [c_r, c_{r+1}) of U^-1, of G = T U^-1 and of H~
+      1. V[:, J_r]  = (U^-1)[:, J_r]                (gs_invert_triangular_cols)
+      2. G[:, J_r]  = T V[:, J_r]                   (gs_to_standard_g_cols)
+      3. exchange: every rank gets every slab V[:, J_s], G[:, J_s]  -- the ONE exchange step
+      4. H~[:, J_r] = V^H G[:, J_r] + G^H V[:, J_r], upper part      (gs_to_standard_cols)
+    and, once the eigenvectors C~ of H~ are known (off the path), rank r forms the eigenvector
+    columns K_r of C = V C~ (gs_backtransform_cols).
+
+A column range of a column-major matrix is one contiguous slab, so the exchange is a plain
+all-gather of unequal slabs (one broadcast per owner; NCCL over NVLink on the GPUs, gloo in the
+CPU test of this host logic).  The cost of column c grows like c^2 in all three steps, so the
+ranges are cut where the CUBE of the column index reaches equal shares.
+
+This module is host logic only: ranges, the order of the calls, the exchange.  All arithmetic runs
+in libgs through the `plan` object (gs.Plan); there is no other implementation behind it.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import torch
+import torch.distributed as dist
+
+from .workloads import colmajor_empty, colmajor_zeros
+
+
+def column_ranges(N: int, world: int, block: int) -> list[tuple[int, int]]:
+    """[(c0, c1)] per rank: contiguous, covering [0, N), boundaries on multiples of `block` (the last
+    ends at N), cut so that sum_{c in J_r} c^2 is about equal (boundary r at N (r/world)^(1/3)).
+    Ranks may get an empty range when there are fewer blocks than ranks."""
+    if N <= 0 or world <= 0 or block <= 0:
+        raise ValueError("N, world and block must be positive")
+    nblk = (N + block - 1) // block
+    cuts = [0]
+    for r in range(1, world):
+        b = round(nblk * (r / world) ** (1.0 / 3.0))
+        cuts.append(min(max(b, cuts[-1]), nblk))
+    cuts.append(nblk)
+    return [(min(cuts[r] * block, N), min(cuts[r + 1] * block, N)) for r in range(world)]
+
+
+def even_ranges(n: int, world: int, align: int = 1) -> list[tuple[int, int]]:
+    """[(k0, k1)] per rank for work that costs the same per column (the back-transformation):
+    equal shares, boundaries on multiples of `align`."""
+    if n < 0 or world <= 0 or align <= 0:
+        raise ValueError("bad arguments")
+    units = (n + align - 1) // align
+    cuts = [min(((units * r) // world) * align, n) for r in range(world)] + [n]
+    return [(cuts[r], cuts[r + 1]) for r in range(world)]
+
+
+def range_cost(c0: int, c1: int) -> float:
+    """Relative cost of a column range in steps 2-3: sum of c^2 ~ (c1^3 - c0^3) / 3."""
+    return (float(c1) ** 3 - float(c0) ** 3) / 3.0
+
+
+def slab(X: torch.Tensor, c0: int, c1: int) -> torch.Tensor:
+    """Columns [c0, c1) of a column-major matrix as a CONTIGUOUS (c1-c0) x rows tensor (a view)."""
+    v = X.t()[c0:c1]
+    if not v.is_contiguous():
+        raise ValueError("expected a column-major matrix")
+    return v
+
+
+def exchange_slabs(mats, ranges, rank: int, world: int, group=None) -> None:
+    """All-gather of unequal column slabs, in place: on return every rank holds columns J_s of every
+    matrix in `mats` as formed by their owner s.  One broadcast per (owner, matrix)."""
+    if world == 1:
+        return
+    for s, (c0, c1) in enumerate(ranges):
+        if c1 <= c0:
+            continue
+        for X in mats:
+            v = slab(X, c0, c1)
+            if X.is_complex():
+                v = torch.view_as_real(v)
+            dist.broadcast(v, src=dist.get_global_rank(group, s) if group is not None else s, group=group)
+
+
+@dataclass
+class ShardedResult:
+    U: torch.Tensor          # replicated
+    Uinv: torch.Tensor       # complete on every rank after the exchange
+    G: torch.Tensor          # complete on every rank after the exchange
+    Htilde: torch.Tensor     # upper triangle; only the columns of `cols` are valid before gather_htilde()
+    cols: tuple[int, int]
+
+
+class ShardedReduction:
+    """Host driver of the sharded path for one rank.  `plan` is a gs.Plan (or, in the CPU test of this
+    host logic, an object with the same column-range methods)."""
+
+    def __init__(self, plan, rank: int = 0, world: int = 1, group=None):
+        self.plan = plan
+        self.rank, self.world, self.group = int(rank), int(world), group
+        self.N, self.nev = plan.N, plan.nev
+        self.ranges = column_ranges(self.N, self.world, plan.block)
+        self.eig_ranges = even_ranges(self.nev, self.world, 2)
+
+    def reduce(self, H: torch.Tensor, S: torch.Tensor, stream=None) -> ShardedResult:
+        """Steps 1-3.  H, S: column-major N x N on this rank's device, identical on all ranks; S is not
+        modified.  Returns this rank's columns of the upper triangle of H~ (and U, U^-1, G in full)."""
+        N, plan = self.N, self.plan
+        c0, c1 = self.ranges[self.rank]
+        U = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
+        U.copy_(S)
+        Uinv = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
+        G = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
+        Ht = colmajor_zeros(N, N, dtype=H.dtype, device=H.device)
+        plan.cholesky(U, stream=stream)                                   # replicated
+        plan.invert_triangular_cols(U, Uinv, c0, c1 - c0, stream=stream)
+        plan.to_standard_g_cols(H, Uinv, G, c0, c1 - c0, stream=stream)
+        plan.last_info(stream=stream)                                     # synchronises: the slabs are final
+        exchange_slabs((Uinv, G), self.ranges, self.rank, self.world, self.group)
+        plan.to_standard_cols(Uinv, G, Ht, c0, c1 - c0, stream=stream)
+        plan.last_info(stream=stream)
+        return ShardedResult(U, Uinv, G, Ht, (c0, c1))
+
+    def gather_htilde(self, res: ShardedResult) -> torch.Tensor:
+        """Every rank gets all columns of the upper triangle of H~ (for an off-path eigensolver)."""
+        exchange_slabs((res.Htilde,), self.ranges, self.rank, self.world, self.group)
+        return res.Htilde
+
+    def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, stream=None) -> torch.Tensor:
+        """C = U^-1 C~, eigenvector columns split evenly over the ranks, then gathered."""
+        C = colmajor_empty(self.N, self.nev, dtype=Ctilde.dtype, device=Ctilde.device)
+        k0, k1 = self.eig_ranges[self.rank]
+        self.plan.backtransform_cols(Uinv, Ctilde, C, k0, k1 - k0, stream=stream)
+        self.plan.last_info(stream=stream)
+        exchange_slabs((C,), self.eig_ranges, self.rank, self.world, self.group)
+        return C
