@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--no-checks", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="NEXT-2: K independent pencils in flight on one GPU (not the headline)")
     ap.add_argument("--batch-n", type=int, default=2048)
+    ap.add_argument("--sharded", action="store_true",
+                    help="NEXT-3: ONE pencil over all ranks (steps 2-4 by column ranges, one exchange); strong scaling, not the headline mode")
     ap.add_argument("--shard-shares", type=int, default=0,
                     help="NEXT-3: time, on ONE GPU and one after the other, the share each of R ranks would run (not the headline)")
     ap.add_argument("--batch-complex", action="store_true")
@@ -491,6 +493,71 @@ def run_batch(args):
                       "data": "synthetic", "detail": out}))
 
 
+def run_sharded(args):
+    """NEXT-3 under torchrun: every rank holds the SAME pencil; step 1 replicated, steps 2-4 by column ranges
+    with one exchange of the U^-1 and G slabs (NCCL broadcasts over NVLink), C gathered at the end."""
+    import torch
+
+    from paper_2502_02460_b200 import gs, metrics as M, replicas, sharded
+    from paper_2502_02460_b200 import workloads as wl
+
+    info = replicas.rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(info.local_rank)
+    dev = torch.device("cuda", info.local_rank)
+    replicas.init(info, "nccl", dev)
+    cfg = wl.CONFIGS[args.config]
+    N, nev, cplx = cfg.N, cfg.nev, cfg.complex
+    pen = wl.make_pencil(N, cfg.box, cfg.seed, complex=cplx, device=dev)      # the same on every rank
+    plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64, device=dev)
+    drv = sharded.ShardedReduction(plan, info.rank, info.world)
+    bufs = drv.alloc(pen.H)
+    Ct = wl.dense_rhs(N, nev, seed=0, complex=cplx, device=dev)
+    C = wl.colmajor_empty(N, nev, dtype=pen.H.dtype, device=dev)
+
+    def step():
+        res = drv.reduce(pen.H, pen.S, out=bufs)
+        drv.backtransform(res.Uinv, Ct, out=C)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    replicas.barrier(info)
+    torch.cuda.synchronize()
+    l0 = plan.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier(info)
+    ms = replicas.max_over_ranks(info, e0.elapsed_time(e1) / args.steps, dev)
+    launches = plan.launch_count() - l0
+    Ht = drv.gather_htilde(bufs)
+    checks = None
+    if info.rank == 0 and not args.no_checks:      # against the whole-matrix calls on this rank
+        V1 = wl.colmajor_empty(N, N, dtype=pen.H.dtype, device=dev)
+        plan.invert_triangular(bufs.U, V1)
+        plan.to_standard(pen.H, V1, bufs.G)        # G is free now; upper triangle of H~ by the one-GPU path
+        plan.last_info()
+        checks = {"Uinv_rel_fro_vs_one_gpu_path": M.rel_frob_upper(bufs.Uinv, V1),
+                  "Htilde_rel_fro_vs_one_gpu_path": M.rel_frob_upper(Ht, bufs.G)}
+        checks["ok"] = bool(max(checks.values()) <= M.TOL_FROB)
+    flops = wl.nominal_flops(N, nev, cplx)["total"]
+    if info.rank == 0:
+        print(json.dumps({"metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": info.world,
+                          "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "c128 (FP64 arithmetic)" if cplx else "f64",
+                          "data": "synthetic",
+                          "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
+                                     "parallelism": f"sharded x{info.world}: step 1 replicated, steps 2-4 by column ranges, "
+                                                    "one exchange of the U^-1 and G slabs (NEXT-3)",
+                                     "column_ranges": drv.ranges},
+                          "gpu_launches": launches, "checks": checks}))
+    replicas.finalize(info)
+
+
 def run_shard_shares(args):
     """NEXT-3: the column-range calls of every one of R ranks, timed on ONE GPU one rank
     after the other.  No multi-GPU hardware is available to this run, so the exchange is not timed: the
@@ -568,6 +635,9 @@ def main():
         return
     if args.shard_shares > 0:
         run_shard_shares(args)
+        return
+    if args.sharded and args.impl == "ours":
+        run_sharded(args)
         return
     if args.impl == "reference":
         run_reference(args)

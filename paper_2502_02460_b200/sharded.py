@@ -106,16 +106,21 @@ class ShardedReduction:
         self.ranges = column_ranges(self.N, self.world, plan.block)
         self.eig_ranges = even_ranges(self.nev, self.world, 2)
 
-    def reduce(self, H: torch.Tensor, S: torch.Tensor, stream=None) -> ShardedResult:
+    def alloc(self, like: torch.Tensor) -> ShardedResult:
+        """The four N x N result buffers of reduce() (so a loop of reductions allocates once)."""
+        N = self.N
+        U, Uinv, G = (colmajor_empty(N, N, dtype=like.dtype, device=like.device) for _ in range(3))
+        Ht = colmajor_zeros(N, N, dtype=like.dtype, device=like.device)
+        return ShardedResult(U, Uinv, G, Ht, self.ranges[self.rank])
+
+    def reduce(self, H: torch.Tensor, S: torch.Tensor, stream=None, out: ShardedResult | None = None) -> ShardedResult:
         """Steps 1-3.  H, S: column-major N x N on this rank's device, identical on all ranks; S is not
         modified.  Returns this rank's columns of the upper triangle of H~ (and U, U^-1, G in full)."""
-        N, plan = self.N, self.plan
-        c0, c1 = self.ranges[self.rank]
-        U = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
+        plan = self.plan
+        res = self.alloc(H) if out is None else out
+        c0, c1 = res.cols
+        U, Uinv, G, Ht = res.U, res.Uinv, res.G, res.Htilde
         U.copy_(S)
-        Uinv = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
-        G = colmajor_empty(N, N, dtype=H.dtype, device=H.device)
-        Ht = colmajor_zeros(N, N, dtype=H.dtype, device=H.device)
         plan.cholesky(U, stream=stream)                                   # replicated
         plan.invert_triangular_cols(U, Uinv, c0, c1 - c0, stream=stream)
         plan.to_standard_g_cols(H, Uinv, G, c0, c1 - c0, stream=stream)
@@ -123,16 +128,16 @@ class ShardedReduction:
         exchange_slabs((Uinv, G), self.ranges, self.rank, self.world, self.group)
         plan.to_standard_cols(Uinv, G, Ht, c0, c1 - c0, stream=stream)
         plan.last_info(stream=stream)
-        return ShardedResult(U, Uinv, G, Ht, (c0, c1))
+        return res
 
     def gather_htilde(self, res: ShardedResult) -> torch.Tensor:
         """Every rank gets all columns of the upper triangle of H~ (for an off-path eigensolver)."""
         exchange_slabs((res.Htilde,), self.ranges, self.rank, self.world, self.group)
         return res.Htilde
 
-    def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, stream=None) -> torch.Tensor:
+    def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, stream=None, out: torch.Tensor | None = None) -> torch.Tensor:
         """C = U^-1 C~, eigenvector columns split evenly over the ranks, then gathered."""
-        C = colmajor_empty(self.N, self.nev, dtype=Ctilde.dtype, device=Ctilde.device)
+        C = colmajor_empty(self.N, self.nev, dtype=Ctilde.dtype, device=Ctilde.device) if out is None else out
         k0, k1 = self.eig_ranges[self.rank]
         self.plan.backtransform_cols(Uinv, Ctilde, C, k0, k1 - k0, stream=stream)
         self.plan.last_info(stream=stream)

@@ -1,0 +1,150 @@
+"""world_size-2 and -3 gloo tests (CPU) of the host logic of the sharded path (paper_2502_02460_b200/sharded.py;
+SURVEY.md section 8(f) NEXT-3): column ranges, the order of the calls, the one
+exchange of unequal column slabs, the gather of H~ and of C.
+
+There is no GPU here, so the `plan` the driver calls is a TEST-ONLY stand-in defined in this file: it
+does each column-range call with numpy from the rank's OWN buffers (poisoning with NaN everything the
+call does not produce), so a slab that the exchange fails to deliver, or a call issued before the data
+it needs has arrived, shows up as NaNs or as a mismatch with the oracle's whole-matrix result.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.multiprocessing as mp
+
+import oracle
+from paper_2502_02460_b200 import sharded
+from paper_2502_02460_b200 import workloads as wl
+
+
+class _NumpyColsPlan:
+    """Same method names and buffer conventions as gs.Plan's column-range calls; CPU, test only."""
+
+    def __init__(self, N, nev, block):
+        self.N, self.nev, self.block = N, nev, block
+        self.calls = []
+
+    def cholesky(self, S, stream=None):
+        S.copy_(torch.from_numpy(oracle.cholesky(S.numpy())))
+        self.calls.append("cholesky")
+
+    def invert_triangular_cols(self, U, Uinv, c0, w, stream=None):
+        V = np.triu(np.linalg.solve(np.triu(U.numpy()), np.eye(self.N, dtype=U.numpy().dtype)))
+        Uinv.fill_(float("nan"))
+        Uinv[:, c0:c0 + w] = torch.from_numpy(V[:, c0:c0 + w].copy())
+        self.calls.append("invert_cols")
+
+    def to_standard_g_cols(self, H, Uinv, G, c0, w, stream=None):
+        Hn = H.numpy()
+        T = np.triu(Hn, 1) + np.diag(np.diag(Hn)) / 2
+        G.fill_(float("nan"))
+        G[:, c0:c0 + w] = torch.from_numpy(T @ Uinv.numpy()[:, c0:c0 + w])
+        self.calls.append("g_cols")
+
+    def to_standard_cols(self, Uinv, G, Ht, c0, w, stream=None):
+        c1 = c0 + w
+        V, Gn = Uinv.numpy()[:, :c1], G.numpy()[:, :c1]        # nothing to the right of the range is read
+        X = V.conj().T @ Gn[:, c0:c1] + Gn.conj().T @ V[:, c0:c1]
+        Ht[:c1, c0:c1] = torch.from_numpy(np.triu(X, -c0))     # rows <= column (global indices)
+        self.calls.append("syr2k_cols")
+
+    def backtransform_cols(self, Uinv, Ct, C, k0, w, stream=None):
+        C.fill_(float("nan"))
+        C[:, k0:k0 + w] = torch.from_numpy(Uinv.numpy() @ Ct.numpy()[:, k0:k0 + w])
+        self.calls.append("back_cols")
+
+    def last_info(self, stream=None):
+        return 0
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, N, nev, block, cplx, out):
+    import torch.distributed as dist
+    os.environ.update({"MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    p = wl.small_pencil(N, seed=11, complex=cplx)                # identical on every rank
+    H, S = wl.to_colmajor(p.H), wl.to_colmajor(p.S)
+    plan = _NumpyColsPlan(N, nev, block)
+    drv = sharded.ShardedReduction(plan, rank, world)
+    res = drv.reduce(H, S)
+    own = res.Htilde[:, res.cols[0]:res.cols[1]].clone()
+    Ht = drv.gather_htilde(res)
+    Ct = wl.to_colmajor(wl.dense_rhs(N, nev, seed=4, complex=cplx))
+    C = drv.backtransform(res.Uinv, Ct)
+    out.put((rank, res.cols, plan.calls, res.Uinv.numpy().copy(), np.triu(Ht.numpy()), C.numpy().copy(),
+             np.triu(own.numpy(), -res.cols[0])))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,N,block,cplx", [(2, 300, 32, False), (3, 257, 16, True), (2, 40, 64, False)])
+def test_sharded_driver_over_gloo(world, N, block, cplx):
+    nev = N // 3
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, N, nev, block, cplx, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=180) for _ in range(world)), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    pen = wl.small_pencil(N, seed=11, complex=cplx)
+    U_o = oracle.cholesky(pen.S.numpy())
+    V_o = oracle.invert_upper(U_o)
+    Ht_o = np.triu(oracle.to_standard(pen.H.numpy(), V_o))
+    C_o = oracle.backtransform(V_o, wl.dense_rhs(N, nev, seed=4, complex=cplx).numpy())
+    ranges = sharded.column_ranges(N, world, block)
+    for rank, cols, calls, V, Ht, C, own in res:
+        assert tuple(cols) == ranges[rank]
+        assert calls == ["cholesky", "invert_cols", "g_cols", "syr2k_cols", "back_cols"]
+        assert np.isfinite(V).all() and np.isfinite(Ht).all() and np.isfinite(C).all()
+        assert np.linalg.norm(V - V_o) <= 1e-11 * np.linalg.norm(V_o)        # every rank ends with all of U^-1
+        assert np.linalg.norm(Ht - Ht_o) <= 1e-11 * np.linalg.norm(Ht_o)     # ... and all of triu(H~)
+        assert np.linalg.norm(C - C_o) <= 1e-11 * np.linalg.norm(C_o)
+        c0, c1 = cols
+        assert np.linalg.norm(own - Ht_o[:, c0:c1]) <= 1e-11 * max(np.linalg.norm(Ht_o[:, c0:c1]), 1e-300)
+
+
+def test_column_ranges_cover_align_and_balance():
+    for N, world, block in ((16384, 8, 128), (16384, 2, 128), (8192, 4, 64), (1000, 8, 128), (100, 3, 128), (32768, 8, 128)):
+        r = sharded.column_ranges(N, world, block)
+        assert len(r) == world and r[0][0] == 0 and r[-1][1] == N
+        for (a0, a1), (b0, b1) in zip(r, r[1:]):
+            assert a1 == b0 and a0 <= a1
+        for c0, c1 in r:
+            assert c0 % block == 0 or c0 == N
+            assert c1 % block == 0 or c1 == N
+    # the cube rule: at the headline size no rank carries more than 1.15 x the mean c^2 cost
+    for world in (2, 4, 8):
+        r = sharded.column_ranges(16384, world, 128)
+        cost = [sharded.range_cost(*c) for c in r]
+        assert max(cost) <= 1.15 * sum(cost) / world
+        assert abs(sum(cost) - 16384.0 ** 3 / 3) <= 1e-6 * 16384.0 ** 3
+
+
+def test_even_ranges():
+    assert sharded.even_ranges(4096, 8, 2) == [(512 * k, 512 * (k + 1)) for k in range(8)]
+    r = sharded.even_ranges(5, 3, 2)
+    assert r[0][0] == 0 and r[-1][1] == 5 and all(a1 == b0 for (_, a1), (b0, _) in zip(r, r[1:]))
+    assert all(k0 % 2 == 0 for k0, _ in r)
+    assert sharded.even_ranges(0, 4) == [(0, 0)] * 4
+
+
+def test_slab_is_a_contiguous_view():
+    X = wl.colmajor_zeros(6, 5)
+    v = sharded.slab(X, 1, 3)
+    assert v.is_contiguous() and v.shape == (2, 6)
+    v.fill_(7.0)
+    assert float(X[:, 1:3].min()) == 7.0 and float(X[:, 0].abs().max()) == 0.0 and float(X[:, 3:].abs().max()) == 0.0
+    with pytest.raises(ValueError):
+        sharded.slab(torch.zeros(6, 5), 1, 3)
