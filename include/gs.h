@@ -108,8 +108,8 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctil
  * column range is therefore one contiguous slab of the buffer, which is what the ranks exchange.
  *
  * gs_invert_triangular_cols: columns J of Uinv = U^-1, rows 0 .. col0+ncols-1, by
- *   blocked back substitution of U X = E_J.  Writes zeros below the diagonal of the whole Uinv buffer
- *   and the inverted diagonal blocks left of J (which it needs and forms itself); the columns right
+ *   blocked back substitution of U X = E_J.  Zeroes the strictly-lower blocks of the whole Uinv buffer
+ *   and writes the inverted diagonal blocks left of J (which it needs and forms itself); the columns right
  *   of J are left untouched above the diagonal blocks.  Reads only the upper triangle of U.
  * gs_to_standard_g_cols: columns J of the intermediate G = T Uinv, T = triu(H,1) + diag(H)/2
  *   (H = T + T^H, so H~ = Uinv^H G + G^H Uinv).  Needs only the columns J of Uinv.
@@ -127,6 +127,36 @@ gs_status_t gs_to_standard_cols(gs_plan_t* plan, const void* Uinv, const void* G
                                 int64_t ncols, void* cuda_stream);
 gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C, int64_t col0,
                                   int64_t ncols, void* cuda_stream);
+
+/* Fused exchange of the sharded path: the column-range calls can store what they produce not only
+ * into their own output buffer but, from the same kernel epilogue, into up to 8 further buffers of
+ * the same shape and layout -- the other ranks' copies, mapped over NVLink/NVSwitch peer memory --
+ * so the slabs travel while the remaining tiles are still being computed and no separate
+ * collective follows.  `kind` selects the result:
+ *   GS_PUSH_UINV    gs_invert_triangular_cols: the columns J of U^-1 (rows above and inside the
+ *                   diagonal blocks).  Here the Uinv ARGUMENT of the call is the rank's private work
+ *                   buffer; the targets are the exchange buffers of ALL ranks including its own,
+ *                   whose strictly-lower part the owner has zeroed once (nothing is pushed there).
+ *   GS_PUSH_G       gs_to_standard_g_cols: the columns J of G      (targets: the other ranks' G)
+ *   GS_PUSH_HTILDE  gs_to_standard_cols:   the columns J of triu(H~) (targets: the other ranks' H~)
+ *   GS_PUSH_C       gs_backtransform_cols: the columns K of C      (targets: the other ranks' C)
+ * Every element of a target has exactly one writer (the owner of its column).  Completion: once the
+ * writer's stream has been synchronised the stores have landed; a barrier between the ranks must
+ * separate them from the first read (and the reads from the next round of stores).  count == 0
+ * clears the set.  Targets are device pointers valid in this process: local buffers, or other
+ * processes' allocations opened with gs_ipc_open. */
+typedef enum { GS_PUSH_UINV = 0, GS_PUSH_G = 1, GS_PUSH_HTILDE = 2, GS_PUSH_C = 3 } gs_push_kind_t;
+gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int count, void* const* targets);
+
+/* CUDA IPC plumbing for the targets (one process per GPU).  gs_ipc_export: the 64-byte handle of the
+ * device allocation that contains dev_ptr and dev_ptr's byte offset inside it (send both to the
+ * peer).  gs_ipc_open (in another process): maps that allocation, enabling peer access, and returns
+ * the pointer that corresponds to dev_ptr.  gs_ipc_close: unmaps (pass the pointer gs_ipc_open
+ * returned and the same offset).  GS_ERR_CUDA if the driver refuses (e.g. memory that was not
+ * allocated with cudaMalloc). */
+gs_status_t gs_ipc_export(const void* dev_ptr, unsigned char* handle64, uint64_t* offset);
+gs_status_t gs_ipc_open(const unsigned char* handle64, uint64_t offset, void** dev_ptr);
+gs_status_t gs_ipc_close(void* dev_ptr, uint64_t offset);
 
 /* Density matrix (the step that follows the path; "single-particle density matrix
  * P_ij = sum_l f_l c*_li c_lj", with c_li = C(i,l), eigenvectors stored as columns):

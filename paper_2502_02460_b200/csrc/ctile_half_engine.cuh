@@ -232,6 +232,23 @@ __global__ void __launch_bounds__(kCThreads, 3) ctile_half_engine_kernel(const _
                     Cz[row + col * p.ldc] = v;
                 }
             }
+    }    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
+        double2* Cd = reinterpret_cast<double2*>(p.peer[d]);
+#pragma unroll
+        for (int mg = 0; mg < 4; ++mg) {
+            const long long row = c_row(mg);
+#pragma unroll
+            for (int ng = 0; ng < 2; ++ng)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const long long col = c_col(ng, e);
+                    if (row < p.c_rows && col < p.c_cols && col >= p.peer_col0 && (!upper_only || row <= col)) {
+                        double2 v = make_double2(alpha * acc[mg][ng][e][0], alpha * acc[mg][ng][e][1]);
+                        if (real_diag && row == col) v.y = 0.0;
+                        Cd[row + col * p.ldc] = v;
+                    }
+                }
+        }
     }
 }
 

@@ -33,12 +33,12 @@ using namespace gs;
 // launch labels for the optional per-launch timing (gs_plan_set_timing)
 enum LaunchLabel : int {
     L_POTRF_LEAF = 0, L_POTRF_TRSM, L_POTRF_GEMM, L_POTRF_SYRK, L_ZERO_LOWER,
-    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_DENS_T, L_DENS_SYRK, L_COUNT
+    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_DENS_T, L_DENS_SYRK, L_PUSH_BAND, L_COUNT
 };
 static const char* const kLabelNames[L_COUNT] = {
     "potrf.leaf", "potrf.trsm_leaf", "potrf.gemm", "potrf.syrk", "zero_lower",
     "trtri.leaf", "trtri.w", "trtri.x", "to_standard.g", "to_standard.syr2k", "backtransform.trmm",
-    "density.transpose", "density.syrk"};
+    "density.transpose", "density.syrk", "shard.push_band"};
 
 struct TimedLaunch {
     int label;
@@ -79,6 +79,7 @@ struct gs_plan {
     int potrf_end = 32;
     int ctile_half = 1;              // complex: two 64 x 32 CTAs per logical tile (3 CTAs/SM) instead of one 64 x 64
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
+    std::vector<void*> push[4];      // fused exchange: push targets per gs_push_kind_t (gs_plan_set_push_targets)
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
@@ -182,6 +183,15 @@ EngineParams blank_params(const gs_plan* plan)
     p.info = info_ptr(plan);
     p.super = plan->super_tile;
     return p;
+}
+
+// fused exchange: the launch also stores its tiles into the plan's push targets of `kind` (include/gs.h)
+void set_peers(const gs_plan* plan, EngineParams& p, int kind, size_t byte_offset = 0)
+{
+    const std::vector<void*>& t = plan->push[kind];
+    p.npeer = int(t.size());
+    p.peer_col0 = 0;
+    for (int d = 0; d < p.npeer; ++d) p.peer[d] = reinterpret_cast<double*>(static_cast<unsigned char*>(t[d]) + byte_offset);
 }
 
 // which: 0 = A, 1 = B, 2 = A2, 3 = B2.  mcontig selects the m-contiguous box of the A operand.
@@ -793,7 +803,8 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H_, const void* Uinv_, v
 }
 
 // C[:, col0 : col0+ncols] = V * C~[:, col0 : col0+ncols]
-static gs_status_t backtransform_cols(gs_plan* plan, const void* Uinv_, const void* Ctilde_, void* C_, int col0, int ncols, cudaStream_t stream)
+static gs_status_t backtransform_cols(gs_plan* plan, const void* Uinv_, const void* Ctilde_, void* C_, int col0, int ncols, cudaStream_t stream,
+                                      bool push = false)
 {
     const int N = int(plan->N);
     Stage st = make_stage(plan, stream);
@@ -806,6 +817,7 @@ static gs_status_t backtransform_cols(gs_plan* plan, const void* Uinv_, const vo
     p.c_rows = N; p.c_cols = ncols;
     p.klo_i = KPB; p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
     p.flags = F_MASK_A;
+    if (push) set_peers(plan, p, GS_PUSH_C, off);
     return launch(st, p, true, L_BACK_TRMM);
 }
 
@@ -867,6 +879,18 @@ gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uin
     GS_TRY(zero_lower(st, Uinv_));
     const MatView vU{U_, N, N, N}, vV{Uinv_, N, N, N}, vT{big_ptr(plan), N, N, N};
     GS_TRY(invert_levels(st, vU, 0, vV, 0, vT, 0, jb1, L_TRTRI_W, L_TRTRI_X, P));
+    if (!plan->push[GS_PUSH_UINV].empty()) {   // the diagonal band of the slab goes out by a copy kernel, the rest from the engine
+        PushTargets pt{};
+        pt.n = int(plan->push[GS_PUSH_UINV].size());
+        for (int d = 0; d < pt.n; ++d) pt.ptr[d] = plan->push[GS_PUSH_UINV][d];
+        const int band = P * lb;
+        dim3 grid((band + 255) / 256, unsigned(ncols));
+        LaunchTimer timer(plan, L_PUSH_BAND, stream);
+        if (plan->z) push_band_kernel<double2><<<grid, 256, 0, stream>>>(static_cast<const double2*>(Uinv_), pt, plan->N, N, int(col0), band, info_ptr(plan));
+        else push_band_kernel<double><<<grid, 256, 0, stream>>>(static_cast<const double*>(Uinv_), pt, plan->N, N, int(col0), band, info_ptr(plan));
+        GS_CUDA(plan, cudaGetLastError());
+        plan->launches += 1;
+    }
     const int npan = (jb1 + P - 1) / P;
     if (npan < 2) return GS_OK;
     {
@@ -886,6 +910,7 @@ gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uin
             p.klo_i = KPB; p.khi_c = P * KPB; p.kmax = P * KPB;
             p.a.x0 = r0 * lb; p.a.k0 = r0 * lb; p.b.k0 = r0 * lb; p.b.x0 = cb * lb;
             p.alpha = -1.0;
+            set_peers(plan, p, GS_PUSH_UINV);
             GS_TRY(launch(st, p, true, L_TRTRI_X));
         }
         if (i == 0) break;
@@ -927,6 +952,7 @@ gs_status_t gs_to_standard_g_cols(gs_plan_t* plan, const void* H_, const void* U
     p.c_rows = N; p.c_cols = int(col0 + ncols);
     p.klo_i = kt; p.khi_c = kt * (jb0 + 1); p.khi_j = kt; p.kmax = (N + st.bk - 1) / st.bk;
     p.flags = F_MASK_A | F_LOWER_A | F_HALF_DIAG_A | F_MASK_B;
+    set_peers(plan, p, GS_PUSH_G);
     return launch(st, p, false, L_TOSTD_G);
 }
 
@@ -957,6 +983,7 @@ gs_status_t gs_to_standard_cols(gs_plan_t* plan, const void* Uinv_, const void* 
     // tiles below the diagonal (I > jb0 + J) get an empty k-range and store nothing: k_lo = kmax (I - jb0 - J)
     p.klo_c = -p.kmax * jb0; p.klo_i = p.kmax; p.klo_j = -p.kmax;
     p.flags = F_DUAL | F_MASK_A | F_MASK_B2 | F_STORE_UPPER | F_REAL_DIAG;
+    set_peers(plan, p, GS_PUSH_HTILDE);
     return launch(st, p, false, L_TOSTD_SYR2K);
 }
 
@@ -971,7 +998,56 @@ gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv_, const void
         !aligned16(Ctilde_) || !aligned16(C_))
         return GS_ERR_INVALID_ARG;
     if (!plan->z && ((col0 * plan->N) % 2 != 0)) return GS_ERR_INVALID_ARG;   // 16-byte aligned column start
-    return backtransform_cols(plan, Uinv_, Ctilde_, C_, int(col0), int(ncols), static_cast<cudaStream_t>(cuda_stream));
+    return backtransform_cols(plan, Uinv_, Ctilde_, C_, int(col0), int(ncols), static_cast<cudaStream_t>(cuda_stream), true);
+}
+
+// Fused exchange: see include/gs.h.
+gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int count, void* const* targets)
+{
+    if (plan == nullptr || int(kind) < 0 || int(kind) > 3 || count < 0 || count > kMaxPeers || (count > 0 && targets == nullptr))
+        return GS_ERR_INVALID_ARG;
+    for (int d = 0; d < count; ++d)
+        if (targets[d] == nullptr || !aligned16(targets[d])) return GS_ERR_INVALID_ARG;
+    plan->push[kind].assign(targets, targets + count);
+    return GS_OK;
+}
+
+// CUDA IPC plumbing for the push targets: a device allocation of another process (one process per GPU) mapped here.
+gs_status_t gs_ipc_export(const void* dev_ptr, unsigned char* handle64, uint64_t* offset)
+{
+    if (dev_ptr == nullptr || handle64 == nullptr || offset == nullptr) return GS_ERR_INVALID_ARG;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+        return GS_ERR_CUDA;
+    CUdeviceptr base = 0;
+    size_t size = 0;
+    if (reinterpret_cast<CUresult (*)(CUdeviceptr*, size_t*, CUdeviceptr)>(fn)(&base, &size, reinterpret_cast<CUdeviceptr>(dev_ptr)) != CUDA_SUCCESS)
+        return GS_ERR_CUDA;
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, reinterpret_cast<void*>(base)) != cudaSuccess) { cudaGetLastError(); return GS_ERR_CUDA; }
+    std::memcpy(handle64, &h, 64);
+    *offset = uint64_t(reinterpret_cast<CUdeviceptr>(dev_ptr) - base);
+    return GS_OK;
+}
+
+gs_status_t gs_ipc_open(const unsigned char* handle64, uint64_t offset, void** dev_ptr)
+{
+    if (handle64 == nullptr || dev_ptr == nullptr) return GS_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, handle64, 64);
+    void* base = nullptr;
+    if (cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return GS_ERR_CUDA; }
+    *dev_ptr = static_cast<unsigned char*>(base) + offset;
+    return GS_OK;
+}
+
+gs_status_t gs_ipc_close(void* dev_ptr, uint64_t offset)
+{
+    if (dev_ptr == nullptr) return GS_ERR_INVALID_ARG;
+    if (cudaIpcCloseMemHandle(static_cast<unsigned char*>(dev_ptr) - offset) != cudaSuccess) { cudaGetLastError(); return GS_ERR_CUDA; }
+    return GS_OK;
 }
 
 // P(i,j) = sum_l f_l conj(C(i,l)) C(j,l) = (X^H X)(i,j) with X(l,i) = sqrt(f_l) C(i,l): one transpose-and-scale

@@ -272,6 +272,28 @@ __global__ void zero_lower_blocks_kernel(T* __restrict__ X, long long ld, int N,
         X[row + (long long)col * ld] = T{};
 }
 
+// Fused-exchange helper of the column-range inversion: copies, for every column c of [col0, col0 + ncols),
+// the rows of the diagonal band it lies in (rows [band * floor(c / band), + band), clipped to N) from src to
+// each of the n push targets (same layout).  That band -- the inverted diagonal panel blocks -- is the only
+// part of a rank's U^-1 slab that the tile engine's own push (EngineParams::peer) does not carry.
+struct PushTargets {
+    void* ptr[8];
+    int n;
+};
+template <typename T>
+__global__ void push_band_kernel(const T* __restrict__ src, PushTargets dst, long long ld, int N, int col0, int band, const int* info)
+{
+    if (*info != 0) return;
+    const int col = col0 + blockIdx.y;
+    const int r0 = (col / band) * band;
+    const int r1 = min(r0 + band, N);
+    for (int row = r0 + blockIdx.x * blockDim.x + threadIdx.x; row < r1; row += gridDim.x * blockDim.x) {
+        const long long off = row + (long long)col * ld;
+        const T v = src[off];
+        for (int d = 0; d < dst.n; ++d) static_cast<T*>(dst.ptr[d])[off] = v;
+    }
+}
+
 // dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid row (blockIdx.y) per column c.
 template <typename T>
 __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst, long long ld, int row0, int rows,

@@ -76,6 +76,8 @@ struct RawOperand {
     int rows, cols;
 };
 
+constexpr int kMaxPeers = 8;   // push targets of one launch: the GPUs of one NVSwitch domain
+
 struct EngineParams {
     CUtensorMap mapA, mapB, mapA2, mapB2;
     RawOperand rawA, rawB, rawA2, rawB2;
@@ -92,6 +94,12 @@ struct EngineParams {
     OperandCoord a, b, a2, b2;
     uint32_t flags;
     double alpha, beta;
+    // Fused exchange (sharded path): every C element this launch stores whose global column is >= peer_col0
+    // is ALSO stored, at the same (row, col, ldc), into each of the npeer matrices peer[d] -- buffers of the
+    // other ranks mapped over NVLink (or further local buffers).  Posted remote stores: the transfer runs
+    // beside the mainloops of the CTAs that follow, tile by tile; nothing is read back.
+    double* peer[kMaxPeers];
+    int npeer, peer_col0;
 };
 
 // Returns false for the padding CTAs of a super-tiled triangular grid (they exit at once).
@@ -447,6 +455,22 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
                 const long long col = c_col(ng, e);
                 if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col))
                     p.C[row + col * p.ldc] = alpha * acc[mg][ng][e];
+            }
+        }
+    }
+    for (int d = 0; d < p.npeer; ++d) {   // fused exchange: the same tile to every push target
+        double* Cd = p.peer[d];
+#pragma unroll
+        for (int mg = 0; mg < 4; ++mg) {
+            const long long row = c_row(mg);
+#pragma unroll
+            for (int ng = 0; ng < 8; ++ng) {
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const long long col = c_col(ng, e);
+                    if (row < p.c_rows && col < p.c_cols && col >= p.peer_col0 && (!upper_only || row <= col))
+                        Cd[row + col * p.ldc] = alpha * acc[mg][ng][e];
+                }
             }
         }
     }

@@ -20,6 +20,7 @@ import torch
 from .workloads import is_colmajor
 
 GS_REAL64, GS_COMPLEX128 = 0, 1
+GS_PUSH_UINV, GS_PUSH_G, GS_PUSH_HTILDE, GS_PUSH_C = 0, 1, 2, 3
 GS_OK = 0
 STATUS_NAMES = {
     0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_NOT_POSDEF", 3: "GS_ERR_SINGULAR",
@@ -29,6 +30,7 @@ EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
     "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
+    "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
@@ -82,6 +84,10 @@ def lib() -> ctypes.CDLL:
         L.gs_to_standard_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_backtransform_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
+        L.gs_plan_set_push_targets.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp)]
+        L.gs_ipc_export.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ctypes.c_uint64)]
+        L.gs_ipc_open.argtypes = [ctypes.c_char_p, ctypes.c_uint64, ctypes.POINTER(vp)]
+        L.gs_ipc_close.argtypes = [vp, ctypes.c_uint64]
         L.gs_reduce_host_scratch_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host_h2d_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_reduce_host_d2h_bytes.argtypes = [vp, ctypes.POINTER(sz)]
@@ -221,6 +227,11 @@ class Plan:
                                                 _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
                                                 _dev_ptr(C, self.N, self.nev, self.tdtype), col0, ncols, _stream_ptr(stream)))
 
+    def set_push_targets(self, kind: int, ptrs):
+        """Fused exchange: device pointers (ints) the column-range call of `kind` also stores into."""
+        arr = (ctypes.c_void_p * max(1, len(ptrs)))(*ptrs)
+        self._check(lib().gs_plan_set_push_targets(self._h, kind, len(ptrs), arr))
+
     def density_matrix(self, C: torch.Tensor, f: torch.Tensor, P: torch.Tensor, stream=None):
         """P(i,j) = sum_l f[l] conj(C(i,l)) C(j,l); upper triangle of P is written."""
         if self.nev == 0:
@@ -290,6 +301,29 @@ class Plan:
         n = ctypes.c_int(0)
         self._check(lib().gs_plan_launch_times(self._h, buf, 16, ctypes.byref(n)))
         return {buf[i].label.decode(): (int(buf[i].launches), float(buf[i].ms)) for i in range(min(n.value, 16))}
+
+
+def ipc_export(t: torch.Tensor):
+    """(64-byte handle, byte offset) of the device allocation behind a CUDA tensor, for another process."""
+    buf = ctypes.create_string_buffer(64)
+    off = ctypes.c_uint64(0)
+    st = lib().gs_ipc_export(t.data_ptr(), buf, ctypes.byref(off))
+    if st != GS_OK:
+        raise GsError(st, 0, "gs_ipc_export")
+    return bytes(buf.raw), int(off.value)
+
+
+def ipc_open(handle: bytes, offset: int) -> int:
+    """Maps a peer's allocation into this process; returns the device pointer of the peer's tensor."""
+    ptr = ctypes.c_void_p()
+    st = lib().gs_ipc_open(handle, offset, ctypes.byref(ptr))
+    if st != GS_OK:
+        raise GsError(st, 0, "gs_ipc_open")
+    return int(ptr.value)
+
+
+def ipc_close(ptr: int, offset: int) -> None:
+    lib().gs_ipc_close(ptr, offset)
 
 
 def generalized_to_standard(H: torch.Tensor, S: torch.Tensor, nev: int | None = None):

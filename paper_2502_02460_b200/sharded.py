@@ -15,10 +15,16 @@ formed:
     and, once the eigenvectors C~ of H~ are known (off the path), rank r forms the eigenvector
     columns K_r of C = V C~ (gs_backtransform_cols).
 
-A column range of a column-major matrix is one contiguous slab, so the exchange is a plain
-all-gather of unequal slabs (one broadcast per owner; NCCL over NVLink on the GPUs, gloo in the
-CPU test of this host logic).  The cost of column c grows like c^2 in all three steps, so the
-ranges are cut where the CUBE of the column index reaches equal shares.
+A column range of a column-major matrix is one contiguous slab.  Two forms of the exchange:
+  exchange="push" (the GPU default): FUSED into the producing kernels.  The other ranks' buffers are mapped
+      over NVLink/NVSwitch peer memory (CUDA IPC) and registered as push targets of the plan; the
+      epilogues of the column-range kernels store every tile they produce into all of them (posted
+      remote stores), so the slabs travel while the rest of the range is still being computed and
+      step 3 is separated from steps 1-2 only by a stream synchronise and a barrier.
+  exchange="collective": an all-gather of unequal slabs after the kernels (one broadcast per owner;
+      NCCL on the GPUs, gloo in the CPU test of this host logic) -- the baseline form.
+The cost of column c grows like c^2 in all three steps, so the ranges are cut where the CUBE of the
+column index reaches equal shares.
 
 This module is host logic only: ranges, the order of the calls, the exchange.  All arithmetic runs
 in libgs through the `plan` object (gs.Plan); there is no other implementation behind it.
@@ -93,53 +99,136 @@ class ShardedResult:
     G: torch.Tensor          # complete on every rank after the exchange
     Htilde: torch.Tensor     # upper triangle; only the columns of `cols` are valid before gather_htilde()
     cols: tuple[int, int]
+    Uinv_work: torch.Tensor | None = None   # push mode: the rank's private work buffer of step 2
+    C: torch.Tensor | None = None           # push mode: the registered N x nev back-transform result
+
+
+class PeerMap:
+    """Push mode: exchanges CUDA IPC handles of the ranks' buffers over the process group, maps the
+    peers' allocations into this process and registers them as push targets of the plan."""
+
+    def __init__(self, plan, rank: int, world: int, group=None):
+        self.plan, self.rank, self.world, self.group = plan, rank, world, group
+        self._bases = {}     # (owner rank, IPC handle) -> base pointer of the mapping (an allocation is mapped once)
+
+    def register(self, kind: int, local: torch.Tensor, include_self: bool) -> None:
+        from . import gs
+        mine = gs.ipc_export(local)
+        infos = [None] * self.world
+        dist.all_gather_object(infos, mine, group=self.group)
+        ptrs = []
+        for s, (handle, off) in enumerate(infos):
+            if s == self.rank:
+                if include_self:
+                    ptrs.append(local.data_ptr())
+                continue
+            if (s, handle) not in self._bases:
+                self._bases[(s, handle)] = gs.ipc_open(handle, 0)
+            ptrs.append(self._bases[(s, handle)] + off)
+        self.plan.set_push_targets(kind, ptrs)
+
+    def close(self) -> None:
+        from . import gs
+        for kind in range(4):
+            self.plan.set_push_targets(kind, [])
+        for base in self._bases.values():
+            gs.ipc_close(base, 0)
+        self._bases = {}
 
 
 class ShardedReduction:
     """Host driver of the sharded path for one rank.  `plan` is a gs.Plan (or, in the CPU test of this
-    host logic, an object with the same column-range methods)."""
+    host logic, an object with the same column-range methods -- exchange="collective" only)."""
 
-    def __init__(self, plan, rank: int = 0, world: int = 1, group=None):
+    def __init__(self, plan, rank: int = 0, world: int = 1, group=None, exchange: str = "collective"):
+        if exchange not in ("collective", "push"):
+            raise ValueError("exchange must be 'collective' or 'push'")
         self.plan = plan
         self.rank, self.world, self.group = int(rank), int(world), group
+        self.push = exchange == "push" and self.world > 1
         self.N, self.nev = plan.N, plan.nev
         self.ranges = column_ranges(self.N, self.world, plan.block)
         self.eig_ranges = even_ranges(self.nev, self.world, 2)
+        self.peers = None
+
+    def _barrier(self) -> None:
+        if self.world > 1:
+            dist.barrier(group=self.group)
 
     def alloc(self, like: torch.Tensor) -> ShardedResult:
-        """The four N x N result buffers of reduce() (so a loop of reductions allocates once)."""
+        """The N x N result buffers of reduce() (so a loop of reductions allocates once).  Push mode:
+        collective over the ranks -- also maps the peers' buffers and registers the push targets."""
         N = self.N
         U, Uinv, G = (colmajor_empty(N, N, dtype=like.dtype, device=like.device) for _ in range(3))
         Ht = colmajor_zeros(N, N, dtype=like.dtype, device=like.device)
-        return ShardedResult(U, Uinv, G, Ht, self.ranges[self.rank])
+        res = ShardedResult(U, Uinv, G, Ht, self.ranges[self.rank])
+        if self.push:
+            from . import gs
+            res.Uinv.zero_()               # exchange buffer: nothing is ever pushed below the diagonal
+            res.Uinv_work = colmajor_empty(N, N, dtype=like.dtype, device=like.device)
+            res.C = colmajor_empty(N, max(self.nev, 1), dtype=like.dtype, device=like.device)[:, :self.nev]
+            torch.cuda.synchronize(like.device)
+            self.peers = PeerMap(self.plan, self.rank, self.world, self.group)
+            self.peers.register(gs.GS_PUSH_UINV, res.Uinv, include_self=True)
+            self.peers.register(gs.GS_PUSH_G, res.G, include_self=False)
+            self.peers.register(gs.GS_PUSH_HTILDE, res.Htilde, include_self=False)
+            if self.nev > 0:
+                self.peers.register(gs.GS_PUSH_C, res.C, include_self=False)
+            self._barrier()
+        return res
+
+    def close(self) -> None:
+        """Push mode: collective; unmaps the peers' buffers (call before the buffers are freed)."""
+        if self.peers is not None:
+            torch.cuda.synchronize()
+            self._barrier()
+            self.peers.close()
+            self.peers = None
+            self._barrier()
 
     def reduce(self, H: torch.Tensor, S: torch.Tensor, stream=None, out: ShardedResult | None = None) -> ShardedResult:
         """Steps 1-3.  H, S: column-major N x N on this rank's device, identical on all ranks; S is not
-        modified.  Returns this rank's columns of the upper triangle of H~ (and U, U^-1, G in full)."""
+        modified.  Returns this rank's columns of the upper triangle of H~ (and U, U^-1, G in full;
+        push mode: H~ in full too, once every rank has returned and a barrier has passed)."""
         plan = self.plan
         res = self.alloc(H) if out is None else out
         c0, c1 = res.cols
         U, Uinv, G, Ht = res.U, res.Uinv, res.G, res.Htilde
+        if self.push:
+            self._barrier()                # the peers have finished reading what the last round pushed
         U.copy_(S)
         plan.cholesky(U, stream=stream)                                   # replicated
-        plan.invert_triangular_cols(U, Uinv, c0, c1 - c0, stream=stream)
-        plan.to_standard_g_cols(H, Uinv, G, c0, c1 - c0, stream=stream)
+        work = res.Uinv_work if self.push else Uinv
+        plan.invert_triangular_cols(U, work, c0, c1 - c0, stream=stream)  # push: slab -> every rank's Uinv
+        plan.to_standard_g_cols(H, work, G, c0, c1 - c0, stream=stream)   # push: slab -> every other rank's G
         plan.last_info(stream=stream)                                     # synchronises: the slabs are final
-        exchange_slabs((Uinv, G), self.ranges, self.rank, self.world, self.group)
+        if self.push:
+            self._barrier()                # ... and have landed everywhere
+        else:
+            exchange_slabs((Uinv, G), self.ranges, self.rank, self.world, self.group)
         plan.to_standard_cols(Uinv, G, Ht, c0, c1 - c0, stream=stream)
         plan.last_info(stream=stream)
         return res
 
     def gather_htilde(self, res: ShardedResult) -> torch.Tensor:
         """Every rank gets all columns of the upper triangle of H~ (for an off-path eigensolver)."""
-        exchange_slabs((res.Htilde,), self.ranges, self.rank, self.world, self.group)
+        if self.push:
+            self._barrier()                # step 3 already pushed them
+        else:
+            exchange_slabs((res.Htilde,), self.ranges, self.rank, self.world, self.group)
         return res.Htilde
 
     def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, stream=None, out: torch.Tensor | None = None) -> torch.Tensor:
-        """C = U^-1 C~, eigenvector columns split evenly over the ranks, then gathered."""
+        """C = U^-1 C~, eigenvector columns split evenly over the ranks, then gathered.  Push mode:
+        `out` must be the registered buffer (ShardedResult.C of alloc())."""
         C = colmajor_empty(self.N, self.nev, dtype=Ctilde.dtype, device=Ctilde.device) if out is None else out
         k0, k1 = self.eig_ranges[self.rank]
+        if self.push and out is None:
+            raise ValueError("push mode: pass out=res.C (the buffer whose peers are registered)")
         self.plan.backtransform_cols(Uinv, Ctilde, C, k0, k1 - k0, stream=stream)
         self.plan.last_info(stream=stream)
-        exchange_slabs((C,), self.eig_ranges, self.rank, self.world, self.group)
+        if self.push:
+            self._barrier()
+        else:
+            exchange_slabs((C,), self.eig_ranges, self.rank, self.world, self.group)
         return C

@@ -131,3 +131,73 @@ def test_column_range_argument_errors():
         plan.backtransform_cols(A, Ct, Co, 32, 64)
     plan.invert_triangular_cols(A, B, 0, 0)      # empty range: no-op
     plan.close()
+
+
+@pytest.mark.parametrize("N,cplx", [(1100, False), (650, True)])
+def test_push_targets_receive_exactly_the_slab(N, cplx):
+    """Fused exchange, kernel side (gs_plan_set_push_targets): with two further LOCAL buffers registered as
+    push targets, every column-range call leaves in each of them bit for bit what it leaves in its own
+    output inside the range (upper part), and touches nothing outside."""
+    gs = _gs()
+    p = wl.small_pencil(N, seed=3, complex=cplx)
+    dt = p.H.dtype
+    H, S = wl.to_colmajor(p.H.cuda()), wl.to_colmajor(p.S.cuda())
+    nev = N // 2
+    plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
+    U = wl.colmajor_empty(N, N, dtype=dt, device="cuda")
+    U.copy_(S)
+    plan.cholesky(U)
+    c0, c1 = sharded.column_ranges(N, 3, plan.block)[1]
+    assert 0 < c0 < c1 < N
+    SENT = -7.25
+
+    def targets(cols):
+        t = [wl.colmajor_empty(N, cols, dtype=dt, device="cuda") for _ in range(2)]
+        for x in t:
+            x.fill_(SENT)
+        return t
+
+    def check(own, tgts, a, b, upper):
+        for x in tgts:
+            inside_own, inside = own[:, a:b], x[:, a:b]
+            if upper:
+                mask = torch.ones(N, N, dtype=torch.bool, device="cuda").triu()[:, a:b]
+                assert torch.equal(inside[mask], inside_own[mask])
+            else:
+                assert torch.equal(inside, inside_own)
+            assert bool((x[:, :a] == SENT).all()) and bool((x[:, b:] == SENT).all())
+
+    V = _nan(N, N, dt)
+    tv = targets(N)
+    plan.set_push_targets(gs.GS_PUSH_UINV, [x.data_ptr() for x in tv])
+    plan.invert_triangular_cols(U, V, c0, c1 - c0)
+    plan.last_info()
+    check(V, tv, c0, c1, upper=True)
+    G = _nan(N, N, dt)
+    tg = targets(N)
+    plan.set_push_targets(gs.GS_PUSH_G, [x.data_ptr() for x in tg])
+    plan.to_standard_g_cols(H, V, G, c0, c1 - c0)
+    plan.last_info()
+    check(G, tg, c0, c1, upper=True)
+    # complete V, G by the whole-range call, then step 3 and the back-transform with targets
+    plan.set_push_targets(gs.GS_PUSH_UINV, [])
+    plan.set_push_targets(gs.GS_PUSH_G, [])
+    plan.invert_triangular_cols(U, V, 0, N)
+    plan.to_standard_g_cols(H, V, G, 0, N)
+    Ht = _nan(N, N, dt)
+    th = targets(N)
+    plan.set_push_targets(gs.GS_PUSH_HTILDE, [x.data_ptr() for x in th])
+    plan.to_standard_cols(V, G, Ht, c0, c1 - c0)
+    plan.last_info()
+    check(Ht, th, c0, c1, upper=True)
+    Ct = wl.to_colmajor(wl.dense_rhs(N, nev, seed=8, complex=cplx).cuda())
+    C = _nan(N, nev, dt)
+    tc = targets(nev)
+    plan.set_push_targets(gs.GS_PUSH_C, [x.data_ptr() for x in tc])
+    k0, k1 = sharded.even_ranges(nev, 3, 2)[1]
+    plan.backtransform_cols(V, Ct, C, k0, k1 - k0)
+    plan.last_info()
+    check(C, tc, k0, k1, upper=False)
+    with pytest.raises(gs.GsError):
+        plan.set_push_targets(gs.GS_PUSH_C, [1] * 9)
+    plan.close()
