@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--batch-n", type=int, default=2048)
     ap.add_argument("--sharded", action="store_true",
                     help="NEXT-3: ONE pencil over all ranks (steps 2-4 by column ranges, one exchange); strong scaling, not the headline mode")
+    ap.add_argument("--exchange", default="push", choices=["push", "collective"],
+                    help="--sharded: slabs stored into the peers' buffers from the kernel epilogues (push) or NCCL broadcasts after the kernels")
     ap.add_argument("--shard-shares", type=int, default=0,
                     help="NEXT-3: time, on ONE GPU and one after the other, the share each of R ranks would run (not the headline)")
     ap.add_argument("--batch-complex", action="store_true")
@@ -511,10 +513,10 @@ def run_sharded(args):
     N, nev, cplx = cfg.N, cfg.nev, cfg.complex
     pen = wl.make_pencil(N, cfg.box, cfg.seed, complex=cplx, device=dev)      # the same on every rank
     plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64, device=dev)
-    drv = sharded.ShardedReduction(plan, info.rank, info.world)
+    drv = sharded.ShardedReduction(plan, info.rank, info.world, exchange=args.exchange)
     bufs = drv.alloc(pen.H)
     Ct = wl.dense_rhs(N, nev, seed=0, complex=cplx, device=dev)
-    C = wl.colmajor_empty(N, nev, dtype=pen.H.dtype, device=dev)
+    C = bufs.C if drv.push else wl.colmajor_empty(N, nev, dtype=pen.H.dtype, device=dev)
 
     def step():
         res = drv.reduce(pen.H, pen.S, out=bufs)
@@ -553,8 +555,11 @@ def run_sharded(args):
                           "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
                                      "parallelism": f"sharded x{info.world}: step 1 replicated, steps 2-4 by column ranges, "
                                                     "one exchange of the U^-1 and G slabs (NEXT-3)",
+                                     "exchange": ("push: fused into the kernel epilogues over peer memory" if drv.push else
+                                                  "collective: broadcasts after the kernels" if info.world > 1 else "none (one rank)"),
                                      "column_ranges": drv.ranges},
                           "gpu_launches": launches, "checks": checks}))
+    drv.close()
     replicas.finalize(info)
 
 
