@@ -55,11 +55,22 @@ __device__ __forceinline__ void cfnma(double2& a, double2 x, double2 y)
 
 __device__ __forceinline__ void cleaf_load_upper(const CLeafSmem& s, const double2* blk, long long ld, int nb, int t)
 {
-    for (int idx = t; idx < CLB * CLB; idx += kCLeafThreads) {
-        const int row = idx & (CLB - 1), col = idx >> 6;
-        double2 v = make_double2((row == col) ? 1.0 : 0.0, 0.0);
-        if (row <= col && col < nb) v = blk[row + (long long)col * ld];
-        s.U[row + col * CLP] = v;
+    constexpr int kBatch = 8;   // independent loads in flight per thread (leaf_kernels.cuh: leaf_load_upper)
+#pragma unroll 1
+    for (int base = t; base < CLB * CLB; base += kCLeafThreads * kBatch) {
+        double2 v[kBatch];
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * kCLeafThreads;
+            const int row = idx & (CLB - 1), col = idx >> 6;
+            v[u] = make_double2((row == col) ? 1.0 : 0.0, 0.0);
+            if (row <= col && col < nb) v[u] = blk[row + (long long)col * ld];
+        }
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * kCLeafThreads;
+            s.U[(idx & (CLB - 1)) + (idx >> 6) * CLP] = v[u];
+        }
     }
 }
 

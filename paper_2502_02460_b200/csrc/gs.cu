@@ -80,6 +80,7 @@ struct gs_plan {
     int ctile_half = 1;              // complex: two 64 x 32 CTAs per logical tile (3 CTAs/SM) instead of one 64 x 64
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
     std::vector<void*> push[4];      // fused exchange: push targets per gs_push_kind_t (gs_plan_set_push_targets)
+    int leaf_blocked = 0;            // real POTRF diagonal blocks: blocked sweep (potrf_leaf4_kernel) instead of the rank-1 sweep
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
@@ -341,7 +342,7 @@ struct Potrf {
             e = launch_pdl(potrf_cleaf_kernel, 1, kCLeafThreads, kCLeafSmemBytes, st.stream, static_cast<double2*>(S), plan->N, int(plan->N),
                            b * st.lb, static_cast<double2*>(w), vW.ld, info_ptr(plan));
         else
-            e = launch_pdl(potrf_leaf_kernel, 1, kLeafThreads, kLeafSmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
+            e = launch_pdl(plan->leaf_blocked ? potrf_leaf4_kernel : potrf_leaf_kernel, 1, kLeafThreads, kLeafSmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
                            b * st.lb, static_cast<double*>(w), vW.ld, info_ptr(plan));
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
@@ -569,6 +570,7 @@ gs_status_t configure_leaf(gs_plan* plan)
     static bool done = false;
     if (done) return GS_OK;
     GS_CUDA(plan, cudaFuncSetAttribute(potrf_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
+    GS_CUDA(plan, cudaFuncSetAttribute(potrf_leaf4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
     GS_CUDA(plan, cudaFuncSetAttribute(trtri_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
     GS_CUDA(plan, cudaFuncSetAttribute(potrf_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
     GS_CUDA(plan, cudaFuncSetAttribute(trtri_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
@@ -620,6 +622,7 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_TILE64", 0, 2, &p->tile64_mode);
     knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
+    knob("GS_LEAF_BLOCKED", 0, 1, &p->leaf_blocked);
     int shard_log2 = p->z ? 4 : 3;   // 1024 rows per panel of the column-range inversion
     knob("GS_SHARD_PANEL_LOG2", 0, 8, &shard_log2);
     p->shard_panel = 1 << shard_log2;

@@ -48,11 +48,24 @@ __device__ __forceinline__ LeafSmem leaf_smem(unsigned char* raw)
 // (identity-padded beyond nb, zero below the diagonal).
 __device__ __forceinline__ void leaf_load_upper(const LeafSmem& s, const double* blk, long long ld, int nb, int t)
 {
-    for (int idx = t; idx < LB * LB; idx += kLeafThreads) {
-        const int row = idx & (LB - 1), col = idx >> 7;
-        double v = (row == col) ? 1.0 : 0.0;
-        if (row <= col && col < nb) v = blk[row + (long long)col * ld];
-        s.U[row + col * LP] = v;
+    // batches of 8 independent (predicated) loads in flight per thread: the one-at-a-time loop spent ~19k
+    // cycles (15 % of the kernel) waiting on global latency (profiles/r01g_sharded.md, leaf notes)
+    constexpr int kBatch = 8;
+#pragma unroll 1
+    for (int base = t; base < LB * LB; base += kLeafThreads * kBatch) {
+        double v[kBatch];
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * kLeafThreads;
+            const int row = idx & (LB - 1), col = idx >> 7;
+            v[u] = (row == col) ? 1.0 : 0.0;
+            if (row <= col && col < nb) v[u] = blk[row + (long long)col * ld];
+        }
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * kLeafThreads;
+            s.U[(idx & (LB - 1)) + (idx >> 7) * LP] = v[u];
+        }
     }
 }
 
@@ -217,6 +230,201 @@ potrf_leaf_kernel(double* __restrict__ S, long long ld, int N, int j0, double* _
             double w = 0.0;
             if (row == col) w = s.dinv[row];
             else if (row > col) w = a[r][c] * s.dinv[row];
+            s.U[col + row * LP] = w;
+        }
+    __syncthreads();
+    leaf_store_all(s, Winv, ldw, LB, t);
+}
+
+// ------------------------------------------------------------------------------------------------
+// potrf_leaf4_kernel: the same result as potrf_leaf_kernel (U_kk in place, W = U_kk^-1 out) by a
+// BLOCKED sweep over 32 panels of 4 rows.  The step of the rank-1 sweep is a latency chain (barrier,
+// broadcast, reciprocal: ~940 cycles, profiles/r01f_leaf_ncu.md); here a panel costs two barriers, and
+// its 4 x 4 diagonal block is factored by EVERY thread redundantly in registers (no communication
+// inside the four dependent pivots), followed by one rank-4 update.
+//
+// The register image Z (thread (ty,tx) holds Z(ty + 16 r, tx + 16 c)) is the elimination applied to
+// [S | I] at once: positions row <= col hold the Schur complement / finished rows of U, positions
+// row > col hold Y = rows of U^-T as they form (W(col,row) at the end).  Panel p = rows 4p .. 4p+3
+// (register row group r = p / 4, threads ty = 4 (p % 4) + q):
+//   A  the owners publish the panel rows Z(K, :)                                            -> barrier
+//   B  every thread: LDL^T of the 4 x 4 diagonal block with Y_KK formed by the same row operations
+//   C  the owners finish their rows: R = U_KK^-T Z(K, :) = dinv (Z + Y_KK Z) over all columns, and publish
+//      R (in-panel columns: the Y part)                                                      -> barrier
+//   D  rank-4 update of every row below the panel: Z(i, c) -= sum_k R(k, i) R(k, c) over the live
+//      columns (Y part: c <= panel end; Schur part: c >= i)
+// ------------------------------------------------------------------------------------------------
+constexpr int LQ = 4;                   // panel rows
+
+// Panels 4r .. 4r+3 (r is a template parameter so that every register index is static).
+// Returns false (in every thread alike) when a pivot is not positive.
+template <int r>
+__device__ __forceinline__ bool leaf4_group(double (&a)[8][8], double* Zp, double* Rb, int tx, int ty, int t, int j0, int* info)
+{
+#pragma unroll 1
+    for (int sgrp = 0; sgrp < 4; ++sgrp) {
+        const int p0 = 16 * r + 4 * sgrp;          // first row / column of the panel
+        const bool owner = (ty >> 2) == sgrp;
+        const int q = ty & 3;
+        // ---- A
+        if (owner) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) Zp[q * LB + tx + 16 * c] = a[r][c];
+        }
+        __syncthreads();
+        // ---- B: 4 x 4 diagonal block, every thread alike (upper part from the image; Y starts as the identity)
+        double z[LQ][LQ];
+#pragma unroll
+        for (int i = 0; i < LQ; ++i)
+#pragma unroll
+            for (int c = 0; c < LQ; ++c) z[i][c] = (c >= i) ? Zp[i * LB + p0 + c] : 0.0;
+        double dinv[LQ];
+#pragma unroll
+        for (int j = 0; j < LQ; ++j) {
+            const double d = z[j][j];
+            if (!(d > 0.0)) {   // the same in every thread: uniform exit
+                if (t == 0) atomicCAS(info, 0, j0 + p0 + j + 1);
+                return false;
+            }
+            const double invd = 1.0 / d;
+            dinv[j] = 1.0 / sqrt(d);
+#pragma unroll
+            for (int i = j + 1; i < LQ; ++i) {
+                const double li = z[j][i] * invd;
+#pragma unroll
+                for (int c = 0; c < LQ; ++c) {
+                    if (c >= i || c < j) z[i][c] = fma(-li, z[j][c], z[i][c]);
+                    else if (c == j) z[i][c] = -li;              // Y(i,j): the pivot row's Y(j,j) is 1
+                }
+            }
+        }
+        // ---- C: the owners finish row q of the panel
+        if (owner) {
+            double yq[LQ - 1], dq = dinv[0], zqq = z[0][0];
+#pragma unroll
+            for (int k = 0; k < LQ - 1; ++k) yq[k] = 0.0;
+#pragma unroll
+            for (int i = 1; i < LQ; ++i)
+                if (q == i) {
+                    dq = dinv[i]; zqq = z[i][i];
+#pragma unroll
+                    for (int k = 0; k < LQ - 1; ++k) yq[k] = (k < i) ? z[i][k] : 0.0;
+                }
+            double acc[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                acc[c] = Zp[q * LB + tx + 16 * c];
+#pragma unroll
+                for (int k = 0; k < LQ - 1; ++k) acc[c] = fma(yq[k], Zp[k * LB + tx + 16 * c], acc[c]);   // yq[k] = 0 for k >= q
+                acc[c] *= dq;
+            }
+            double pub = acc[r];
+            const int qc = tx - 4 * sgrp;             // column inside the panel (c == r only)
+            if (qc >= 0 && qc < LQ) {
+                // row q of the factored block: z[q][qc] (static indexing through selects)
+                double zq = 0.0;
+#pragma unroll
+                for (int i = 0; i < LQ; ++i)
+#pragma unroll
+                    for (int c = 0; c < LQ; ++c)
+                        if (i == q && c == qc) zq = z[i][c];
+                if (qc > q) { acc[r] = zq * dq; pub = 0.0; }              // U(q,qc)    | Y part above the diagonal is 0
+                else if (qc == q) { acc[r] = zqq * dq; pub = dq; }         // U(k,k)     | W(k,k)
+                else { acc[r] = zq * dq; pub = acc[r]; }                   // W(qc,q)
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                a[r][c] = acc[c];
+                Rb[q * LB + tx + 16 * c] = (c == r) ? pub : acc[c];
+            }
+        }
+        __syncthreads();
+        // ---- D: rank-4 update of the rows below the panel
+        const bool ylive = tx <= 4 * sgrp + 3;        // column group r: Y part (columns up to the panel's end)
+        const bool upper = tx >= ty;                  // diagonal register blocks: Schur part
+        const bool rowact = ty >= 4 * sgrp + 4;       // row group r: rows below the panel
+#pragma unroll
+        for (int k = 0; k < LQ; ++k) {
+            double cv[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) cv[c] = Rb[k * LB + tx + 16 * c];
+            {   // rows of the panel's own group
+                const double u = rowact ? -Rb[k * LB + ty + 16 * r] : 0.0;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    if (c < r || c > r) a[r][c] = fma(u, cv[c], a[r][c]);
+                    else if (ylive || upper) a[r][c] = fma(u, cv[c], a[r][c]);
+                }
+            }
+#pragma unroll
+            for (int rr = r + 1; rr < 8; ++rr) {
+                const double u = -Rb[k * LB + ty + 16 * rr];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    if (c < r || c > rr) a[rr][c] = fma(u, cv[c], a[rr][c]);
+                    else if (c == r) { if (ylive) a[rr][c] = fma(u, cv[c], a[rr][c]); }
+                    else if (c == rr) { if (upper) a[rr][c] = fma(u, cv[c], a[rr][c]); }
+                }
+            }
+        }
+        // (the next panel's step A writes Zp, which nobody reads after step C; Rb is rewritten after the next barrier)
+    }
+    return true;
+}
+
+__global__ void __launch_bounds__(kLeafThreads, 1)
+potrf_leaf4_kernel(double* __restrict__ S, long long ld, int N, int j0, double* __restrict__ Winv, long long ldw, int* info)
+{
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*info != 0) return;
+    extern __shared__ __align__(16) unsigned char leaf_raw[];
+    const LeafSmem s = leaf_smem(leaf_raw);
+    const int t = threadIdx.x, tx = t & 15, ty = t >> 4;
+    const int nb = min(LB, N - j0);
+    double* blk = S + j0 + (long long)j0 * ld;
+
+    leaf_load_upper(s, blk, ld, nb, t);
+    __syncthreads();
+    double a[8][8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) a[r][c] = s.U[ty + 16 * r + (tx + 16 * c) * LP];
+    __syncthreads();   // the image is free now: the panel buffers live in it
+    double* Zp = s.U;                        // [4][128] panel rows as published
+    double* Rb = s.U + LQ * LB;              // [4][128] finished panel rows (in-panel columns: Y part)
+
+    if (!leaf4_group<0>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<1>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<2>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<3>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<4>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<5>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<6>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    if (!leaf4_group<7>(a, Zp, Rb, tx, ty, t, j0, info)) return;
+    __syncthreads();
+
+    // shared image = U (upper) with zeros below; write it out
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            s.U[row + col * LP] = (row <= col) ? a[r][c] : 0.0;
+        }
+    __syncthreads();
+    leaf_store_all(s, blk, ld, nb, t);
+    __syncthreads();
+    // W = U^-1: the register at (row, col), row > col, is W(col, row); W(k,k) = 1 / U(k,k)
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int row = ty + 16 * r, col = tx + 16 * c;
+            double w = 0.0;
+            if (row == col) w = 1.0 / a[r][c];
+            else if (row > col) w = a[r][c];
             s.U[col + row * LP] = w;
         }
     __syncthreads();
