@@ -80,6 +80,13 @@ gs_status_t gs_plan_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t b
  * trailing update on FP64 tensor-core (DMMA) tiles. */
 gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream);
 
+/* Step 1 restricted to the leading ncols x ncols block of S_inout (ncols a multiple of the block
+ * order -- 128 real, 64 complex -- or equal to N): the leading principal blocks of the factor nest,
+ * chol(S[:k,:k]) = U[:k,:k], so a rank of the sharded path that owns columns up to k factors only
+ * that block.  Upper triangle of the leading block: U; strictly-lower blocks of the whole buffer:
+ * zero; everything else in columns >= ncols is left as it was (still S).  ncols == 0 is a no-op. */
+gs_status_t gs_cholesky_leading(gs_plan_t* plan, void* S_inout, int64_t ncols, void* cuda_stream);
+
 /* Step 2.  Reads the upper triangle of U (N x N); writes Uinv = U^-1 (upper
  * triangle) and zeros below the diagonal.  Uinv must not alias U.  Blocked TRTRI. */
 gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U, void* Uinv, void* cuda_stream);

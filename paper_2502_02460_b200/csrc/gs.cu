@@ -666,7 +666,8 @@ gs_status_t gs_plan_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t b
     return GS_OK;
 }
 
-gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
+// the leading nlead blocks (leading principal blocks of a Cholesky factor nest: chol(S[:k,:k]) = U[:k,:k])
+static gs_status_t cholesky_blocks(gs_plan_t* plan, void* S_inout, int nlead, void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
     if (S_inout == nullptr || !aligned16(S_inout)) return GS_ERR_INVALID_ARG;
@@ -689,7 +690,7 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     f.st.stream = plan->side;
     const gs_status_t zs = zero_lower(f.st, S);
     f.st.stream = stream;
-    const gs_status_t fs = zs == GS_OK ? f.factor(plan->nblk, stream) : zs;
+    const gs_status_t fs = zs == GS_OK ? f.factor(nlead, stream) : zs;
     // factor() joins the side stream after every panel; a single-panel factorisation has no join of its own
     const cudaError_t e1 = cudaEventRecord(plan->ev_join, plan->side);
     const cudaError_t e2 = cudaStreamWaitEvent(stream, plan->ev_join, 0);
@@ -697,6 +698,19 @@ gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
     GS_CUDA(plan, e1);
     GS_CUDA(plan, e2);
     return GS_OK;
+}
+
+gs_status_t gs_cholesky(gs_plan_t* plan, void* S_inout, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    return cholesky_blocks(plan, S_inout, plan->nblk, cuda_stream);
+}
+
+gs_status_t gs_cholesky_leading(gs_plan_t* plan, void* S_inout, int64_t ncols, void* cuda_stream)
+{
+    if (plan == nullptr || ncols < 0 || ncols > plan->N || (ncols % plan->lb != 0 && ncols != plan->N)) return GS_ERR_INVALID_ARG;
+    if (ncols == 0) return check_ready(plan);
+    return cholesky_blocks(plan, S_inout, int((ncols + plan->lb - 1) / plan->lb), cuda_stream);
 }
 
 // V = U^-1: every diagonal 128-block inverted by the leaf kernel, then block-recursive doubling.

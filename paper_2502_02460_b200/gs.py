@@ -28,7 +28,7 @@ STATUS_NAMES = {
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
-    "gs_cholesky", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
+    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
     "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
@@ -75,6 +75,7 @@ def lib() -> ctypes.CDLL:
         L.gs_plan_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_plan_set_workspace.argtypes = [vp, vp, sz]
         L.gs_cholesky.argtypes = [vp, vp, vp]
+        L.gs_cholesky_leading.argtypes = [vp, vp, i64, vp]
         L.gs_invert_triangular.argtypes = [vp, vp, vp, vp]
         L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
         L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
@@ -183,6 +184,10 @@ class Plan:
     # ---- the four steps of PAPER.md:61-67 ----
     def cholesky(self, S: torch.Tensor, stream=None):
         self._check(lib().gs_cholesky(self._h, _dev_ptr(S, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+
+    def cholesky_leading(self, S: torch.Tensor, ncols: int, stream=None):
+        """Step 1 on the leading ncols x ncols block only (sharded path)."""
+        self._check(lib().gs_cholesky_leading(self._h, _dev_ptr(S, self.N, self.N, self.tdtype), ncols, _stream_ptr(stream)))
 
     def invert_triangular(self, U: torch.Tensor, Uinv: torch.Tensor, stream=None):
         self._check(lib().gs_invert_triangular(self._h, _dev_ptr(U, self.N, self.N, self.tdtype),

@@ -2,10 +2,11 @@
 (SURVEY.md section 8(f) NEXT-3; the paper's multi-GPU direction, PAPER.md:118, PAPER.md:138;
 DESIGN.md section 9).
 
-One process per GPU.  Every rank holds H, S and forms U itself (step 1 does not shard: each panel
-depends on all earlier trailing updates -- it is replicated, the same kernels give the same bits on
-every rank).  After that the work is split by COLUMN RANGES, which need no exchange while they are
-formed:
+One process per GPU.  Every rank holds H, S and forms the part of U it needs itself: step 1 does not
+shard (each panel depends on all earlier trailing updates), but the leading principal blocks of a
+Cholesky factor nest -- chol(S[:k,:k]) = U[:k,:k] -- and a rank that owns columns up to k needs no more
+than that block (gs_cholesky_leading; the same kernels give the same bits on every rank).  After that
+the work is split by COLUMN RANGES, which need no exchange while they are formed:
 
     rank r owns the block columns J_r = [c_r, c_{r+1}) of U^-1, of G = T U^-1 and of H~
       1. V[:, J_r]  = (U^-1)[:, J_r]                (gs_invert_triangular_cols)
@@ -23,8 +24,9 @@ A column range of a column-major matrix is one contiguous slab.  Two forms of th
       step 3 is separated from steps 1-2 only by a stream synchronise and a barrier.
   exchange="collective": an all-gather of unequal slabs after the kernels (one broadcast per owner;
       NCCL on the GPUs, gloo in the CPU test of this host logic) -- the baseline form.
-The cost of column c grows like c^2 in all three steps, so the ranges are cut where the CUBE of the
-column index reaches equal shares.
+With x = (c/N)^3, a range [c0, c1) costs kappa x1 (its leading Cholesky) + (x1 - x0) (steps 2-3: the cost
+of column c grows like c^2 in all of them); the ranges are cut so that every rank carries the same sum
+(column_ranges; kappa = time of step 1 / time of steps 2-3 on one GPU, 0.30 measured at N = 16384).
 
 This module is host logic only: ranges, the order of the calls, the exchange.  All arithmetic runs
 in libgs through the `plan` object (gs.Plan); there is no other implementation behind it.
@@ -39,16 +41,23 @@ import torch.distributed as dist
 from .workloads import colmajor_empty, colmajor_zeros
 
 
-def column_ranges(N: int, world: int, block: int) -> list[tuple[int, int]]:
+CHOL_WEIGHT = 0.30   # step 1 / (steps 2 + 3) on one GPU: 50.4 ms / 167.6 ms at N = 16384 (profiles/r01f_bench.json.txt)
+
+
+def column_ranges(N: int, world: int, block: int, chol_weight: float = CHOL_WEIGHT) -> list[tuple[int, int]]:
     """[(c0, c1)] per rank: contiguous, covering [0, N), boundaries on multiples of `block` (the last
-    ends at N), cut so that sum_{c in J_r} c^2 is about equal (boundary r at N (r/world)^(1/3)).
-    Ranks may get an empty range when there are fewer blocks than ranks."""
-    if N <= 0 or world <= 0 or block <= 0:
+    ends at N).  With x = (c/N)^3 rank r carries chol_weight * x1 + (x1 - x0) (range_cost); equal sums
+    give x1_r = (1 - rho^(r+1)) / (1 - rho^world), rho = 1 / (1 + chol_weight) (chol_weight = 0: the
+    plain cube rule x1_r = (r+1)/world).  Ranks may get an empty range when there are fewer blocks
+    than ranks."""
+    if N <= 0 or world <= 0 or block <= 0 or chol_weight < 0:
         raise ValueError("N, world and block must be positive")
     nblk = (N + block - 1) // block
+    rho = 1.0 / (1.0 + chol_weight)
     cuts = [0]
     for r in range(1, world):
-        b = round(nblk * (r / world) ** (1.0 / 3.0))
+        x = r / world if chol_weight == 0 else (1.0 - rho ** r) / (1.0 - rho ** world)
+        b = round(nblk * x ** (1.0 / 3.0))
         cuts.append(min(max(b, cuts[-1]), nblk))
     cuts.append(nblk)
     return [(min(cuts[r] * block, N), min(cuts[r + 1] * block, N)) for r in range(world)]
@@ -64,9 +73,11 @@ def even_ranges(n: int, world: int, align: int = 1) -> list[tuple[int, int]]:
     return [(cuts[r], cuts[r + 1]) for r in range(world)]
 
 
-def range_cost(c0: int, c1: int) -> float:
-    """Relative cost of a column range in steps 2-3: sum of c^2 ~ (c1^3 - c0^3) / 3."""
-    return (float(c1) ** 3 - float(c0) ** 3) / 3.0
+def range_cost(c0: int, c1: int, N: int, chol_weight: float = CHOL_WEIGHT) -> float:
+    """Relative cost of owning [c0, c1): its leading Cholesky plus its share of steps 2-3, in units of
+    the one-GPU time of steps 2-3."""
+    x0, x1 = (float(c0) / N) ** 3, (float(c1) / N) ** 3
+    return (chol_weight * x1 if c1 > c0 else 0.0) + (x1 - x0)
 
 
 def slab(X: torch.Tensor, c0: int, c1: int) -> torch.Tensor:
@@ -94,7 +105,7 @@ def exchange_slabs(mats, ranges, rank: int, world: int, group=None) -> None:
 
 @dataclass
 class ShardedResult:
-    U: torch.Tensor          # replicated
+    U: torch.Tensor          # the leading cols[1] x cols[1] block holds U (all of U on the last rank); the rest is still S
     Uinv: torch.Tensor       # complete on every rank after the exchange
     G: torch.Tensor          # complete on every rank after the exchange
     Htilde: torch.Tensor     # upper triangle; only the columns of `cols` are valid before gather_htilde()
@@ -197,7 +208,7 @@ class ShardedReduction:
         if self.push:
             self._barrier()                # the peers have finished reading what the last round pushed
         U.copy_(S)
-        plan.cholesky(U, stream=stream)                                   # replicated
+        plan.cholesky_leading(U, c1, stream=stream)                       # the leading block this rank needs
         work = res.Uinv_work if self.push else Uinv
         plan.invert_triangular_cols(U, work, c0, c1 - c0, stream=stream)  # push: slab -> every rank's Uinv
         plan.to_standard_g_cols(H, work, G, c0, c1 - c0, stream=stream)   # push: slab -> every other rank's G

@@ -42,11 +42,17 @@ def _run(N, cplx, world, nev, seed):
     plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
     ranges = sharded.column_ranges(N, world, plan.block)
     U = wl.colmajor_empty(N, N, dtype=dt, device="cuda")
-    U.copy_(S)
-    plan.cholesky(U)
     V_all, G_all, Ht_all = _nan(N, N, dt), _nan(N, N, dt), _nan(N, N, dt)
     for c0, c1 in ranges:                      # steps 1-2 of rank r, then its slabs "go out"
         V_r, G_r = _nan(N, N, dt), _nan(N, N, dt)
+        U.copy_(S)
+        plan.cholesky_leading(U, c1)           # the rank factors only the leading block it needs ...
+        plan.last_info()
+        if c1 > 0:
+            assert M.rel_frob_upper(U[:c1, :c1].cpu(), U_o[:c1, :c1]) <= M.TOL_FROB
+        if c1 < N:
+            assert torch.equal(torch.triu(U)[:c1, c1:], torch.triu(S)[:c1, c1:])     # ... and leaves the rest as it was
+        U[:, c1:] = float("nan")
         plan.invert_triangular_cols(U, V_r, c0, c1 - c0)
         plan.to_standard_g_cols(H, V_r, G_r, c0, c1 - c0)
         plan.last_info()
@@ -106,7 +112,7 @@ def test_one_rank_equals_whole_matrix_calls():
     plan, U, V, Ht = gs.generalized_to_standard(H, S, 0)
     drv = sharded.ShardedReduction(plan, 0, 1)
     res = drv.reduce(H, S)
-    assert torch.equal(res.U, U)
+    assert torch.equal(res.U, U)            # one rank: the leading block is the whole matrix
     assert M.rel_frob_upper(res.Uinv.cpu(), V.cpu()) <= 1e-13
     assert M.rel_frob_upper(res.Htilde.cpu(), Ht.cpu()) <= 1e-13
     plan.close()

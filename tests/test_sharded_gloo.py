@@ -27,14 +27,21 @@ class _NumpyColsPlan:
         self.N, self.nev, self.block = N, nev, block
         self.calls = []
 
-    def cholesky(self, S, stream=None):
-        S.copy_(torch.from_numpy(oracle.cholesky(S.numpy())))
+    def cholesky_leading(self, S, ncols, stream=None):
+        full = S.numpy().copy()
+        full[:ncols, :ncols] = oracle.cholesky(np.ascontiguousarray(full[:ncols, :ncols]))
+        full[:, ncols:] = np.nan                      # nothing right of the leading block may be used
+        S.copy_(torch.from_numpy(full))
         self.calls.append("cholesky")
 
     def invert_triangular_cols(self, U, Uinv, c0, w, stream=None):
-        V = np.triu(np.linalg.solve(np.triu(U.numpy()), np.eye(self.N, dtype=U.numpy().dtype)))
+        c1 = c0 + w
         Uinv.fill_(float("nan"))
-        Uinv[:, c0:c0 + w] = torch.from_numpy(V[:, c0:c0 + w].copy())
+        if w > 0:
+            Ul = np.triu(U.numpy()[:c1, :c1])
+            V = np.zeros((self.N, w), dtype=U.numpy().dtype)
+            V[:c1] = np.triu(np.linalg.solve(Ul, np.eye(c1, dtype=Ul.dtype)))[:, c0:c1]
+            Uinv[:, c0:c1] = torch.from_numpy(V)
         self.calls.append("invert_cols")
 
     def to_standard_g_cols(self, H, Uinv, G, c0, w, stream=None):
@@ -117,19 +124,26 @@ def test_sharded_driver_over_gloo(world, N, block, cplx):
 
 def test_column_ranges_cover_align_and_balance():
     for N, world, block in ((16384, 8, 128), (16384, 2, 128), (8192, 4, 64), (1000, 8, 128), (100, 3, 128), (32768, 8, 128)):
-        r = sharded.column_ranges(N, world, block)
+      for kappa in (0.0, sharded.CHOL_WEIGHT):
+        r = sharded.column_ranges(N, world, block, kappa)
         assert len(r) == world and r[0][0] == 0 and r[-1][1] == N
         for (a0, a1), (b0, b1) in zip(r, r[1:]):
             assert a1 == b0 and a0 <= a1
         for c0, c1 in r:
             assert c0 % block == 0 or c0 == N
             assert c1 % block == 0 or c1 == N
-    # the cube rule: at the headline size no rank carries more than 1.15 x the mean c^2 cost
+    # equal sums of (leading Cholesky + share of steps 2-3): at the headline size no rank carries more than
+    # 1.12 x the mean, with and without the Cholesky term
     for world in (2, 4, 8):
-        r = sharded.column_ranges(16384, world, 128)
-        cost = [sharded.range_cost(*c) for c in r]
-        assert max(cost) <= 1.15 * sum(cost) / world
-        assert abs(sum(cost) - 16384.0 ** 3 / 3) <= 1e-6 * 16384.0 ** 3
+        for kappa in (0.0, sharded.CHOL_WEIGHT):
+            r = sharded.column_ranges(16384, world, 128, kappa)
+            cost = [sharded.range_cost(c0, c1, 16384, kappa) for c0, c1 in r]
+            assert max(cost) <= 1.12 * sum(cost) / world, (world, kappa, cost)
+    # the plain cube rule is the kappa = 0 case
+    assert sharded.column_ranges(16384, 8, 128, 0.0)[0] == (0, 8192)
+    # with the Cholesky term the last rank, which factors all of S, gets the narrowest range
+    r = sharded.column_ranges(16384, 8, 128)
+    assert r[-1][1] - r[-1][0] == min(c1 - c0 for c0, c1 in r)
 
 
 def test_even_ranges():
