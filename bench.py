@@ -615,12 +615,18 @@ def run_shard_shares(args):
         plan.cholesky_leading(Us, ncols)
     for r, ((c0, c1), (k0, k1)) in enumerate(zip(ranges, eig)):
         w = c1 - c0
+        def ranged(name, fn):       # NVTX range per stage and rank: `ncu --nvtx --nvtx-include "shard.<stage>.r<rank>/"`
+            def run():
+                torch.cuda.nvtx.range_push(f"shard.{name}.r{r}")
+                fn()
+                torch.cuda.nvtx.range_pop()
+            return run
         t = {"cols": [c0, c1], "eig_cols": [k0, k1],
-             "cholesky_leading": (timed(lambda: chol_lead(c1)) - t_copy) if w > 0 else 0.0,
-             "invert": timed(lambda: plan.invert_triangular_cols(U, Vr, c0, w)),
-             "g": timed(lambda: plan.to_standard_g_cols(pen.H, V, G, c0, w)),
-             "syr2k": timed(lambda: plan.to_standard_cols(V, G, Ht, c0, w)),
-             "backtransform": timed(lambda: plan.backtransform_cols(V, Ct, C, k0, k1 - k0))}
+             "cholesky_leading": (timed(ranged("cholesky", lambda: chol_lead(c1))) - t_copy) if w > 0 else 0.0,
+             "invert": timed(ranged("invert", lambda: plan.invert_triangular_cols(U, Vr, c0, w))),
+             "g": timed(ranged("g", lambda: plan.to_standard_g_cols(pen.H, V, G, c0, w))),
+             "syr2k": timed(ranged("syr2k", lambda: plan.to_standard_cols(V, G, Ht, c0, w))),
+             "backtransform": timed(ranged("back", lambda: plan.backtransform_cols(V, Ct, C, k0, k1 - k0)))}
         t["sum_ms"] = t["cholesky_leading"] + t["invert"] + t["g"] + t["syr2k"] + t["backtransform"]
         ranks.append(t)
     plan.last_info()

@@ -240,6 +240,8 @@ __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid
     }
 
     // ===================== epilogue: C = alpha * acc (predicated 16-byte stores) =====================
+    // (+ fused exchange: the same element to every push target, tile_engine.cuh: EngineParams::peer)
+    const int npeer = p.npeer;
 #pragma unroll
     for (int mg = 0; mg < 4; ++mg) {
         const long long row = c_row(mg);
@@ -251,26 +253,12 @@ __global__ void __launch_bounds__(kCThreads, 2) ctile_engine_kernel(const __grid
                 if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col)) {
                     double2 v = make_double2(alpha * acc[mg][ng][e][0], alpha * acc[mg][ng][e][1]);
                     if (real_diag && row == col) v.y = 0.0;
-                    Cz[row + col * p.ldc] = v;
+                    const long long off = row + col * p.ldc;
+                    Cz[off] = v;
+                    if (npeer > 0 && col >= p.peer_col0)
+                        for (int d = 0; d < npeer; ++d) reinterpret_cast<double2*>(p.peer[d])[off] = v;
                 }
             }
-    }    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
-        double2* Cd = reinterpret_cast<double2*>(p.peer[d]);
-#pragma unroll
-        for (int mg = 0; mg < 4; ++mg) {
-            const long long row = c_row(mg);
-#pragma unroll
-            for (int ng = 0; ng < 4; ++ng)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const long long col = c_col(ng, e);
-                    if (row < p.c_rows && col < p.c_cols && col >= p.peer_col0 && (!upper_only || row <= col)) {
-                        double2 v = make_double2(alpha * acc[mg][ng][e][0], alpha * acc[mg][ng][e][1]);
-                        if (real_diag && row == col) v.y = 0.0;
-                        Cd[row + col * p.ldc] = v;
-                    }
-                }
-        }
     }
 }
 

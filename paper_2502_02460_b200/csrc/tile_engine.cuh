@@ -445,6 +445,8 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
     }
 
     // ===================== epilogue: C = alpha * acc (predicated, direct to global) =====================
+    // (+ fused exchange: the same element to every push target whose column filter it passes)
+    const int npeer = p.npeer;
 #pragma unroll
     for (int mg = 0; mg < 4; ++mg) {
         const long long row = c_row(mg);
@@ -453,23 +455,12 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const long long col = c_col(ng, e);
-                if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col))
-                    p.C[row + col * p.ldc] = alpha * acc[mg][ng][e];
-            }
-        }
-    }
-    for (int d = 0; d < p.npeer; ++d) {   // fused exchange: the same tile to every push target
-        double* Cd = p.peer[d];
-#pragma unroll
-        for (int mg = 0; mg < 4; ++mg) {
-            const long long row = c_row(mg);
-#pragma unroll
-            for (int ng = 0; ng < 8; ++ng) {
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const long long col = c_col(ng, e);
-                    if (row < p.c_rows && col < p.c_cols && col >= p.peer_col0 && (!upper_only || row <= col))
-                        Cd[row + col * p.ldc] = alpha * acc[mg][ng][e];
+                if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col)) {
+                    const long long off = row + col * p.ldc;
+                    const double v = alpha * acc[mg][ng][e];
+                    p.C[off] = v;
+                    if (npeer > 0 && col >= p.peer_col0)
+                        for (int d = 0; d < npeer; ++d) p.peer[d][off] = v;
                 }
             }
         }
