@@ -166,6 +166,21 @@ class ShardedReduction:
         if self.world > 1:
             dist.barrier(group=self.group)
 
+    def _check_all(self, device, stream=None) -> None:
+        """Synchronises this rank's stream and agrees on the numerical status over ALL ranks: a rank
+        whose leading block is fine must not run on into an exchange that a failing rank never joins.
+        Raises GsError(GS_ERR_NOT_POSDEF, first bad pivot) on every rank alike."""
+        info = self.plan.last_info(stream=stream, raise_on_failure=False)
+        bad = abs(int(info)) if info else (1 << 62)
+        if self.world > 1:
+            on_cpu = dist.get_backend(self.group) == "gloo"
+            t = torch.tensor([bad], dtype=torch.int64, device="cpu" if on_cpu else device)
+            dist.all_reduce(t, op=dist.ReduceOp.MIN, group=self.group)
+            bad = int(t.item())
+        if bad != (1 << 62):
+            from .gs import GsError
+            raise GsError(2, bad, "sharded reduction: S is not positive definite (first bad pivot over all ranks)")
+
     def alloc(self, like: torch.Tensor) -> ShardedResult:
         """The N x N result buffers of reduce() (so a loop of reductions allocates once).  Push mode:
         collective over the ranks -- also maps the peers' buffers and registers the push targets."""
@@ -212,7 +227,7 @@ class ShardedReduction:
         work = res.Uinv_work if self.push else Uinv
         plan.invert_triangular_cols(U, work, c0, c1 - c0, stream=stream)  # push: slab -> every rank's Uinv
         plan.to_standard_g_cols(H, work, G, c0, c1 - c0, stream=stream)   # push: slab -> every other rank's G
-        plan.last_info(stream=stream)                                     # synchronises: the slabs are final
+        self._check_all(H.device, stream)                                 # synchronises: the slabs are final; all ranks agree
         if self.push:
             self._barrier()                # ... and have landed everywhere
         else:

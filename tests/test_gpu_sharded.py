@@ -207,3 +207,17 @@ def test_push_targets_receive_exactly_the_slab(N, cplx):
     with pytest.raises(gs.GsError):
         plan.set_push_targets(gs.GS_PUSH_C, [1] * 9)
     plan.close()
+
+
+def test_sharded_reduction_reports_a_non_positive_definite_s():
+    gs = _gs()
+    N = 640
+    p = wl.small_pencil(N, seed=4)
+    S = p.S.clone()
+    S[300, 300] = -1.0
+    plan = gs.Plan(N, 0)
+    drv = sharded.ShardedReduction(plan, 0, 1)
+    with pytest.raises(gs.GsError) as e:
+        drv.reduce(wl.to_colmajor(p.H.cuda()), wl.to_colmajor(S.cuda()))
+    assert e.value.status == 2 and e.value.info == 301
+    plan.close()

@@ -26,6 +26,7 @@ class _NumpyColsPlan:
     def __init__(self, N, nev, block):
         self.N, self.nev, self.block = N, nev, block
         self.calls = []
+        self.fail_info = 0
 
     def cholesky_leading(self, S, ncols, stream=None):
         full = S.numpy().copy()
@@ -63,14 +64,42 @@ class _NumpyColsPlan:
         C[:, k0:k0 + w] = torch.from_numpy(Uinv.numpy() @ Ct.numpy()[:, k0:k0 + w])
         self.calls.append("back_cols")
 
-    def last_info(self, stream=None):
-        return 0
+    def last_info(self, stream=None, raise_on_failure=True):
+        return self.fail_info
 
 
 def _free_port() -> int:
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
         return s.getsockname()[1]
+
+
+def _spawn(target, world, extra_args, timeout=240, attempts=2):
+    """Runs `target(rank, world, port, *extra_args, out)` in `world` spawned processes and returns their
+    results sorted by rank.  A rendezvous that does not come up (port taken between _free_port() and the
+    workers' bind, a slow import under load) is retried once on a fresh port; a real failure fails twice."""
+    last = None
+    for _ in range(attempts):
+        ctx = mp.get_context("spawn")
+        out = ctx.Queue()
+        port = _free_port()
+        procs = [ctx.Process(target=target, args=(r, world, port) + tuple(extra_args) + (out,)) for r in range(world)]
+        for p in procs:
+            p.start()
+        try:
+            res = sorted((out.get(timeout=timeout) for _ in range(world)), key=lambda t: t[0])
+            for p in procs:
+                p.join(timeout=60)
+            if all(p.exitcode == 0 for p in procs):
+                return res
+            last = AssertionError(f"worker exit codes {[p.exitcode for p in procs]}")
+        except Exception as e:  # noqa: BLE001 -- queue.Empty on a hung rendezvous
+            last = e
+        finally:
+            for p in procs:
+                if p.is_alive():
+                    p.terminate()
+    raise last
 
 
 def _worker(rank, world, port, N, nev, block, cplx, out):
@@ -95,16 +124,7 @@ def _worker(rank, world, port, N, nev, block, cplx, out):
 @pytest.mark.parametrize("world,N,block,cplx", [(2, 300, 32, False), (3, 257, 16, True), (2, 40, 64, False)])
 def test_sharded_driver_over_gloo(world, N, block, cplx):
     nev = N // 3
-    ctx = mp.get_context("spawn")
-    out = ctx.Queue()
-    port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, world, port, N, nev, block, cplx, out)) for r in range(world)]
-    for p in procs:
-        p.start()
-    res = sorted((out.get(timeout=180) for _ in range(world)), key=lambda t: t[0])
-    for p in procs:
-        p.join(timeout=60)
-        assert p.exitcode == 0
+    res = _spawn(_worker, world, (N, nev, block, cplx))
     pen = wl.small_pencil(N, seed=11, complex=cplx)
     U_o = oracle.cholesky(pen.S.numpy())
     V_o = oracle.invert_upper(U_o)
@@ -162,3 +182,27 @@ def test_slab_is_a_contiguous_view():
     assert float(X[:, 1:3].min()) == 7.0 and float(X[:, 0].abs().max()) == 0.0 and float(X[:, 3:].abs().max()) == 0.0
     with pytest.raises(ValueError):
         sharded.slab(torch.zeros(6, 5), 1, 3)
+
+
+def _failing_worker(rank, world, port, out):
+    import torch.distributed as dist
+    from paper_2502_02460_b200.gs import GsError
+    os.environ.update({"MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    N = 96
+    p = wl.small_pencil(N, seed=2)
+    plan = _NumpyColsPlan(N, 8, 16)
+    plan.fail_info = 77 if rank == 1 else 0          # only rank 1's leading block hits the bad pivot
+    drv = sharded.ShardedReduction(plan, rank, world)
+    try:
+        drv.reduce(wl.to_colmajor(p.H), wl.to_colmajor(p.S))
+        out.put((rank, None))
+    except GsError as e:
+        out.put((rank, (e.status, e.info)))
+    dist.barrier()                                   # nobody is left behind in the exchange
+    dist.destroy_process_group()
+
+
+def test_a_failing_rank_stops_every_rank():
+    res = _spawn(_failing_worker, 2, ())
+    assert res == [(0, (2, 77)), (1, (2, 77))]
