@@ -222,17 +222,19 @@ class ShardedReduction:
         U, Uinv, G, Ht = res.U, res.Uinv, res.G, res.Htilde
         if self.push:
             self._barrier()                # the peers have finished reading what the last round pushed
-        U.copy_(S)
-        plan.cholesky_leading(U, c1, stream=stream)                       # the leading block this rank needs
         work = res.Uinv_work if self.push else Uinv
-        plan.invert_triangular_cols(U, work, c0, c1 - c0, stream=stream)  # push: slab -> every rank's Uinv
-        plan.to_standard_g_cols(H, work, G, c0, c1 - c0, stream=stream)   # push: slab -> every other rank's G
+        if c1 > c0:                        # (a rank without columns -- more ranks than blocks -- only takes part in the exchange)
+            U.copy_(S)
+            plan.cholesky_leading(U, c1, stream=stream)                       # the leading block this rank needs
+            plan.invert_triangular_cols(U, work, c0, c1 - c0, stream=stream)  # push: slab -> every rank's Uinv
+            plan.to_standard_g_cols(H, work, G, c0, c1 - c0, stream=stream)   # push: slab -> every other rank's G
         self._check_all(H.device, stream)                                 # synchronises: the slabs are final; all ranks agree
         if self.push:
             self._barrier()                # ... and have landed everywhere
         else:
             exchange_slabs((Uinv, G), self.ranges, self.rank, self.world, self.group)
-        plan.to_standard_cols(Uinv, G, Ht, c0, c1 - c0, stream=stream)
+        if c1 > c0:
+            plan.to_standard_cols(Uinv, G, Ht, c0, c1 - c0, stream=stream)
         plan.last_info(stream=stream)
         return res
 

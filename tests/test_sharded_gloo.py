@@ -121,7 +121,7 @@ def _worker(rank, world, port, N, nev, block, cplx, out):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,N,block,cplx", [(2, 300, 32, False), (3, 257, 16, True), (2, 40, 64, False)])
+@pytest.mark.parametrize("world,N,block,cplx", [(2, 300, 32, False), (3, 257, 16, True), (2, 40, 64, False), (3, 100, 64, False)])
 def test_sharded_driver_over_gloo(world, N, block, cplx):
     nev = N // 3
     res = _spawn(_worker, world, (N, nev, block, cplx))
@@ -133,7 +133,7 @@ def test_sharded_driver_over_gloo(world, N, block, cplx):
     ranges = sharded.column_ranges(N, world, block)
     for rank, cols, calls, V, Ht, C, own in res:
         assert tuple(cols) == ranges[rank]
-        assert calls == ["cholesky", "invert_cols", "g_cols", "syr2k_cols", "back_cols"]
+        assert calls == (["cholesky", "invert_cols", "g_cols", "syr2k_cols", "back_cols"] if cols[1] > cols[0] else ["back_cols"])
         assert np.isfinite(V).all() and np.isfinite(Ht).all() and np.isfinite(C).all()
         assert np.linalg.norm(V - V_o) <= 1e-11 * np.linalg.norm(V_o)        # every rank ends with all of U^-1
         assert np.linalg.norm(Ht - Ht_o) <= 1e-11 * np.linalg.norm(Ht_o)     # ... and all of triu(H~)
