@@ -24,7 +24,9 @@
  * Pointers   Every matrix argument is a DEVICE pointer (cudaMalloc-class memory on the current
  *            device), 16-byte aligned, caller-owned.  The library never allocates device memory
  *            for matrices; scratch is the caller-provided workspace (gs_plan_set_workspace).
- *            Outputs must not alias inputs except the documented in-place S_inout.
+ *            Outputs must not OVERLAP inputs (byte ranges, not only equal pointers) except the
+ *            documented in-place S_inout: GS_ERR_INVALID_ARG.  NULL or misaligned matrix pointers:
+ *            GS_ERR_INVALID_ARG.  Workspace / scratch missing, too small or misaligned: GS_ERR_WORKSPACE.
  * Streams    `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *            Compute calls only enqueue work on it and return without synchronising.
  * Errors     Every call returns a gs_status_t and never throws or exits.  Argument errors are
@@ -32,10 +34,12 @@
  *            gs_cholesky; a zero diagonal entry in gs_invert_triangular) is recorded in a
  *            device-side flag as the 1-based index of the first bad pivot; all later compute
  *            calls on the same plan become no-ops while the flag is set; gs_last_info synchronises
- *            the stream and reports it.  gs_cholesky clears the flag when it starts.
+ *            the stream and reports it.  gs_cholesky clears the flag when it starts; a plan used
+ *            for the later steps only clears it with gs_plan_clear_info.
  * No CPU fallback exists: without a device of compute capability 10.x plan creation fails with
  *            GS_ERR_UNSUPPORTED_DEVICE.
- * Domain     N >= 1, 0 <= nev <= N.  Any N is accepted (ragged edges are handled in the kernels).
+ * Domain     1 <= N <= 2^20, 0 <= nev <= N.  Any such N is accepted (ragged edges are handled in the
+ *            kernels; odd N takes a loader without tensor maps).
  */
 #ifndef GS_H_
 #define GS_H_
@@ -180,6 +184,10 @@ gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C, const double* f, v
  * (LAPACK-style).  GS_ERR_CUDA if the stream reports an asynchronous error. */
 gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
 
+/* Clears the plan's numerical-failure flag (enqueued on `cuda_stream`): the way back to a usable plan
+ * after GS_ERR_SINGULAR / GS_ERR_NOT_POSDEF when the next call is not gs_cholesky (which clears it itself). */
+gs_status_t gs_plan_clear_info(gs_plan_t* plan, void* cuda_stream);
+
 /* Host-buffer entry points (the calls an application with H, S in host memory makes; used for the
  * end-to-end measurement).  gs_reduce_host copies S and H from HOST memory into device scratch
  * inside [dev_scratch, dev_scratch + scratch_bytes) -- only the triangles the steps reference: the
@@ -194,7 +202,7 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info);
  * in the scratch: gs_backtransform_host, called later with the SAME scratch, copies C~ (N x nev) in,
  * forms C = U^-1 C~ and copies C out.  Both synchronise the stream before returning and report
  * numerical failure like gs_last_info.  Scratch size: gs_reduce_host_scratch_bytes(); 256-byte
- * aligned.  gs_reduce_host_h2d_bytes / gs_reduce_host_d2h_bytes report the bytes gs_reduce_host
+ * aligned (NULL, too small or misaligned: GS_ERR_WORKSPACE).  gs_reduce_host_h2d_bytes / gs_reduce_host_d2h_bytes report the bytes gs_reduce_host
  * copies in for S and H / back for H~. */
 gs_status_t gs_reduce_host_scratch_bytes(const gs_plan_t* plan, size_t* bytes);
 gs_status_t gs_reduce_host_h2d_bytes(const gs_plan_t* plan, size_t* bytes);

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <cstring>
+#include <mutex>
 
 #include "ctile_engine.cuh"
 #include "ctile_half_engine.cuh"
@@ -17,16 +18,38 @@ namespace gs {
 // not link libcuda directly.
 inline PFN_cuTensorMapEncodeTiled tensor_map_encoder()
 {
+    static std::once_flag once;
     static PFN_cuTensorMapEncodeTiled fn = nullptr;
-    if (fn == nullptr) {
+    std::call_once(once, [] {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult qres;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
             qres == cudaDriverEntryPointSuccess)
             fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(p);
-    }
+    });
     return fn;
 }
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a PER-DEVICE setting: a process that creates plans on
+// several devices (gs.Plan(device=...), Batch(device=...)) must opt in on each of them.  `configure` runs once
+// per (caller-supplied state, current device), under a mutex (plans may be used from several host threads).
+constexpr int kMaxDevices = 64;
+struct PerDeviceOnce {
+    std::mutex mu;
+    bool done[kMaxDevices] = {};
+    template <typename F>
+    cudaError_t run(F&& configure)
+    {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        std::lock_guard<std::mutex> lock(mu);
+        if (dev >= 0 && dev < kMaxDevices && done[dev]) return cudaSuccess;
+        e = configure();
+        if (e == cudaSuccess && dev >= 0 && dev < kMaxDevices) done[dev] = true;
+        return e;
+    }
+};
 
 // Column-major FP64 matrix view: rows x cols, leading dimension ld (elements).  TMA needs a
 // 16-byte aligned base and a row pitch that is a multiple of 16 bytes (even ld).
@@ -84,10 +107,8 @@ inline int num_tiles(const EngineParams& p)
     return per * p.batch;
 }
 
-inline cudaError_t engine_configure()
+inline cudaError_t engine_configure_device()
 {
-    static bool done = false;
-    if (done) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(tile_engine_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(tile_engine_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
@@ -107,9 +128,13 @@ inline cudaError_t engine_configure()
     e = cudaFuncSetAttribute(ctile_engine_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(ctile_engine_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCSmemBytes);
-    if (e != cudaSuccess) return e;
-    done = true;
-    return cudaSuccess;
+    return e;
+}
+
+inline cudaError_t engine_configure()
+{
+    static PerDeviceOnce once;
+    return once.run(engine_configure_device);
 }
 
 // a_nn: A operand is m-contiguous (A stored M x K).  Returns cudaSuccess or the launch error.

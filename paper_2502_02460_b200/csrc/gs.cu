@@ -152,6 +152,16 @@ void clear_timed(gs_plan* p)
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// byte ranges [a, a + na) and [b, b + nb) intersect (the aliasing rule of include/gs.h is about ranges:
+// an output that starts inside an input is as wrong as one that equals it)
+bool overlaps(const void* a, size_t na, const void* b, size_t nb)
+{
+    const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+    return a0 < b0 + nb && b0 < a0 + na;
+}
+size_t mat_bytes(const gs_plan* p) { return size_t(p->N) * size_t(p->N) * p->es; }
+size_t vec_bytes(const gs_plan* p) { return size_t(p->N) * size_t(p->nev) * p->es; }
+
 // A stage under construction: knows whether every operand can go through TMA.
 struct Stage {
     gs_plan* plan;
@@ -250,7 +260,7 @@ gs_status_t zero_lower(Stage& st, void* X)
     const gs_plan* plan = st.plan;
     const int N = int(plan->N);
     if (N <= st.lb) return GS_OK;
-    dim3 grid(N > 2048 ? 8 : (N + 255) / 256, N);
+    dim3 grid(N, N > 2048 ? 8 : (N + 255) / 256);   // columns on grid.x: gridDim.y stops at 65535
     LaunchTimer timer(st.plan, L_ZERO_LOWER, st.stream);
     if (st.z) zero_lower_blocks_kernel<double2, CLB><<<grid, 256, 0, st.stream>>>(static_cast<double2*>(X), plan->N, N, info_ptr(plan));
     else zero_lower_blocks_kernel<double, LB><<<grid, 256, 0, st.stream>>>(static_cast<double*>(X), plan->N, N, info_ptr(plan));
@@ -458,7 +468,7 @@ struct Potrf {
         const int N = int(plan->N);
         const int rows = (b2 * st.lb < N ? b2 * st.lb : N) - b1 * st.lb;
         const int cols = (c1 * st.lb < N ? c1 * st.lb : N) - c0 * st.lb;
-        dim3 grid((rows + 255) / 256, cols);
+        dim3 grid(cols, (rows + 255) / 256);
         LaunchTimer timer(plan, L_POTRF_TRSM, st.stream);
         cudaError_t e;
         if (st.z)
@@ -565,16 +575,19 @@ gs_status_t ensure_side_stream(gs_plan* plan)
     return GS_OK;
 }
 
+// the opt-in to > 48 KB of dynamic shared memory is a per-device attribute (engine_host.cuh: PerDeviceOnce)
 gs_status_t configure_leaf(gs_plan* plan)
 {
-    static bool done = false;
-    if (done) return GS_OK;
-    GS_CUDA(plan, cudaFuncSetAttribute(potrf_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
-    GS_CUDA(plan, cudaFuncSetAttribute(potrf_leaf4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
-    GS_CUDA(plan, cudaFuncSetAttribute(trtri_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes));
-    GS_CUDA(plan, cudaFuncSetAttribute(potrf_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
-    GS_CUDA(plan, cudaFuncSetAttribute(trtri_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes));
-    done = true;
+    static PerDeviceOnce once;
+    const cudaError_t e = once.run([]() -> cudaError_t {
+        cudaError_t r = cudaFuncSetAttribute(potrf_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(potrf_leaf4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(trtri_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(potrf_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(trtri_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes);
+        return r;
+    });
+    if (e != cudaSuccess) return cuda_fail(plan, e);
     return GS_OK;
 }
 
@@ -713,11 +726,24 @@ gs_status_t gs_cholesky_leading(gs_plan_t* plan, void* S_inout, int64_t ncols, v
     return cholesky_blocks(plan, S_inout, int((ncols + plan->lb - 1) / plan->lb), cuda_stream);
 }
 
+// first exact zero among the first n diagonal entries of U -> info = -(index + 1), deterministically
+static gs_status_t check_diagonal(gs_plan* plan, const void* U, int64_t n, cudaStream_t stream)
+{
+    LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
+    if (plan->z) check_diagonal_kernel<double2><<<1, 1024, 0, stream>>>(static_cast<const double2*>(U), plan->N, int(n), info_ptr(plan));
+    else check_diagonal_kernel<double><<<1, 1024, 0, stream>>>(static_cast<const double*>(U), plan->N, int(n), info_ptr(plan));
+    GS_CUDA(plan, cudaGetLastError());
+    plan->launches += 1;
+    return GS_OK;
+}
+
 // V = U^-1: every diagonal 128-block inverted by the leaf kernel, then block-recursive doubling.
 gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
-    if (U_ == nullptr || Uinv_ == nullptr || U_ == Uinv_ || !aligned16(U_) || !aligned16(Uinv_)) return GS_ERR_INVALID_ARG;
+    if (U_ == nullptr || Uinv_ == nullptr || !aligned16(U_) || !aligned16(Uinv_) ||
+        overlaps(U_, mat_bytes(plan), Uinv_, mat_bytes(plan)))
+        return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     GS_TRY(configure_leaf(plan));
     const void* U = U_;
@@ -725,6 +751,7 @@ gs_status_t gs_invert_triangular(gs_plan_t* plan, const void* U_, void* Uinv_, v
     const int N = int(plan->N), nblk = plan->nblk;
     Stage st = make_stage(plan, stream);
 
+    GS_TRY(check_diagonal(plan, U, N, stream));
     {
         LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
         if (plan->z)
@@ -781,8 +808,8 @@ static gs_status_t to_standard_rows(gs_plan* plan, Stage& st, const MatView& vV,
 static gs_status_t to_standard_impl(gs_plan* plan, const void* H_, const void* Uinv_, void* Htilde_, void* cuda_stream, RowRanges* ranges)
 {
     GS_TRY(check_ready(plan));
-    if (H_ == nullptr || Uinv_ == nullptr || Htilde_ == nullptr || Htilde_ == H_ || Htilde_ == Uinv_ ||
-        !aligned16(H_) || !aligned16(Uinv_) || !aligned16(Htilde_))
+    if (H_ == nullptr || Uinv_ == nullptr || Htilde_ == nullptr || !aligned16(H_) || !aligned16(Uinv_) || !aligned16(Htilde_) ||
+        overlaps(Htilde_, mat_bytes(plan), H_, mat_bytes(plan)) || overlaps(Htilde_, mat_bytes(plan), Uinv_, mat_bytes(plan)))
         return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const int N = int(plan->N), nblk = plan->nblk;
@@ -842,8 +869,8 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv_, const void* Cti
 {
     GS_TRY(check_ready(plan));
     if (plan->nev == 0) return GS_OK;
-    if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || C_ == Ctilde_ || C_ == Uinv_ || !aligned16(Uinv_) ||
-        !aligned16(Ctilde_) || !aligned16(C_))
+    if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || !aligned16(Uinv_) || !aligned16(Ctilde_) || !aligned16(C_) ||
+        overlaps(C_, vec_bytes(plan), Ctilde_, vec_bytes(plan)) || overlaps(C_, vec_bytes(plan), Uinv_, mat_bytes(plan)))
         return GS_ERR_INVALID_ARG;
     return backtransform_cols(plan, Uinv_, Ctilde_, C_, 0, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
 }
@@ -872,7 +899,7 @@ static bool col_range_ok(const gs_plan* plan, int64_t col0, int64_t ncols, int64
 gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uinv_, int64_t col0, int64_t ncols, void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
-    if (U_ == nullptr || Uinv_ == nullptr || U_ == Uinv_ || !aligned16(U_) || !aligned16(Uinv_) ||
+    if (U_ == nullptr || Uinv_ == nullptr || !aligned16(U_) || !aligned16(Uinv_) || overlaps(U_, mat_bytes(plan), Uinv_, mat_bytes(plan)) ||
         !col_range_ok(plan, col0, ncols, plan->N))
         return GS_ERR_INVALID_ARG;
     if (ncols == 0) return GS_OK;
@@ -883,6 +910,7 @@ gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uin
     const int P = plan->shard_panel;
     Stage st = make_stage(plan, stream);
     double* V = static_cast<double*>(Uinv_);
+    GS_TRY(check_diagonal(plan, U_, std::min<int64_t>(int64_t(jb1) * lb, N), stream));
     {
         LaunchTimer timer(plan, L_TRTRI_LEAF, stream);
         if (plan->z)
@@ -901,7 +929,7 @@ gs_status_t gs_invert_triangular_cols(gs_plan_t* plan, const void* U_, void* Uin
         pt.n = int(plan->push[GS_PUSH_UINV].size());
         for (int d = 0; d < pt.n; ++d) pt.ptr[d] = plan->push[GS_PUSH_UINV][d];
         const int band = P * lb;
-        dim3 grid((band + 255) / 256, unsigned(ncols));
+        dim3 grid(unsigned(ncols), (band + 255) / 256);
         LaunchTimer timer(plan, L_PUSH_BAND, stream);
         if (plan->z) push_band_kernel<double2><<<grid, 256, 0, stream>>>(static_cast<const double2*>(Uinv_), pt, plan->N, N, int(col0), band, info_ptr(plan));
         else push_band_kernel<double><<<grid, 256, 0, stream>>>(static_cast<const double*>(Uinv_), pt, plan->N, N, int(col0), band, info_ptr(plan));
@@ -953,8 +981,9 @@ gs_status_t gs_to_standard_g_cols(gs_plan_t* plan, const void* H_, const void* U
                                   void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
-    if (H_ == nullptr || Uinv_ == nullptr || G_ == nullptr || G_ == H_ || G_ == Uinv_ || !aligned16(H_) || !aligned16(Uinv_) ||
-        !aligned16(G_) || !col_range_ok(plan, col0, ncols, plan->N))
+    if (H_ == nullptr || Uinv_ == nullptr || G_ == nullptr || !aligned16(H_) || !aligned16(Uinv_) || !aligned16(G_) ||
+        overlaps(G_, mat_bytes(plan), H_, mat_bytes(plan)) || overlaps(G_, mat_bytes(plan), Uinv_, mat_bytes(plan)) ||
+        !col_range_ok(plan, col0, ncols, plan->N))
         return GS_ERR_INVALID_ARG;
     if (ncols == 0) return GS_OK;
     const int N = int(plan->N), lb = plan->lb, kt = KPB;
@@ -979,8 +1008,9 @@ gs_status_t gs_to_standard_cols(gs_plan_t* plan, const void* Uinv_, const void* 
                                 void* cuda_stream)
 {
     GS_TRY(check_ready(plan));
-    if (Uinv_ == nullptr || G_ == nullptr || Htilde_ == nullptr || Htilde_ == G_ || Htilde_ == Uinv_ || G_ == Uinv_ ||
-        !aligned16(Uinv_) || !aligned16(G_) || !aligned16(Htilde_) || !col_range_ok(plan, col0, ncols, plan->N))
+    if (Uinv_ == nullptr || G_ == nullptr || Htilde_ == nullptr || !aligned16(Uinv_) || !aligned16(G_) || !aligned16(Htilde_) ||
+        overlaps(Htilde_, mat_bytes(plan), G_, mat_bytes(plan)) || overlaps(Htilde_, mat_bytes(plan), Uinv_, mat_bytes(plan)) ||
+        overlaps(G_, mat_bytes(plan), Uinv_, mat_bytes(plan)) || !col_range_ok(plan, col0, ncols, plan->N))
         return GS_ERR_INVALID_ARG;
     if (ncols == 0) return GS_OK;
     const int N = int(plan->N), lb = plan->lb, kt = KPB;
@@ -1011,8 +1041,8 @@ gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv_, const void
     GS_TRY(check_ready(plan));
     if (col0 < 0 || ncols < 0 || col0 + ncols > plan->nev) return GS_ERR_INVALID_ARG;
     if (ncols == 0) return GS_OK;
-    if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || C_ == Ctilde_ || C_ == Uinv_ || !aligned16(Uinv_) ||
-        !aligned16(Ctilde_) || !aligned16(C_))
+    if (Uinv_ == nullptr || Ctilde_ == nullptr || C_ == nullptr || !aligned16(Uinv_) || !aligned16(Ctilde_) || !aligned16(C_) ||
+        overlaps(C_, vec_bytes(plan), Ctilde_, vec_bytes(plan)) || overlaps(C_, vec_bytes(plan), Uinv_, mat_bytes(plan)))
         return GS_ERR_INVALID_ARG;
     if (!plan->z && ((col0 * plan->N) % 2 != 0)) return GS_ERR_INVALID_ARG;   // 16-byte aligned column start
     return backtransform_cols(plan, Uinv_, Ctilde_, C_, int(col0), int(ncols), static_cast<cudaStream_t>(cuda_stream), true);
@@ -1074,7 +1104,8 @@ gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C_, const double* f, 
     GS_TRY(check_ready(plan));
     if (P_ == nullptr || !aligned16(P_)) return GS_ERR_INVALID_ARG;
     const int N = int(plan->N), nev = int(plan->nev);
-    if (nev > 0 && (C_ == nullptr || f == nullptr || C_ == P_ || !aligned16(C_))) return GS_ERR_INVALID_ARG;
+    if (nev > 0 && (C_ == nullptr || f == nullptr || !aligned16(C_) || overlaps(P_, mat_bytes(plan), C_, vec_bytes(plan))))
+        return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     Stage st = make_stage(plan, stream);
     void* X = big_ptr(plan);
@@ -1115,6 +1146,14 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)
     GS_CUDA(plan, cudaStreamSynchronize(stream));
     if (h > 0) { *info = h; return GS_ERR_NOT_POSDEF; }
     if (h < 0) { *info = -int64_t(h); return GS_ERR_SINGULAR; }
+    return GS_OK;
+}
+
+gs_status_t gs_plan_clear_info(gs_plan_t* plan, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    if (plan->ws == nullptr) return GS_ERR_WORKSPACE;
+    GS_CUDA(plan, cudaMemsetAsync(info_ptr(plan), 0, sizeof(int), static_cast<cudaStream_t>(cuda_stream)));
     return GS_OK;
 }
 
@@ -1265,9 +1304,8 @@ gs_status_t gs_reduce_host(gs_plan_t* plan, const void* host_H, const void* host
     GS_TRY(check_ready(plan));
     size_t need = 0;
     gs_reduce_host_scratch_bytes(plan, &need);
-    if (host_H == nullptr || host_S == nullptr || host_Htilde == nullptr || dev_scratch == nullptr || scratch_bytes < need ||
-        (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
-        return GS_ERR_INVALID_ARG;
+    if (dev_scratch == nullptr || scratch_bytes < need || (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0) return GS_ERR_WORKSPACE;
+    if (host_H == nullptr || host_S == nullptr || host_Htilde == nullptr) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const size_t bytes = size_t(plan->N) * size_t(plan->N) * plan->es;
     const size_t mat = need / 4;
@@ -1344,7 +1382,7 @@ gs_status_t gs_backtransform_host(gs_plan_t* plan, const void* host_Ctilde, void
     size_t need = 0;
     gs_reduce_host_scratch_bytes(plan, &need);
     if (dev_scratch == nullptr || scratch_bytes < need || (reinterpret_cast<uintptr_t>(dev_scratch) & 255u) != 0)
-        return GS_ERR_INVALID_ARG;
+        return GS_ERR_WORKSPACE;
     if (plan->nev == 0) return GS_OK;
     if (host_Ctilde == nullptr || host_C == nullptr) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);

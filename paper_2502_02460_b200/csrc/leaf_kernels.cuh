@@ -467,6 +467,28 @@ trtri_leaf_kernel(const double* __restrict__ U, double* __restrict__ V, long lon
     leaf_store_all(s, vb, ld, nb, t);
 }
 
+// Scans the first n diagonal entries of U (one CTA) and records the FIRST exact zero as info = -(index + 1)
+// (GS_ERR_SINGULAR).  The leaf kernels find zeros too, but one CTA per block in no particular order: which
+// block reports first would be a race, and "the first bad pivot" (include/gs.h) must not be.
+template <typename T>
+__global__ void __launch_bounds__(1024, 1) check_diagonal_kernel(const T* __restrict__ U, long long ld, int n, int* info)
+{
+    if (*info != 0) return;
+    __shared__ int first;
+    if (threadIdx.x == 0) first = n;
+    __syncthreads();
+    int mine = n;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const T u = U[i + (long long)i * ld];
+        bool zero;
+        if constexpr (sizeof(T) == 16) zero = (u.x == 0.0 && u.y == 0.0); else zero = (u == 0.0);
+        if (zero && i < mine) mine = i;
+    }
+    if (mine < n) atomicMin(&first, mine);
+    __syncthreads();
+    if (threadIdx.x == 0 && first < n) atomicCAS(info, 0, -(first + 1));
+}
+
 // Zero the strictly-lower part of an N x N column-major matrix outside its 128 x 128 diagonal
 // blocks (those are written whole by the leaf kernels): the "strictly-lower part is zero" contract
 // of U and U^-1 (include/gs.h).
@@ -474,9 +496,9 @@ template <typename T, int kLB>
 __global__ void zero_lower_blocks_kernel(T* __restrict__ X, long long ld, int N, const int* info)
 {
     if (*info != 0) return;
-    const int col = blockIdx.y;
+    const int col = blockIdx.x;                // columns on grid.x (gridDim.y stops at 65535, N does not)
     const int first = (col / kLB + 1) * kLB;   // first row below the diagonal block of this column
-    for (int row = first + blockIdx.x * blockDim.x + threadIdx.x; row < N; row += gridDim.x * blockDim.x)
+    for (int row = first + blockIdx.y * blockDim.x + threadIdx.x; row < N; row += gridDim.y * blockDim.x)
         X[row + (long long)col * ld] = T{};
 }
 
@@ -492,17 +514,17 @@ template <typename T>
 __global__ void push_band_kernel(const T* __restrict__ src, PushTargets dst, long long ld, int N, int col0, int band, const int* info)
 {
     if (*info != 0) return;
-    const int col = col0 + blockIdx.y;
+    const int col = col0 + blockIdx.x;
     const int r0 = (col / band) * band;
     const int r1 = min(r0 + band, N);
-    for (int row = r0 + blockIdx.x * blockDim.x + threadIdx.x; row < r1; row += gridDim.x * blockDim.x) {
+    for (int row = r0 + blockIdx.y * blockDim.x + threadIdx.x; row < r1; row += gridDim.y * blockDim.x) {
         const long long off = row + (long long)col * ld;
         const T v = src[off];
         for (int d = 0; d < dst.n; ++d) static_cast<T*>(dst.ptr[d])[off] = v;
     }
 }
 
-// dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid row (blockIdx.y) per column c.
+// dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid column (blockIdx.x) per column c.
 template <typename T>
 __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst, long long ld, int row0, int rows,
                                   int col0, const int* info)
@@ -510,9 +532,9 @@ __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst
     grid_dep_launch();
     grid_dep_wait();
     if (*info != 0) return;
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = blockIdx.y * blockDim.x + threadIdx.x;
     if (r < rows) {
-        const long long off = row0 + r + (long long)(col0 + blockIdx.y) * ld;
+        const long long off = row0 + r + (long long)(col0 + blockIdx.x) * ld;
         dst[off] = src[off];
     }
 }

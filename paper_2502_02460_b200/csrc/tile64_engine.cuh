@@ -251,7 +251,8 @@ __global__ void __launch_bounds__(k64Threads, 3) tile64_engine_kernel(const __gr
                 if (row < p.c_rows && col < p.c_cols && (!upper_only || row <= col))
                     p.C[row + col * p.ldc] = alpha * acc[mg][ng][e];
             }
-    }    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
+    }
+    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
         double* Cd = p.peer[d];
 #pragma unroll
         for (int mg = 0; mg < 4; ++mg) {

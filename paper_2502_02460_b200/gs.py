@@ -28,7 +28,7 @@ STATUS_NAMES = {
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
-    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info",
+    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info", "gs_plan_clear_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
     "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
@@ -85,6 +85,7 @@ def lib() -> ctypes.CDLL:
         L.gs_to_standard_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_backtransform_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
+        L.gs_plan_clear_info.argtypes = [vp, vp]
         L.gs_plan_set_push_targets.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp)]
         L.gs_ipc_export.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ctypes.c_uint64)]
         L.gs_ipc_open.argtypes = [ctypes.c_char_p, ctypes.c_uint64, ctypes.POINTER(vp)]
@@ -250,9 +251,14 @@ class Plan:
     def last_info(self, stream=None, raise_on_failure: bool = True) -> int:
         info = ctypes.c_int64(0)
         status = lib().gs_last_info(self._h, _stream_ptr(stream), ctypes.byref(info))
+        self.last_status = int(status)     # which failure `info` belongs to (NOT_POSDEF / SINGULAR)
         if status != GS_OK and raise_on_failure:
             self._check(status, int(info.value))
         return int(info.value)
+
+    def clear_info(self, stream=None):
+        """Clears the numerical-failure flag (gs_cholesky does so itself when it starts)."""
+        self._check(lib().gs_plan_clear_info(self._h, _stream_ptr(stream)))
 
     def launch_count(self) -> int:
         n = ctypes.c_int64(0)

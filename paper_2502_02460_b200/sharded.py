@@ -169,17 +169,23 @@ class ShardedReduction:
     def _check_all(self, device, stream=None) -> None:
         """Synchronises this rank's stream and agrees on the numerical status over ALL ranks: a rank
         whose leading block is fine must not run on into an exchange that a failing rank never joins.
-        Raises GsError(GS_ERR_NOT_POSDEF, first bad pivot) on every rank alike."""
-        info = self.plan.last_info(stream=stream, raise_on_failure=False)
-        bad = abs(int(info)) if info else (1 << 62)
+        Raises GsError(status, first bad pivot) on every rank alike: GS_ERR_NOT_POSDEF (a pivot of S that
+        is not positive) or GS_ERR_SINGULAR (a zero on the diagonal of U in the column-range inversion)."""
+        info = int(self.plan.last_info(stream=stream, raise_on_failure=False))
+        # last_info reports |index|; the status says which failure it was (gs.h: gs_last_info)
+        status = self.plan.last_status if hasattr(self.plan, "last_status") else (2 if info else 0)
+        # one MIN reduction orders by pivot index first, then by status: key = 8 * index + status
+        key = (8 * abs(info) + int(status)) if info else (1 << 62)
         if self.world > 1:
             on_cpu = dist.get_backend(self.group) == "gloo"
-            t = torch.tensor([bad], dtype=torch.int64, device="cpu" if on_cpu else device)
+            t = torch.tensor([key], dtype=torch.int64, device="cpu" if on_cpu else device)
             dist.all_reduce(t, op=dist.ReduceOp.MIN, group=self.group)
-            bad = int(t.item())
-        if bad != (1 << 62):
+            key = int(t.item())
+        if key != (1 << 62):
             from .gs import GsError
-            raise GsError(2, bad, "sharded reduction: S is not positive definite (first bad pivot over all ranks)")
+            bad, status = key >> 3, key & 7
+            what = "a zero on the diagonal of U" if status == 3 else "S is not positive definite"
+            raise GsError(status or 2, bad, f"sharded reduction: {what} (first bad pivot over all ranks)")
 
     def alloc(self, like: torch.Tensor) -> ShardedResult:
         """The N x N result buffers of reduce() (so a loop of reductions allocates once).  Push mode:
@@ -190,6 +196,11 @@ class ShardedReduction:
         res = ShardedResult(U, Uinv, G, Ht, self.ranges[self.rank])
         if self.push:
             from . import gs
+            if self.peers is not None:
+                # a second alloc() would leak the first one's IPC mappings (and re-open handles the caching
+                # allocator may hand out again): push mode works on ONE persistent result
+                raise RuntimeError("push mode: alloc() was already called; pass out=<that result> to reduce(), "
+                                   "or close() first")
             res.Uinv.zero_()               # exchange buffer: nothing is ever pushed below the diagonal
             res.Uinv_work = colmajor_empty(N, N, dtype=like.dtype, device=like.device)
             res.C = colmajor_empty(N, max(self.nev, 1), dtype=like.dtype, device=like.device)[:, :self.nev]
@@ -218,6 +229,11 @@ class ShardedReduction:
         push mode: H~ in full too, once every rank has returned and a barrier has passed)."""
         plan = self.plan
         res = self.alloc(H) if out is None else out
+        if stream is not None and stream != torch.cuda.current_stream(H.device):
+            # the torch-side operations below (the copy of S, NCCL broadcasts, all-reduces) run on torch's
+            # CURRENT stream: make `stream` current so that they are ordered with the libgs kernels
+            with torch.cuda.stream(stream):
+                return self.reduce(H, S, stream=stream, out=res)
         c0, c1 = res.cols
         U, Uinv, G, Ht = res.U, res.Uinv, res.G, res.Htilde
         if self.push:
@@ -249,6 +265,9 @@ class ShardedReduction:
     def backtransform(self, Uinv: torch.Tensor, Ctilde: torch.Tensor, stream=None, out: torch.Tensor | None = None) -> torch.Tensor:
         """C = U^-1 C~, eigenvector columns split evenly over the ranks, then gathered.  Push mode:
         `out` must be the registered buffer (ShardedResult.C of alloc())."""
+        if stream is not None and stream != torch.cuda.current_stream(Ctilde.device):
+            with torch.cuda.stream(stream):   # see reduce(): the exchange runs on torch's current stream
+                return self.backtransform(Uinv, Ctilde, stream=stream, out=out)
         C = colmajor_empty(self.N, self.nev, dtype=Ctilde.dtype, device=Ctilde.device) if out is None else out
         k0, k1 = self.eig_ranges[self.rank]
         if self.push and out is None:

@@ -113,11 +113,35 @@ def test_complex_not_positive_definite():
     plan.close()
 
 
+@pytest.mark.slow
+def test_complex_n4160_all_three_potrf_tiers_full_oracle():
+    """65 complex blocks of 64: every panel tier of the POTRF schedule at its default width, look-ahead on
+    two streams, long-k inversion levels and HER2K -- against the WHOLE complex oracle, element by element."""
+    gs = _gs()
+    N, nev = 4160, 1040
+    p = wl.make_pencil(N, wl.scaled_box(N), wl.BASE_SEED + 78, complex=True, device="cuda")
+    plan, U, V, Ht = gs.generalized_to_standard(p.H, p.S, nev)
+    H, S = p.H.cpu().numpy(), p.S.cpu().numpy()
+    U_o = oracle.cholesky(S)
+    V_o = oracle.invert_upper(U_o)
+    Ht_o = oracle.to_standard(H, V_o)
+    for name, X, X_o in (("U", U, U_o), ("Uinv", V, V_o), ("Htilde", Ht, Ht_o)):
+        assert M.rel_frob_upper(X.cpu(), X_o) <= M.TOL_FROB, name
+        d = torch.triu(X.cpu() - torch.from_numpy(X_o)).abs().max().item()
+        assert d <= 1e-11 * np.abs(X_o).max(), name
+    Ct = wl.dense_rhs(N, nev, seed=13, complex=True, device="cuda")
+    Cg = _z(N, nev)
+    plan.backtransform(_dev(V_o), Ct, Cg)
+    plan.last_info()
+    assert M.rel_frob(Cg.cpu(), oracle.backtransform(V_o, Ct.cpu().numpy())) <= M.TOL_FROB
+    plan.close()
+
+
 def test_config3_full_size_leading_block_phase_identity_and_invariants():
     """BASELINE config 3 (N = 8192 complex Hermitian, nev = 2048), in the configuration bench.py times."""
     gs = _gs()
     cfg = wl.CONFIGS[3]
-    N, nev, k = cfg.N, cfg.nev, 1024
+    N, nev, k = cfg.N, cfg.nev, 2048      # 32 complex blocks: first panel + look-ahead iterations
     dev = "cuda"
     pz = wl.make_pencil(N, cfg.box, cfg.seed, complex=True, device=dev)
     plan, U, V, Ht = gs.generalized_to_standard(pz.H, pz.S, nev)
@@ -136,6 +160,22 @@ def test_config3_full_size_leading_block_phase_identity_and_invariants():
     # trailing rows of C nest
     C_o = oracle.backtransform(V[N - 512:, N - 512:].cpu().numpy(), Ct[N - 512:, :32].cpu().numpy())
     assert M.rel_frob(C[N - 512:, :32].cpu(), C_o) <= M.TOL_FROB
+    # far corner of step 2: trailing blocks of an upper inverse nest
+    Vf_o = oracle.invert_upper(U[N - 1024:, N - 1024:].cpu().numpy())
+    assert M.rel_frob_upper(V[N - 1024:, N - 1024:].cpu(), Vf_o) <= M.TOL_FROB
+    # sampled entries H~_ij = v_i^H H v_j from the definition (CPU, extended precision), far half of the matrix
+    rng = np.random.default_rng(21)
+    Hh = pz.H.cpu().numpy()
+    for _ in range(4):
+        j = int(rng.integers(N // 2, N))
+        vj = V[:j + 1, j].cpu().numpy().astype(np.clongdouble)
+        t = np.concatenate([Hh[r0:min(j + 1, r0 + 1024), :j + 1].astype(np.clongdouble) @ vj for r0 in range(0, j + 1, 1024)])
+        for _ in range(8):
+            i = int(rng.integers(max(0, j - N // 2), j + 1))
+            vi = V[:i + 1, i].cpu().numpy().astype(np.clongdouble)
+            ref = complex(np.dot(np.conj(vi), t[:i + 1]))
+            scale = float(np.linalg.norm(vi.astype(np.complex128)) * np.linalg.norm(t[:i + 1].astype(np.complex128)))
+            assert abs(Ht[i, j].item() - ref) <= 1e-11 * scale, (i, j)
 
     # invariants at full size (plain torch complex128 on the device, off the hot path)
     assert torch.tril(U, -1).abs().max().item() == 0.0 and torch.tril(V, -1).abs().max().item() == 0.0

@@ -6,9 +6,16 @@ The full oracle does not finish at N >= 16384, so:
   * configs 2 and 4 (N = 16384, 32768): the leading-block pin -- for upper-triangular factors the
     leading k x k blocks nest, chol(S[:k,:k]) = U[:k,:k], U[:k,:k]^-1 = V[:k,:k],
     V[:k,:k]^H H[:k,:k] V[:k,:k] = H~[:k,:k], and the trailing rows of C = V C~ nest -- so the oracle
-    on the leading k = 1024 block of the SAME device buffers pins the GPU result there; sampled
-    entries of C are recomputed one by one; and size-independent invariants (U^T U = S, U V = I,
-    U^T H~ U = H) evaluated off the hot path in torch FP64 cover the rest of the matrix.
+    on the leading k = 4096 block of the SAME device buffers pins the GPU result there (32 blocks:
+    the first 8-block POTRF panel plus three look-ahead iterations of the schedule bench.py times);
+    the FAR corner is pinned too: trailing blocks of an upper inverse nest,
+    V[N-k:, N-k:] = (U[N-k:, N-k:])^-1, and sampled entries H~_ij = v_i^H H v_j (biased towards
+    i, j > N/2, where the k-ranges of the SYR2K-shaped launch are longest) and C_ij are recomputed one
+    by one from the definition in extended precision on the CPU; and size-independent invariants
+    (U^T U = S, U V = I, U^T H~ U = H) evaluated off the hot path in torch FP64 cover the rest;
+  * N = 8320 (65 blocks: one 8-block panel, then 4-block panels, then single blocks -- all three tiers
+    of the POTRF schedule at their default widths, with look-ahead, split solves on two streams and the
+    long-k levels of the inversion): the WHOLE oracle, element by element (slow: ~1 min of CPU).
 """
 import numpy as np
 import pytest
@@ -20,7 +27,7 @@ from paper_2502_02460_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-K_LEAD = 1024
+K_LEAD = 4096
 
 
 def _run_path(cfg, dev="cuda"):
@@ -74,6 +81,43 @@ def _sampled_entries_check(V, Ct, C, samples=64, seed=5):
         assert abs(float(C[i, j]) - ref) <= 1e-11 * scale
 
 
+def _far_corner_inverse_check(U, V, k=1024):
+    """Trailing blocks of the inverse of an upper triangular matrix nest: V[N-k:, N-k:] = (U[N-k:, N-k:])^-1.
+    The oracle's back substitution on the GPU's own trailing block of U pins the far corner of step 2."""
+    N = U.shape[0]
+    V_o = oracle.invert_upper(U[N - k:, N - k:].cpu().numpy())
+    assert M.rel_frob_upper(V[N - k:, N - k:].cpu(), V_o) <= M.TOL_FROB
+
+
+def _sampled_htilde_check(p, V, Ht, ncols=8, per_col=8, seed=9):
+    """64 entries H~_ij = v_i^H H v_j (i <= j) from the definition, numpy longdouble on the
+    CPU: t_j = H[:, :j+1] v_j[:j+1] once per sampled column j (row chunks), then one dot product per i.
+    Columns and rows are biased towards the far half of the matrix."""
+    N = V.shape[0]
+    rng = np.random.default_rng(seed)
+    Hh = p.H.cpu().numpy()                                  # column-major view or copy; only read
+    for _ in range(ncols):
+        j = int(rng.integers(N // 2, N))
+        vj = V[:j + 1, j].cpu().numpy().astype(np.longdouble)
+        t = np.empty(j + 1, dtype=np.longdouble)
+        for r0 in range(0, j + 1, 1024):
+            r1 = min(j + 1, r0 + 1024)
+            t[r0:r1] = Hh[r0:r1, :j + 1].astype(np.longdouble) @ vj
+        for _ in range(per_col):
+            i = int(rng.integers(max(0, j - N // 2), j + 1))
+            vi = V[:i + 1, i].cpu().numpy().astype(np.longdouble)
+            ref = float(np.dot(vi, t[:i + 1]))
+            scale = float(np.linalg.norm(vi.astype(np.float64)) * np.linalg.norm(t[:i + 1].astype(np.float64))) + 1e-300
+            assert abs(Ht[i, j].item() - ref) <= 1e-11 * scale, (i, j, Ht[i, j].item(), ref)
+
+
+def _max_abs_upper(X, X_ref) -> float:
+    """max |X_ij - Xref_ij| over i <= j, relative to max |Xref|: the element-wise check beside the Frobenius one."""
+    X_ref = torch.as_tensor(X_ref)
+    d = torch.triu(torch.as_tensor(X) - X_ref).abs().max().item()
+    return d / max(X_ref.abs().max().item(), 1e-300)
+
+
 def _invariants(p, U, V, Ht):
     """Properties that hold at any size, evaluated with plain torch FP64 on the device (off the path)."""
     N = U.shape[0]
@@ -122,10 +166,51 @@ def test_config1_full_oracle_and_eigen_metrics():
     plan.close()
 
 
+@pytest.mark.slow
+def test_n8320_all_three_potrf_tiers_full_oracle():
+    """65 blocks: left = 65 > potrf_tail = 64 -> one 8-block panel; then 4-block panels while more than 32
+    blocks remain; then single blocks.  Every panel tier of the default schedule, the two-stream look-ahead
+    with its F1/F2 split solves, the long-k doubling levels and a SYR2K with k up to N meet the oracle
+    element by element here (the headline N = 16384 runs exactly these code paths, only longer)."""
+    from paper_2502_02460_b200 import gs
+    N, nev = 8320, 2080
+    p = wl.make_pencil(N, wl.scaled_box(N), wl.BASE_SEED + 77, device="cuda")
+    U = wl.colmajor_empty(N, N, device="cuda")
+    U.copy_(p.S)
+    V = wl.colmajor_empty(N, N, device="cuda")
+    Ht = wl.colmajor_zeros(N, N, device="cuda")
+    Ct = wl.dense_rhs(N, nev, seed=12, device="cuda")
+    C = wl.colmajor_empty(N, nev, device="cuda")
+    plan = gs.Plan(N, nev)
+    plan.cholesky(U)
+    plan.invert_triangular(U, V)
+    plan.to_standard(p.H, V, Ht)
+    plan.backtransform(V, Ct, C)
+    assert plan.last_info() == 0
+    H, S = p.H.cpu().numpy(), p.S.cpu().numpy()
+    U_o = oracle.cholesky(S)
+    V_o = oracle.invert_upper(U_o)
+    Ht_o = oracle.to_standard(H, V_o)
+    for name, X, X_o in (("U", U, U_o), ("Uinv", V, V_o), ("Htilde", Ht, Ht_o)):
+        assert M.rel_frob_upper(X.cpu(), X_o) <= M.TOL_FROB, name
+        assert _max_abs_upper(X.cpu(), X_o) <= 1e-11, name
+    # back-transform on the identical C~ with the oracle's V (the stage judged on its own)
+    Cg = wl.colmajor_empty(N, nev, device="cuda")
+    plan.backtransform(wl.to_colmajor(torch.from_numpy(np.ascontiguousarray(V_o)).cuda()), Ct, Cg)
+    plan.last_info()
+    C_o = oracle.backtransform(V_o, Ct.cpu().numpy())
+    assert M.rel_frob(Cg.cpu(), C_o) <= M.TOL_FROB
+    assert (Cg.cpu() - torch.from_numpy(C_o)).abs().max().item() <= 1e-11 * np.abs(C_o).max()
+    assert M.rel_frob(C.cpu(), C_o) <= 1e-10          # chained (GPU's own V): kappa(U)-amplified
+    plan.close()
+
+
 def test_config2_headline_leading_block_and_invariants():
     cfg = wl.CONFIGS[2]
     plan, p, U, V, Ht, Ct, C = _run_path(cfg)
     _leading_block_checks(p, U, V, Ht)
+    _far_corner_inverse_check(U, V)
+    _sampled_htilde_check(p, V, Ht)
     _trailing_rows_check(V, Ct, C)
     _sampled_entries_check(V, Ct, C)
     _invariants(p, U, V, Ht)
@@ -142,6 +227,8 @@ def test_config4_n32768_leading_block_and_invariants():
         pytest.skip("needs ~90 GiB of free device memory")
     plan, p, U, V, Ht, Ct, C = _run_path(cfg)
     _leading_block_checks(p, U, V, Ht)
+    _far_corner_inverse_check(U, V)
+    _sampled_htilde_check(p, V, Ht, ncols=4, per_col=8)
     _trailing_rows_check(V, Ct, C)
     _sampled_entries_check(V, Ct, C, samples=32)
     del Ct, C
