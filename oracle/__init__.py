@@ -47,6 +47,14 @@ def _load():
             getattr(lib, f"orc_jacobi_{t}").restype = i64
             getattr(lib, f"orc_density_{t}").argtypes = [i64, i64, p, p, p]
             getattr(lib, f"orc_density_{t}").restype = None
+            getattr(lib, f"orc_inertia_{t}").argtypes = [i64, p, ctypes.c_double]
+            getattr(lib, f"orc_inertia_{t}").restype = i64
+        lib.orc_sturm_count.argtypes = [i64, p, p, ctypes.c_double]
+        lib.orc_sturm_count.restype = i64
+        lib.orc_tridiag_eigenvalue.argtypes = [i64, p, p, i64]
+        lib.orc_tridiag_eigenvalue.restype = ctypes.c_double
+        lib.orc_tridiag_eigenvalues.argtypes = [i64, p, p, i64, p]
+        lib.orc_tridiag_eigenvalues.restype = None
         lib.orc_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -144,6 +152,43 @@ def jacobi(A):
     if sweeps < 0:
         raise RuntimeError("Jacobi did not converge in 60 sweeps")
     return eps, Q, int(sweeps)
+
+
+def _tri(d, e):
+    d = np.ascontiguousarray(np.asarray(d, dtype=np.float64))
+    e = np.ascontiguousarray(np.asarray(e, dtype=np.float64))
+    n = d.shape[0]
+    assert d.ndim == 1 and e.shape == (max(n - 1, 0),)
+    if e.size == 0:
+        e = np.zeros(1)
+    return n, d, e
+
+
+def sturm_count(d, e, x: float) -> int:
+    """O8: number of eigenvalues of tridiag(e, d, e) that are < x."""
+    n, d, e = _tri(d, e)
+    return int(_load().orc_sturm_count(n, _ptr(d), _ptr(e), float(x)))
+
+
+def tridiag_eigenvalues(d, e, nev=None) -> np.ndarray:
+    """O9: the lowest nev eigenvalues (ascending) of tridiag(e, d, e) by Sturm bisection."""
+    n, d, e = _tri(d, e)
+    nev = n if nev is None else int(nev)
+    out = np.zeros(nev, dtype=np.float64)
+    if nev > 0:
+        _load().orc_tridiag_eigenvalues(n, _ptr(d), _ptr(e), nev, _ptr(out))
+    return out
+
+
+def inertia_count(A, sigma: float) -> int:
+    """O10: number of eigenvalues of the Hermitian matrix A (upper triangle read) that are < sigma, by LDL^H
+    without pivoting.  Raises ZeroDivisionError if a pivot is exactly zero."""
+    A = _f(A)
+    N = A.shape[0]
+    r = int(getattr(_load(), f"orc_inertia_{_sfx(A)}")(N, _ptr(A), float(sigma)))
+    if r < 0:
+        raise ZeroDivisionError("zero pivot in LDL^H: choose another sigma")
+    return r
 
 
 def hermitian_from_upper(Ht_upper) -> np.ndarray:

@@ -34,6 +34,13 @@
  * at tiny N, planted factor, complex = real (x) phase identity, scipy/LAPACK cross-checks; the density
  * matrix (O7): hand-computed case fixing the conjugate, electron count sum_ij P_ij S_ij = sum_l f_l,
  * projector identity, numpy einsum (tests/test_oracle_density.py).
+ * NEXT-4 helpers (the standard eigenproblem between steps 3 and 4, whose stages the paper's
+ * Table 1 calls "Tridiag. / Solve / Back"): the oracle for eps and C~ stays the Jacobi
+ * method above; O8/O9 (Sturm count and bisection on a symmetric tridiagonal matrix) check the INTERMEDIATE
+ * tridiagonal matrix a GPU tridiagonalisation emits (same eigenvalues as H~), and O10 (inertia of A - sigma I
+ * by LDL^H without pivoting) proves that a set of computed eigenvalues is the LOWEST nev with none missing.
+ * Pins (tests/test_oracle_tridiag.py): closed-form spectrum of tridiag(-1,2,-1), diagonal and 2 x 2 cases,
+ * Jacobi on the same matrix, inertia against brute-force eigenvalue counts and a hand-computed LDL^T.
  * No function here is "parity unpinned".
  */
 #include <complex.h>
@@ -409,4 +416,98 @@ void orc_density_z(int64_t N, int64_t nev, const zdouble *C, const double *f, zd
             for (int64_t l = 0; l < nev; ++l) s += f[l] * conj(AT(C, i, l)) * AT(C, j, l);
             AT(P, i, j) = s;
         }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O8. Sturm count: the number of eigenvalues of the real symmetric tridiagonal matrix          */
+/* T = tridiag(e, d, e) (d: n diagonal, e: n-1 off-diagonal entries) that are < x.              */
+/* Sylvester's law of inertia applied to T - x I = L D L^T (Golub & Van Loan sec. 8.4.2;        */
+/* Parlett, The Symmetric Eigenvalue Problem, sec. 3.3):                                        */
+/*   q_0 = d_0 - x,   q_i = d_i - x - e_{i-1}^2 / q_{i-1},   count = #{ i : q_i < 0 }.          */
+/* A pivot that is exactly zero is replaced by -tiny (the usual convention: it counts as        */
+/* negative, i.e. an eigenvalue equal to x is counted as "< x" only through rounding).          */
+/* ------------------------------------------------------------------------------------------ */
+int64_t orc_sturm_count(int64_t n, const double *d, const double *e, double x)
+{
+    int64_t count = 0;
+    double q = 1.0;
+    for (int64_t i = 0; i < n; ++i) {
+        const double off = (i == 0) ? 0.0 : e[i - 1] * e[i - 1] / q;
+        q = d[i] - x - off;
+        if (q == 0.0) q = -1e-300;
+        if (q < 0.0) ++count;
+    }
+    return count;
+}
+
+/* O9. The k-th smallest eigenvalue (k = 0 .. n-1) of T by bisection on the Gershgorin interval:   */
+/* invariant count(lo) <= k < count(hi); stops when the interval cannot be halved any more in FP64. */
+double orc_tridiag_eigenvalue(int64_t n, const double *d, const double *e, int64_t k)
+{
+    double lo = d[0], hi = d[0];
+    for (int64_t i = 0; i < n; ++i) {
+        const double r = (i > 0 ? fabs(e[i - 1]) : 0.0) + (i + 1 < n ? fabs(e[i]) : 0.0);
+        if (d[i] - r < lo) lo = d[i] - r;
+        if (d[i] + r > hi) hi = d[i] + r;
+    }
+    const double pad = 2.0 * ldexp(1.0, -52) * (fabs(lo) > fabs(hi) ? fabs(lo) : fabs(hi)) * (double)n + 1e-300;
+    lo -= pad;
+    hi += pad;
+    for (int it = 0; it < 2000; ++it) {
+        const double mid = lo + 0.5 * (hi - lo);
+        if (!(mid > lo && mid < hi)) break;
+        if (orc_sturm_count(n, d, e, mid) <= k) lo = mid; else hi = mid;
+    }
+    return lo + 0.5 * (hi - lo);
+}
+
+void orc_tridiag_eigenvalues(int64_t n, const double *d, const double *e, int64_t nev, double *eps)
+{
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < nev; ++k) eps[k] = orc_tridiag_eigenvalue(n, d, e, k);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O10. Inertia: the number of eigenvalues of the Hermitian matrix A that are < sigma, as the    */
+/* number of negative pivots of A - sigma I = L D L^H (symmetric Gaussian elimination WITHOUT    */
+/* pivoting; Sylvester's law of inertia).  A: full N x N on entry (the upper triangle is read),  */
+/* destroyed.  Returns -1 if a pivot is exactly zero (sigma hit an eigenvalue of a leading       */
+/* block: choose another sigma).  Independent of Cholesky, Jacobi and of any tridiagonalisation. */
+/*   for j: p_j = A(j,j);  for i > j: l = conj(A(j,i)) / p_j;  A(i, c) -= l A(j, c), c >= i.      */
+/* ------------------------------------------------------------------------------------------ */
+int64_t orc_inertia_d(int64_t N, double *A, double sigma)
+{
+    int64_t neg = 0;
+    for (int64_t j = 0; j < N; ++j) AT(A, j, j) -= sigma;
+    for (int64_t j = 0; j < N; ++j) {
+        const double p = AT(A, j, j);
+        if (p == 0.0 || p != p) return -1;
+        if (p < 0.0) ++neg;
+#pragma omp parallel for schedule(static)
+        for (int64_t c = j + 1; c < N; ++c) {
+            const double ajc = AT(A, j, c);
+            if (ajc == 0.0) continue;
+            for (int64_t i = j + 1; i <= c; ++i) AT(A, i, c) -= (AT(A, j, i) / p) * ajc;
+        }
+    }
+    return neg;
+}
+
+int64_t orc_inertia_z(int64_t N, zdouble *A, double sigma)
+{
+    int64_t neg = 0;
+    for (int64_t j = 0; j < N; ++j) AT(A, j, j) = creal(AT(A, j, j)) - sigma;
+    for (int64_t j = 0; j < N; ++j) {
+        const double p = creal(AT(A, j, j));
+        if (p == 0.0 || p != p) return -1;
+        if (p < 0.0) ++neg;
+#pragma omp parallel for schedule(static)
+        for (int64_t c = j + 1; c < N; ++c) {
+            const zdouble ajc = AT(A, j, c);
+            if (ajc == 0.0) continue;
+            for (int64_t i = j + 1; i <= c; ++i) AT(A, i, c) -= (conj(AT(A, j, i)) / p) * ajc;
+            AT(A, c, c) = creal(AT(A, c, c));
+        }
+    }
+    return neg;
 }

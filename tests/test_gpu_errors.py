@@ -209,7 +209,7 @@ def test_reduce_host_scratch_errors():
     assert L.gs_backtransform_host(h, None, hC.data_ptr(), sp, need, st) == INVALID
     # and the good call still works afterwards (S = H = I: H~ = I)
     assert L.gs_reduce_host(h, *args, sp, need, st) == OK
-    assert torch.equal(torch.triu(hHt), torch.eye(N, dtype=torch.float64))
+    assert torch.equal(torch.triu(hHt.t()), torch.eye(N, dtype=torch.float64))     # the buffer is the column-major image
     plan.close()
 
 
