@@ -62,7 +62,8 @@ typedef enum {
     GS_ERR_SINGULAR = 3,           /* gs_last_info: U(info,info) == 0                            */
     GS_ERR_CUDA = 4,               /* a CUDA runtime/driver call failed                          */
     GS_ERR_WORKSPACE = 5,          /* workspace missing, too small or misaligned                 */
-    GS_ERR_UNSUPPORTED_DEVICE = 6  /* current device is not compute capability 10.x              */
+    GS_ERR_UNSUPPORTED_DEVICE = 6, /* current device is not compute capability 10.x              */
+    GS_ERR_NO_CONVERGENCE = 7      /* gs_last_info: the tridiagonal eigensolver did not converge */
 } gs_status_t;
 
 /* Create a plan for problems of order N, element type dtype, and nev wanted eigenvectors
@@ -178,6 +179,44 @@ gs_status_t gs_ipc_close(void* dev_ptr, uint64_t offset);
  * One weighted SYRK / HERK on the tensor-core tile engine over sqrt(f)-scaled, transposed C (held
  * in the plan's workspace). */
 gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C, const double* f, void* P, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------------
+ * NEXT-4: the standard eigenproblem  H~ C~ = C~ eps  that sits between step 3 and the
+ * back-transformation ("This reduces the generalized eigenproblem to the standard one, H~ C~ = eps C~, which has
+ * the same set of eigenvalues"), for the LOWEST nev eigenpairs of the plan (ascending), in the
+ * three stages of the paper's Table 1 under "Standard EVP":
+ *
+ *   gs_evp_tridiagonalize  "Tridiag."  H~ = Q T Q^H by the one-stage Householder reduction ("ELPA1", the
+ *                          conventional one-stage method, which the paper reports as the faster one on GPUs,
+ *                          PAPER.md:120).  A_inout: N x N, ld N; on entry its UPPER triangle holds H~ (what
+ *                          gs_to_standard writes; the strictly-lower part is never read); on exit column i holds
+ *                          the Householder vector v_i (rows 0 .. i-1, v_i(i-1) = 1, zeros below) of
+ *                          H(i) = I - tau(i) v_i v_i^H, Q = H(N-1) ... H(1): H~ is destroyed.  d (N) and e (N-1
+ *                          used) receive the diagonal and off-diagonal of the real symmetric tridiagonal T; tau
+ *                          (N elements of the plan's dtype) the reflector scalars.  All device pointers.
+ *   gs_evp_tridiag_solve   "Solve"     the lowest nev eigenvalues of T -> eps (nev, ascending) and their
+ *                          eigenvectors -> Z (N x nev REAL, ld N), by divide and conquer (secular equation
+ *                          solved per root, Gu-Eisenstat vectors, the block products on the tile engine).
+ *                          d, e are not modified.  SYNCHRONISES the stream once per level of the recursion
+ *                          (the deflation counts decide the shapes of the launches that follow).
+ *   gs_evp_backtransform   "Back"      C~ = Q Z (N x nev, the plan's dtype, ld N): blocked reflectors (compact
+ *                          WY, one panel = one block) applied on the tile engine.  A_reflectors is the matrix
+ *                          gs_evp_tridiagonalize left; the triangular factors of the blocks are kept in the
+ *                          plan's EVP workspace, so the call belongs to the LAST gs_evp_tridiagonalize on the plan.
+ *   gs_standard_eigh       the three in a row: eps (nev) and C~ (N x nev) from the upper triangle of Htilde_inout
+ *                          (destroyed).  C~ is what gs_backtransform takes.
+ *
+ * Scratch: a second caller-owned device buffer (about 3 N^2 + N nev doubles), gs_evp_workspace_bytes /
+ * gs_evp_set_workspace, 256-byte aligned; GS_ERR_WORKSPACE if missing or too small.  The plan's ordinary
+ * workspace must be set as well.  C~ is unique only up to the phase of each column (and up to rotations inside
+ * clusters of equal eigenvalues): compare residuals and orthonormality, not elements.
+ * Numerical failure: GS_ERR_NO_CONVERGENCE from gs_last_info if the QL iteration of a leaf does not converge. */
+gs_status_t gs_evp_workspace_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_evp_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t bytes);
+gs_status_t gs_evp_tridiagonalize(gs_plan_t* plan, void* A_inout, double* d, double* e, void* tau, void* cuda_stream);
+gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double* e, double* eps, double* Z, void* cuda_stream);
+gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream);
+gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream);
 
 /* Synchronises `cuda_stream`, then reports the plan's numerical status: GS_OK with *info = 0, or
  * GS_ERR_NOT_POSDEF / GS_ERR_SINGULAR with *info = 1-based index of the first bad pivot

@@ -1,0 +1,482 @@
+// evp_dc.cuh -- kernels of the tridiagonal eigensolver (NEXT-4: the "Solve" stage of the standard eigenproblem,
+// PAPER.md:126-133 Table 1 column "Solve"; "the solve step of the tridiagonal matrix"):
+// Cuppen's divide and conquer with Gu / Eisenstat's stable eigenvector formula -- the method of LAPACK's xSTEDC
+// and of ELPA's solve step, restated here for the GPU (nothing is copied from either).
+//
+//   T = diag(T1, T2) + beta (e_a e_b^T + e_b e_a^T) = diag(T1', T2') + |beta| w w^T,  w = e_a + sign(beta) e_b,
+//   T1' = T1 - |beta| e_a e_a^T, T2' = T2 - |beta| e_b e_b^T.  With T1' = Q1 D1 Q1^T, T2' = Q2 D2 Q2^T:
+//   T = Q (D + rho z z^T) Q^T,  Q = diag(Q1, Q2),  z = Q^T w / sqrt2,  rho = 2 |beta|.
+//   * deflation: entries with rho |z_j| tiny, and pairs of (nearly) equal d rotated so that one z vanishes, are
+//     eigenpairs already;
+//   * the other k eigenvalues are the roots of  1 + rho sum_i z_i^2 / (d_i - lambda) = 0, one per interval
+//     (d_j, d_j+1): found by bisection on mu = lambda - d_origin with the origin at the NEARER pole, so that every
+//     difference d_i - lambda_j = (d_i - d_origin) - mu is formed without cancellation;
+//   * z is replaced by the z^ for which the computed lambda are the EXACT eigenvalues (Loewner's formula): the
+//     eigenvectors x_j = (D - lambda_j)^-1 z^ / ||.|| are then orthogonal to working precision;
+//   * the new eigenvector block is  Q X: two GEMMs on the FP64 tensor-core tile engine (top rows use only the
+//     columns that come from Q1 or were mixed by a deflation rotation, bottom rows likewise) -- all the O(N^3) work.
+// Leaves (128 x 128) are solved by the implicit QL iteration, one CTA each.
+//
+// Eigenvalues of a solved block are kept sorted through an index (dcur ascending, idx -> physical column of Q),
+// so no column is ever moved for the sake of ordering.  All arrays below are indexed by GLOBAL position
+// (block offset + local index).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cfloat>
+
+namespace gs {
+namespace evp {
+
+constexpr int kDcLeaf = 128;
+
+struct MergeDesc {
+    int off, n1, n2;     // block [off, off + n1 + n2): children [off, off + n1), [off + n1, off + n1 + n2)
+    int k;               // number of non-deflated eigenvalues (device -> host)
+    int c1, c2, c3;      // of those: columns from Q1 only / mixed by a rotation / from Q2 only (grouped order)
+    int nrot;            // deflation rotations recorded
+    int r;               // roots whose eigenVECTORS are wanted (host -> device; k except at the top level)
+    int fail;
+    double rho;
+    double pad;
+};
+
+struct DcArrays {
+    double* Qcur; double* Qnew; double* G; long long ldq;   // eigenvector blocks (block diagonal), gather buffer
+    double* dcur; int* idx;        // solved blocks: eigenvalues ascending, physical column of each
+    double* dnew; int* idxnew;     // the same for the level being formed
+    double* dm; double* zs; int* srcm; int* typ;      // merged (sorted) D, z, source column, type 1 / 2 / 3
+    double* dlam; double* wz; int* gsrc; int* gpos; int* gtyp;   // non-deflated: sorted d, z, source column, grouped position, type
+    double* dval; int* dsrc; int* dtyp;                // deflated eigenvalues, their columns and types
+    double* mu; int* org;          // roots: lambda_j = dlam[org_j] + mu_j
+    double* zhat;
+    int* rota; int* rotb; int* rotta; int* rottb; double* rotc; double* rots;   // rotations: columns, prior types, c, s
+    MergeDesc* desc;
+    int* info;                     // plan's failure flag
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// d(b-1) -= |e(b-1)|, d(b) -= |e(b-1)| at every leaf boundary b (all of them are cut points of some level)
+// ---------------------------------------------------------------------------------------------------------
+__global__ void dc_cut_kernel(double* d, const double* e, int N)
+{
+    const int b = (blockIdx.x * blockDim.x + threadIdx.x + 1) * kDcLeaf;
+    if (b < N) {
+        const double a = fabs(e[b - 1]);
+        d[b - 1] -= a;
+        d[b] -= a;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Leaf: all eigenpairs of the n x n (n <= 128) tridiagonal block at offset off by the implicit QL iteration with
+// Wilkinson shifts (EISPACK tql2 / LAPACK xSTEQR scheme).  Thread 0 runs the scalar recurrences of one sweep and
+// leaves its rotations in shared memory; then every thread applies them to its own ROW of Q (kept in registers?
+// no: in the Q block in global memory, 128 KB per leaf, L2-resident; loads of successive columns are coalesced
+// over the rows).  Result: dcur ascending, idx = physical column.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restrict__ dd, const double* __restrict__ ee, int N, DcArrays a)
+{
+    if (*a.info != 0) return;
+    const int off = blockIdx.x * kDcLeaf;
+    const int n = min(kDcLeaf, N - off);
+    const int t = threadIdx.x;
+    __shared__ double d[kDcLeaf], e[kDcLeaf], cs[kDcLeaf], sn[kDcLeaf];
+    __shared__ int s_l, s_m, s_cnt, s_fail;
+    if (t < n) { d[t] = dd[off + t]; e[t] = (t + 1 < n) ? ee[off + t] : 0.0; }
+    double* Q = a.Qcur + off + (long long)off * a.ldq;
+    for (int c = 0; c < n; ++c)
+        if (t < n) Q[t + (long long)c * a.ldq] = (t == c) ? 1.0 : 0.0;
+    if (t == 0) { s_fail = 0; }
+    __syncthreads();
+    for (int l = 0; l < n; ++l) {
+        int iter = 0;
+        while (true) {
+            if (t == 0) {
+                int m = l;
+                for (; m < n - 1; ++m) {
+                    const double ds = fabs(d[m]) + fabs(d[m + 1]);
+                    if (fabs(e[m]) <= DBL_EPSILON * 0.5 * ds) break;
+                }
+                s_m = m;
+                s_cnt = 0;
+                if (m != l) {
+                    if (iter == 60) s_fail = 1;
+                    double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                    double r = hypot(g, 1.0);
+                    g = d[m] - d[l] + e[l] / (g + copysign(r, g));
+                    double s = 1.0, c = 1.0, p = 0.0;
+                    int i = m - 1;
+                    bool early = false;
+                    for (; i >= l; --i) {
+                        double f = s * e[i];
+                        const double b = c * e[i];
+                        r = hypot(f, g);
+                        e[i + 1] = r;
+                        if (r == 0.0) { d[i + 1] -= p; e[m] = 0.0; early = true; break; }
+                        s = f / r;
+                        c = g / r;
+                        g = d[i + 1] - p;
+                        r = (d[i] - g) * s + 2.0 * c * b;
+                        p = s * r;
+                        d[i + 1] = g + p;
+                        g = c * r - b;
+                        cs[i] = c; sn[i] = s;          // rotation of columns (i, i+1)
+                    }
+                    s_l = early ? i + 1 : l;           // rotations recorded for i = m-1 .. s_l
+                    s_cnt = (m - 1) - s_l + 1;
+                    if (!early) { d[l] -= p; e[l] = g; e[m] = 0.0; }
+                }
+            }
+            __syncthreads();
+            const int m = s_m;
+            if (s_fail) break;
+            if (m == l) break;
+            // apply the sweep's rotations, i = m-1 down to s_l, to row t of Q
+            if (t < n && s_cnt > 0) {
+                const int lo = s_l;
+                double hi_val = Q[t + (long long)m * a.ldq];            // z(t, i+1)
+                for (int i = m - 1; i >= lo; --i) {
+                    const double zi = Q[t + (long long)i * a.ldq];
+                    const double c = cs[i], s = sn[i];
+                    Q[t + (long long)(i + 1) * a.ldq] = s * zi + c * hi_val;
+                    hi_val = c * zi - s * hi_val;
+                }
+                Q[t + (long long)lo * a.ldq] = hi_val;
+            }
+            ++iter;
+            __syncthreads();
+        }
+        if (s_fail) break;
+    }
+    __syncthreads();
+    if (s_fail) { if (t == 0) atomicCAS(a.info, 0, -(1 << 30)); return; }
+    // ascending order through an index (rank sort, ties by position)
+    if (t < n) {
+        const double v = d[t];
+        int rank = 0;
+        for (int j = 0; j < n; ++j) rank += (d[j] < v || (d[j] == v && j < t)) ? 1 : 0;
+        a.dcur[off + rank] = v;
+        a.idx[off + rank] = off + t;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M1: z = Q^T w / sqrt2 and the merge of the two sorted eigenvalue lists of a pair of children.
+// grid.x = merge, 256 threads.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_setup_kernel(const double* __restrict__ e, DcArrays a)
+{
+    if (*a.info != 0) return;
+    MergeDesc& ds = a.desc[blockIdx.x];
+    const int off = ds.off, n1 = ds.n1, n2 = ds.n2, n = n1 + n2;
+    const double beta = e[off + n1 - 1];
+    const double sgn = beta < 0.0 ? -1.0 : 1.0;
+    if (threadIdx.x == 0) ds.rho = 2.0 * fabs(beta);
+    const double is2 = 0.70710678118654752440;
+    const double* d1 = a.dcur + off;
+    const double* d2 = a.dcur + off + n1;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) {
+        double dv, zv;
+        int col, rank, ty;
+        if (j < n1) {
+            dv = d1[j]; col = a.idx[off + j]; ty = 1;
+            zv = a.Qcur[(off + n1 - 1) + (long long)col * a.ldq] * is2;            // last row of Q1
+            int lo = 0, hi = n2;                                                    // # of d2 < dv
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (d2[mid] < dv) lo = mid + 1; else hi = mid; }
+            rank = j + lo;
+        } else {
+            const int j2 = j - n1;
+            dv = d2[j2]; col = a.idx[off + j]; ty = 3;
+            zv = sgn * a.Qcur[(off + n1) + (long long)col * a.ldq] * is2;          // first row of Q2
+            int lo = 0, hi = n1;                                                    // # of d1 <= dv
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (d1[mid] <= dv) lo = mid + 1; else hi = mid; }
+            rank = j2 + lo;
+        }
+        a.dm[off + rank] = dv; a.zs[off + rank] = zv; a.srcm[off + rank] = col; a.typ[off + rank] = ty;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M2: deflation scan (sequential in the sorted order: one thread per merge after a parallel max-reduction).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_deflate_kernel(DcArrays a)
+{
+    if (*a.info != 0) return;
+    MergeDesc& ds = a.desc[blockIdx.x];
+    const int off = ds.off, n = ds.n1 + ds.n2;
+    __shared__ double s_max[256];
+    double mx = 0.0;
+    for (int j = threadIdx.x; j < n; j += 256) mx = fmax(mx, fmax(fabs(a.dm[off + j]), fabs(a.zs[off + j])));
+    s_max[threadIdx.x] = mx;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s_max[threadIdx.x] = fmax(s_max[threadIdx.x], s_max[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    const double tol = 8.0 * (DBL_EPSILON * 0.5) * s_max[0];
+    const double rho = ds.rho;
+    double* dm = a.dm + off; double* z = a.zs + off; int* src = a.srcm + off; int* typ = a.typ + off;
+    int k = 0, ndef = 0, nrot = 0, pj = -1;
+    // non-deflated entries are compacted in place at the front (index k <= j always), deflated ones go to dval
+    auto defl = [&](int j) { a.dval[off + ndef] = dm[j]; a.dsrc[off + ndef] = src[j]; a.dtyp[off + ndef] = typ[j]; ++ndef; };
+    auto keep = [&](int j) { a.dlam[off + k] = dm[j]; a.wz[off + k] = z[j]; a.gsrc[off + k] = src[j]; a.gtyp[off + k] = typ[j]; ++k; };
+    for (int j = 0; j < n; ++j) {
+        if (rho * fabs(z[j]) <= tol) { defl(j); continue; }
+        if (pj < 0) { pj = j; continue; }
+        double s = z[pj], c = z[j];
+        const double tau = hypot(c, s);
+        const double tdiff = dm[j] - dm[pj];
+        c /= tau;
+        s = -s / tau;
+        if (fabs(tdiff * c * s) <= tol) {
+            z[j] = tau; z[pj] = 0.0;
+            a.rota[off + nrot] = src[pj]; a.rotb[off + nrot] = src[j];
+            a.rotta[off + nrot] = typ[pj]; a.rottb[off + nrot] = typ[j];
+            a.rotc[off + nrot] = c; a.rots[off + nrot] = s;
+            ++nrot;
+            if (typ[pj] != typ[j]) { typ[pj] = 2; typ[j] = 2; }
+            const double tt = dm[pj] * c * c + dm[j] * s * s;
+            dm[j] = dm[pj] * s * s + dm[j] * c * c;
+            dm[pj] = tt;
+            defl(pj);
+            pj = j;
+        } else {
+            keep(pj);
+            pj = j;
+        }
+    }
+    if (pj >= 0) keep(pj);
+    // grouped order of the non-deflated columns: [from Q1 only | mixed | from Q2 only]
+    int c1 = 0, c2 = 0, c3 = 0;
+    for (int q = 0; q < k; ++q) { const int ty = a.gtyp[off + q]; c1 += ty == 1; c2 += ty == 2; c3 += ty == 3; }
+    int p1 = 0, p2 = c1, p3 = c1 + c2;
+    for (int q = 0; q < k; ++q) {
+        const int ty = a.gtyp[off + q];
+        a.gpos[off + q] = ty == 1 ? p1++ : ty == 2 ? p2++ : p3++;
+    }
+    ds.k = k; ds.c1 = c1; ds.c2 = c2; ds.c3 = c3; ds.nrot = nrot; ds.fail = 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M3: the deflation rotations applied to the columns of Q, one thread per row of the merged block.  A column
+// that still belongs to one child only is zero outside that child's rows (the storage there is not read).
+// grid = (row chunks, merges).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_rotate_kernel(DcArrays a)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, n1 = ds.n1, n = ds.n1 + ds.n2;
+    const int lr = blockIdx.x * 256 + threadIdx.x;
+    if (lr >= n || ds.nrot == 0) return;
+    const bool top = lr < n1;
+    double* Qr = a.Qcur + off + lr;
+    for (int q = 0; q < ds.nrot; ++q) {
+        const int ca = a.rota[off + q], cb = a.rotb[off + q];
+        const int ta = a.rotta[off + q], tb = a.rottb[off + q];
+        const double c = a.rotc[off + q], s = a.rots[off + q];
+        const bool ina = ta == 2 || (ta == 1) == top, inb = tb == 2 || (tb == 1) == top;
+        const double x = ina ? Qr[(long long)ca * a.ldq] : 0.0;
+        const double y = inb ? Qr[(long long)cb * a.ldq] : 0.0;
+        if (ta == tb && ta != 2 && !ina) continue;            // both columns are zero in this row and stay so
+        Qr[(long long)ca * a.ldq] = c * x + s * y;
+        Qr[(long long)cb * a.ldq] = c * y - s * x;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M4: gather.  Non-deflated column q -> G[:, off + gpos(q)]; deflated column q' -> Qnew[:, off + k + q'].  All rows
+// are written, zeros outside the column's support (the k-range of the bottom GEMM may start one column early,
+// inside the columns that come from Q1 only: a TMA box of FP64 elements must start at an even row of X).
+// grid = (columns of the block, merges), 256 threads stride over the rows.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_gather_kernel(DcArrays a)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, n1 = ds.n1, n = ds.n1 + ds.n2, k = ds.k;
+    const int q = blockIdx.x;
+    if (q >= n) return;
+    int src, ty;
+    double* dst;
+    bool nondefl = q < k;
+    if (nondefl) { src = a.gsrc[off + q]; ty = a.gtyp[off + q]; dst = a.G + off + (long long)(off + a.gpos[off + q]) * a.ldq; }
+    else { src = a.dsrc[off + q - k]; ty = a.dtyp[off + q - k]; dst = a.Qnew + off + (long long)(off + q) * a.ldq; }
+    const double* s = a.Qcur + off + (long long)src * a.ldq;
+    for (int r = threadIdx.x; r < n; r += 256) {
+        const bool in = ty == 2 || (ty == 1) == (r < n1);
+        dst[r] = in ? s[r] : 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M5: secular equation.  One warp per root j of every merge: bisection on mu = lambda - d_origin.
+// grid = (ceil(maxk / 8), merges), 256 threads.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double secular_f(const double* __restrict__ dl, const double* __restrict__ w, int k, double dorg, double mu, double rho, int lane)
+{
+    double s = 0.0;
+    for (int i = lane; i < k; i += 32) {
+        const double wi = w[i];
+        s += wi * wi / ((dl[i] - dorg) - mu);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    return 1.0 + rho * s;
+}
+
+__global__ void __launch_bounds__(256) dc_secular_kernel(DcArrays a)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, k = ds.k;
+    const int j = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (j >= k) return;
+    const double* dl = a.dlam + off;
+    const double* w = a.wz + off;
+    const double rho = ds.rho;
+    int org;
+    double lo, hi;
+    if (j < k - 1) {
+        const double gap = dl[j + 1] - dl[j];
+        const double fm = secular_f(dl, w, k, dl[j], 0.5 * gap, rho, lane);
+        if (fm >= 0.0) { org = j; lo = 0.0; hi = 0.5 * gap; }             // root in the left half: origin d_j
+        else { org = j + 1; lo = -0.5 * gap; hi = 0.0; }                  // right half: origin d_j+1
+    } else {
+        double w2 = 0.0;
+        for (int i = lane; i < k; i += 32) w2 += w[i] * w[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w2 += __shfl_xor_sync(0xffffffffu, w2, o);
+        org = j; lo = 0.0; hi = rho * w2 * (1.0 + 4.0 * DBL_EPSILON);
+        if (!(hi > 0.0)) hi = DBL_MIN;
+    }
+    const double dorg = dl[org];
+    for (int it = 0; it < 1200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (!(mid > lo && mid < hi)) break;
+        const double f = secular_f(dl, w, k, dorg, mid, rho, lane);
+        if (f >= 0.0) hi = mid; else lo = mid;
+    }
+    double mu = 0.5 * (lo + hi);
+    if (mu == 0.0) mu = (org == j) ? hi : lo;          // never on the pole itself
+    if (lane == 0) { a.mu[off + j] = mu; a.org[off + j] = org; }
+}
+
+// d_i - lambda_j from the shifted representation
+__device__ __forceinline__ double dc_diff(const double* __restrict__ dl, const double* __restrict__ mu, const int* __restrict__ org, int i, int j)
+{
+    return (dl[i] - dl[org[j]]) - mu[j];
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M6: z^_i (Loewner / Gu-Eisenstat), one warp per i:
+//   z^_i^2 = (lambda_{k-1} - d_i) / rho * prod_{j<i} (d_i - lambda_j)/(d_i - d_j) * prod_{j>i} (lambda_{j-1} - d_i)/(d_j - d_i)
+// every factor is positive by interlacing; sign taken from z_i.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_zhat_kernel(DcArrays a)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, k = ds.k;
+    const int i = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (i >= k) return;
+    const double* dl = a.dlam + off;
+    const double* mu = a.mu + off;
+    const int* org = a.org + off;
+    double prod = 1.0;
+    const double di = dl[i];
+    for (int j = lane; j < k; j += 32) {
+        if (j < i) prod *= dc_diff(dl, mu, org, i, j) / (di - dl[j]);
+        else if (j > i) prod *= -dc_diff(dl, mu, org, i, j - 1) / (dl[j] - di);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) prod *= __shfl_xor_sync(0xffffffffu, prod, o);
+    if (lane == 0) {
+        const double last = -dc_diff(dl, mu, org, i, k - 1);        // lambda_{k-1} - d_i > 0
+        const double z2 = prod * last / ds.rho;
+        a.zhat[off + i] = copysign(sqrt(fmax(z2, 0.0)), a.wz[off + i]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M7: eigenvector x_j = (D - lambda_j)^-1 z^, normalised, written with its rows in the grouped order of the
+// gathered columns: X[off + gpos(i), off + j].  One warp per root j < r.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_xcols_kernel(DcArrays a, double* __restrict__ X)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, k = ds.k;
+    const int j = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (j >= ds.r) return;
+    const double* dl = a.dlam + off;
+    const double* mu = a.mu + off;
+    const int* org = a.org + off;
+    double n2 = 0.0;
+    for (int i = lane; i < k; i += 32) {
+        const double x = a.zhat[off + i] / dc_diff(dl, mu, org, i, j);
+        n2 += x * x;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) n2 += __shfl_xor_sync(0xffffffffu, n2, o);
+    const double inv = 1.0 / sqrt(n2);
+    double* col = X + off + (long long)(off + j) * a.ldq;
+    for (int i = lane; i < k; i += 32) col[a.gpos[off + i]] = a.zhat[off + i] / dc_diff(dl, mu, org, i, j) * inv;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// M8: eigenvalues of the merged block (roots, then deflated values) and their ascending index.
+// Root j lives in column off + j of Qnew (j < r; no column otherwise: idx = -1), deflated q in column off + k + q.
+// grid = (ceil(n / 256), merges).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dc_values_kernel(DcArrays a, double* __restrict__ val)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, n = ds.n1 + ds.n2, k = ds.k;
+    const int x = blockIdx.x * 256 + threadIdx.x;
+    if (x >= n) return;
+    val[off + x] = x < k ? a.dlam[off + a.org[off + x]] + a.mu[off + x] : a.dval[off + x - k];
+}
+
+__global__ void __launch_bounds__(256) dc_rank_kernel(DcArrays a, const double* __restrict__ val)
+{
+    if (*a.info != 0) return;
+    const MergeDesc ds = a.desc[blockIdx.y];
+    const int off = ds.off, n = ds.n1 + ds.n2, k = ds.k;
+    const int x = blockIdx.x * 256 + threadIdx.x;
+    if (x >= n) return;
+    const double v = val[off + x];
+    int rank = 0;
+    for (int y = 0; y < n; ++y) {
+        const double vy = val[off + y];
+        rank += (vy < v || (vy == v && y < x)) ? 1 : 0;
+    }
+    a.dnew[off + rank] = v;
+    a.idxnew[off + rank] = (x < k && x >= ds.r) ? -1 : off + x;
+}
+
+// a block without a partner at this level passes through: its columns are copied to the other Q buffer
+__global__ void __launch_bounds__(256) dc_copy_block_kernel(const double* __restrict__ src, double* __restrict__ dst, long long ld, int off, int n)
+{
+    const int c = blockIdx.x;
+    for (int r = threadIdx.x; r < n; r += 256) dst[off + r + (long long)(off + c) * ld] = src[off + r + (long long)(off + c) * ld];
+}
+
+// Z(:, c) = Q(:, idx(c)), eps(c) = d(c) for the lowest nev pairs
+__global__ void __launch_bounds__(256) dc_output_kernel(const double* __restrict__ Q, long long ldq, const double* __restrict__ d, const int* __restrict__ idx,
+                                                        int N, int nev, double* __restrict__ eps, double* __restrict__ Z, long long ldz, int* info)
+{
+    if (*info != 0) return;
+    const int c = blockIdx.x;
+    if (c >= nev) return;
+    const int src = idx[c];
+    if (src < 0) { if (threadIdx.x == 0) atomicCAS(info, 0, -(1 << 30) - 1); return; }
+    if (threadIdx.x == 0) eps[c] = d[c];
+    for (int r = threadIdx.x; r < N; r += 256) Z[r + (long long)c * ldz] = Q[r + (long long)src * ldq];
+}
+
+}  // namespace evp
+}  // namespace gs

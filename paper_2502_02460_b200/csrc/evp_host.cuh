@@ -1,0 +1,465 @@
+// evp_host.cuh -- host drivers of NEXT-4, the standard eigenproblem  H~ C~ = C~ eps  between step 3 and the
+// back-transformation, in the three stages of the paper's Table 1:
+//   gs_evp_tridiagonalize  "Tridiag."  one-stage Householder reduction H~ = Q T Q^H     (evp_tridiag.cuh)
+//   gs_evp_tridiag_solve   "Solve"     divide and conquer on T, lowest nev pairs        (evp_dc.cuh)
+//   gs_evp_backtransform   "Back"      C~ = Q Z, blocked reflectors on the tile engine
+// Included by gs.cu (same translation unit: it uses the plan, Stage and launch() defined there).
+#pragma once
+
+#include "evp_dc.cuh"
+#include "evp_tridiag.cuh"
+
+namespace {
+
+using namespace gs::evp;
+
+// ---- workspace carving (the same walk computes the size and the pointers) ----
+struct EvpLayout {
+    size_t total = 0;
+    unsigned char* base = nullptr;
+    template <typename T>
+    T* take(size_t count)
+    {
+        const size_t off = total;
+        total += ((count * sizeof(T) + 255) / 256) * 256;
+        return base != nullptr ? reinterpret_cast<T*>(base + off) : nullptr;
+    }
+};
+
+struct EvpBuffers {
+    // tridiagonalisation
+    unsigned int* tickets; void* sc;
+    void *u, *wp, *corr2, *tfin, *Pd, *Vt, *Wt, *Pt, *P1, *P2, *R, *Rinv, *Y, *Y2;
+    long long ldp;
+    int nb, npanels;
+    // results kept for gs_standard_eigh
+    double *d, *e, *dwork; void* tau; double* Z;
+    // divide and conquer
+    DcArrays dc;
+    double* val;
+    long long ldq;
+};
+
+EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes)
+{
+    EvpLayout L;
+    L.base = base;
+    EvpBuffers b{};
+    const size_t N = size_t(p->N), es = p->es, nev = size_t(p->nev);
+    const int nb = p->lb;
+    const size_t th = p->z ? 64 : 128;
+    const size_t nJ = (N + 127) / 128, nI = (N + th - 1) / th;
+    b.nb = nb;
+    b.npanels = int((N + nb - 1) / nb) + 1;
+    b.ldp = (long long)((N + 1) & ~size_t(1));
+    b.ldq = (long long)((N + 1) & ~size_t(1));
+    auto takeb = [&](size_t elems) { return static_cast<void*>(L.take<unsigned char>(elems * es)); };
+    b.tickets = L.take<unsigned int>(16);
+    b.sc = L.take<unsigned char>(256);
+    b.d = L.take<double>(N); b.e = L.take<double>(N + 1); b.dwork = L.take<double>(N); b.tau = takeb(N);
+    b.u = takeb(N + 1); b.wp = takeb(N + 1); b.corr2 = takeb(N + 1); b.tfin = takeb(2 * size_t(nb)); b.Pd = takeb(N + 64);
+    b.Vt = takeb(size_t(nb) * N); b.Wt = takeb(size_t(nb) * N);
+    b.Pt = takeb(nJ * 2 * size_t(nb));
+    b.P1 = takeb(nJ * size_t(b.ldp)); b.P2 = takeb(nI * size_t(b.ldp));
+    b.R = takeb(size_t(b.npanels) * nb * (nb + 1)); b.Rinv = takeb(size_t(b.npanels) * nb * (nb + 1));
+    b.Y = takeb(size_t(nb) * (nev + 2)); b.Y2 = takeb(size_t(nb) * (nev + 2));
+    b.Z = L.take<double>(N * (nev > 0 ? nev : 1));
+    DcArrays& a = b.dc;
+    a.ldq = b.ldq;
+    a.Qcur = L.take<double>(size_t(b.ldq) * N); a.Qnew = L.take<double>(size_t(b.ldq) * N); a.G = L.take<double>(size_t(b.ldq) * N);
+    a.dcur = L.take<double>(N); a.dnew = L.take<double>(N); a.dm = L.take<double>(N); a.zs = L.take<double>(N);
+    a.dlam = L.take<double>(N); a.wz = L.take<double>(N); a.dval = L.take<double>(N); a.mu = L.take<double>(N); a.zhat = L.take<double>(N);
+    a.rotc = L.take<double>(N); a.rots = L.take<double>(N); b.val = L.take<double>(N);
+    a.idx = L.take<int>(N); a.idxnew = L.take<int>(N); a.srcm = L.take<int>(N); a.typ = L.take<int>(N); a.gsrc = L.take<int>(N);
+    a.gpos = L.take<int>(N); a.gtyp = L.take<int>(N); a.dsrc = L.take<int>(N); a.dtyp = L.take<int>(N); a.org = L.take<int>(N);
+    a.rota = L.take<int>(N); a.rotb = L.take<int>(N); a.rotta = L.take<int>(N); a.rottb = L.take<int>(N);
+    a.desc = L.take<MergeDesc>((N + kDcLeaf - 1) / kDcLeaf + 1);
+    a.info = base != nullptr ? info_ptr(p) : nullptr;
+    if (bytes != nullptr) *bytes = L.total;
+    return b;
+}
+
+gs_status_t evp_ready(const gs_plan* plan, EvpBuffers* b)
+{
+    GS_TRY(check_ready(plan));
+    size_t need = 0;
+    evp_carve(plan, nullptr, &need);
+    if (plan->evp_ws == nullptr || plan->evp_ws_bytes < need) return GS_ERR_WORKSPACE;
+    *b = evp_carve(plan, plan->evp_ws, nullptr);
+    return GS_OK;
+}
+
+template <typename T>
+StepParams<T> step_params(const gs_plan* plan, const EvpBuffers& b, void* A, double* d, double* e, void* tau)
+{
+    StepParams<T> p{};
+    p.A = static_cast<T*>(A); p.ld = plan->N; p.N = int(plan->N); p.nb = b.nb; p.lb = b.nb;
+    p.u = static_cast<T*>(b.u); p.wp = static_cast<T*>(b.wp); p.corr2 = static_cast<T*>(b.corr2);
+    p.Vt = static_cast<T*>(b.Vt); p.Wt = static_cast<T*>(b.Wt);
+    p.P1 = static_cast<T*>(b.P1); p.P2 = static_cast<T*>(b.P2); p.ldp = b.ldp;
+    p.Pt = static_cast<T*>(b.Pt); p.tfin = static_cast<T*>(b.tfin); p.Pd = static_cast<T*>(b.Pd);
+    p.sc = static_cast<StepScalars<T>*>(b.sc); p.tickets = b.tickets;
+    p.d = d; p.e = e; p.tau = static_cast<T*>(tau); p.R = static_cast<T*>(b.R);
+    p.info = info_ptr(plan);
+    return p;
+}
+
+// GS_EVP_TRACE=1: synchronise after every launch of the eigensolver and name it on stderr (debugging aid)
+inline bool evp_trace_on()
+{
+    static const bool on = std::getenv("GS_EVP_TRACE") != nullptr;
+    return on;
+}
+inline void evp_trace(cudaStream_t stream, const char* what, int a = 0, int b = 0)
+{
+    if (!evp_trace_on()) return;
+    const cudaError_t e = cudaStreamSynchronize(stream);
+    std::fprintf(stderr, "[evp] %s %d %d -> %s\n", what, a, b, cudaGetErrorString(e));
+    std::fflush(stderr);
+}
+
+// step kernels: programmatic dependent launch unless GS_EVP_PDL=0
+template <typename... KArgs, typename... Args>
+inline cudaError_t evp_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args)
+{
+    static const bool pdl = !(std::getenv("GS_EVP_PDL") != nullptr && std::atoi(std::getenv("GS_EVP_PDL")) == 0);
+    if (pdl) return launch_pdl(kernel, grid, block, 0, stream, args...);
+    kernel<<<grid, block, 0, stream>>>(KArgs(args)...);
+    return cudaGetLastError();
+}
+
+#define GS_LAUNCH_OK(plan)                                       \
+    do {                                                         \
+        const cudaError_t le__ = cudaGetLastError();             \
+        if (le__ != cudaSuccess) return cuda_fail((plan), le__); \
+        (plan)->launches += 1;                                   \
+    } while (0)
+
+// A[0:m, 0:m] -= V W^H + W V^H (upper tiles) from the panel's conjugate-transposed images Vt, Wt (cnt x m, ld nb)
+gs_status_t evp_her2k(gs_plan* plan, const EvpBuffers& b, void* A, int m, int cnt, cudaStream_t stream)
+{
+    Stage st = make_stage(plan, stream);
+    st.tma = true;                       // the operands are the panels (even pitch by construction), also for odd N
+    const MatView vV{b.Vt, cnt, m, b.nb}, vW{b.Wt, cnt, m, b.nb};
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vV, false) || !set_operand(st, p, 1, vW, false) || !set_operand(st, p, 2, vW, false) ||
+        !set_operand(st, p, 3, vV, false))
+        return GS_ERR_CUDA;
+    p.C = static_cast<double*>(A); p.ldc = plan->N;
+    p.tiles_m = (m + st.lb - 1) / st.lb; p.tiles_n = p.tiles_m; p.order = ORDER_TRI_ROW_DESC;
+    p.c_rows = m; p.c_cols = m;
+    p.khi_c = (cnt + st.bk - 1) / st.bk; p.kmax = p.khi_c;
+    p.alpha = -1.0; p.beta = 1.0;
+    p.flags = F_DUAL | F_STORE_UPPER | F_REAL_DIAG;
+    return launch(st, p, false, L_EVP_HER2K);
+}
+
+template <typename T>
+gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, double* d, double* e, void* tau, cudaStream_t stream)
+{
+    constexpr int TH = SymvGeom<T>::TH, TW = kSymvTW;
+    const int N = int(plan->N), nb = b.nb;
+    GS_CUDA(plan, cudaMemsetAsync(b.tickets, 0, 16 * sizeof(unsigned int), stream));
+    GS_CUDA(plan, cudaMemsetAsync(b.sc, 0, 256, stream));
+    init_r_kernel<T><<<64, 256, 0, stream>>>(static_cast<T*>(b.R), nb, b.npanels);
+    GS_LAUNCH_OK(plan);
+    StepParams<T> p = step_params<T>(plan, b, A, d, e, tau);
+    const bool vec = (N % 2 == 0);
+    const int fgrid = std::max(1, std::min(64, (N + 255) / 256));
+    auto finish = [&](int i, int jp, int mode) -> gs_status_t {
+        p.i = i; p.jp = jp; p.mode = mode;
+        LaunchTimer timer(plan, L_EVP_STEP, stream);
+        const cudaError_t le = evp_launch(finish_kernel<T>, fgrid, 256, stream, p);
+        if (le != cudaSuccess) return cuda_fail(plan, le);
+        plan->launches += 1;
+        evp_trace(stream, "finish", i, mode);
+        return GS_OK;
+    };
+    GS_TRY(finish(N, 0, 1));                      // fresh load of column N-1
+    int i = N - 1, panel = 0;
+    while (i >= 1) {
+        const int itop = i;
+        int jp = 0;
+        p.itop = itop; p.panel = panel;
+        while (i >= 1 && jp < nb) {
+            p.i = i; p.jp = jp; p.mode = 0;
+            const int nJ = (i + TW - 1) / TW, nI = (i + TH - 1) / TH;
+            {
+                LaunchTimer timer(plan, L_EVP_SYMV, stream);
+                const dim3 grid(nJ, nI + (jp > 0 ? 1 : 0));
+                const cudaError_t le = vec ? evp_launch(symv_kernel<T, true>, grid, kSymvThreads, stream, p)
+                                           : evp_launch(symv_kernel<T, false>, grid, kSymvThreads, stream, p);
+                if (le != cudaSuccess) return cuda_fail(plan, le);
+                plan->launches += 1;
+                evp_trace(stream, "symv", i, jp);
+            }
+            {
+                LaunchTimer timer(plan, L_EVP_STEP, stream);
+                const cudaError_t le = evp_launch(combine_kernel<T>, (i + kCombineRows - 1) / kCombineRows, 256, stream, p);
+                if (le != cudaSuccess) return cuda_fail(plan, le);
+                plan->launches += 1;
+                evp_trace(stream, "combine", i, jp);
+            }
+            const bool last = (jp == nb - 1) || (i == 1);
+            GS_TRY(finish(i, jp, last ? 2 : 0));
+            --i; ++jp;
+        }
+        // the panel's rank-2 jp update of the leading (i + 1) x (i + 1) block, then the next column from the updated matrix
+        GS_TRY(evp_her2k(plan, b, A, i + 1, jp, stream));
+        evp_trace(stream, "her2k", i + 1, jp);
+        GS_TRY(finish(i + 1, 0, 1));
+        ++panel;
+    }
+    // T' = (D + stril(V^H V))^-1 per panel, kept as R^-1 with R = (T'^-1)^H upper triangular (one leaf launch)
+    GS_TRY(configure_leaf(plan));
+    const int nblocks = panel > 0 ? panel : 1;
+    {
+        LaunchTimer timer(plan, L_EVP_STEP, stream);
+        if (plan->z)
+            trtri_cleaf_kernel<<<nblocks, kCLeafThreads, kCLeafSmemBytes, stream>>>(static_cast<const double2*>(b.R), static_cast<double2*>(b.Rinv),
+                                                                                   (long long)nb, nblocks * nb, info_ptr(plan));
+        else
+            trtri_leaf_kernel<<<nblocks, kLeafThreads, kLeafSmemBytes, stream>>>(static_cast<const double*>(b.R), static_cast<double*>(b.Rinv),
+                                                                                 (long long)nb, nblocks * nb, info_ptr(plan));
+        GS_LAUNCH_OK(plan);
+        evp_trace(stream, "trtri_blocks", nblocks, 0);
+    }
+    return GS_OK;
+}
+
+// C~ = Q Z:  Q = H(N-1) ... H(1) applied panel by panel, lowest reflectors first:
+//   Y = Vp^H C~[0:m, :],  Y2 = T'p Y = (Rp^-1)^H Y,  C~[0:m, :] -= Vp Y2.
+gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const void* A, const double* Z, long long ldz, void* Ct, cudaStream_t stream)
+{
+    const int N = int(plan->N), nev = int(plan->nev), nb = b.nb;
+    if (nev == 0) return GS_OK;
+    {
+        LaunchTimer timer(plan, L_EVP_BACK, stream);
+        const dim3 grid((N + 255) / 256, std::min(nev, 4096));
+        if (plan->z) widen_kernel<double2><<<grid, 256, 0, stream>>>(Z, ldz, static_cast<double2*>(Ct), plan->N, N, nev);
+        else widen_kernel<double><<<grid, 256, 0, stream>>>(Z, ldz, static_cast<double*>(Ct), plan->N, N, nev);
+        GS_LAUNCH_OK(plan);
+        evp_trace(stream, "back.widen", N, nev);
+    }
+    if (N < 2) return GS_OK;
+    Stage st = make_stage(plan, stream);
+    const int lb = st.lb, bk = st.bk;
+    const int npan = (N - 1 + nb - 1) / nb;           // reflectors i = 1 .. N-1 in panels counted from the top
+    const int tn = (nev + lb - 1) / lb;
+    for (int pnl = npan - 1; pnl >= 0; --pnl) {
+        const int itop = N - 1 - pnl * nb;
+        int cnt = std::min(nb, itop);                  // reflectors itop - cnt + 1 .. itop
+        int i0 = itop - cnt + 1, first = nb - cnt;
+        const int m = itop;
+        // a TMA box of FP64 elements must start at an even row: an odd start takes in the reflector below it, which for
+        // the (only) partial panel is column 0 of the reflector matrix -- a zero vector with T' = 1, i.e. no reflector
+        if (first % 2 != 0) { first -= 1; i0 -= 1; cnt += 1; }
+        const MatView vA{A, m, i0 + cnt, N}, vC{Ct, m, nev, N};
+        const MatView vY{b.Y, cnt, nev, nb}, vY2{b.Y2, cnt, nev, nb};
+        const MatView vR{static_cast<const unsigned char*>(b.Rinv) + size_t(pnl) * nb * (nb + 1) * plan->es, nb, nb, nb};
+        {   // Y = Vp^H C~
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vA, false) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
+            p.C = static_cast<double*>(b.Y); p.ldc = nb;
+            p.tiles_m = 1; p.tiles_n = tn; p.order = ORDER_ROW;
+            p.c_rows = cnt; p.c_cols = nev;
+            p.khi_c = (m + bk - 1) / bk; p.kmax = p.khi_c;
+            p.a.x0 = i0;
+            GS_TRY(launch(st, p, false, L_EVP_BACK));
+            evp_trace(stream, "back.y", pnl, cnt);
+        }
+        {   // Y2 = (Rp^-1)^H Y  (the panel's block of R^-1 is upper triangular with zeros below)
+            Stage s2 = st;
+            s2.tma = true;
+            EngineParams p = blank_params(plan);
+            if (!set_operand(s2, p, 0, vR, false) || !set_operand(s2, p, 1, vY, false)) return GS_ERR_CUDA;
+            p.C = static_cast<double*>(b.Y2); p.ldc = nb;
+            p.tiles_m = 1; p.tiles_n = tn; p.order = ORDER_ROW;
+            p.c_rows = cnt; p.c_cols = nev;
+            p.khi_c = (cnt + bk - 1) / bk; p.kmax = p.khi_c;
+            p.a.k0 = first; p.a.x0 = first;
+            GS_TRY(launch(s2, p, false, L_EVP_BACK));
+            evp_trace(stream, "back.ty", pnl, first);
+        }
+        {   // C~[0:m, :] -= Vp Y2
+            EngineParams p = blank_params(plan);
+            if (!set_operand(st, p, 0, vA, true) || !set_operand(st, p, 1, vY2, false)) return GS_ERR_CUDA;
+            p.C = static_cast<double*>(Ct); p.ldc = N;
+            p.tiles_m = (m + lb - 1) / lb; p.tiles_n = tn; p.order = ORDER_ROW;
+            p.c_rows = m; p.c_cols = nev;
+            p.khi_c = (cnt + bk - 1) / bk; p.kmax = p.khi_c;
+            p.a.k0 = i0;
+            p.alpha = -1.0; p.beta = 1.0;
+            GS_TRY(launch(st, p, true, L_EVP_BACK));
+            evp_trace(stream, "back.update", pnl, m);
+        }
+    }
+    return GS_OK;
+}
+
+// Divide and conquer on tridiag(e, d, e): lowest nev eigenvalues -> eps, their eigenvectors -> Z (N x nev, ld ldz).
+// d is modified (cut points).  Synchronises the stream once per level: the deflation counts decide the shapes of
+// the launches that follow.
+gs_status_t evp_solve_impl(gs_plan* plan, EvpBuffers& b, double* d, const double* e, double* eps, double* Z, long long ldz, cudaStream_t stream)
+{
+    const int N = int(plan->N), nev = int(plan->nev);
+    DcArrays a = b.dc;
+    const int nleaf = (N + kDcLeaf - 1) / kDcLeaf;
+    {
+        LaunchTimer timer(plan, L_EVP_DC, stream);
+        if (nleaf > 1) { dc_cut_kernel<<<(nleaf + 255) / 256, 256, 0, stream>>>(d, e, N); GS_LAUNCH_OK(plan); }
+        dc_leaf_kernel<<<nleaf, kDcLeaf, 0, stream>>>(d, e, N, a);
+        GS_LAUNCH_OK(plan);
+    }
+    // real engine launches, also inside a complex plan
+    Stage st = make_stage(plan, stream);
+    st.z = false; st.lb = LB; st.bk = BK; st.tma = true;
+    std::vector<MergeDesc> hd;
+    for (int span = 1; span < nleaf; span *= 2) {           // blocks of `span` leaves are solved; merge neighbours
+        hd.clear();
+        std::vector<std::pair<int, int>> pass;             // (off, n) of blocks without a partner
+        for (int g = 0; g * span < nleaf; g += 2) {
+            const int off = g * span * kDcLeaf;
+            const int end1 = std::min((g + 1) * span * kDcLeaf, N);
+            const int end2 = std::min((g + 2) * span * kDcLeaf, N);
+            if (end2 > end1) { MergeDesc m{}; m.off = off; m.n1 = end1 - off; m.n2 = end2 - end1; hd.push_back(m); }
+            else pass.emplace_back(off, end1 - off);
+        }
+        const int nm = int(hd.size());
+        const bool top = span * 2 >= nleaf;
+        int nmax = 0;
+        for (const MergeDesc& m : hd) nmax = std::max(nmax, m.n1 + m.n2);
+        GS_CUDA(plan, cudaMemcpyAsync(a.desc, hd.data(), sizeof(MergeDesc) * nm, cudaMemcpyHostToDevice, stream));
+        {
+            LaunchTimer timer(plan, L_EVP_DC, stream);
+            dc_setup_kernel<<<nm, 256, 0, stream>>>(e, a); GS_LAUNCH_OK(plan);
+            dc_deflate_kernel<<<nm, 256, 0, stream>>>(a); GS_LAUNCH_OK(plan);
+            dc_rotate_kernel<<<dim3((nmax + 255) / 256, nm), 256, 0, stream>>>(a); GS_LAUNCH_OK(plan);
+            dc_gather_kernel<<<dim3(nmax, nm), 256, 0, stream>>>(a); GS_LAUNCH_OK(plan);
+            dc_secular_kernel<<<dim3((nmax + 7) / 8, nm), 256, 0, stream>>>(a); GS_LAUNCH_OK(plan);
+            dc_zhat_kernel<<<dim3((nmax + 7) / 8, nm), 256, 0, stream>>>(a); GS_LAUNCH_OK(plan);
+        }
+        GS_CUDA(plan, cudaMemcpyAsync(hd.data(), a.desc, sizeof(MergeDesc) * nm, cudaMemcpyDeviceToHost, stream));
+        GS_CUDA(plan, cudaStreamSynchronize(stream));
+        for (MergeDesc& m : hd) m.r = top ? std::min(m.k, nev) : m.k;
+        GS_CUDA(plan, cudaMemcpyAsync(a.desc, hd.data(), sizeof(MergeDesc) * nm, cudaMemcpyHostToDevice, stream));
+        double* X = a.Qcur;                                  // the old eigenvector blocks are dead once gathered
+        {
+            LaunchTimer timer(plan, L_EVP_DC, stream);
+            dc_xcols_kernel<<<dim3((nmax + 7) / 8, nm), 256, 0, stream>>>(a, X); GS_LAUNCH_OK(plan);
+        }
+        const long long ldq = a.ldq;
+        for (const MergeDesc& m : hd) {
+            if (m.r == 0) continue;
+            const int off = m.off, n = m.n1 + m.n2;
+            for (int half = 0; half < 2; ++half) {
+                const int row0 = half == 0 ? off : off + m.n1, rows = half == 0 ? m.n1 : m.n2;
+                // (the bottom k-range starts at an even row of X: one column of the Q1-only group, zero in these rows, may be taken in)
+                const int kc0 = half == 0 ? 0 : (m.c1 & ~1), kk = half == 0 ? m.c1 + m.c2 : m.k - (m.c1 & ~1);
+                const MatView vG{a.G, row0 + rows, off + kc0 + kk, ldq}, vX{X, off + kc0 + kk, off + m.r, ldq};
+                EngineParams p = blank_params(plan);
+                if (!set_operand(st, p, 0, vG, true) || !set_operand(st, p, 1, vX, false)) return GS_ERR_CUDA;
+                p.C = a.Qnew; p.ldc = ldq;
+                p.tiles_m = (rows + LB - 1) / LB; p.tiles_n = (m.r + LB - 1) / LB; p.order = ORDER_COL;
+                p.c_row0 = row0; p.c_col0 = off; p.c_rows = row0 + rows; p.c_cols = off + m.r;
+                p.khi_c = (kk + BK - 1) / BK; p.kmax = p.khi_c;
+                p.a.x0 = row0; p.a.k0 = off + kc0;
+                p.b.k0 = off + kc0; p.b.x0 = off;
+                GS_TRY(launch(st, p, true, L_EVP_DC_GEMM));
+            }
+            (void)n;
+        }
+        {
+            LaunchTimer timer(plan, L_EVP_DC, stream);
+            dc_values_kernel<<<dim3((nmax + 255) / 256, nm), 256, 0, stream>>>(a, b.val); GS_LAUNCH_OK(plan);
+            dc_rank_kernel<<<dim3((nmax + 255) / 256, nm), 256, 0, stream>>>(a, b.val); GS_LAUNCH_OK(plan);
+            for (const auto& pb : pass) {
+                dc_copy_block_kernel<<<pb.second, 256, 0, stream>>>(a.Qcur, a.Qnew, ldq, pb.first, pb.second); GS_LAUNCH_OK(plan);
+                GS_CUDA(plan, cudaMemcpyAsync(a.dnew + pb.first, a.dcur + pb.first, sizeof(double) * pb.second, cudaMemcpyDeviceToDevice, stream));
+                GS_CUDA(plan, cudaMemcpyAsync(a.idxnew + pb.first, a.idx + pb.first, sizeof(int) * pb.second, cudaMemcpyDeviceToDevice, stream));
+            }
+        }
+        std::swap(a.Qcur, a.Qnew);
+        std::swap(a.dcur, a.dnew);
+        std::swap(a.idx, a.idxnew);
+    }
+    if (nev > 0) {
+        LaunchTimer timer(plan, L_EVP_DC, stream);
+        dc_output_kernel<<<nev, 256, 0, stream>>>(a.Qcur, a.ldq, a.dcur, a.idx, N, nev, eps, Z, ldz, info_ptr(plan));
+        GS_LAUNCH_OK(plan);
+    }
+    return GS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+gs_status_t gs_evp_workspace_bytes(const gs_plan_t* plan, size_t* bytes)
+{
+    if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
+    evp_carve(plan, nullptr, bytes);
+    return GS_OK;
+}
+
+gs_status_t gs_evp_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t bytes)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    size_t need = 0;
+    evp_carve(plan, nullptr, &need);
+    if (dev_workspace == nullptr || bytes < need || (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) != 0) return GS_ERR_WORKSPACE;
+    plan->evp_ws = static_cast<unsigned char*>(dev_workspace);
+    plan->evp_ws_bytes = bytes;
+    return GS_OK;
+}
+
+gs_status_t gs_evp_tridiagonalize(gs_plan_t* plan, void* A_inout, double* d, double* e, void* tau, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));
+    if (A_inout == nullptr || d == nullptr || e == nullptr || tau == nullptr || !aligned16(A_inout) || !aligned16(tau)) return GS_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    return plan->z ? evp_tridiagonalize_t<double2>(plan, b, A_inout, d, e, tau, stream)
+                   : evp_tridiagonalize_t<double>(plan, b, A_inout, d, e, tau, stream);
+}
+
+gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double* e, double* eps, double* Z, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));
+    if (d == nullptr || e == nullptr || eps == nullptr || (plan->nev > 0 && Z == nullptr)) return GS_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    GS_CUDA(plan, cudaMemcpyAsync(b.dwork, d, sizeof(double) * size_t(plan->N), cudaMemcpyDeviceToDevice, stream));
+    return evp_solve_impl(plan, b, b.dwork, e, eps, Z, plan->N, stream);
+}
+
+gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));
+    if (plan->nev == 0) return GS_OK;
+    if (A_reflectors == nullptr || Z == nullptr || Ctilde == nullptr || !aligned16(A_reflectors) || !aligned16(Ctilde) ||
+        overlaps(Ctilde, vec_bytes(plan), A_reflectors, mat_bytes(plan)))
+        return GS_ERR_INVALID_ARG;
+    return evp_backtransform_impl(plan, b, A_reflectors, Z, plan->N, Ctilde, static_cast<cudaStream_t>(cuda_stream));
+}
+
+gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));
+    if (Htilde_inout == nullptr || eps == nullptr || (plan->nev > 0 && Ctilde == nullptr) || !aligned16(Htilde_inout) ||
+        (Ctilde != nullptr && (!aligned16(Ctilde) || overlaps(Ctilde, vec_bytes(plan), Htilde_inout, mat_bytes(plan)))))
+        return GS_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    GS_TRY(plan->z ? evp_tridiagonalize_t<double2>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream)
+                   : evp_tridiagonalize_t<double>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream));
+    GS_TRY(evp_solve_impl(plan, b, b.d, b.e, eps, b.Z, plan->N, stream));
+    return evp_backtransform_impl(plan, b, Htilde_inout, b.Z, plan->N, Ctilde, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,496 @@
+// evp_tridiag.cuh -- kernels of the one-stage Householder tridiagonalisation  H~ = Q T Q^H  (NEXT-4: the
+// "Tridiag." stage of the standard eigenproblem, "conventional one-stage diagonalization method
+// (ELPA1)", Table 1 column "Tridiag."; the paper notes that on GPUs the one-stage solver is
+// typically the faster one).
+//
+// Upper-triangle form: column i = N-1 .. 1 of the leading (unreduced) block is annihilated above the first
+// superdiagonal by H(i) = I - tau v v^H, v(i-1) = 1, v(i:) = 0; Q = H(N-1) ... H(1).  Panels of nb columns are
+// reduced against the STALE leading block with the usual lazy rank-2 corrections (V, W), and one HER2K-shaped
+// launch of the tile engine applies  A -= V W^H + W V^H  after every panel.
+//
+// Half of the 4N^3/3 flop are the N matrix-vector products with the leading block: 0.5 flop per byte, i.e.
+// HBM-bound (the FP64 ridge of this part is ~5.7 flop/B).  So the design goal of the step kernels is HBM
+// traffic, not arithmetic: the symmetric product reads ONE triangle (4 m^2 bytes per step instead of 8 m^2:
+// 4N^3/3 bytes over the whole reduction), every element feeding both y(r) += a u(c) and y(c) += conj(a) u(r).
+//
+// A step is three launches (S, C, F) because it contains three global reductions that depend on each other
+// (the matrix-vector product, the dot product w'^H v, the norm of the next column).  Two identities shorten
+// that chain:
+//   * with u = the updated column a(0:i) BEFORE scaling, v = s (u - beta e_{i-1}), s = 1 / (alpha - beta): every
+//     product with v is linear in u, so S multiplies by u and never waits for the norm; the scaling is applied
+//     in C:  A v = s (A u - beta A(:, i-1)),  W^H v = s (W^H u - beta conj(W(i-1, :)));
+//   * the part of the NEXT column's lazy update that involves the old panel columns is formed in the same pass
+//     over the panels as the correction of w (C), so the panels are read once per step.
+// Partial sums are combined in a fixed order (per-CTA partial buffers; the last CTA to arrive -- an atomic ticket
+// -- adds them up), so the reduction is bit-reproducible.
+//
+// Panels are stored as conjugate transposes  Vt = V^H, Wt = W^H  (nb x N, leading dimension nb): that is the
+// k-contiguous operand layout of the tile engine's HER2K-shaped launch, and it makes W^H u a plain product.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "ptx.cuh"
+
+namespace gs {
+namespace evp {
+
+// ---- scalar helpers: T = double (real symmetric) or double2 (complex Hermitian, interleaved re/im) ----
+__device__ __forceinline__ double zero_of(double) { return 0.0; }
+__device__ __forceinline__ double2 zero_of(double2) { return make_double2(0.0, 0.0); }
+__device__ __forceinline__ double cj(double a) { return a; }
+__device__ __forceinline__ double2 cj(double2 a) { return make_double2(a.x, -a.y); }
+__device__ __forceinline__ double re(double a) { return a; }
+__device__ __forceinline__ double re(double2 a) { return a.x; }
+__device__ __forceinline__ double abs2(double a) { return a * a; }
+__device__ __forceinline__ double abs2(double2 a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ double mul(double a, double b) { return a * b; }
+__device__ __forceinline__ double2 mul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double add(double a, double b) { return a + b; }
+__device__ __forceinline__ double2 add(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double sub(double a, double b) { return a - b; }
+__device__ __forceinline__ double2 sub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double rscale(double a, double r) { return a * r; }
+__device__ __forceinline__ double2 rscale(double2 a, double r) { return make_double2(a.x * r, a.y * r); }
+// acc + a * b
+__device__ __forceinline__ double fmad(double a, double b, double acc) { return fma(a, b, acc); }
+__device__ __forceinline__ double2 fmad(double2 a, double2 b, double2 acc)
+{
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+    return acc;
+}
+// acc + conj(a) * b
+__device__ __forceinline__ double cfmad(double a, double b, double acc) { return fma(a, b, acc); }
+__device__ __forceinline__ double2 cfmad(double2 a, double2 b, double2 acc)
+{
+    acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+    return acc;
+}
+__device__ __forceinline__ bool is_zero(double a) { return a == 0.0; }
+__device__ __forceinline__ bool is_zero(double2 a) { return a.x == 0.0 && a.y == 0.0; }
+__device__ __forceinline__ double real_only(double a) { return a; }
+__device__ __forceinline__ double2 real_only(double2 a) { return make_double2(a.x, 0.0); }
+__device__ __forceinline__ double from_real(double r, double) { return r; }
+__device__ __forceinline__ double2 from_real(double r, double2) { return make_double2(r, 0.0); }
+__device__ __forceinline__ double shfl_xor(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+__device__ __forceinline__ double2 shfl_xor(double2 v, int m)
+{
+    return make_double2(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
+}
+__device__ __forceinline__ double ldcg(const double* p) { return __ldcg(p); }
+__device__ __forceinline__ double2 ldcg(const double2* p) { return __ldcg(p); }
+
+// Per-step scalars of the reduction, produced by the finalising CTAs and read by the next kernels.
+template <typename T>
+struct StepScalars {
+    T tau;          // reflector scalar of the CURRENT step (H = I - tau v v^H); 0: H = I
+    T s;            // 1 / (alpha - beta) (0 when tau == 0)
+    T alpha2;       // -1/2 |tau|^2 (w'^H v), set by C's finaliser
+    double beta;    // the new off-diagonal entry e(i-1)
+    double xnorm2;  // ||x||^2 of the current column
+    int pad[2];
+};
+
+constexpr int kSymvThreads = 256;
+constexpr int kSymvTW = 128;                        // tile width (columns): 8 warps x 16 columns
+template <typename T> struct SymvGeom { static constexpr int RPT = 32 / int(sizeof(T)); static constexpr int TH = 32 * RPT; };
+
+// Everything a step kernel needs.
+template <typename T>
+struct StepParams {
+    T* A;                 // N x N column-major, ld = N; upper triangle of the leading m x m block is live
+    long long ld;
+    int N;
+    int i;                // current column (S, C, F); the active block is A[0:i, 0:i]
+    int jp;               // number of reflectors already in the panel (panel column of this step)
+    int nb;               // panel width = leading dimension of Vt, Wt
+    int itop;             // column index of panel column 0 (i = itop - jp)
+    T* u;                 // N: the updated, unscaled current column a(0:i+1)
+    T* wp;                // N: w' (C -> F)
+    T* corr2;             // N: old-panel part of the next column's lazy update (C -> F)
+    T* Vt;                // nb x N (ld nb): V^H of the panel
+    T* Wt;                // nb x N (ld nb): W^H of the panel
+    T* P1;                // [nJ][ldp] row-direction partials of y = A u, indexed by column block
+    T* P2;                // [nI][ldp] column-direction partials, indexed by row block
+    long long ldp;
+    T* Pt;                // [nJ][2 nb] partials of W^H u, V^H u
+    T* tfin;              // 2 nb: tW' = W^H v, tV' = V^H v (scaled), final
+    T* Pd;                // dot / norm partials (one per CTA)
+    StepScalars<T>* sc;   // sc[0]: current step
+    unsigned int* tickets;   // [4] atomic tickets (S panel-dot, C, F)
+    double* d;            // N
+    double* e;            // N
+    T* tau;               // N
+    T* R;                 // per-panel upper triangular M^H = conj(D) + striu(V^H V), block p at R + p * lb * (lb + 1), ld = lb
+    int lb;               // block order of R (= nb)
+    int panel;            // panel number (block of R)
+    int mode;             // F: 0 = lazy next column (stale A + panel corrections), 1 = fresh (A is up to date), 2 = none
+    const int* info;
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// S: partial sums of y = A[0:m, 0:m] u (m = i) from the UPPER triangle only, one CTA per (TH x 128) tile; the
+// extra grid row (blockIdx.y == nI) forms W^H u and V^H u over 128-row chunks, and its last CTA finalises them.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, bool kVec>
+__global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> p)
+{
+    constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW;
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const int m = p.i;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const int nI = (m + TH - 1) / TH;
+    __shared__ T red[8][TH];
+    __shared__ unsigned int s_last;
+
+    if (int(blockIdx.y) == nI) {
+        // ---- panel dots: Pt[x][c] = sum_{r in chunk} Wt[c, r] u[r],  Pt[x][nb + c] likewise for Vt ----
+        const int jp = p.jp, nb = p.nb;
+        if (jp == 0) return;
+        const int x = blockIdx.x;
+        const int r0 = x * TW, r1 = min(r0 + TW, m);
+        const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
+        const int c = t % nb, g = t / nb;
+        T aw = zero_of(T{}), av = zero_of(T{});
+        if (c < jp) {
+            for (int r = r0 + g; r < r1; r += groups) {
+                const T ur = p.u[r];
+                aw = fmad(p.Wt[c + (long long)r * nb], ur, aw);
+                av = fmad(p.Vt[c + (long long)r * nb], ur, av);
+            }
+        }
+        T* sm = &red[0][0];                               // 8 * TH elements >= 2 * 256
+        sm[t] = aw; sm[kSymvThreads + t] = av;
+        __syncthreads();
+        if (t < nb) {
+            T sw = zero_of(T{}), sv = zero_of(T{});
+            for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
+            p.Pt[(long long)x * 2 * nb + t] = sw;
+            p.Pt[(long long)x * 2 * nb + nb + t] = sv;
+        }
+        __threadfence();
+        __syncthreads();
+        if (t == 0) s_last = (atomicAdd(&p.tickets[0], 1u) == gridDim.x - 1) ? 1u : 0u;
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+        // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
+        const StepScalars<T> sc = *p.sc;
+        if (t < 2 * nb) {
+            const int cc = t % nb;
+            const bool isV = t >= nb;
+            T acc = zero_of(T{});
+            if (cc < jp) {
+                for (int xx = 0; xx < int(gridDim.x); ++xx) acc = add(acc, ldcg(&p.Pt[(long long)xx * 2 * nb + t]));
+                const T rowv = (isV ? p.Vt : p.Wt)[cc + (long long)(m - 1) * nb];   // conj(W(i-1, c))
+                acc = mul(sc.s, sub(acc, rscale(rowv, sc.beta)));
+            }
+            p.tfin[t] = acc;
+            if (isV && cc < jp) {
+                // G(a, b) = v_a^H v_b for a = itop - cc > b = i;  M^H(b - i0, a - i0) = conj(G(a, b)) with i0 = itop - lb + 1
+                const int lb = p.lb, rowb = lb - 1 - p.jp, cola = lb - 1 - cc;
+                p.R[(long long)p.panel * lb * (lb + 1) + rowb + (long long)cola * lb] = cj(acc);
+            }
+        }
+        if (t == 0) p.tickets[0] = 0u;
+        return;
+    }
+
+    // ---- one tile of the upper triangle ----
+    const int I = blockIdx.y, J = blockIdx.x;
+    if (I * TH > J * TW + TW - 1 || I * TH >= m || J * TW >= m) return;
+    const int r0 = I * TH + lane * RPT;
+    const int c0 = J * TW + warp * 16;
+    T ur[RPT], yr[RPT];
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+        ur[k] = (r0 + k < m) ? p.u[r0 + k] : zero_of(T{});
+        yr[k] = zero_of(T{});
+    }
+    const bool rows_in = r0 + RPT <= m;
+#pragma unroll
+    for (int cc = 0; cc < 16; cc += 8) {
+        T a[8][RPT];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int c = c0 + cc + q;
+            const T* src = p.A + r0 + (long long)c * p.ld;
+            // only tiles that reach the upper triangle are loaded: a thread whose rows lie below column c skips
+            if (c < m && r0 <= c) {
+                if (kVec && rows_in) {
+                    if constexpr (sizeof(T) == 8) {
+                        const double2 v0 = *reinterpret_cast<const double2*>(src);       // 16-byte aligned: even ld
+                        const double2 v1 = *reinterpret_cast<const double2*>(src + 2);
+                        a[q][0] = v0.x; a[q][1] = v0.y; a[q][2] = v1.x; a[q][3] = v1.y;
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < RPT; ++k) a[q][k] = src[k];
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < RPT; ++k) a[q][k] = (r0 + k < m) ? src[k] : zero_of(T{});
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < RPT; ++k) a[q][k] = zero_of(T{});
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int c = c0 + cc + q;
+            const T uc = (c < m) ? p.u[c] : zero_of(T{});
+            T yc = zero_of(T{});
+#pragma unroll
+            for (int k = 0; k < RPT; ++k) {
+                const int r = r0 + k;
+                T av = a[q][k];
+                if (r > c || c >= m) av = zero_of(T{});          // strictly-lower part of the buffer is never used
+                if (r == c) av = real_only(av);                   // Hermitian: real diagonal
+                yr[k] = fmad(av, uc, yr[k]);
+                if (r < c) yc = cfmad(av, ur[k], yc);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) yc = add(yc, shfl_xor(yc, o));
+            if (lane == 0 && c < m) p.P2[(long long)I * p.ldp + c] = yc;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) red[warp][lane * RPT + k] = yr[k];
+    __syncthreads();
+    if (t < TH) {
+        T s = red[0][t];
+#pragma unroll
+        for (int w = 1; w < 8; ++w) s = add(s, red[w][t]);
+        const int r = I * TH + t;
+        if (r < m) p.P1[(long long)J * p.ldp + r] = s;
+    }
+}
+
+// Householder scalars of a column with off-diagonal part (x, alpha):  H [x; alpha] = [0; beta]  (LAPACK xLARFG
+// without the safmin rescaling loop).
+__device__ __forceinline__ void householder_scalars(double alpha, double xnorm2, StepScalars<double>& sc)
+{
+    sc.xnorm2 = xnorm2;
+    if (xnorm2 == 0.0) { sc.tau = 0.0; sc.s = 0.0; sc.beta = alpha; return; }
+    const double beta = -copysign(sqrt(alpha * alpha + xnorm2), alpha);
+    sc.beta = beta;
+    sc.tau = (beta - alpha) / beta;
+    sc.s = 1.0 / (alpha - beta);
+}
+__device__ __forceinline__ void householder_scalars(double2 alpha, double xnorm2, StepScalars<double2>& sc)
+{
+    sc.xnorm2 = xnorm2;
+    if (xnorm2 == 0.0 && alpha.y == 0.0) { sc.tau = make_double2(0.0, 0.0); sc.s = make_double2(0.0, 0.0); sc.beta = alpha.x; return; }
+    const double beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
+    sc.beta = beta;
+    sc.tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+    const double dr = alpha.x - beta, di = alpha.y, den = dr * dr + di * di;     // 1 / (alpha - beta)
+    sc.s = make_double2(dr / den, -di / den);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// C: per row r < m = i (32 rows per CTA, 8 threads per row):
+//   y      = sum of the partials of S
+//   v(r)   = s (u(r) - beta [r == i-1])                       -> Vt[jp, r] = conj(v), A(r, i) = v   (clean reflector)
+//   w'(r)  = s (y - beta A(r, i-1)) - sum_c ( V(r,c) tW'(c) + W(r,c) tV'(c) )
+//   corr2  = sum_c ( V(r,c) conj(W(i-1,c)) + W(r,c) conj(V(i-1,c)) )     (old panel columns of the next lazy update)
+//   partial of w'^H v; the last CTA sets alpha2 = -1/2 |tau|^2 (w'^H v) and records d(i), e(i-1), tau(i).
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kCombineRows = 32;
+template <typename T>
+__global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
+{
+    constexpr int TH = SymvGeom<T>::TH, TW = kSymvTW;
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const int m = p.i, jp = p.jp, nb = p.nb;
+    const int t = threadIdx.x, l8 = t & 7, rr = t >> 3;
+    const int r = blockIdx.x * kCombineRows + rr;
+    const StepScalars<T> sc = *p.sc;
+    __shared__ T s_t[2 * 128];           // tW', tV'
+    __shared__ T s_row[2 * 128];         // Wt[:, i-1], Vt[:, i-1]
+    __shared__ T s_dot[8];
+    __shared__ unsigned int s_last;
+    for (int c = t; c < 2 * nb; c += 256) {
+        const int cc = c % nb;
+        s_t[c] = (cc < jp) ? p.tfin[c] : zero_of(T{});
+        s_row[c] = (cc < jp) ? (c < nb ? p.Wt : p.Vt)[cc + (long long)(m - 1) * nb] : zero_of(T{});
+    }
+    __syncthreads();
+    T dotp = zero_of(T{});
+    T y = zero_of(T{}), c1 = zero_of(T{}), c2 = zero_of(T{});
+    if (r < m) {
+        // y(r): P1[J][r] for J >= r / TW, P2[I][r] for I <= r / TH
+        const int nJ = (m + TW - 1) / TW;
+        for (int J = r / TW + l8; J < nJ; J += 8) y = add(y, p.P1[(long long)J * p.ldp + r]);
+        for (int I = l8; I <= r / TH; I += 8) y = add(y, p.P2[(long long)I * p.ldp + r]);
+        const T* vt = p.Vt + (long long)r * nb;
+        const T* wt = p.Wt + (long long)r * nb;
+        for (int c = l8; c < jp; c += 8) {
+            const T vrc = cj(vt[c]), wrc = cj(wt[c]);             // V(r,c), W(r,c)
+            c1 = fmad(vrc, s_t[c], c1);
+            c1 = fmad(wrc, s_t[nb + c], c1);
+            c2 = fmad(vrc, s_row[c], c2);                          // V(r,c) conj(W(i-1,c)) : s_row[c] = Wt[c, i-1] = conj(W(i-1,c))
+            c2 = fmad(wrc, s_row[nb + c], c2);
+        }
+    }
+    // (all 32 lanes take part in the shuffles: a warp holds four rows, some of which may lie beyond m)
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) { y = add(y, shfl_xor(y, o)); c1 = add(c1, shfl_xor(c1, o)); c2 = add(c2, shfl_xor(c2, o)); }
+    if (r < m) {
+        if (l8 == 0) {
+            const T ur = p.u[r];
+            T v = mul(sc.s, (r == m - 1) ? sub(ur, from_real(sc.beta, T{})) : ur);
+            if (r == m - 1 && !is_zero(sc.s)) v = from_real(1.0, T{});   // (an identity reflector keeps v = 0)
+            T acol = p.A[r + (long long)(m - 1) * p.ld];
+            if (r == m - 1) acol = real_only(acol);
+            T wpr = sub(mul(sc.s, sub(y, rscale(acol, sc.beta))), c1);
+            p.Vt[jp + (long long)r * nb] = cj(v);
+            p.A[r + (long long)m * p.ld] = v;
+            p.wp[r] = wpr;
+            p.corr2[r] = c2;
+            dotp = cfmad(wpr, v, dotp);
+        }
+    }
+    // block partial of w'^H v: lanes with l8 == 0 hold one row each
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dotp = add(dotp, shfl_xor(dotp, o));
+    if ((t & 31) == 0) s_dot[t >> 5] = dotp;
+    __syncthreads();
+    if (t == 0) {
+        T s = s_dot[0];
+        for (int w = 1; w < 8; ++w) s = add(s, s_dot[w]);
+        p.Pd[blockIdx.x] = s;
+        __threadfence();
+        s_last = (atomicAdd(&p.tickets[1], 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (t == 0) {
+        T dot = zero_of(T{});
+        for (int b = 0; b < int(gridDim.x); ++b) dot = add(dot, ldcg(&p.Pd[b]));
+        p.sc->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
+        p.d[m] = re(p.u[m]);
+        p.e[m - 1] = sc.beta;
+        p.tau[m] = sc.tau;
+        // diagonal of M^H = conj(D) + striu(V^H V): conj(1 / tau) (1 for an identity reflector)
+        const int lb = p.lb, pos = lb - 1 - jp;
+        T dinv;
+        if (is_zero(sc.tau)) dinv = from_real(1.0, T{});
+        else { const double n2 = abs2(sc.tau); dinv = cj(rscale(cj(sc.tau), 1.0 / n2)); }   // conj(1/tau) = conj(conj(tau)/|tau|^2)
+        p.R[(long long)p.panel * lb * (lb + 1) + pos + (long long)pos * lb] = dinv;
+        p.tickets[1] = 0u;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// F: finishes step i and prepares column inext = i - 1.
+//   mode 0 (inside a panel):   w(r) = tau w'(r) + alpha2 v(r) -> Wt[jp, r] = conj(w);
+//                              u(r) = A(r, i-1) - corr2(r) - v(r) conj(w(i-1)) - w(r)       (r <= i-1; v(i-1) = 1)
+//   mode 2 (last of a panel):  only w (the HER2K-shaped launch and a fresh load follow)
+//   mode 1 (fresh load):       u(r) = A(r, inext), A up to date; p.i = inext + 1
+//   rows >= i of column i of A are zeroed (clean reflector matrix for the back-transformation);
+//   partial ||u(0 : inext-1)||^2; the last CTA derives beta, tau, s of the next step (and d(0) at the very end).
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) finish_kernel(const StepParams<T> p)
+{
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const int i = p.i, inext = i - 1, jp = p.jp, nb = p.nb, mode = p.mode;
+    const int t = threadIdx.x;
+    const StepScalars<T> sc = *p.sc;
+    __shared__ double s_n[8];
+    __shared__ unsigned int s_last;
+    T wlast = zero_of(T{}), vlast = zero_of(T{});
+    if (mode != 1) {   // w(i-1) and v(i-1) (= 1, or 0 for an identity reflector): every thread forms them itself
+        vlast = cj(p.Vt[jp + (long long)(i - 1) * nb]);
+        wlast = add(mul(sc.tau, p.wp[i - 1]), mul(sc.alpha2, vlast));
+    }
+    double nrm = 0.0;
+    for (int r = blockIdx.x * 256 + t; r < p.N; r += gridDim.x * 256) {
+        if (mode != 1) {
+            if (r < i) {
+                const T v = cj(p.Vt[jp + (long long)r * nb]);
+                const T w = add(mul(sc.tau, p.wp[r]), mul(sc.alpha2, v));
+                p.Wt[jp + (long long)r * nb] = cj(w);
+                if (mode == 0) {
+                    T un = sub(sub(sub(p.A[r + (long long)inext * p.ld], p.corr2[r]), mul(v, cj(wlast))), mul(w, cj(vlast)));
+                    if (r == inext) un = real_only(un);
+                    p.u[r] = un;
+                    if (r < inext - 1) nrm += abs2(un);
+                }
+            } else {
+                p.A[r + (long long)i * p.ld] = zero_of(T{});
+            }
+        } else {
+            if (r <= inext) {
+                T un = p.A[r + (long long)inext * p.ld];
+                if (r == inext) un = real_only(un);
+                p.u[r] = un;
+                if (r < inext - 1) nrm += abs2(un);
+            }
+            if (inext == 0) p.A[r] = zero_of(T{});      // column 0 carries no reflector: the reflector matrix has a zero column there
+        }
+    }
+    if (mode == 2) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+    if ((t & 31) == 0) s_n[t >> 5] = nrm;
+    __syncthreads();
+    if (t == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += s_n[w];
+        reinterpret_cast<double*>(p.Pd)[blockIdx.x] = s;
+        __threadfence();
+        s_last = (atomicAdd(&p.tickets[2], 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (t == 0) {
+        double x2 = 0.0;
+        for (int b = 0; b < int(gridDim.x); ++b) x2 += __ldcg(&reinterpret_cast<const double*>(p.Pd)[b]);
+        if (inext >= 1) {
+            StepScalars<T> nx;
+            nx.alpha2 = zero_of(T{});
+            householder_scalars(ldcg(&p.u[inext - 1]), x2, nx);
+            nx.pad[0] = nx.pad[1] = 0;
+            *p.sc = nx;
+        } else {
+            p.d[0] = re(ldcg(&p.u[0]));
+            p.tau[0] = zero_of(T{});
+        }
+        p.tickets[2] = 0u;
+    }
+}
+
+// identity blocks of R (lb x lb, stride lb (lb + 1)): a partial last panel leaves part of its block unset
+template <typename T>
+__global__ void init_r_kernel(T* R, int lb, int npanels)
+{
+    const long long total = (long long)npanels * lb * (lb + 1);
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const long long within = idx % ((long long)lb * (lb + 1));
+        const int row = int(within % lb), col = int(within / lb);
+        R[idx] = (row == col && col < lb) ? from_real(1.0, T{}) : zero_of(T{});
+    }
+}
+
+// C~(r, c) = Z(r, c) as T (real -> complex widening for the Hermitian path; a plain copy for the real one)
+template <typename T>
+__global__ void widen_kernel(const double* __restrict__ Z, long long ldz, T* __restrict__ C, long long ldc, int rows, int cols)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= rows) return;
+    for (int c = blockIdx.y; c < cols; c += gridDim.y) C[r + (long long)c * ldc] = from_real(Z[r + (long long)c * ldz], T{});
+}
+
+}  // namespace evp
+}  // namespace gs

@@ -33,12 +33,14 @@ using namespace gs;
 // launch labels for the optional per-launch timing (gs_plan_set_timing)
 enum LaunchLabel : int {
     L_POTRF_LEAF = 0, L_POTRF_TRSM, L_POTRF_GEMM, L_POTRF_SYRK, L_ZERO_LOWER,
-    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_DENS_T, L_DENS_SYRK, L_PUSH_BAND, L_COUNT
+    L_TRTRI_LEAF, L_TRTRI_W, L_TRTRI_X, L_TOSTD_G, L_TOSTD_SYR2K, L_BACK_TRMM, L_DENS_T, L_DENS_SYRK, L_PUSH_BAND,
+    L_EVP_SYMV, L_EVP_STEP, L_EVP_HER2K, L_EVP_DC, L_EVP_DC_GEMM, L_EVP_BACK, L_COUNT
 };
 static const char* const kLabelNames[L_COUNT] = {
     "potrf.leaf", "potrf.trsm_leaf", "potrf.gemm", "potrf.syrk", "zero_lower",
     "trtri.leaf", "trtri.w", "trtri.x", "to_standard.g", "to_standard.syr2k", "backtransform.trmm",
-    "density.transpose", "density.syrk", "shard.push_band"};
+    "density.transpose", "density.syrk", "shard.push_band",
+    "evp.tridiag.symv", "evp.tridiag.step", "evp.tridiag.her2k", "evp.solve.dc", "evp.solve.gemm", "evp.back"};
 
 struct TimedLaunch {
     int label;
@@ -57,6 +59,8 @@ struct gs_plan {
     int nblk = 0;                    // ceil(N / lb)
     unsigned char* ws = nullptr;     // caller-owned device workspace
     size_t ws_bytes = 0;
+    unsigned char* evp_ws = nullptr; // caller-owned device workspace of the standard eigensolver (gs_evp_set_workspace)
+    size_t evp_ws_bytes = 0;
     int64_t launches = 0;
     int timing_mode = 0;
     std::vector<TimedLaunch> timed;
@@ -1145,6 +1149,7 @@ gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)
     GS_CUDA(plan, cudaMemcpyAsync(&h, info_ptr(plan), sizeof(int), cudaMemcpyDeviceToHost, stream));
     GS_CUDA(plan, cudaStreamSynchronize(stream));
     if (h > 0) { *info = h; return GS_ERR_NOT_POSDEF; }
+    if (h <= -(1 << 30)) { *info = 0; return GS_ERR_NO_CONVERGENCE; }   // the tridiagonal eigensolver gave up (evp_dc.cuh)
     if (h < 0) { *info = -int64_t(h); return GS_ERR_SINGULAR; }
     return GS_OK;
 }
@@ -1496,6 +1501,7 @@ const char* gs_status_string(gs_status_t status)
         case GS_ERR_CUDA: return "GS_ERR_CUDA";
         case GS_ERR_WORKSPACE: return "GS_ERR_WORKSPACE";
         case GS_ERR_UNSUPPORTED_DEVICE: return "GS_ERR_UNSUPPORTED_DEVICE";
+        case GS_ERR_NO_CONVERGENCE: return "GS_ERR_NO_CONVERGENCE";
     }
     return "GS_ERR_UNKNOWN";
 }
@@ -1503,3 +1509,5 @@ const char* gs_status_string(gs_status_t status)
 const char* gs_plan_last_cuda_error(const gs_plan_t* plan) { return plan != nullptr ? plan->cuda_error : ""; }
 
 }  // extern "C"
+
+#include "evp_host.cuh"

@@ -24,7 +24,7 @@ GS_PUSH_UINV, GS_PUSH_G, GS_PUSH_HTILDE, GS_PUSH_C = 0, 1, 2, 3
 GS_OK = 0
 STATUS_NAMES = {
     0: "GS_OK", 1: "GS_ERR_INVALID_ARG", 2: "GS_ERR_NOT_POSDEF", 3: "GS_ERR_SINGULAR",
-    4: "GS_ERR_CUDA", 5: "GS_ERR_WORKSPACE", 6: "GS_ERR_UNSUPPORTED_DEVICE",
+    4: "GS_ERR_CUDA", 5: "GS_ERR_WORKSPACE", 6: "GS_ERR_UNSUPPORTED_DEVICE", 7: "GS_ERR_NO_CONVERGENCE",
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
@@ -34,6 +34,8 @@ EXPORTS = (
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
+    "gs_evp_workspace_bytes", "gs_evp_set_workspace", "gs_evp_tridiagonalize", "gs_evp_tridiag_solve", "gs_evp_backtransform",
+    "gs_standard_eigh",
 )
 
 
@@ -99,6 +101,12 @@ def lib() -> ctypes.CDLL:
         L.gs_plan_launch_times.argtypes = [vp, ctypes.POINTER(LaunchTime), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.gs_plan_launch_trace.argtypes = [vp, ctypes.POINTER(LaunchTrace), ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         L.gs_plan_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
+        L.gs_evp_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        L.gs_evp_set_workspace.argtypes = [vp, vp, sz]
+        L.gs_evp_tridiagonalize.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.gs_evp_tridiag_solve.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.gs_evp_backtransform.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_standard_eigh.argtypes = [vp, vp, vp, vp, vp]
         L.gs_status_string.argtypes = [ctypes.c_int]
         L.gs_status_string.restype = ctypes.c_char_p
         L.gs_plan_last_cuda_error.argtypes = [vp]
@@ -248,6 +256,66 @@ class Plan:
         self._check(lib().gs_density_matrix(self._h, _dev_ptr(C, self.N, self.nev, self.tdtype), f.data_ptr(),
                                             _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
 
+    # ---- NEXT-4: the standard eigenproblem H~ C~ = C~ eps between step 3 and the back-transformation ----
+    def evp_workspace_bytes(self) -> int:
+        n = ctypes.c_size_t(0)
+        self._check(lib().gs_evp_workspace_bytes(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    def ensure_evp_workspace(self, alloc=None):
+        """Allocates (once) and registers the eigensolver's scratch; `alloc(nbytes)` may supply the uint8 buffer."""
+        if getattr(self, "evp_workspace", None) is None:
+            n = self.evp_workspace_bytes()
+            self.evp_workspace = alloc(n) if alloc is not None else torch.empty(n, dtype=torch.uint8, device=self.device)
+            self._check(lib().gs_evp_set_workspace(self._h, self.evp_workspace.data_ptr(), n))
+
+    def _vec(self, n: int, dtype=torch.float64) -> torch.Tensor:
+        return torch.empty(n, dtype=dtype, device=self.device)
+
+    def evp_tridiagonalize(self, A: torch.Tensor, stream=None):
+        """"Tridiag.": A (upper triangle = H~) -> Householder vectors in A, returns (d, e, tau)."""
+        self.ensure_evp_workspace()
+        d, e, tau = self._vec(self.N), self._vec(self.N), self._vec(self.N, self.tdtype)
+        self._check(lib().gs_evp_tridiagonalize(self._h, _dev_ptr(A, self.N, self.N, self.tdtype), d.data_ptr(), e.data_ptr(),
+                                                tau.data_ptr(), _stream_ptr(stream)))
+        return d, e[:max(self.N - 1, 0)], tau
+
+    def evp_tridiag_solve(self, d: torch.Tensor, e: torch.Tensor, stream=None):
+        """"Solve": lowest nev eigenvalues of tridiag(e, d, e) and their eigenvectors Z (N x nev, real)."""
+        from .workloads import colmajor_empty
+        self.ensure_evp_workspace()
+        ebuf = self._vec(self.N)
+        ebuf[:e.numel()].copy_(e)
+        eps = self._vec(max(self.nev, 1))[:self.nev]
+        Z = colmajor_empty(self.N, max(self.nev, 1), device=self.device)[:, :self.nev]
+        self._check(lib().gs_evp_tridiag_solve(self._h, d.contiguous().data_ptr(), ebuf.data_ptr(), eps.data_ptr(), Z.data_ptr(),
+                                               _stream_ptr(stream)))
+        return eps, Z
+
+    def evp_backtransform(self, A: torch.Tensor, Z: torch.Tensor, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """"Back": C~ = Q Z with the reflectors evp_tridiagonalize left in A."""
+        from .workloads import colmajor_empty
+        self.ensure_evp_workspace()
+        Ct = colmajor_empty(self.N, max(self.nev, 1), dtype=self.tdtype, device=self.device)[:, :self.nev] if out is None else out
+        if self.nev > 0:
+            self._check(lib().gs_evp_backtransform(self._h, _dev_ptr(A, self.N, self.N, self.tdtype),
+                                                   _dev_ptr(Z, self.N, self.nev, torch.float64),
+                                                   _dev_ptr(Ct, self.N, self.nev, self.tdtype), _stream_ptr(stream)))
+        return Ct
+
+    def standard_eigh(self, Htilde: torch.Tensor, eps: torch.Tensor | None = None, out: torch.Tensor | None = None,
+                      workspace_alloc=None, stream=None):
+        """The three stages in a row on the upper triangle of Htilde (DESTROYED): returns (eps, C~), lowest nev pairs."""
+        from .workloads import colmajor_empty
+        self.ensure_evp_workspace(workspace_alloc)
+        if eps is None:
+            eps = self._vec(max(self.nev, 1))[:self.nev]
+        Ct = colmajor_empty(self.N, max(self.nev, 1), dtype=self.tdtype, device=self.device)[:, :self.nev] if out is None else out
+        self._check(lib().gs_standard_eigh(self._h, _dev_ptr(Htilde, self.N, self.N, self.tdtype), eps.data_ptr(),
+                                           _dev_ptr(Ct, self.N, self.nev, self.tdtype) if self.nev > 0 else None,
+                                           _stream_ptr(stream)))
+        return eps, Ct
+
     def last_info(self, stream=None, raise_on_failure: bool = True) -> int:
         info = ctypes.c_int64(0)
         status = lib().gs_last_info(self._h, _stream_ptr(stream), ctypes.byref(info))
@@ -308,10 +376,10 @@ class Plan:
 
     def launch_times(self) -> dict:
         """{label: (launches, total_ms)} since the last set_timing; call after a stream synchronise."""
-        buf = (LaunchTime * 16)()
+        buf = (LaunchTime * 32)()
         n = ctypes.c_int(0)
-        self._check(lib().gs_plan_launch_times(self._h, buf, 16, ctypes.byref(n)))
-        return {buf[i].label.decode(): (int(buf[i].launches), float(buf[i].ms)) for i in range(min(n.value, 16))}
+        self._check(lib().gs_plan_launch_times(self._h, buf, 32, ctypes.byref(n)))
+        return {buf[i].label.decode(): (int(buf[i].launches), float(buf[i].ms)) for i in range(min(n.value, 32))}
 
 
 def ipc_export(t: torch.Tensor):

@@ -65,7 +65,7 @@ def check_size(N: int, cplx: bool, standard_evp: bool = False) -> dict:
     out["cols_inv"] = _rel(torch.triu(Vx), torch.triu(V))
     out["cols_std"] = _rel(torch.triu(Htx), torch.triu(Ht))
     if standard_evp and hasattr(plan, "standard_eigh"):
-        eps, Q = plan.standard_eigh(Ht, nev)
+        eps, Q = plan.standard_eigh(Ht.clone())
         plan.last_info()
         R = Hs @ Q - Q * eps.to(dt).unsqueeze(0)
         out["evp_resid"] = (R.norm() / (Hs.norm() * N * 2.0 ** -52)).item()
