@@ -44,6 +44,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-checks", action="store_true")
+    ap.add_argument("--no-evp", action="store_true", help="skip the standard-eigensolver block (NEXT-4, outside the metric)")
     ap.add_argument("--batch", type=int, default=0, help="NEXT-2: K independent pencils in flight on one GPU (not the headline)")
     ap.add_argument("--batch-n", type=int, default=2048)
     ap.add_argument("--sharded", action="store_true",
@@ -130,6 +131,22 @@ def oracle_step(k: int, inputs=None):
     return t4 - t0, dict(zip(STAGES, (t1 - t0, t2 - t1, t3 - t2, t4 - t3))), inputs
 
 
+def _one_thread_oracle(k: int):
+    """The same oracle on ONE host thread (OMP_NUM_THREADS=1 in a child process), at a smaller order so that it
+    stays within seconds.  Returns {"value", "sample_N", "seconds"} or None."""
+    import subprocess
+    code = ("import json, bench; sec, st, _ = bench.oracle_step(%d); "
+            "print(json.dumps({'seconds': sec}))" % k)
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS="1", CUDA_VISIBLE_DEVICES="")
+        out = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=env, capture_output=True, text=True, timeout=300)
+        sec = json.loads(out.stdout.strip().splitlines()[-1])["seconds"]
+    except Exception:
+        return None
+    from paper_2502_02460_b200 import workloads as wl
+    return {"value": wl.nominal_flops(k, k // 4)["total"] / sec / 1e12, "unit": UNIT, "cores": 1, "sample_N": k, "seconds": sec}
+
+
 def cpu_baseline(k: int) -> dict:
     import oracle
     from paper_2502_02460_b200 import workloads as wl
@@ -139,7 +156,8 @@ def cpu_baseline(k: int) -> dict:
     return {"value": fl / sec / 1e12, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
             "sample": f"one pass of the four oracle stages on the BASELINE recipe at N={k}, nev={k // 4} "
                       f"(configs[1] size; the full N=16384 oracle would take hours)",
-            "seconds": sec, "stage_seconds": stages}
+            "seconds": sec, "stage_seconds": stages,
+            "one_thread": _one_thread_oracle(min(k, 1536))}
 
 
 def run_reference(args):
@@ -191,13 +209,28 @@ def _measured_peaks() -> dict:
         return {}
 
 
+TRAFFIC_FILE = os.path.join("profiles", "dominant_kernel_traffic.json")
+
+
 def _ncu_traffic(label: str):
     """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture (profiles/), or None."""
     try:
-        d = json.load(open(os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")))
+        d = json.load(open(os.path.join(ROOT, TRAFFIC_FILE)))
         return d.get(label)
     except Exception:
         return None
+
+
+def _traffic_source() -> dict:
+    """Where `roofline.traffic` comes from: the committed file, its git blob id (so that a stale capture is visible
+    in the bench line: the id changes only when the capture is regenerated) and the capture it was made from."""
+    import hashlib
+    try:
+        raw = open(os.path.join(ROOT, TRAFFIC_FILE), "rb").read()
+        blob = hashlib.sha1(b"blob %d\0" % len(raw) + raw).hexdigest()
+        return {"file": TRAFFIC_FILE, "git_blob": blob, "capture": json.loads(raw).get("_source")}
+    except Exception:
+        return {"file": TRAFFIC_FILE, "git_blob": None}
 
 
 def _nvml_index(local_rank: int) -> int:
@@ -324,6 +357,7 @@ def run_ours(args):
         "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
         "frac": (achieved / fp64_peak) if achieved else None,
         "traffic": _ncu_traffic("to_standard.syr2k.complex" if cplx else "to_standard.syr2k") if N == (8192 if cplx else 16384) else None,
+        "traffic_source": _traffic_source(),
         "algorithmic_flop_per_launch": dom_flop, "launch_ms": dom_ms, "launches_timed": dom[0],
         "peak_source": "measured live on this device: sustained mma.sync.m8n8k4.f64 (DMMA) microbenchmark "
                        "(libgs_peak.so); MEASURED_PEAKS.json has no FP64 entry",
@@ -350,6 +384,13 @@ def run_ours(args):
                                       "nominal_flop": dens_flop}}
     plan.to_standard(H, V, Ht)            # restore H~ for the checks below
     plan.last_info()
+
+    # NEXT-4 (outside the metric): the standard eigenproblem H~ C~ = C~ eps between step 3 and the back-transformation
+    # (Table 1 "Tridiag. / Solve / Back"), and the WHOLE generalized solve as one chain
+    if not args.no_evp:
+        next_stages["standard_evp"] = standard_evp_block(plan, H, S0, U, V, Ht, C, N, nev, cplx, fp64_peak, _measured_peaks().get("hbm_gbs"))
+        plan.to_standard(H, V, Ht)        # (the eigensolver destroyed H~)
+        plan.last_info()
 
     stages = {}
     for name, ms in zip(STAGES, stage_ms):
@@ -420,6 +461,10 @@ def run_ours(args):
             plan.last_info()
             checks["e2e_Htilde_equals_device_path"] = bool(torch.equal(torch.triu(hHt.t().to(dev)), torch.triu(Ht2)))
             del Ht2
+            Cref = V @ Ct
+            checks["e2e_C_rel_fro_vs_torch"] = ((hC.t().to(dev) - Cref).norm() / Cref.norm()).item()
+            del Cref
+            checks["ok"] = bool(checks["ok"] and checks["e2e_Htilde_equals_device_path"] and checks["e2e_C_rel_fro_vs_torch"] < 1e-11)
         del scratch, hH, hS, hHt, hCt, hC
 
     cpu = None
@@ -444,6 +489,74 @@ def run_ours(args):
                              "Invert 1.8 s, Multiply 18.8 s, Backtr. 6.8 s = 29.7 s, i.e. ~6.2 TFLOP/s on 4 GPUs (context only)",
         }))
     replicas.finalize(info)
+
+
+def standard_evp_block(plan, H, S0, U, V, Ht, C, N, nev, cplx, fp64_peak, hbm_gbs):
+    """Times the three stages of the standard eigensolver on the H~ the path just formed, then the whole generalized
+    solve (steps 1-3, eigensolver, back-transformation) as one chain; checks the acceptance metrics on the result."""
+    import torch
+    from paper_2502_02460_b200 import metrics as M
+
+    plan.ensure_evp_workspace()
+    C = torch.empty_like(C)               # (the caller's C keeps the back-transform of its own C~ for the checks)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    A = Ht.clone()
+    plan.evp_tridiagonalize(A)            # warm-up (module load, workspace touch)
+    A.copy_(Ht)
+    ev[0].record()
+    d, e, tau = plan.evp_tridiagonalize(A)
+    ev[1].record()
+    eps, Z = plan.evp_tridiag_solve(d, e)
+    ev[2].record()
+    Ct = plan.evp_backtransform(A, Z)
+    ev[3].record()
+    plan.last_info()
+    t_tri, t_solve, t_back = (ev[i].elapsed_time(ev[i + 1]) for i in range(3))
+    f = 4.0 if cplx else 1.0
+    es = 16 if cplx else 8
+    tri_bytes = 4.0 * float(N) ** 3 / 3.0 * (es / 8.0)       # one triangle of the leading block per step: sum_m 4 m^2 (x2 complex)
+    back_flop = f * 2.0 * float(N) ** 2 * nev
+    her2k_flop = f * 2.0 * float(N) ** 3 / 3.0
+    # per-label device times of one more pass
+    A.copy_(Ht)
+    plan.set_timing(1)
+    d, e, tau = plan.evp_tridiagonalize(A)
+    eps, Z = plan.evp_tridiag_solve(d, e)
+    Ct = plan.evp_backtransform(A, Z)
+    plan.last_info()
+    kern = {k: {"launches": n, "ms": round(ms, 3)} for k, (n, ms) in plan.launch_times().items() if k.startswith("evp.")}
+    plan.set_timing(0)
+    out = {
+        "method": "one-stage Householder tridiagonalisation (ELPA1 route, PAPER.md:120) / divide and conquer / compact-WY back-transformation",
+        "tridiag": {"ms": round(t_tri, 3), "bound": "hbm", "algorithmic_bytes": tri_bytes,
+                    "achieved_gbs": tri_bytes / (t_tri * 1e-3) / 1e9,
+                    "frac_of_hbm": (tri_bytes / (t_tri * 1e-3) / 1e9 / hbm_gbs) if hbm_gbs else None, "hbm_gbs_peak": hbm_gbs,
+                    "her2k_tflops": (her2k_flop / (kern["evp.tridiag.her2k"]["ms"] * 1e-3) / 1e12) if "evp.tridiag.her2k" in kern else None},
+        "solve": {"ms": round(t_solve, 3), "bound": "tensor (block products) + latency (secular equation, deflation)",
+                  "gemm_ms": kern.get("evp.solve.gemm", {}).get("ms")},
+        "back": {"ms": round(t_back, 3), "bound": "tensor", "nominal_flop": back_flop,
+                 "tflops": back_flop / (t_back * 1e-3) / 1e12, "frac_of_fp64_peak": back_flop / (t_back * 1e-3) / 1e12 / fp64_peak},
+        "total_ms": round(t_tri + t_solve + t_back, 3), "kernels": kern,
+    }
+    # the whole generalized solve, one chain on one stream
+    evc = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    U.copy_(S0)
+    evc[0].record()
+    plan.cholesky(U)
+    plan.invert_triangular(U, V)
+    plan.to_standard(H, V, Ht)
+    eps, Ct = plan.standard_eigh(Ht)
+    plan.backtransform(V, Ct, C)
+    evc[1].record()
+    plan.last_info()
+    out["generalized_solve_ms"] = round(evc[0].elapsed_time(evc[1]), 3)
+    out["checks"] = {"eig_residual": M.eig_residual(H, S0, C, eps), "s_orthonormality": M.s_orthonormality(S0, C),
+                     "tolerances": {"eig_residual": M.TOL_RESIDUAL, "s_orthonormality": M.TOL_SORTH}}
+    out["checks"]["ok"] = bool(out["checks"]["eig_residual"] <= M.TOL_RESIDUAL and out["checks"]["s_orthonormality"] <= M.TOL_SORTH)
+    out["paper_context"] = ("PAPER.md:133 Table 1 (ELPA 2024.05, NCCL, 4x A100-40GB, N=40960, nev=N): Tridiag. 49.5 s, Solve 40.1 s, "
+                            "Back 14.6 s; whole generalized solve 134 s (context only)")
+    del A, Z, Ct
+    return out
 
 
 def run_batch(args):
