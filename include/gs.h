@@ -218,6 +218,31 @@ gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double*
 gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream);
 gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------------
+ * (5) Ill-conditioned overlap matrix.  "In the latter case (high condition number of S),
+ * electronic structure calculations can then be carried out by transforming the eigenproblem (2) to the basis of
+ * eigenvectors D_i of the overlap matrix, but omitting any D_i for which sigma_i is smaller than a small positive
+ * number delta (typically delta <= 1e-5)".  The route that replaces steps 1-3 when S is close to
+ * singular (steps 1-3 need "S must not be numerically singular"):
+ *
+ *   gs_truncated_to_standard   S = D Sigma D^H by the eigensolver above (all N pairs);  X = D Sigma^-1/2 on the kept
+ *                              directions (sigma_i >= delta), ZERO columns for the dropped ones (the lowest sigma:
+ *                              the first columns);  Hr = X^H H X.  S_inout (upper triangle = S) is destroyed.
+ *                              X, Hr: N x N outputs (Hr: upper triangle written; rows / columns of dropped directions
+ *                              are zero except for a diagonal entry above the spectrum of Hr, so they never enter the
+ *                              lowest eigenvalues).  sigma: N eigenvalues of S, ascending.  H: both triangles filled.
+ *   gs_truncated_rank          synchronises; number of kept directions (must be >= nev for the lowest nev to be meaningful).
+ *   then  gs_standard_eigh(plan, Hr, eps, Ctilde)  and
+ *   gs_backtransform_dense     C = X Ctilde (X dense N x N, Ctilde N x nev).  C^H S C = I, X^H (H C - S C eps) = 0.
+ *
+ * EVP workspace: gs_truncated_workspace_bytes (larger than gs_evp_workspace_bytes when nev < N: all N eigenvectors
+ * of S are formed), registered with gs_evp_set_workspace. */
+gs_status_t gs_truncated_workspace_bytes(const gs_plan_t* plan, size_t* bytes);
+gs_status_t gs_truncated_to_standard(gs_plan_t* plan, const void* H, void* S_inout, double delta, void* X, void* Hr, double* sigma,
+                                     void* cuda_stream);
+gs_status_t gs_truncated_rank(gs_plan_t* plan, void* cuda_stream, int64_t* kept);
+gs_status_t gs_backtransform_dense(gs_plan_t* plan, const void* X, const void* Ctilde, void* C, void* cuda_stream);
+
 /* Synchronises `cuda_stream`, then reports the plan's numerical status: GS_OK with *info = 0, or
  * GS_ERR_NOT_POSDEF / GS_ERR_SINGULAR with *info = 1-based index of the first bad pivot
  * (LAPACK-style).  GS_ERR_CUDA if the stream reports an asynchronous error. */

@@ -47,6 +47,9 @@ def _load():
             getattr(lib, f"orc_jacobi_{t}").restype = i64
             getattr(lib, f"orc_density_{t}").argtypes = [i64, i64, p, p, p]
             getattr(lib, f"orc_density_{t}").restype = None
+            for nm in ("hn", "nn"):
+                getattr(lib, f"orc_matmul_{nm}_{t}").argtypes = [i64, i64, i64, p, p, p]
+                getattr(lib, f"orc_matmul_{nm}_{t}").restype = None
             getattr(lib, f"orc_inertia_{t}").argtypes = [i64, p, ctypes.c_double]
             getattr(lib, f"orc_inertia_{t}").restype = i64
         lib.orc_sturm_count.argtypes = [i64, p, p, ctypes.c_double]
@@ -189,6 +192,54 @@ def inertia_count(A, sigma: float) -> int:
     if r < 0:
         raise ZeroDivisionError("zero pivot in LDL^H: choose another sigma")
     return r
+
+
+def _common(A, B):
+    A, B = np.asarray(A), np.asarray(B)
+    dt = np.complex128 if (np.iscomplexobj(A) or np.iscomplexobj(B)) else np.float64
+    return _f(A, dt), _f(B, dt)
+
+
+def matmul_hn(A, B) -> np.ndarray:
+    """O11: C = A^H B by the plain triple loop (A: K x M, B: K x N)."""
+    A, B = _common(A, B)
+    K, Mm = A.shape
+    K2, Nn = B.shape
+    assert K == K2
+    C = np.zeros((Mm, Nn), dtype=A.dtype, order="F")
+    if Mm and Nn:
+        getattr(_load(), f"orc_matmul_hn_{_sfx(A)}")(Mm, Nn, K, _ptr(A), _ptr(B), _ptr(C))
+    return C
+
+
+def matmul_nn(A, B) -> np.ndarray:
+    """O11: C = A B by the plain triple loop (A: M x K, B: K x N)."""
+    A, B = _common(A, B)
+    Mm, K = A.shape
+    K2, Nn = B.shape
+    assert K == K2
+    C = np.zeros((Mm, Nn), dtype=A.dtype, order="F")
+    if Mm and Nn:
+        getattr(_load(), f"orc_matmul_nn_{_sfx(A)}")(Mm, Nn, K, _ptr(A), _ptr(B), _ptr(C))
+    return C
+
+
+def truncated_eigh(H, S, delta: float, nev=None):
+    """The route for an ill-conditioned S, step by step: eigenvectors D_i of the overlap matrix
+    (Jacobi), omit every D_i with sigma_i < delta, transform the eigenproblem to that basis (scaled so that it is
+    orthonormal in the S inner product: X = D_kept Sigma_kept^-1/2), solve the standard problem there (Jacobi),
+    transform back.  Returns dict(sigma (all, ascending), kept, X (N x kept), Hr, eps, y, C)."""
+    H, S = _f(H), _f(S)
+    sigma, D, _ = jacobi(S)
+    keep = sigma >= delta
+    m = int(keep.sum())
+    X = np.asfortranarray(D[:, keep] / np.sqrt(sigma[keep])[None, :])
+    Hr = matmul_hn(X, matmul_nn(H, X))
+    Hr = 0.5 * (Hr + Hr.conj().T)
+    eps, y, _ = jacobi(Hr)
+    nev = m if nev is None else min(int(nev), m)
+    y = np.asfortranarray(y[:, :nev])
+    return {"sigma": sigma, "kept": m, "X": X, "Hr": Hr, "eps": eps[:nev], "y": y, "C": matmul_nn(X, y)}
 
 
 def hermitian_from_upper(Ht_upper) -> np.ndarray:

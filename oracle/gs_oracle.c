@@ -41,6 +41,11 @@
  * by LDL^H without pivoting) proves that a set of computed eigenvalues is the LOWEST nev with none missing.
  * Pins (tests/test_oracle_tridiag.py): closed-form spectrum of tridiag(-1,2,-1), diagonal and 2 x 2 cases,
  * Jacobi on the same matrix, inertia against brute-force eigenvalue counts and a hand-computed LDL^T.
+ * (5) truncated-basis route for an ill-conditioned S: O11 plain triple-loop products C = A^H B and
+ * C = A B; the route itself is assembled from O5 (Jacobi on S and on H_r) and O11 in oracle/__init__.py,
+ * step by step in the paper's order.  Pins (tests/test_oracle_truncated.py): commuting pencil with planted
+ * near-null directions (closed form eps_i = h_i / sigma_i on the kept directions), delta = 0 reproduces the
+ * Cholesky route's eigenvalues, numpy products.
  * No function here is "parity unpinned".
  */
 #include <complex.h>
@@ -510,4 +515,54 @@ int64_t orc_inertia_z(int64_t N, zdouble *A, double sigma)
         }
     }
     return neg;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O11. Plain triple-loop products (column-major, leading dimensions = row counts):             */
+/*   orc_matmul_hn:  C (M x N) = A^H B,  A is K x M, B is K x N                                 */
+/*   orc_matmul_nn:  C (M x N) = A B,    A is M x K, B is K x N                                 */
+/* Used by the truncated-basis route of PAPER.md:73 (H_r = X^H H X, C = X y).                   */
+/* ------------------------------------------------------------------------------------------ */
+void orc_matmul_hn_d(int64_t M, int64_t N, int64_t K, const double *A, const double *B, double *C)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < M; ++i) {
+            double s = 0.0;
+            for (int64_t k = 0; k < K; ++k) s += A[k + i * K] * B[k + j * K];
+            C[i + j * M] = s;
+        }
+}
+
+void orc_matmul_hn_z(int64_t M, int64_t N, int64_t K, const zdouble *A, const zdouble *B, zdouble *C)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < M; ++i) {
+            zdouble s = 0.0;
+            for (int64_t k = 0; k < K; ++k) s += conj(A[k + i * K]) * B[k + j * K];
+            C[i + j * M] = s;
+        }
+}
+
+void orc_matmul_nn_d(int64_t M, int64_t N, int64_t K, const double *A, const double *B, double *C)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < M; ++i) {
+            double s = 0.0;
+            for (int64_t k = 0; k < K; ++k) s += A[i + k * M] * B[k + j * K];
+            C[i + j * M] = s;
+        }
+}
+
+void orc_matmul_nn_z(int64_t M, int64_t N, int64_t K, const zdouble *A, const zdouble *B, zdouble *C)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t i = 0; i < M; ++i) {
+            zdouble s = 0.0;
+            for (int64_t k = 0; k < K; ++k) s += A[i + k * M] * B[k + j * K];
+            C[i + j * M] = s;
+        }
 }

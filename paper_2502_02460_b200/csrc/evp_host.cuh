@@ -40,12 +40,15 @@ struct EvpBuffers {
     long long ldq;
 };
 
-EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes)
+// nev_cap: number of eigenvectors the carved buffers must hold (the plan's nev; N for the truncated-basis route,
+// which needs ALL eigenvectors of S).  Everything that depends on it lies behind the R blocks, so the triangular
+// factors a tridiagonalisation leaves are found again whatever nev_cap the next call carves with.
+EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes, int64_t nev_cap)
 {
     EvpLayout L;
     L.base = base;
     EvpBuffers b{};
-    const size_t N = size_t(p->N), es = p->es, nev = size_t(p->nev);
+    const size_t N = size_t(p->N), es = p->es, nev = size_t(nev_cap);
     const int nb = p->lb;
     const size_t th = p->z ? 64 : 128;
     const size_t nJ = (N + 127) / 128, nI = (N + th - 1) / th;
@@ -79,13 +82,14 @@ EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes)
     return b;
 }
 
-gs_status_t evp_ready(const gs_plan* plan, EvpBuffers* b)
+gs_status_t evp_ready(const gs_plan* plan, EvpBuffers* b, int64_t nev_cap = -1)
 {
     GS_TRY(check_ready(plan));
+    if (nev_cap < 0) nev_cap = plan->nev;
     size_t need = 0;
-    evp_carve(plan, nullptr, &need);
+    evp_carve(plan, nullptr, &need, nev_cap);
     if (plan->evp_ws == nullptr || plan->evp_ws_bytes < need) return GS_ERR_WORKSPACE;
-    *b = evp_carve(plan, plan->evp_ws, nullptr);
+    *b = evp_carve(plan, plan->evp_ws, nullptr, nev_cap);
     return GS_OK;
 }
 
@@ -229,9 +233,9 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
 
 // C~ = Q Z:  Q = H(N-1) ... H(1) applied panel by panel, lowest reflectors first:
 //   Y = Vp^H C~[0:m, :],  Y2 = T'p Y = (Rp^-1)^H Y,  C~[0:m, :] -= Vp Y2.
-gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const void* A, const double* Z, long long ldz, void* Ct, cudaStream_t stream)
+gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const void* A, const double* Z, long long ldz, void* Ct, int nev, cudaStream_t stream)
 {
-    const int N = int(plan->N), nev = int(plan->nev), nb = b.nb;
+    const int N = int(plan->N), nb = b.nb;
     if (nev == 0) return GS_OK;
     {
         LaunchTimer timer(plan, L_EVP_BACK, stream);
@@ -300,9 +304,9 @@ gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const voi
 // Divide and conquer on tridiag(e, d, e): lowest nev eigenvalues -> eps, their eigenvectors -> Z (N x nev, ld ldz).
 // d is modified (cut points).  Synchronises the stream once per level: the deflation counts decide the shapes of
 // the launches that follow.
-gs_status_t evp_solve_impl(gs_plan* plan, EvpBuffers& b, double* d, const double* e, double* eps, double* Z, long long ldz, cudaStream_t stream)
+gs_status_t evp_solve_impl(gs_plan* plan, EvpBuffers& b, double* d, const double* e, double* eps, double* Z, long long ldz, int nev, cudaStream_t stream)
 {
-    const int N = int(plan->N), nev = int(plan->nev);
+    const int N = int(plan->N);
     DcArrays a = b.dc;
     const int nleaf = (N + kDcLeaf - 1) / kDcLeaf;
     {
@@ -391,6 +395,15 @@ gs_status_t evp_solve_impl(gs_plan* plan, EvpBuffers& b, double* d, const double
     return GS_OK;
 }
 
+// tridiagonalise, solve, back-transform: the lowest nev pairs of the upper triangle of A (destroyed)
+gs_status_t evp_eigh_impl(gs_plan* plan, EvpBuffers& b, void* A, double* eps, void* Ct, int nev, cudaStream_t stream)
+{
+    GS_TRY(plan->z ? evp_tridiagonalize_t<double2>(plan, b, A, b.d, b.e, b.tau, stream)
+                   : evp_tridiagonalize_t<double>(plan, b, A, b.d, b.e, b.tau, stream));
+    GS_TRY(evp_solve_impl(plan, b, b.d, b.e, eps, b.Z, plan->N, nev, stream));
+    return evp_backtransform_impl(plan, b, A, b.Z, plan->N, Ct, nev, stream);
+}
+
 }  // namespace
 
 extern "C" {
@@ -398,7 +411,7 @@ extern "C" {
 gs_status_t gs_evp_workspace_bytes(const gs_plan_t* plan, size_t* bytes)
 {
     if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
-    evp_carve(plan, nullptr, bytes);
+    evp_carve(plan, nullptr, bytes, plan->nev);
     return GS_OK;
 }
 
@@ -406,7 +419,7 @@ gs_status_t gs_evp_set_workspace(gs_plan_t* plan, void* dev_workspace, size_t by
 {
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
     size_t need = 0;
-    evp_carve(plan, nullptr, &need);
+    evp_carve(plan, nullptr, &need, plan->nev);
     if (dev_workspace == nullptr || bytes < need || (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) != 0) return GS_ERR_WORKSPACE;
     plan->evp_ws = static_cast<unsigned char*>(dev_workspace);
     plan->evp_ws_bytes = bytes;
@@ -432,7 +445,7 @@ gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double*
     if (d == nullptr || e == nullptr || eps == nullptr || (plan->nev > 0 && Z == nullptr)) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     GS_CUDA(plan, cudaMemcpyAsync(b.dwork, d, sizeof(double) * size_t(plan->N), cudaMemcpyDeviceToDevice, stream));
-    return evp_solve_impl(plan, b, b.dwork, e, eps, Z, plan->N, stream);
+    return evp_solve_impl(plan, b, b.dwork, e, eps, Z, plan->N, int(plan->nev), stream);
 }
 
 gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream)
@@ -444,7 +457,7 @@ gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, cons
     if (A_reflectors == nullptr || Z == nullptr || Ctilde == nullptr || !aligned16(A_reflectors) || !aligned16(Ctilde) ||
         overlaps(Ctilde, vec_bytes(plan), A_reflectors, mat_bytes(plan)))
         return GS_ERR_INVALID_ARG;
-    return evp_backtransform_impl(plan, b, A_reflectors, Z, plan->N, Ctilde, static_cast<cudaStream_t>(cuda_stream));
+    return evp_backtransform_impl(plan, b, A_reflectors, Z, plan->N, Ctilde, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
 }
 
 gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream)
@@ -455,11 +468,110 @@ gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, v
     if (Htilde_inout == nullptr || eps == nullptr || (plan->nev > 0 && Ctilde == nullptr) || !aligned16(Htilde_inout) ||
         (Ctilde != nullptr && (!aligned16(Ctilde) || overlaps(Ctilde, vec_bytes(plan), Htilde_inout, mat_bytes(plan)))))
         return GS_ERR_INVALID_ARG;
+    return evp_eigh_impl(plan, b, Htilde_inout, eps, Ctilde, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ------------------------------------------------------------------------------------------------------
+// (5) Ill-conditioned overlap: "electronic structure calculations can then be carried out by
+// transforming the eigenproblem (2) to the basis of eigenvectors D_i of the overlap matrix, but omitting any D_i
+// for which sigma_i is smaller than a small positive number delta".
+//   S = D Sigma D^H (the eigensolver above, ALL N pairs);  X = D_kept Sigma_kept^-1/2  (X^H S X = I on the kept
+//   directions; the dropped ones -- the lowest sigma, i.e. the first columns -- become zero columns);
+//   H_r = X^H H X (two products on the tile engine; zero rows / columns for the dropped directions, whose diagonal
+//   entries are set to a shift above the spectrum of H_r so that they can never be among the lowest nev);
+//   then H_r y = eps y by gs_standard_eigh and C = X y by gs_backtransform_dense.
+// ------------------------------------------------------------------------------------------------------
+gs_status_t gs_truncated_workspace_bytes(const gs_plan_t* plan, size_t* bytes)
+{
+    if (plan == nullptr || bytes == nullptr) return GS_ERR_INVALID_ARG;
+    evp_carve(plan, nullptr, bytes, plan->N);
+    return GS_OK;
+}
+
+gs_status_t gs_truncated_to_standard(gs_plan_t* plan, const void* H, void* S_inout, double delta, void* X, void* Hr, double* sigma,
+                                     void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b, plan->N));
+    if (H == nullptr || S_inout == nullptr || X == nullptr || Hr == nullptr || sigma == nullptr || !(delta >= 0.0) || !aligned16(H) ||
+        !aligned16(S_inout) || !aligned16(X) || !aligned16(Hr) || overlaps(X, mat_bytes(plan), H, mat_bytes(plan)) ||
+        overlaps(X, mat_bytes(plan), S_inout, mat_bytes(plan)) || overlaps(Hr, mat_bytes(plan), H, mat_bytes(plan)) ||
+        overlaps(Hr, mat_bytes(plan), X, mat_bytes(plan)) || overlaps(Hr, mat_bytes(plan), S_inout, mat_bytes(plan)))
+        return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    GS_TRY(plan->z ? evp_tridiagonalize_t<double2>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream)
-                   : evp_tridiagonalize_t<double>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream));
-    GS_TRY(evp_solve_impl(plan, b, b.d, b.e, eps, b.Z, plan->N, stream));
-    return evp_backtransform_impl(plan, b, Htilde_inout, b.Z, plan->N, Ctilde, stream);
+    const int N = int(plan->N);
+    GS_TRY(evp_eigh_impl(plan, b, S_inout, sigma, X, N, stream));          // X = D (all eigenvectors), sigma ascending
+    int* kept = info_ptr(plan) + 16;                                       // (a slot of the plan's 256-byte flag area)
+    {
+        LaunchTimer timer(plan, L_EVP_BACK, stream);
+        const dim3 grid((N + 255) / 256, std::min(N, 4096));
+        if (plan->z) truncate_scale_kernel<double2><<<grid, 256, 0, stream>>>(static_cast<double2*>(X), plan->N, N, sigma, delta, kept, info_ptr(plan));
+        else truncate_scale_kernel<double><<<grid, 256, 0, stream>>>(static_cast<double*>(X), plan->N, N, sigma, delta, kept, info_ptr(plan));
+        GS_LAUNCH_OK(plan);
+    }
+    Stage st = make_stage(plan, stream);
+    const MatView vH{H, N, N, N}, vX{X, N, N, N}, vW{big_ptr(plan), N, N, N};
+    const int kt = (N + st.bk - 1) / st.bk, nt = plan->nblk;
+    {   // W = H X  (as H^H X: H is Hermitian, and the k-contiguous operand is the fast one)
+        EngineParams p = blank_params(plan);
+        if (!set_operand(st, p, 0, vH, false) || !set_operand(st, p, 1, vX, false)) return GS_ERR_CUDA;
+        p.C = static_cast<double*>(big_ptr(plan)); p.ldc = N;
+        p.tiles_m = nt; p.tiles_n = nt; p.order = ORDER_COL;
+        p.c_rows = N; p.c_cols = N;
+        p.khi_c = kt; p.kmax = kt;
+        GS_TRY(launch(st, p, false, L_EVP_DC_GEMM));
+    }
+    {   // H_r = X^H W, upper triangle
+        EngineParams p = blank_params(plan);
+        if (!set_operand(st, p, 0, vX, false) || !set_operand(st, p, 1, vW, false)) return GS_ERR_CUDA;
+        p.C = static_cast<double*>(Hr); p.ldc = N;
+        p.tiles_m = nt; p.tiles_n = nt; p.order = ORDER_TRI_ROW_DESC;
+        p.c_rows = N; p.c_cols = N;
+        p.khi_c = kt; p.kmax = kt;
+        p.flags = F_STORE_UPPER | F_REAL_DIAG;
+        GS_TRY(launch(st, p, false, L_EVP_DC_GEMM));
+    }
+    {   // shift = 2 ||triu(H_r)||_F sqrt2 + 1 > lambda_max(H_r) on the diagonal of the dropped directions
+        LaunchTimer timer(plan, L_EVP_BACK, stream);
+        const int nb = std::min(64, (N + 255) / 256);
+        if (plan->z) shift_dropped_kernel<double2><<<nb, 256, 0, stream>>>(static_cast<double2*>(Hr), plan->N, N, sigma, delta, static_cast<double*>(b.Pd), b.tickets + 3, info_ptr(plan));
+        else shift_dropped_kernel<double><<<nb, 256, 0, stream>>>(static_cast<double*>(Hr), plan->N, N, sigma, delta, static_cast<double*>(b.Pd), b.tickets + 3, info_ptr(plan));
+        GS_LAUNCH_OK(plan);
+    }
+    return GS_OK;
+}
+
+gs_status_t gs_truncated_rank(gs_plan_t* plan, void* cuda_stream, int64_t* kept)
+{
+    if (plan == nullptr || kept == nullptr) return GS_ERR_INVALID_ARG;
+    GS_TRY(check_ready(plan));
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int h = 0;
+    GS_CUDA(plan, cudaMemcpyAsync(&h, info_ptr(plan) + 16, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    GS_CUDA(plan, cudaStreamSynchronize(stream));
+    *kept = h;
+    return GS_OK;
+}
+
+// C = X C~ with a DENSE X (N x N): the back-transformation of the truncated-basis route
+gs_status_t gs_backtransform_dense(gs_plan_t* plan, const void* X, const void* Ctilde, void* C, void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (plan->nev == 0) return GS_OK;
+    if (X == nullptr || Ctilde == nullptr || C == nullptr || !aligned16(X) || !aligned16(Ctilde) || !aligned16(C) ||
+        overlaps(C, vec_bytes(plan), Ctilde, vec_bytes(plan)) || overlaps(C, vec_bytes(plan), X, mat_bytes(plan)))
+        return GS_ERR_INVALID_ARG;
+    const int N = int(plan->N), nev = int(plan->nev);
+    Stage st = make_stage(plan, static_cast<cudaStream_t>(cuda_stream));
+    const MatView vX{X, N, N, N}, vC{Ctilde, N, nev, N};
+    EngineParams p = blank_params(plan);
+    if (!set_operand(st, p, 0, vX, true) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
+    p.C = static_cast<double*>(C); p.ldc = N;
+    p.tiles_m = plan->nblk; p.tiles_n = (nev + st.lb - 1) / st.lb; p.order = ORDER_ROW;
+    p.c_rows = N; p.c_cols = nev;
+    p.khi_c = (N + st.bk - 1) / st.bk; p.kmax = p.khi_c;
+    return launch(st, p, true, L_BACK_TRMM);
 }
 
 }  // extern "C"

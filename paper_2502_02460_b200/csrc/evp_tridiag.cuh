@@ -492,5 +492,59 @@ __global__ void widen_kernel(const double* __restrict__ Z, long long ldz, T* __r
     for (int c = blockIdx.y; c < cols; c += gridDim.y) C[r + (long long)c * ldc] = from_real(Z[r + (long long)c * ldz], T{});
 }
 
+// Truncated-basis route: column i of X (= eigenvector D_i of S) is scaled by sigma_i^-1/2 if
+// sigma_i >= delta and zeroed otherwise; *kept = number of kept directions.
+template <typename T>
+__global__ void truncate_scale_kernel(T* __restrict__ X, long long ld, int N, const double* __restrict__ sigma, double delta, int* kept, const int* info)
+{
+    if (*info != 0) return;
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+        int k = 0;
+        for (int c = 0; c < N; ++c) k += (sigma[c] >= delta && sigma[c] > 0.0) ? 1 : 0;
+        *kept = k;
+    }
+    if (r >= N) return;
+    for (int c = blockIdx.y; c < N; c += gridDim.y) {
+        const double s = sigma[c];
+        const double f = (s >= delta && s > 0.0) ? 1.0 / sqrt(s) : 0.0;
+        X[r + (long long)c * ld] = rscale(X[r + (long long)c * ld], f);
+    }
+}
+
+// H_r(i,i) = 2 sqrt2 ||triu(H_r)||_F + 1 for the dropped directions i (whose rows and columns of H_r are zero): a
+// value above the spectrum of H_r, so that these decoupled 1 x 1 blocks are never among the lowest eigenvalues.
+template <typename T>
+__global__ void __launch_bounds__(256) shift_dropped_kernel(T* __restrict__ Hr, long long ld, int N, const double* __restrict__ sigma, double delta,
+                                                            double* partial, unsigned int* ticket, const int* info)
+{
+    if (*info != 0) return;
+    __shared__ double s_n[8];
+    __shared__ unsigned int s_last;
+    double acc = 0.0;
+    for (long long c = blockIdx.x; c < N; c += gridDim.x)
+        for (int r = threadIdx.x; r <= c; r += 256) acc += abs2(Hr[r + c * ld]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) s_n[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += s_n[w];
+        partial[blockIdx.x] = s;
+        __threadfence();
+        s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double tot = 0.0;
+    for (int b = 0; b < int(gridDim.x); ++b) tot += __ldcg(&partial[b]);
+    const double shift = 2.0 * sqrt(2.0 * tot) + 1.0;
+    for (int c = threadIdx.x; c < N; c += 256)
+        if (!(sigma[c] >= delta && sigma[c] > 0.0)) Hr[c + (long long)c * ld] = from_real(shift, T{});
+    if (threadIdx.x == 0) *ticket = 0u;
+}
+
 }  // namespace evp
 }  // namespace gs

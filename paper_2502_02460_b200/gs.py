@@ -35,7 +35,7 @@ EXPORTS = (
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
     "gs_evp_workspace_bytes", "gs_evp_set_workspace", "gs_evp_tridiagonalize", "gs_evp_tridiag_solve", "gs_evp_backtransform",
-    "gs_standard_eigh",
+    "gs_standard_eigh", "gs_truncated_workspace_bytes", "gs_truncated_to_standard", "gs_truncated_rank", "gs_backtransform_dense",
 )
 
 
@@ -107,6 +107,10 @@ def lib() -> ctypes.CDLL:
         L.gs_evp_tridiag_solve.argtypes = [vp, vp, vp, vp, vp, vp]
         L.gs_evp_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_standard_eigh.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_truncated_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
+        L.gs_truncated_to_standard.argtypes = [vp, vp, vp, ctypes.c_double, vp, vp, vp, vp]
+        L.gs_truncated_rank.argtypes = [vp, vp, ctypes.POINTER(i64)]
+        L.gs_backtransform_dense.argtypes = [vp, vp, vp, vp, vp]
         L.gs_status_string.argtypes = [ctypes.c_int]
         L.gs_status_string.restype = ctypes.c_char_p
         L.gs_plan_last_cuda_error.argtypes = [vp]
@@ -262,10 +266,15 @@ class Plan:
         self._check(lib().gs_evp_workspace_bytes(self._h, ctypes.byref(n)))
         return int(n.value)
 
-    def ensure_evp_workspace(self, alloc=None):
-        """Allocates (once) and registers the eigensolver's scratch; `alloc(nbytes)` may supply the uint8 buffer."""
-        if getattr(self, "evp_workspace", None) is None:
-            n = self.evp_workspace_bytes()
+    def ensure_evp_workspace(self, alloc=None, truncated: bool = False):
+        """Allocates (once) and registers the eigensolver's scratch; `alloc(nbytes)` may supply the uint8 buffer.
+        truncated=True sizes it for the truncated-basis route (all N eigenvectors of S)."""
+        n = self.evp_workspace_bytes()
+        if truncated:
+            nt = ctypes.c_size_t(0)
+            self._check(lib().gs_truncated_workspace_bytes(self._h, ctypes.byref(nt)))
+            n = max(n, int(nt.value))
+        if getattr(self, "evp_workspace", None) is None or self.evp_workspace.numel() < n:
             self.evp_workspace = alloc(n) if alloc is not None else torch.empty(n, dtype=torch.uint8, device=self.device)
             self._check(lib().gs_evp_set_workspace(self._h, self.evp_workspace.data_ptr(), n))
 
@@ -315,6 +324,30 @@ class Plan:
                                            _dev_ptr(Ct, self.N, self.nev, self.tdtype) if self.nev > 0 else None,
                                            _stream_ptr(stream)))
         return eps, Ct
+
+    # ---- (5) ill-conditioned S: the truncated-basis route of PAPER.md:73 ----
+    def truncated_to_standard(self, H: torch.Tensor, S: torch.Tensor, delta: float, stream=None):
+        """S (upper triangle) is DESTROYED.  Returns (X, Hr, sigma): then standard_eigh(Hr) and backtransform_dense(X, C~)."""
+        from .workloads import colmajor_empty, colmajor_zeros
+        self.ensure_evp_workspace(truncated=True)
+        X = colmajor_empty(self.N, self.N, dtype=self.tdtype, device=self.device)
+        Hr = colmajor_zeros(self.N, self.N, dtype=self.tdtype, device=self.device)
+        sigma = self._vec(self.N)
+        self._check(lib().gs_truncated_to_standard(self._h, _dev_ptr(H, self.N, self.N, self.tdtype), _dev_ptr(S, self.N, self.N, self.tdtype),
+                                                   float(delta), X.data_ptr(), Hr.data_ptr(), sigma.data_ptr(), _stream_ptr(stream)))
+        return X, Hr, sigma
+
+    def truncated_rank(self, stream=None) -> int:
+        n = ctypes.c_int64(0)
+        self._check(lib().gs_truncated_rank(self._h, _stream_ptr(stream), ctypes.byref(n)))
+        return int(n.value)
+
+    def backtransform_dense(self, X: torch.Tensor, Ctilde: torch.Tensor, C: torch.Tensor, stream=None):
+        if self.nev == 0:
+            return
+        self._check(lib().gs_backtransform_dense(self._h, _dev_ptr(X, self.N, self.N, self.tdtype),
+                                                 _dev_ptr(Ctilde, self.N, self.nev, self.tdtype),
+                                                 _dev_ptr(C, self.N, self.nev, self.tdtype), _stream_ptr(stream)))
 
     def last_info(self, stream=None, raise_on_failure: bool = True) -> int:
         info = ctypes.c_int64(0)
