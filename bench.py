@@ -39,6 +39,9 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2 = headline)")
+    ap.add_argument("--n", type=int, default=0, help="context runs only: a real pencil of this order instead of a BASELINE config "
+                                                     "(e.g. 40960 = the size of the paper's Table 1, PAPER.md:136)")
+    ap.add_argument("--nev", type=int, default=0, help="with --n: number of eigenvectors (default n / 4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-sample", type=int, default=4096, help="order of the leading block the oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -264,6 +267,8 @@ def run_ours(args):
         return replicas.max_over_ranks(info, x, dev)
 
     cfg = wl.CONFIGS[args.config]
+    if args.n > 0:      # a context run at another size (same recipe, box scaled like configs 1-4): never the headline
+        cfg = wl.Config(9, args.n, args.nev if args.nev > 0 else args.n // 4, False, wl.scaled_box(args.n))
     N, nev = cfg.N, cfg.nev
     cplx = cfg.complex
     tdt = torch.complex128 if cplx else torch.float64
@@ -477,7 +482,8 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "c128 (FP64 arithmetic)" if cplx else "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
-                       "recipe": "BASELINE.json configs[%d]: Gaussian-overlap S, H = -S(1+0.1g)+diag" % cfg.index,
+                       "recipe": ("BASELINE.json configs[%d]: Gaussian-overlap S, H = -S(1+0.1g)+diag" % cfg.index) if args.n <= 0 else
+                                 "CONTEXT RUN, not a BASELINE config: the same recipe at N=%d (Table 1's size is 40960, PAPER.md:136)" % N,
                        "parallelism": "replicas x%d (one independent pencil per GPU)" % world,
                        "cache": "inputs_larger_than_L2 (each matrix %.1f GiB vs 126 MB L2)" % (N * N * (16 if cplx else 8) / 2 ** 30),
                        "timing": "CUDA events per step on the launching stream; S restored between steps outside the events"},

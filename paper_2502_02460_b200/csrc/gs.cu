@@ -15,6 +15,7 @@
 #include "../../include/gs.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>   // header-only NVTX v3: no-ops unless a profiler injects itself
 
 #include <cstdio>
 #include <cstdlib>
@@ -26,6 +27,7 @@
 
 #include "engine_host.cuh"
 #include "leaf_kernels.cuh"
+#include "leaf32_kernel.cuh"
 #include "cleaf_kernels.cuh"
 
 using namespace gs;
@@ -85,6 +87,7 @@ struct gs_plan {
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
     std::vector<void*> push[4];      // fused exchange: push targets per gs_push_kind_t (gs_plan_set_push_targets)
     int leaf_blocked = 0;            // real POTRF diagonal blocks: blocked sweep (potrf_leaf4_kernel) instead of the rank-1 sweep
+    int leaf_mode = 0;               // 0: rank-1 sweep (potrf_leaf_kernel, default: the fastest measured); 1: 4-row panels; 2: 32 x 32 sub-blocks by warp shuffles + in-CTA DMMA (leaf32_kernel.cuh)
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};
@@ -119,8 +122,17 @@ struct LaunchTimer {
     cudaStream_t stream;
     bool on;
     TimedLaunch t;
-    LaunchTimer(gs_plan* p, int label, cudaStream_t s) : plan(p), stream(s), on(false)
+    bool nvtx;
+    // GS_NVTX=1: every launch sits in an NVTX range named after its label ("to_standard.syr2k", ...), so that
+    // `ncu --nvtx --print-nvtx-rename kernel` lists launches by label (profiles/r02_perkernel.md)
+    static bool nvtx_on()
     {
+        static const bool v = std::getenv("GS_NVTX") != nullptr && std::atoi(std::getenv("GS_NVTX")) != 0;
+        return v;
+    }
+    LaunchTimer(gs_plan* p, int label, cudaStream_t s) : plan(p), stream(s), on(false), nvtx(nvtx_on())
+    {
+        if (nvtx) nvtxRangePushA(kLabelNames[label]);
         if (p->timing_mode == 1 || (p->timing_mode == 2 && label == L_TOSTD_SYR2K)) {
             t.label = label;
             t.side = (p->side != nullptr && s == p->side) ? 1 : 0;
@@ -132,6 +144,7 @@ struct LaunchTimer {
     }
     ~LaunchTimer()
     {
+        if (nvtx) nvtxRangePop();
         if (on) {
             cudaEventRecord(t.e1, stream);
             plan->timed.push_back(t);
@@ -355,8 +368,11 @@ struct Potrf {
         if (st.z)
             e = launch_pdl(potrf_cleaf_kernel, 1, kCLeafThreads, kCLeafSmemBytes, st.stream, static_cast<double2*>(S), plan->N, int(plan->N),
                            b * st.lb, static_cast<double2*>(w), vW.ld, info_ptr(plan));
+        else if (plan->leaf_mode == 2)
+            e = launch_pdl(potrf_leaf32_kernel, 1, kLeaf32Threads, kLeaf32SmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
+                           b * st.lb, static_cast<double*>(w), vW.ld, info_ptr(plan));
         else
-            e = launch_pdl(plan->leaf_blocked ? potrf_leaf4_kernel : potrf_leaf_kernel, 1, kLeafThreads, kLeafSmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
+            e = launch_pdl(plan->leaf_mode == 1 ? potrf_leaf4_kernel : potrf_leaf_kernel, 1, kLeafThreads, kLeafSmemBytes, st.stream, static_cast<double*>(S), plan->N, int(plan->N),
                            b * st.lb, static_cast<double*>(w), vW.ld, info_ptr(plan));
         if (e != cudaSuccess) return cuda_fail(plan, e);
         plan->launches += 1;
@@ -586,6 +602,7 @@ gs_status_t configure_leaf(gs_plan* plan)
     const cudaError_t e = once.run([]() -> cudaError_t {
         cudaError_t r = cudaFuncSetAttribute(potrf_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
         if (r == cudaSuccess) r = cudaFuncSetAttribute(potrf_leaf4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(potrf_leaf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeaf32SmemBytes);
         if (r == cudaSuccess) r = cudaFuncSetAttribute(trtri_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLeafSmemBytes);
         if (r == cudaSuccess) r = cudaFuncSetAttribute(potrf_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes);
         if (r == cudaSuccess) r = cudaFuncSetAttribute(trtri_cleaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCLeafSmemBytes);
@@ -640,6 +657,8 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
     knob("GS_LEAF_BLOCKED", 0, 1, &p->leaf_blocked);
+    if (p->leaf_blocked) p->leaf_mode = 1;
+    knob("GS_LEAF", 0, 2, &p->leaf_mode);
     int shard_log2 = p->z ? 4 : 3;   // 1024 rows per panel of the column-range inversion
     knob("GS_SHARD_PANEL_LOG2", 0, 8, &shard_log2);
     p->shard_panel = 1 << shard_log2;

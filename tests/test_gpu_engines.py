@@ -45,6 +45,7 @@ print("OK" if bad == 0 else "FAILED")
     {"GS_POTRF_NB": "2", "GS_POTRF_TAIL": "6", "GS_POTRF_NB_TAIL": "2", "GS_POTRF_END": "3", "GS_POTRF_NB_END": "1"},
     {"GS_POTRF_NB": "16", "GS_POTRF_TAIL": "0", "GS_POTRF_END": "0"},
     {"GS_LEAF_BLOCKED": "1"},
+    {"GS_LEAF": "2"},
 ])
 def test_engine_configuration(env):
     e = dict(os.environ)
