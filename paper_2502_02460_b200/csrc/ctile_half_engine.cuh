@@ -43,6 +43,9 @@ __global__ void __launch_bounds__(kCThreads, 3) ctile_half_engine_kernel(const _
     int b, I, J;
     if (!decode_tile(p, blockIdx.x >> 1, b, I, J)) return;
     const int qj = blockIdx.x & 1;   // which 32-column half of the logical 64 x 64 tile
+    if (p.c_row0 + (long long)b * p.c_brow + (long long)CT * I >= p.c_rows ||
+        p.c_col0 + (long long)b * p.c_bcol + (long long)CT * J + 32 * qj >= p.c_cols)
+        return;   // entirely outside the C bounds: nothing to store
     int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
     int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
     if (k_lo < 0) k_lo = 0;

@@ -63,6 +63,11 @@ __global__ void __launch_bounds__(k64Threads, 3) tile64_engine_kernel(const __gr
     int b, I, J;
     if (!decode_tile(p, blockIdx.x >> 2, b, I, J)) return;
     const int qi = blockIdx.x & 1, qj = (blockIdx.x >> 1) & 1;
+    // a tile that lies entirely outside the C bounds stores nothing: skip it (batched launches over a matrix whose
+    // block count is not a power of two -- the doubling levels of the triangular inversion -- have many of them)
+    if (p.c_row0 + (long long)b * p.c_brow + (long long)BM * I + T64 * qi >= p.c_rows ||
+        p.c_col0 + (long long)b * p.c_bcol + (long long)BN * J + T64 * qj >= p.c_cols)
+        return;
     int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
     int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
     if (k_lo < 0) k_lo = 0;

@@ -235,6 +235,8 @@ __global__ void __launch_bounds__(kThreads, 1) tile_engine_kernel(const __grid_c
 
     int b, I, J;
     if (!decode_tile(p, blockIdx.x, b, I, J)) return;
+    if (p.c_row0 + (long long)b * p.c_brow + (long long)BM * I >= p.c_rows || p.c_col0 + (long long)b * p.c_bcol + (long long)BN * J >= p.c_cols)
+        return;   // entirely outside the C bounds: nothing to store
     int k_lo = p.klo_c + p.klo_i * I + p.klo_j * J;
     int k_hi = p.khi_c + p.khi_i * I + p.khi_j * J;
     if (k_lo < 0) k_lo = 0;
