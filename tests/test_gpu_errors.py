@@ -229,3 +229,47 @@ def test_second_device_or_reconfiguration_after_set_device():
             R = torch.triu(U).t() @ torch.triu(U) - p.S.to(dev)
             assert (R.norm() / p.S.norm()).item() < 1e-13
             plan.close()
+
+
+def test_evp_and_truncated_argument_errors():
+    """NEXT-4 / (5) entry points: workspace and pointer errors come back as statuses, nothing is launched."""
+    gs = _gs()
+    L = gs.lib()
+    N, nev = 200, 64
+    plan = gs.Plan(N, nev)
+    h, st = plan._h, _stream()
+    A = wl.colmajor_zeros(N, N, device="cuda")
+    B = wl.colmajor_zeros(N, N, device="cuda")
+    X = wl.colmajor_zeros(N, nev, device="cuda")
+    v = torch.zeros(N, dtype=torch.float64, device="cuda")
+    a, b, x, vp = A.data_ptr(), B.data_ptr(), X.data_ptr(), v.data_ptr()
+    # no eigensolver workspace yet
+    assert L.gs_evp_tridiagonalize(h, a, vp, vp, vp, st) == WORKSPACE
+    assert L.gs_standard_eigh(h, a, vp, x, st) == WORKSPACE
+    assert L.gs_truncated_to_standard(h, a, b, 1e-5, a, b, vp, st) == WORKSPACE
+    n = ctypes.c_size_t(0)
+    assert L.gs_evp_workspace_bytes(h, ctypes.byref(n)) == OK and n.value > 3 * N * N * 8
+    nt = ctypes.c_size_t(0)
+    assert L.gs_truncated_workspace_bytes(h, ctypes.byref(nt)) == OK and nt.value > n.value      # all N eigenvectors of S
+    ws = torch.empty(nt.value + 512, dtype=torch.uint8, device="cuda")
+    assert L.gs_evp_set_workspace(h, None, n.value) == WORKSPACE
+    assert L.gs_evp_set_workspace(h, ws.data_ptr(), n.value - 1) == WORKSPACE
+    assert L.gs_evp_set_workspace(h, ws.data_ptr() + 16, n.value) == WORKSPACE
+    assert L.gs_evp_set_workspace(h, ws.data_ptr(), n.value) == OK
+    assert L.gs_truncated_to_standard(h, a, b, 1e-5, x, b, vp, st) == WORKSPACE                # sized for nev only: too small
+    assert L.gs_evp_set_workspace(h, ws.data_ptr(), nt.value) == OK
+    # pointers
+    assert L.gs_evp_tridiagonalize(h, None, vp, vp, vp, st) == INVALID
+    assert L.gs_evp_tridiagonalize(h, a + 8, vp, vp, vp, st) == INVALID
+    assert L.gs_evp_tridiagonalize(h, a, None, vp, vp, st) == INVALID
+    assert L.gs_evp_tridiag_solve(h, vp, vp, None, x, st) == INVALID
+    assert L.gs_evp_backtransform(h, a, vp, a + 64, st) == INVALID                              # C~ inside the reflector matrix
+    assert L.gs_standard_eigh(h, a, vp, a + 16, st) == INVALID
+    assert L.gs_standard_eigh(h, a, None, x, st) == INVALID
+    assert L.gs_truncated_to_standard(h, a, b, -1.0, A.data_ptr(), b, vp, st) == INVALID        # delta < 0, X aliases H
+    assert L.gs_truncated_to_standard(h, a, b, float("nan"), x, b, vp, st) == INVALID
+    assert L.gs_backtransform_dense(h, a, x, x, st) == INVALID
+    assert L.gs_truncated_rank(h, st, None) == INVALID
+    torch.cuda.synchronize()
+    assert plan.last_info() == 0 and plan.launch_count() == 0
+    plan.close()

@@ -235,3 +235,40 @@ def test_config4_n32768_leading_block_and_invariants():
     torch.cuda.empty_cache()
     _invariants(p, U, V, Ht)
     plan.close()
+
+
+@pytest.mark.slow
+def test_n65664_cholesky_beyond_the_65535_grid_limit():
+    """N = 65664 (513 blocks, not a power of two, > 65535): the helper kernels put the column index on grid.x
+    (gridDim.y stops at 65535) and the engines skip tiles beyond the matrix.  S is a Toeplitz SPD matrix
+    generated in place (no second N x N buffer: 34.5 GB each); checked by the leading-block oracle pin, the zeroing
+    contract on sampled columns and sampled entries of U^T U = S computed one by one."""
+    from paper_2502_02460_b200 import gs
+    N = 65664
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90 * 2 ** 30:
+        pytest.skip("needs ~75 GiB of free device memory")
+    idx = torch.arange(N, dtype=torch.float64, device="cuda")
+    U = wl.colmajor_empty(N, N, device="cuda")
+    for c0 in range(0, N, 4096):
+        c1 = min(N, c0 + 4096)
+        blk = torch.exp(-(idx[:, None] - idx[None, c0:c1]).abs() / 8.0)      # S_ij = exp(-|i - j| / 8): SPD (AR(1) covariance)
+        blk[c0:c1, :].diagonal().add_(1e-3)
+        U[:, c0:c1] = blk
+    def s_entry(i, j):
+        return float(np.exp(-abs(i - j) / 8.0) + (1e-3 if i == j else 0.0))
+    plan = gs.Plan(N, 0)
+    plan.cholesky(U)
+    assert plan.last_info() == 0
+    k = 1024
+    S_k = np.array([[s_entry(i, j) for j in range(k)] for i in range(k)])
+    assert M.rel_frob_upper(U[:k, :k].cpu(), oracle.cholesky(S_k)) <= M.TOL_FROB
+    rng = np.random.default_rng(4)
+    for _ in range(48):
+        j = int(rng.integers(N // 2, N))
+        i = int(rng.integers(max(0, j - 40), j + 1))
+        col_j = U[:j + 1, j]
+        assert torch.count_nonzero(U[j + 1:, j]).item() == 0                 # zeroing contract below the diagonal
+        got = torch.dot(U[:i + 1, i], col_j[:i + 1]).item()
+        assert abs(got - s_entry(i, j)) <= 1e-12
+    plan.close()
