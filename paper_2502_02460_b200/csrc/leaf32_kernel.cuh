@@ -50,10 +50,9 @@ __device__ __forceinline__ double leaf32_rcp(double d)
 }
 
 // ---- P1: 32 x 32 diagonal sub-block at (b0, b0): A = L D L^T, then U = D^1/2 L^T.  One warp, lane = row. ----
-// The row stays in registers.  Per pivot J: lane J publishes its row in a double-buffered shared row (one __syncwarp);
-// by symmetry the multiplier of row i is the pivot row's own element i, so every lane reads rowbuf[lane]; the NEXT
-// pivot (the lane's running diagonal, one FMA behind) is broadcast with __shfl_sync and its reciprocal started at once,
-// so that the reciprocal's latency overlaps the row update instead of heading the next step.
+// The row stays in registers, the whole (symmetric) Schur complement is kept.  Per pivot J: lane J publishes its row in
+// a double-buffered shared row (one __syncwarp) for the row updates; the NEXT pivot (the lane's running diagonal, one
+// FMA behind the reciprocal) is broadcast with __shfl_sync and its reciprocal started at once.
 // Template on the 8-column register group, run-time loop over the pivot inside it: the fully unrolled 32 x 31 / 2 nest is
 // ~3500 instructions that every launch would have to fetch once -- slower than the arithmetic it saves.
 __device__ __forceinline__ void sts64(uint32_t addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
@@ -64,7 +63,7 @@ __device__ __forceinline__ double lds64(uint32_t addr)
     return v;
 }
 
-#ifdef LEAF32_PROF
+#ifdef LEAF32_PROF_FINE
 __device__ long long g_leaf32_fine[8];
 __device__ __forceinline__ long long leaf32_clk_after(double v)
 {
@@ -85,20 +84,17 @@ __device__ __forceinline__ void leaf32_potrf_group(double (&a)[32], uint32_t row
 #pragma unroll 1
     for (int jo = 0; jo < 8; ++jo) {
         const int J = 8 * G + jo;
-#ifdef LEAF32_PROF
+#ifdef LEAF32_PROF_FINE
         long long tprev = clock64();
 #endif
-        const uint32_t rb = rowbuf + (J & 1) * 256;
-        if (lane == J) {
+        // The multiplier of row `lane` is A(lane, J) / d -- the lane's OWN register of column J (the Schur complement is
+        // kept symmetric in registers), so the scalar chain  inv -> diagonal -> next pivot -> reciprocal  never waits for
+        // the published pivot row; that row (lane J's registers through shared memory) only feeds the row update.
+        double aj = a[8 * G];
 #pragma unroll
-            for (int c = 8 * G; c < 32; ++c) sts64(rb + 8 * c, a[c]);
-        }
-        __syncwarp();
-        LEAF32_FINE(0, d);
+        for (int u = 1; u < 8; ++u) aj = (jo == u) ? a[8 * G + u] : aj;
         if (!(d > 0.0)) { if (bad < 0) bad = J; }              // uniform: every lane holds the same d
         if (lane == J) dr = d;
-        const double aj = lds64(rb + 8 * lane);                  // A(J, lane) = A(lane, J)
-        LEAF32_FINE(1, aj);
         const double l = (lane > J) ? aj * inv : 0.0;            // multiplier; 0: row not updated
         const double t2 = (lane > J) ? aj * aj : 0.0;
         dii = fma(-t2, inv, dii);                                // this row's diagonal after the step: ONE op behind inv
@@ -107,6 +103,13 @@ __device__ __forceinline__ void leaf32_potrf_group(double (&a)[32], uint32_t row
         LEAF32_FINE(3, dn);
         const double invn = leaf32_rcp(dn);
         LEAF32_FINE(4, invn);
+        const uint32_t rb = rowbuf + (J & 1) * 256;
+        if (lane == J) {
+#pragma unroll
+            for (int c = 8 * G; c < 32; ++c) sts64(rb + 8 * c, a[c]);
+        }
+        __syncwarp();
+        LEAF32_FINE(0, d);
 #pragma unroll
         for (int c = 8 * G; c < 32; c += 2) {
             const double2 p = lds128(rb + 8 * c);
