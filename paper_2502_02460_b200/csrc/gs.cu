@@ -87,7 +87,7 @@ struct gs_plan {
     int tile64_mode = 2, tile64_below = 74;   // 64 x 64-tile engine for launches below this many logical tiles
     std::vector<void*> push[4];      // fused exchange: push targets per gs_push_kind_t (gs_plan_set_push_targets)
     int leaf_blocked = 0;            // real POTRF diagonal blocks: blocked sweep (potrf_leaf4_kernel) instead of the rank-1 sweep
-    int leaf_mode = 0;               // 0: rank-1 sweep (potrf_leaf_kernel, default: the fastest measured); 1: 4-row panels; 2: 32 x 32 sub-blocks by warp shuffles + in-CTA DMMA (leaf32_kernel.cuh)
+    int leaf_mode = 2;               // 2: 32 x 32 sub-blocks, warp-level sweeps + in-CTA DMMA (leaf32_kernel.cuh, default); 1: 4-row panels; 0: rank-1 sweep over 256 threads
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     char cuda_error[256] = {0};

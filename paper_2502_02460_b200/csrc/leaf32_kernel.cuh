@@ -34,8 +34,13 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// The sweeps below are written as template recursions over the step index: with `#pragma unroll` alone nvcc gives up on
-// the 32 x 31 / 2 triangular nests and keeps the row in local memory behind a dynamically indexed loop.
+// (the pivot rows are addressed through their 32-bit shared-memory address: explicit ld / st.shared)
+__device__ __forceinline__ double lds64(uint32_t addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+    return v;
+}
 
 // 1 / d to ~1 ulp without the IEEE-rounding division sequence: the hardware seed (MUFU.RCP64H, ~20 bits) and two
 // Newton steps.  The reciprocal of the pivot sits on the dependent chain of every elimination step.
@@ -45,112 +50,72 @@ __device__ __forceinline__ double leaf32_rcp(double d)
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
     const double e = fma(-d, x, 1.0);      // 1 - d x0
     const double x1 = fma(x, e, x);        // x0 (1 + e)
-    const double e2 = e * e;               // 1 - d x1 = e^2 exactly: formed beside x1, not behind it (FP64 ops are ~40 cycles deep)
+    const double e2 = e * e;               // 1 - d x1 = e^2 exactly: formed beside x1, not behind it
     return fma(x1, e2, x1);
 }
 
-// ---- P1: 32 x 32 diagonal sub-block at (b0, b0): A = L D L^T, then U = D^1/2 L^T.  One warp, lane = row. ----
-// The row stays in registers, the whole (symmetric) Schur complement is kept.  Per pivot J: lane J publishes its row in
-// a double-buffered shared row (one __syncwarp) for the row updates; the NEXT pivot (the lane's running diagonal, one
-// FMA behind the reciprocal) is broadcast with __shfl_sync and its reciprocal started at once.
-// Template on the 8-column register group, run-time loop over the pivot inside it: the fully unrolled 32 x 31 / 2 nest is
-// ~3500 instructions that every launch would have to fetch once -- slower than the arithmetic it saves.
-__device__ __forceinline__ void sts64(uint32_t addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
-__device__ __forceinline__ double lds64(uint32_t addr)
+// ---- P1: 32 x 32 diagonal sub-block at (b0, b0): A = L D L^T, then U = D^1/2 L^T.  FOUR warps, lane = row, warp w holds
+// columns 8 w .. 8 w + 7 of every row in registers (the whole symmetric Schur complement is kept).  Per pivot J: lane J
+// of every warp publishes its eight entries of the pivot row in a double-buffered shared row, one 128-thread named
+// barrier, then every lane reads its multiplier A(J, lane) = A(lane, J) and its warp's eight pivot-row entries back.
+// The running diagonal of every row is carried redundantly by the four warps, so the next pivot is one __shfl_sync and
+// its reciprocal starts one FMA behind the previous one.  (One warp doing the whole row update alone spends 280 of its
+// 530 cycles per pivot on the shared-memory round trip of 24 values and 75 on 32 FMAs: profiles/r02_leaf32.md.)
+// Returns the local index of the first pivot that is not > 0, or -1 (the same value in all four warps).
+__device__ __forceinline__ int leaf32_potrf_4warps(double* S, double* dinv, uint32_t rowbuf, int b0, int lane, int w)
 {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
-    return v;
-}
-
-#ifdef LEAF32_PROF_FINE
-__device__ long long g_leaf32_fine[8];
-__device__ __forceinline__ long long leaf32_clk_after(double v)
-{
-    long long c;
-    asm volatile("{ .reg .b64 t; mov.b64 t, %1; mov.u64 %0, %%clock64; }" : "=l"(c) : "d"(v) : "memory");
-    return c;
-}
-#define LEAF32_FINE(i, v) do { const long long c__ = leaf32_clk_after(v); if (lane == 0) { g_leaf32_fine[i] += c__ - tprev; } tprev = c__; } while (0)
-#else
-#define LEAF32_FINE(i, v) do { } while (0)
-#endif
-
-// (rowbuf is addressed through its 32-bit shared-memory address: with a generic pointer the compiler re-derives the
-// shared window from SR_CgaCtaId inside the pivot loop, an S2R per step on the critical path)
-template <int G>
-__device__ __forceinline__ void leaf32_potrf_group(double (&a)[32], uint32_t rowbuf, int lane, int& bad, double& dr, double& dii, double& d, double& inv)
-{
-#pragma unroll 1
-    for (int jo = 0; jo < 8; ++jo) {
-        const int J = 8 * G + jo;
-#ifdef LEAF32_PROF_FINE
-        long long tprev = clock64();
-#endif
-        // The multiplier of row `lane` is A(lane, J) / d -- the lane's OWN register of column J (the Schur complement is
-        // kept symmetric in registers), so the scalar chain  inv -> diagonal -> next pivot -> reciprocal  never waits for
-        // the published pivot row; that row (lane J's registers through shared memory) only feeds the row update.
-        double aj = a[8 * G];
+    double a[8];
 #pragma unroll
-        for (int u = 1; u < 8; ++u) aj = (jo == u) ? a[8 * G + u] : aj;
-        if (!(d > 0.0)) { if (bad < 0) bad = J; }              // uniform: every lane holds the same d
-        if (lane == J) dr = d;
-        const double l = (lane > J) ? aj * inv : 0.0;            // multiplier; 0: row not updated
-        const double t2 = (lane > J) ? aj * aj : 0.0;
-        dii = fma(-t2, inv, dii);                                // this row's diagonal after the step: ONE op behind inv
-        LEAF32_FINE(2, dii);
-        const double dn = __shfl_sync(0xffffffffu, dii, (J + 1) & 31);
-        LEAF32_FINE(3, dn);
-        const double invn = leaf32_rcp(dn);
-        LEAF32_FINE(4, invn);
-        const uint32_t rb = rowbuf + (J & 1) * 256;
-        if (lane == J) {
-#pragma unroll
-            for (int c = 8 * G; c < 32; ++c) sts64(rb + 8 * c, a[c]);
-        }
-        __syncwarp();
-        LEAF32_FINE(0, d);
-#pragma unroll
-        for (int c = 8 * G; c < 32; c += 2) {
-            const double2 p = lds128(rb + 8 * c);
-            a[c] = fma(-l, p.x, a[c]);          // (columns <= J of the group are dead: updating them too costs less
-            a[c + 1] = fma(-l, p.y, a[c + 1]);  //  than the selects that would spare them)
-        }
-        LEAF32_FINE(5, a[31]);
-        LEAF32_FINE(6, a[8 * G]);
-        d = dn;
-        inv = invn;
-    }
-    if constexpr (G + 1 < 4) leaf32_potrf_group<G + 1>(a, rowbuf, lane, bad, dr, dii, d, inv);
-}
-
-// Returns the local index of the first pivot that is not > 0, or -1.  rowbuf: 64 doubles of shared memory.
-__device__ __forceinline__ int leaf32_potrf_warp(double* S, double* dinv, double* rowbuf, int b0, int lane)
-{
-    double a[32];
-    // the full symmetric sub-block, row `lane`, from the upper triangle: a[c] = A(min, max)
-#pragma unroll
-    for (int c = 0; c < 32; ++c) {
+    for (int u = 0; u < 8; ++u) {
+        const int c = 8 * w + u;
         const int lo = c < lane ? c : lane, hi = c < lane ? lane : c;
-        a[c] = S[(b0 + lo) + (b0 + hi) * P32];
+        a[u] = S[(b0 + lo) + (b0 + hi) * P32];                   // A(min, max): the upper triangle holds the block
     }
     int bad = -1;
     double dr = 1.0;                                             // this lane's own pivot d(lane)
     double dii = S[(b0 + lane) + (b0 + lane) * P32];
     double d = __shfl_sync(0xffffffffu, dii, 0);
     double inv = leaf32_rcp(d);
-    leaf32_potrf_group<0>(a, smem_u32(rowbuf), lane, bad, dr, dii, d, inv);
+#pragma unroll 1
+    for (int J = 0; J < 32; ++J) {
+        const uint32_t rb = rowbuf + (J & 1) * 256;
+        if (lane == J) {
+#pragma unroll
+            for (int u = 0; u < 8; u += 2)
+                asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(rb + 8 * (8 * w + u)), "d"(a[u]), "d"(a[u + 1]) : "memory");
+        }
+        named_bar_sync(2, 128);
+        if (!(d > 0.0)) { if (bad < 0) bad = J; }              // uniform: every thread holds the same d
+        if (lane == J) dr = d;
+        const double aj = lds64(rb + 8 * lane);                  // A(J, lane) = A(lane, J)
+        const double l = (lane > J) ? aj * inv : 0.0;            // multiplier; 0: row not updated
+        dii = fma(-l, aj, dii);
+        const double dn = __shfl_sync(0xffffffffu, dii, (J + 1) & 31);
+        const double invn = leaf32_rcp(dn);
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) {
+            const double2 p = lds128(rb + 8 * (8 * w + u));
+            a[u] = fma(-l, p.x, a[u]);          // (columns <= J are dead: updating them too costs less than sparing them)
+            a[u + 1] = fma(-l, p.y, a[u + 1]);
+        }
+        d = dn;
+        inv = invn;
+    }
     if (bad >= 0) return bad;
     // row `lane` of D L^T -> row of U = D^1/2 L^T
     const double s = 1.0 / sqrt(dr);
 #pragma unroll
-    for (int c = 0; c < 32; ++c) {
-        if (c > lane) S[(b0 + lane) + (b0 + c) * P32] = a[c] * s;
+    for (int u = 0; u < 8; ++u) {
+        const int c = 8 * w + u;
+        if (c > lane) S[(b0 + lane) + (b0 + c) * P32] = a[u] * s;
         else if (c == lane) S[(b0 + lane) + (b0 + c) * P32] = dr * s;
     }
-    dinv[b0 + lane] = s;
+    if (w == 0) dinv[b0 + lane] = s;
     return -1;
 }
+
+// The two substitutions below are template recursions over the step index: with `#pragma unroll` alone nvcc gives up on
+// the 32 x 31 / 2 triangular nests and keeps the column in local memory behind a dynamically indexed loop.
 
 // ---- P2a: column cg of the panel right of the sub-block: x = U_bb^-T a (right-looking substitution), one thread ----
 template <int I>
@@ -196,6 +161,8 @@ __device__ __forceinline__ void leaf32_invert_warp(double* S, const double* dinv
 }
 
 // ---- P3: one 16 x 32 unit of the trailing update: S(r0:r0+16, c0:c0+32) -= P^T P, P = rows b0 .. b0+31 ----
+// All 48 operand fragments are loaded before the first DMMA: with one or two warps per sub-partition nothing else
+// hides the shared-memory latency, and a load -> DMMA -> load -> DMMA sequence costs ~275 cycles per k-step.
 __device__ __forceinline__ void leaf32_update_unit(double* S, int b0, int r0, int c0, int lane)
 {
     const int g = lane >> 2, q = lane & 3;
@@ -204,19 +171,21 @@ __device__ __forceinline__ void leaf32_update_unit(double* S, int b0, int r0, in
     for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
         for (int ni = 0; ni < 4; ++ni) { acc[mi][ni][0] = 0.0; acc[mi][ni][1] = 0.0; }
+    double af[8][2], bf[8][4];
 #pragma unroll
     for (int ks = 0; ks < 8; ++ks) {
         const int kr = b0 + 4 * ks + q;
-        double af[2], bf[4];
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi) af[mi] = S[kr + (r0 + 8 * mi + g) * P32];
+        for (int mi = 0; mi < 2; ++mi) af[ks][mi] = S[kr + (r0 + 8 * mi + g) * P32];
 #pragma unroll
-        for (int ni = 0; ni < 4; ++ni) bf[ni] = S[kr + (c0 + 8 * ni + g) * P32];
+        for (int ni = 0; ni < 4; ++ni) bf[ks][ni] = S[kr + (c0 + 8 * ni + g) * P32];
+    }
+#pragma unroll
+    for (int ks = 0; ks < 8; ++ks)
 #pragma unroll
         for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
-            for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[mi], bf[ni]);
-    }
+            for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[ks][mi], bf[ks][ni]);
 #pragma unroll
     for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
@@ -235,6 +204,8 @@ __device__ __forceinline__ double leaf32_w(const double* S, const double* dinv, 
 }
 
 // ---- inverse assembly, unit 16 x 32 of T = U12 W22 (s x s blocks at (o, o+s) and (o+s, o+s)); k runs to the unit's last column ----
+// k in chunks of 32 (8 k-steps), the fragments of a chunk loaded before its DMMAs (see leaf32_update_unit).  W22 is upper
+// triangular: the chunk k0 = n0 is the diagonal 32-block (diagonal from dinv, zeros below), the chunks before it are plain.
 __device__ __forceinline__ void leaf32_t_unit(const double* S, const double* dinv, double* T, int o, int s, int m0, int n0, int lane)
 {
     const int g = lane >> 2, q = lane & 3;
@@ -243,18 +214,25 @@ __device__ __forceinline__ void leaf32_t_unit(const double* S, const double* din
     for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
         for (int ni = 0; ni < 4; ++ni) { acc[mi][ni][0] = 0.0; acc[mi][ni][1] = 0.0; }
-    const int ksteps = (n0 + 32) / 4;                            // W22 is upper triangular: k <= n
-    for (int ks = 0; ks < ksteps; ++ks) {
-        const int k = 4 * ks + q;
-        double af[2], bf[4];
+#pragma unroll 1
+    for (int k0 = 0; k0 <= n0; k0 += 32) {
+        double af[8][2], bf[8][4];
+        const bool diag = k0 == n0;
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi) af[mi] = S[(o + m0 + 8 * mi + g) + (o + s + k) * P32];
+        for (int ks = 0; ks < 8; ++ks) {
+            const int k = k0 + 4 * ks + q;
 #pragma unroll
-        for (int ni = 0; ni < 4; ++ni) bf[ni] = leaf32_w(S, dinv, o + s + k, o + s + n0 + 8 * ni + g);
+            for (int mi = 0; mi < 2; ++mi) af[ks][mi] = S[(o + m0 + 8 * mi + g) + (o + s + k) * P32];
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi)
+            for (int ni = 0; ni < 4; ++ni)
+                bf[ks][ni] = diag ? leaf32_w(S, dinv, o + s + k, o + s + n0 + 8 * ni + g) : S[(o + s + n0 + 8 * ni + g) + (o + s + k) * P32];
+        }
 #pragma unroll
-            for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[mi], bf[ni]);
+        for (int ks = 0; ks < 8; ++ks)
+#pragma unroll
+            for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[ks][mi], bf[ks][ni]);
     }
 #pragma unroll
     for (int mi = 0; mi < 2; ++mi)
@@ -265,6 +243,7 @@ __device__ __forceinline__ void leaf32_t_unit(const double* S, const double* din
 }
 
 // ---- unit 16 x 32 of W12 = -W11 T, stored transposed: S(o + s + n, o + m) = W12(m, n); k runs from the unit's first row ----
+// W11 is upper triangular: k >= m.  Chunks of 32 from the 32-block that holds row m0 (masked loads) to s (plain loads).
 __device__ __forceinline__ void leaf32_x_unit(double* S, const double* dinv, const double* T, int o, int s, int m0, int n0, int lane)
 {
     const int g = lane >> 2, q = lane & 3;
@@ -273,17 +252,26 @@ __device__ __forceinline__ void leaf32_x_unit(double* S, const double* dinv, con
     for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
         for (int ni = 0; ni < 4; ++ni) { acc[mi][ni][0] = 0.0; acc[mi][ni][1] = 0.0; }
-    for (int ks = m0 / 4; ks < s / 4; ++ks) {                    // W11 is upper triangular: k >= m
-        const int k = 4 * ks + q;
-        double af[2], bf[4];
+    const int kfirst = m0 & ~31;
+#pragma unroll 1
+    for (int k0 = kfirst; k0 < s; k0 += 32) {
+        double af[8][2], bf[8][4];
+        const bool diag = k0 == kfirst;
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi) af[mi] = leaf32_w(S, dinv, o + m0 + 8 * mi + g, o + k);
+        for (int ks = 0; ks < 8; ++ks) {
+            const int k = k0 + 4 * ks + q;
 #pragma unroll
-        for (int ni = 0; ni < 4; ++ni) bf[ni] = T[k + (n0 + 8 * ni + g) * PT32];
+            for (int mi = 0; mi < 2; ++mi)
+                af[ks][mi] = diag ? leaf32_w(S, dinv, o + m0 + 8 * mi + g, o + k) : S[(o + k) + (o + m0 + 8 * mi + g) * P32];
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi)
+            for (int ni = 0; ni < 4; ++ni) bf[ks][ni] = T[k + (n0 + 8 * ni + g) * PT32];
+        }
 #pragma unroll
-            for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[mi], bf[ni]);
+        for (int ks = 0; ks < 8; ++ks)
+#pragma unroll
+            for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni) dmma_8x8x4(acc[mi][ni][0], acc[mi][ni][1], af[ks][mi], bf[ks][ni]);
     }
 #pragma unroll
     for (int mi = 0; mi < 2; ++mi)
@@ -292,6 +280,17 @@ __device__ __forceinline__ void leaf32_x_unit(double* S, const double* dinv, con
 #pragma unroll
             for (int e = 0; e < 2; ++e)
                 S[(o + s + n0 + 8 * ni + 2 * q + e) + (o + m0 + 8 * mi + g) * P32] = -acc[mi][ni][e];
+}
+
+// rows r0 .. r0+31 of U (all 128 columns: the upper part from the image, zeros below the diagonal) to global memory,
+// by 128 threads (tt = 0 .. 127): 32 consecutive rows of a column per warp instruction
+__device__ __forceinline__ void leaf32_store_u_rows(const double* S, double* blk, long long ld, int nb, int r0, int tt)
+{
+#pragma unroll 8
+    for (int idx = tt; idx < 32 * LB; idx += 128) {
+        const int r = r0 + (idx & 31), c = idx >> 5;
+        if (r < nb && c < nb) blk[r + (long long)c * ld] = (r <= c) ? S[r + c * P32] : 0.0;
+    }
 }
 
 #ifdef LEAF32_PROF
@@ -339,9 +338,11 @@ potrf_leaf32_kernel(double* __restrict__ Sg, long long ld, int N, int j0, double
 #pragma unroll 1
     for (int kb = 0; kb < 4; ++kb) {
         const int b0 = 32 * kb;
-        if (warp == 0) {
-            const int bad = leaf32_potrf_warp(S, dinv, rowbuf, b0, lane);
-            if (bad >= 0 && lane == 0) *s_fail = b0 + bad;
+        if (warp < 4) {
+            const int bad = leaf32_potrf_4warps(S, dinv, smem_u32(rowbuf), b0, lane, warp);
+            if (bad >= 0 && t == 0) *s_fail = b0 + bad;
+        } else if (kb > 0) {
+            leaf32_store_u_rows(S, blk, ld, nb, b0 - 32, t - 128);      // rows of the previous step are final: the idle warps store them
         }
         __syncthreads();
         LEAF32_STAMP(2 + 3 * kb);
@@ -368,16 +369,11 @@ potrf_leaf32_kernel(double* __restrict__ Sg, long long ld, int N, int j0, double
         LEAF32_STAMP(4 + 3 * kb);
     }
 
-    // ---- write U (upper triangle, zeros below) while the image still holds it untouched above the diagonal ----
-    for (int idx = t; idx < LB * LB; idx += kLeaf32Threads) {
-        const int r = idx & (LB - 1), c = idx >> 7;
-        if (r < nb && c < nb) blk[r + (long long)c * ld] = (r <= c) ? S[r + c * P32] : 0.0;
-    }
-
     LEAF32_STAMP(14);
     // ---- W = U^-1: the diagonal 32-blocks are inverted; two doubling levels, [A B; 0 D]^-1 = [A^-1, -A^-1 B D^-1; 0, D^-1] ----
     // level 1: pairs (0,1) and (2,3), s = 32: 2 units per pair; warps 0..3
     if (warp < 4) leaf32_t_unit(S, dinv, T + (warp >> 1) * 32 * PT32, (warp >> 1) * 64, 32, 16 * (warp & 1), 0, lane);
+    else leaf32_store_u_rows(S, blk, ld, nb, 96, t - 128);            // the last 32 rows of U, beside the level-1 products
     __syncthreads();
     if (warp < 4) leaf32_x_unit(S, dinv, T + (warp >> 1) * 32 * PT32, (warp >> 1) * 64, 32, 16 * (warp & 1), 0, lane);
     __syncthreads();
@@ -389,6 +385,7 @@ potrf_leaf32_kernel(double* __restrict__ Sg, long long ld, int N, int j0, double
     LEAF32_STAMP(15);
 
     // ---- write W (upper triangle from the transposed image, dinv on the diagonal, zeros below; identity-padded) ----
+#pragma unroll 8
     for (int idx = t; idx < LB * LB; idx += kLeaf32Threads) {
         const int r = idx & (LB - 1), c = idx >> 7;
         Winv[r + (long long)c * ldw] = leaf32_w(S, dinv, r, c);
