@@ -160,6 +160,21 @@ gs_status_t gs_backtransform_cols(gs_plan_t* plan, const void* Uinv, const void*
 typedef enum { GS_PUSH_UINV = 0, GS_PUSH_G = 1, GS_PUSH_HTILDE = 2, GS_PUSH_C = 3 } gs_push_kind_t;
 gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int count, void* const* targets);
 
+/* Device-side ordering of the fused exchange (instead of a host `stream synchronise + barrier` between producing a
+ * slab and consuming the peers' slabs): every rank owns a small array of 32-bit flags in device memory, mapped into
+ * its peers like the push targets.
+ *   gs_exchange_signal  enqueues on `cuda_stream`, BEHIND everything already enqueued there (so behind the kernels whose
+ *                       epilogues pushed the slabs; a memory barrier precedes the write), the write of `value` to each
+ *                       of the `count` flag addresses (local, or a peer's opened with gs_ipc_open);
+ *   gs_exchange_wait    enqueues a wait until every one of the `count` LOCAL flags is >= `value` (wrap-around aware
+ *                       comparison of the driver); later work of the stream starts only then.
+ * Both are stream memory operations of the driver (cuStreamWriteValue32 / cuStreamWaitValue32): no kernel spins, no SM
+ * is held, the host is not synchronised.  Flags are 4-byte aligned device addresses; use increasing epochs as values.
+ * A wait whose signal is never enqueued blocks its stream for good: every rank must signal, also after a numerical
+ * failure (the compute calls are no-ops then, the signals are not). */
+gs_status_t gs_exchange_signal(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream);
+gs_status_t gs_exchange_wait(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream);
+
 /* CUDA IPC plumbing for the targets (one process per GPU).  gs_ipc_export: the 64-byte handle of the
  * device allocation that contains dev_ptr and dev_ptr's byte offset inside it (send both to the
  * peer).  gs_ipc_open (in another process): maps that allocation, enabling peer access, and returns

@@ -1082,6 +1082,46 @@ gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int c
     return GS_OK;
 }
 
+// Device-side ordering of the fused exchange: stream memory operations (see include/gs.h).
+namespace {
+typedef CUresult (*StreamValue32Fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+StreamValue32Fn stream_value_fn(const char* name)
+{
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint(name, &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return nullptr;
+    return reinterpret_cast<StreamValue32Fn>(fn);
+}
+gs_status_t stream_values(gs_plan* plan, bool wait, int count, void* const* flags, uint32_t value, void* cuda_stream)
+{
+    if (plan == nullptr || count < 0 || count > 64 || (count > 0 && flags == nullptr)) return GS_ERR_INVALID_ARG;
+    for (int d = 0; d < count; ++d)
+        if (flags[d] == nullptr || (reinterpret_cast<uintptr_t>(flags[d]) & 3u) != 0) return GS_ERR_INVALID_ARG;
+    static StreamValue32Fn wr = stream_value_fn("cuStreamWriteValue32"), wt = stream_value_fn("cuStreamWaitValue32");
+    StreamValue32Fn fn = wait ? wt : wr;
+    if (fn == nullptr) return GS_ERR_CUDA;
+    for (int d = 0; d < count; ++d) {
+        const CUresult r = fn(static_cast<CUstream>(cuda_stream), reinterpret_cast<CUdeviceptr>(flags[d]), value,
+                              wait ? unsigned(CU_STREAM_WAIT_VALUE_GEQ) : unsigned(CU_STREAM_WRITE_VALUE_DEFAULT));
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(plan->cuda_error, sizeof(plan->cuda_error), "%s failed (CUresult %d)", wait ? "cuStreamWaitValue32" : "cuStreamWriteValue32", int(r));
+            return GS_ERR_CUDA;
+        }
+    }
+    return GS_OK;
+}
+}  // namespace
+
+gs_status_t gs_exchange_signal(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream)
+{
+    return stream_values(plan, false, count, flags, value, cuda_stream);
+}
+
+gs_status_t gs_exchange_wait(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream)
+{
+    return stream_values(plan, true, count, flags, value, cuda_stream);
+}
+
 // CUDA IPC plumbing for the push targets: a device allocation of another process (one process per GPU) mapped here.
 gs_status_t gs_ipc_export(const void* dev_ptr, unsigned char* handle64, uint64_t* offset)
 {

@@ -30,7 +30,7 @@ EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
     "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info", "gs_plan_clear_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
-    "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close",
+    "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close", "gs_exchange_signal", "gs_exchange_wait",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
@@ -89,6 +89,8 @@ def lib() -> ctypes.CDLL:
         L.gs_last_info.argtypes = [vp, vp, ctypes.POINTER(i64)]
         L.gs_plan_clear_info.argtypes = [vp, vp]
         L.gs_plan_set_push_targets.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp)]
+        L.gs_exchange_signal.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.c_uint32, vp]
+        L.gs_exchange_wait.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.c_uint32, vp]
         L.gs_ipc_export.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ctypes.c_uint64)]
         L.gs_ipc_open.argtypes = [ctypes.c_char_p, ctypes.c_uint64, ctypes.POINTER(vp)]
         L.gs_ipc_close.argtypes = [vp, ctypes.c_uint64]
@@ -249,6 +251,16 @@ class Plan:
         """Fused exchange: device pointers (ints) the column-range call of `kind` also stores into."""
         arr = (ctypes.c_void_p * max(1, len(ptrs)))(*ptrs)
         self._check(lib().gs_plan_set_push_targets(self._h, kind, len(ptrs), arr))
+
+    def exchange_signal(self, flag_ptrs, value: int, stream=None):
+        """Behind everything enqueued on the stream: write `value` to every flag address (device-side ordering)."""
+        arr = (ctypes.c_void_p * max(1, len(flag_ptrs)))(*flag_ptrs)
+        self._check(lib().gs_exchange_signal(self._h, len(flag_ptrs), arr, value & 0xFFFFFFFF, _stream_ptr(stream)))
+
+    def exchange_wait(self, flag_ptrs, value: int, stream=None):
+        """The stream continues only when every (local) flag is >= value."""
+        arr = (ctypes.c_void_p * max(1, len(flag_ptrs)))(*flag_ptrs)
+        self._check(lib().gs_exchange_wait(self._h, len(flag_ptrs), arr, value & 0xFFFFFFFF, _stream_ptr(stream)))
 
     def density_matrix(self, C: torch.Tensor, f: torch.Tensor, P: torch.Tensor, stream=None):
         """P(i,j) = sum_l f[l] conj(C(i,l)) C(j,l); upper triangle of P is written."""

@@ -20,8 +20,14 @@ A column range of a column-major matrix is one contiguous slab.  Two forms of th
   exchange="push" (the GPU default): FUSED into the producing kernels.  The other ranks' buffers are mapped
       over NVLink/NVSwitch peer memory (CUDA IPC) and registered as push targets of the plan; the
       epilogues of the column-range kernels store every tile they produce into all of them (posted
-      remote stores), so the slabs travel while the rest of the range is still being computed and
-      step 3 is separated from steps 1-2 only by a stream synchronise and a barrier.
+      remote stores), so the slabs travel while the rest of the range is still being computed.  Steps 1-2
+      and step 3 are then ordered either on the host (sync="host": stream synchronise + barrier) or ON THE
+      DEVICE (sync="device"): every rank owns 2 x world 32-bit flags, mapped into its peers like the buffers;
+      behind its producing kernels a rank writes the round's epoch into its "ready" slot of every peer
+      (gs_exchange_signal) and its consuming launch waits until all ready slots of its own array carry the
+      epoch (gs_exchange_wait) -- stream memory operations, no spinning kernel, no host round trip between
+      producing and consuming; a second set of slots ("done") keeps a round's stores behind the previous
+      round's reads.
   exchange="collective": an all-gather of unequal slabs after the kernels (one broadcast per owner;
       NCCL on the GPUs, gloo in the CPU test of this host logic) -- the baseline form.
 With x = (c/N)^3, a range [c0, c1) costs kappa x1 (its leading Cholesky) + (x1 - x0) (steps 2-3: the cost
@@ -122,7 +128,8 @@ class PeerMap:
         self.plan, self.rank, self.world, self.group = plan, rank, world, group
         self._bases = {}     # (owner rank, IPC handle) -> base pointer of the mapping (an allocation is mapped once)
 
-    def register(self, kind: int, local: torch.Tensor, include_self: bool) -> None:
+    def map_all(self, local: torch.Tensor) -> list:
+        """Device pointers, valid in this process, of the buffer every rank passes here (own rank: the local one)."""
         from . import gs
         mine = gs.ipc_export(local)
         infos = [None] * self.world
@@ -130,12 +137,17 @@ class PeerMap:
         ptrs = []
         for s, (handle, off) in enumerate(infos):
             if s == self.rank:
-                if include_self:
-                    ptrs.append(local.data_ptr())
+                ptrs.append(local.data_ptr())
                 continue
             if (s, handle) not in self._bases:
                 self._bases[(s, handle)] = gs.ipc_open(handle, 0)
             ptrs.append(self._bases[(s, handle)] + off)
+        return ptrs
+
+    def register(self, kind: int, local: torch.Tensor, include_self: bool) -> None:
+        ptrs = self.map_all(local)
+        if not include_self:
+            ptrs = [p for s, p in enumerate(ptrs) if s != self.rank]
         self.plan.set_push_targets(kind, ptrs)
 
     def close(self) -> None:
@@ -151,12 +163,18 @@ class ShardedReduction:
     """Host driver of the sharded path for one rank.  `plan` is a gs.Plan (or, in the CPU test of this
     host logic, an object with the same column-range methods -- exchange="collective" only)."""
 
-    def __init__(self, plan, rank: int = 0, world: int = 1, group=None, exchange: str = "collective"):
+    def __init__(self, plan, rank: int = 0, world: int = 1, group=None, exchange: str = "collective", sync: str = "host"):
         if exchange not in ("collective", "push"):
             raise ValueError("exchange must be 'collective' or 'push'")
+        if sync not in ("host", "device"):
+            raise ValueError("sync must be 'host' or 'device'")
         self.plan = plan
         self.rank, self.world, self.group = int(rank), int(world), group
         self.push = exchange == "push" and self.world > 1
+        self.device_sync = self.push and sync == "device"
+        self.epoch = 0
+        self.flags = None            # int32[2 * world]: ready slots, then done slots (device sync)
+        self.flag_ptrs = None        # this rank's view of every rank's flag array
         self.N, self.nev = plan.N, plan.nev
         self.ranges = column_ranges(self.N, self.world, plan.block)
         self.eig_ranges = even_ranges(self.nev, self.world, 2)
@@ -211,6 +229,11 @@ class ShardedReduction:
             self.peers.register(gs.GS_PUSH_HTILDE, res.Htilde, include_self=False)
             if self.nev > 0:
                 self.peers.register(gs.GS_PUSH_C, res.C, include_self=False)
+            if self.device_sync:
+                self.flags = torch.zeros(2 * self.world, dtype=torch.int32, device=like.device)
+                torch.cuda.synchronize(like.device)
+                self.flag_ptrs = self.peers.map_all(self.flags)
+                self.epoch = 0
             self._barrier()
         return res
 
@@ -236,6 +259,8 @@ class ShardedReduction:
                 return self.reduce(H, S, stream=stream, out=res)
         c0, c1 = res.cols
         U, Uinv, G, Ht = res.U, res.Uinv, res.G, res.Htilde
+        if self.device_sync:
+            return self._reduce_device_sync(H, S, res, stream)
         if self.push:
             self._barrier()                # the peers have finished reading what the last round pushed
         work = res.Uinv_work if self.push else Uinv
@@ -254,9 +279,44 @@ class ShardedReduction:
         plan.last_info(stream=stream)
         return res
 
+    def _slots(self, which: int):
+        """(addresses of MY slot `which` (0 ready, 1 done) in every rank's flag array, addresses of all ranks' slots in mine)"""
+        w, r = self.world, self.rank
+        mine_everywhere = [p + 4 * (which * w + r) for p in self.flag_ptrs]
+        all_in_mine = [self.flag_ptrs[r] + 4 * (which * w + s) for s in range(w)]
+        return mine_everywhere, all_in_mine
+
+    def _reduce_device_sync(self, H, S, res, stream):
+        """reduce() with the producing and the consuming launches ordered by device-side flags: nothing between
+        step 2 and step 3 waits for the host.  Every rank signals, whatever its own numerical status (a failed rank's
+        compute calls are no-ops; its signals are not), so no stream waits for ever; the status is agreed at the end."""
+        plan = self.plan
+        c0, c1 = res.cols
+        self.epoch += 1
+        e = self.epoch
+        ready_out, ready_in = self._slots(0)
+        done_out, done_in = self._slots(1)
+        if e > 1:
+            plan.exchange_wait(done_in, e - 1, stream=stream)     # the peers have read what the last round pushed
+        if c1 > c0:
+            res.U.copy_(S)
+            plan.cholesky_leading(res.U, c1, stream=stream)
+            plan.invert_triangular_cols(res.U, res.Uinv_work, c0, c1 - c0, stream=stream)
+            plan.to_standard_g_cols(H, res.Uinv_work, res.G, c0, c1 - c0, stream=stream)
+        plan.exchange_signal(ready_out, e, stream=stream)          # behind the kernels whose epilogues pushed the slabs
+        plan.exchange_wait(ready_in, e, stream=stream)             # every rank's slabs have landed here
+        if c1 > c0:
+            plan.to_standard_cols(res.Uinv, res.G, res.Htilde, c0, c1 - c0, stream=stream)
+        plan.exchange_signal(done_out, e, stream=stream)           # ... and my columns of H~ are out as well
+        self._check_all(H.device, stream)
+        return res
+
     def gather_htilde(self, res: ShardedResult) -> torch.Tensor:
         """Every rank gets all columns of the upper triangle of H~ (for an off-path eigensolver)."""
-        if self.push:
+        if self.device_sync:
+            _, done_in = self._slots(1)
+            self.plan.exchange_wait(done_in, self.epoch)           # step 3 of every rank has pushed its columns
+        elif self.push:
             self._barrier()                # step 3 already pushed them
         else:
             exchange_slabs((res.Htilde,), self.ranges, self.rank, self.world, self.group)
