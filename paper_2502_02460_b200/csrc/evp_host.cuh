@@ -442,7 +442,7 @@ gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double*
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
     EvpBuffers b;
     GS_TRY(evp_ready(plan, &b));
-    if (d == nullptr || e == nullptr || eps == nullptr || (plan->nev > 0 && Z == nullptr)) return GS_ERR_INVALID_ARG;
+    if (d == nullptr || e == nullptr || (plan->nev > 0 && (eps == nullptr || Z == nullptr))) return GS_ERR_INVALID_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     GS_CUDA(plan, cudaMemcpyAsync(b.dwork, d, sizeof(double) * size_t(plan->N), cudaMemcpyDeviceToDevice, stream));
     return evp_solve_impl(plan, b, b.dwork, e, eps, Z, plan->N, int(plan->nev), stream);
@@ -465,7 +465,7 @@ gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, v
     if (plan == nullptr) return GS_ERR_INVALID_ARG;
     EvpBuffers b;
     GS_TRY(evp_ready(plan, &b));
-    if (Htilde_inout == nullptr || eps == nullptr || (plan->nev > 0 && Ctilde == nullptr) || !aligned16(Htilde_inout) ||
+    if (Htilde_inout == nullptr || (plan->nev > 0 && (eps == nullptr || Ctilde == nullptr)) || !aligned16(Htilde_inout) ||
         (Ctilde != nullptr && (!aligned16(Ctilde) || overlaps(Ctilde, vec_bytes(plan), Htilde_inout, mat_bytes(plan)))))
         return GS_ERR_INVALID_ARG;
     return evp_eigh_impl(plan, b, Htilde_inout, eps, Ctilde, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));

@@ -184,6 +184,24 @@ def test_stage_calls_chain_like_standard_eigh():
     plan.close()
 
 
+def test_nev_zero_and_single_eigenpair():
+    """nev = 0: the stages run (tridiagonalisation, eigenvalue-free solve) and return nothing; nev = 1: the lowest pair."""
+    gs = _gs()
+    N = 200
+    _, _, Ht = _htilde(N, False, seed=12)
+    eps_o, _, _ = oracle.jacobi(Ht)
+    plan0 = gs.Plan(N, 0)
+    eps, Ct = plan0.standard_eigh(_upper_poisoned(Ht))
+    assert plan0.last_info() == 0 and eps.numel() == 0 and Ct.shape == (N, 0)
+    plan0.close()
+    plan1 = gs.Plan(N, 1)
+    eps, Ct = plan1.standard_eigh(_upper_poisoned(Ht))
+    assert plan1.last_info() == 0
+    assert abs(eps.item() - eps_o[0]) <= 1e-12 * np.abs(eps_o).max()
+    _validity(Ht, eps, Ct, 1)
+    plan1.close()
+
+
 def test_config0_end_to_end_without_any_library_eigensolver():
     """BASELINE config 0 through the GPU path ONLY -- reduction, standard eigensolver, back-transformation -- against
     the three acceptance tolerances and the oracle's eigenvalues (no torch.linalg anywhere)."""
