@@ -195,6 +195,24 @@ gs_status_t gs_ipc_close(void* dev_ptr, uint64_t offset);
  * in the plan's workspace). */
 gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C, const double* f, void* P, void* cuda_stream);
 
+/* The same operation for callers that cannot allocate device memory -- code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc: identical kernels and results, but the scratch
+ * (the status flag and the sqrt(f)-scaled, transposed eigenvector block) lives in a static device array of
+ * GS_STATIC_SCRATCH_BYTES inside libgs, which every GPU that loads the library holds until the process exits.
+ * The plan needs NO workspace (gs_plan_set_workspace may never have been called); the call allocates nothing
+ * (no cudaMalloc / cudaFree, no allocating library routine) and, like the other compute calls, only enqueues
+ * work.  C, f, P are the caller's device buffers as above.
+ * Limit: 256 + N * nev' * sizeof(element) <= GS_STATIC_SCRATCH_BYTES, nev' = nev rounded up to even for
+ * GS_REAL64 (2 for nev == 0) -- e.g. N = nev = 1024 complex, or N = 2048 with nev = 1024 real / 512 complex.
+ * Beyond it: GS_ERR_WORKSPACE, and gs_plan_last_cuda_error names the sizes; use gs_density_matrix.
+ * ALL calls in the process on one device share the one array, whatever their plan or stream: two calls whose
+ * GPU work may overlap (different streams without an edge between them, several host threads) RACE on it --
+ * order them.  The array keeps the previous call's contents; the call clears what must start at zero.
+ * There is no numerical status to report (a negative occupation gives NaN, as above); the plan's own status
+ * flag (gs_last_info) is neither read nor written. */
+#define GS_STATIC_SCRATCH_BYTES (16u * 1024u * 1024u + 256u)
+gs_status_t gs_density_matrix_static(gs_plan_t* plan, const void* C, const double* f, void* P, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------------
  * NEXT-4: the standard eigenproblem  H~ C~ = C~ eps  that sits between step 3 and the
  * back-transformation ("This reduces the generalized eigenproblem to the standard one, H~ C~ = eps C~, which has

@@ -1198,6 +1198,84 @@ gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C_, const double* f, 
     return launch(st, p, false, L_DENS_SYRK);
 }
 
+// ------------------------------------------------------------------------------------------------
+// gs_density_matrix_static: the same two launches with their scratch (the status flag and the scaled,
+// transposed eigenvector block X) in a file-scope device array instead of the caller's workspace, for callers
+// that cannot allocate device memory (CUDA graph capture, serving loops).  The array's name is a host-side
+// stand-in in host code: its device address comes from cudaGetSymbolAddress, looked up once per device with
+// that device current.  Every call shares the array: calls that overlap on the GPU race (include/gs.h).
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[GS_STATIC_SCRATCH_BYTES];
+
+static cudaError_t static_scratch_address(unsigned char** out)
+{
+    static std::mutex mu;
+    static unsigned char* addr[kMaxDevices] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (addr[dev] == nullptr) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (p == nullptr || (reinterpret_cast<uintptr_t>(p) & 255u) != 0) return cudaErrorInvalidSymbol;
+        addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = addr[dev];
+    return cudaSuccess;
+}
+
+gs_status_t gs_density_matrix_static(gs_plan_t* plan, const void* C_, const double* f, void* P_, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;   // the plan's own workspace is not used: none has to be set
+    if (P_ == nullptr || !aligned16(P_)) return GS_ERR_INVALID_ARG;
+    const int N = int(plan->N), nev = int(plan->nev);
+    if (nev > 0 && (C_ == nullptr || f == nullptr || !aligned16(C_) || overlaps(P_, mat_bytes(plan), C_, vec_bytes(plan))))
+        return GS_ERR_INVALID_ARG;
+    const long long ldx = nev == 0 ? 2 : (plan->z ? nev : ((nev + 1) & ~1LL));   // as in gs_density_matrix
+    const size_t need = kInfoBytes + size_t(N) * size_t(ldx) * plan->es;
+    if (need > size_t(GS_STATIC_SCRATCH_BYTES)) {
+        std::snprintf(plan->cuda_error, sizeof(plan->cuda_error),
+                      "gs_density_matrix_static: N = %d, nev = %d needs %zu bytes of scratch, the static array holds %zu "
+                      "(GS_STATIC_SCRATCH_BYTES); use gs_density_matrix with a workspace", N, nev, need, size_t(GS_STATIC_SCRATCH_BYTES));
+        return GS_ERR_WORKSPACE;
+    }
+    unsigned char* scratch = nullptr;
+    GS_CUDA(plan, static_scratch_address(&scratch));
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    // the array keeps the previous call's contents: the status flag the kernels test must start at zero
+    // (X is overwritten in full before it is read: rows l < nev by the transpose, TMA zero-fills the ragged k tail)
+    int* info = reinterpret_cast<int*>(scratch);
+    GS_CUDA(plan, cudaMemsetAsync(info, 0, kInfoBytes, stream));
+    void* X = scratch + kInfoBytes;
+    Stage st = make_stage(plan, stream);
+    if (nev > 0) {
+        dim3 grid((N + 31) / 32, (nev + 31) / 32), block(32, 8);
+        LaunchTimer timer(plan, L_DENS_T, stream);
+        if (plan->z)
+            transpose_scale_kernel<double2><<<grid, block, 0, stream>>>(static_cast<const double2*>(C_), plan->N, f,
+                                                                       static_cast<double2*>(X), ldx, N, nev, info);
+        else
+            transpose_scale_kernel<double><<<grid, block, 0, stream>>>(static_cast<const double*>(C_), plan->N, f,
+                                                                     static_cast<double*>(X), ldx, N, nev, info);
+        GS_CUDA(plan, cudaGetLastError());
+        plan->launches += 1;
+    }
+    const MatView vX{X, nev > 0 ? nev : 1, N, ldx};
+    st.tma = true;
+    EngineParams p = blank_params(plan);
+    p.info = info;
+    if (!set_operand(st, p, 0, vX, false) || !set_operand(st, p, 1, vX, false)) return GS_ERR_CUDA;
+    p.C = static_cast<double*>(P_); p.ldc = N;
+    p.tiles_m = plan->nblk; p.tiles_n = plan->nblk; p.order = ORDER_TRI_ROW_DESC;
+    p.c_rows = N; p.c_cols = N;
+    p.khi_c = (nev + st.bk - 1) / st.bk; p.kmax = p.khi_c;
+    p.flags = F_STORE_UPPER | F_REAL_DIAG;
+    return launch(st, p, false, L_DENS_SYRK);
+}
+
 gs_status_t gs_last_info(gs_plan_t* plan, void* cuda_stream, int64_t* info)
 {
     if (plan == nullptr || info == nullptr) return GS_ERR_INVALID_ARG;

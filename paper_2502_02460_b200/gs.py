@@ -28,7 +28,7 @@ STATUS_NAMES = {
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
-    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_last_info", "gs_plan_clear_info",
+    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_density_matrix_static", "gs_last_info", "gs_plan_clear_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
     "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close", "gs_exchange_signal", "gs_exchange_wait",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
@@ -82,6 +82,7 @@ def lib() -> ctypes.CDLL:
         L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
         L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_density_matrix.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_density_matrix_static.argtypes = [vp, vp, vp, vp, vp]
         L.gs_invert_triangular_cols.argtypes = [vp, vp, vp, i64, i64, vp]
         L.gs_to_standard_g_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
         L.gs_to_standard_cols.argtypes = [vp, vp, vp, vp, i64, i64, vp]
@@ -271,6 +272,17 @@ class Plan:
             raise ValueError("f: expected a contiguous CUDA float64 vector of length nev")
         self._check(lib().gs_density_matrix(self._h, _dev_ptr(C, self.N, self.nev, self.tdtype), f.data_ptr(),
                                             _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+
+    def density_matrix_static(self, C: torch.Tensor, f: torch.Tensor, P: torch.Tensor, stream=None):
+        """gs_density_matrix_static: the same result with the scratch in libgs's static device array -- no allocation,
+        no plan workspace; N * nev is limited (GS_STATIC_SCRATCH_BYTES) and overlapping calls race (include/gs.h)."""
+        if self.nev == 0:
+            self._check(lib().gs_density_matrix_static(self._h, None, None, _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
+            return
+        if not (f.is_cuda and f.dtype == torch.float64 and f.dim() == 1 and f.numel() == self.nev and f.is_contiguous()):
+            raise ValueError("f: expected a contiguous CUDA float64 vector of length nev")
+        self._check(lib().gs_density_matrix_static(self._h, _dev_ptr(C, self.N, self.nev, self.tdtype), f.data_ptr(),
+                                                   _dev_ptr(P, self.N, self.N, self.tdtype), _stream_ptr(stream)))
 
     # ---- NEXT-4: the standard eigenproblem H~ C~ = C~ eps between step 3 and the back-transformation (PAPER.md:67) ----
     def evp_workspace_bytes(self) -> int:
