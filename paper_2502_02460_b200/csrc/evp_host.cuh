@@ -132,12 +132,50 @@ inline cudaError_t evp_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, c
     return cudaGetLastError();
 }
 
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_smem(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    static const bool pdl = !(std::getenv("GS_EVP_PDL") != nullptr && std::atoi(std::getenv("GS_EVP_PDL")) == 0);
+    if (pdl) return launch_pdl(kernel, grid, block, smem, stream, args...);
+    kernel<<<grid, block, smem, stream>>>(KArgs(args)...);
+    return cudaGetLastError();
+}
+
 #define GS_LAUNCH_OK(plan)                                       \
     do {                                                         \
         const cudaError_t le__ = cudaGetLastError();             \
         if (le__ != cudaSuccess) return cuda_fail((plan), le__); \
         (plan)->launches += 1;                                   \
     } while (0)
+
+// tensor map of symv_tma_kernel: A as an (N * w8) x N FP64 tensor, box = 128 doubles (TH rows) x 16 columns, no swizzle
+inline bool make_symv_map(CUtensorMap* out, const void* A, long long N, int w8)
+{
+    PFN_cuTensorMapEncodeTiled enc = tensor_map_encoder();
+    if (enc == nullptr) return false;
+    cuuint64_t dims[2] = {static_cast<cuuint64_t>(N) * w8, static_cast<cuuint64_t>(N)};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(N) * 8 * w8};
+    cuuint32_t box[2] = {128, 16};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(A), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// per-device opt-in of symv_tma_kernel to its dynamic shared memory; *sms = SM count of the current device
+inline cudaError_t configure_symv(int* sms)
+{
+    static PerDeviceOnce once;
+    cudaError_t e = once.run([]() -> cudaError_t {
+        cudaError_t r = cudaFuncSetAttribute(symv_tma_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, SvCfg<double>::kSmemBytes);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(symv_tma_kernel<double2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SvCfg<double2>::kSmemBytes);
+        return r;
+    });
+    if (e != cudaSuccess) return e;
+    int dev = 0;
+    e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    return cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev);
+}
 
 // A[0:m, 0:m] -= V W^H + W V^H (upper tiles) from the panel's conjugate-transposed images Vt, Wt (cnt x m, ld nb)
 gs_status_t evp_her2k(gs_plan* plan, const EvpBuffers& b, void* A, int m, int cnt, cudaStream_t stream)
@@ -169,6 +207,19 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     GS_LAUNCH_OK(plan);
     StepParams<T> p = step_params<T>(plan, b, A, d, e, tau);
     const bool vec = (N % 2 == 0);
+    // S through TMA (symv_tma_kernel) whenever A admits a tensor map; GS_EVP_SYMV=0 keeps the plain-load kernel,
+    // GS_EVP_CHUNK fixes the strip length (128-row blocks per work item: 1, 2 or 4)
+    static const bool tma_off = std::getenv("GS_EVP_SYMV") != nullptr && std::atoi(std::getenv("GS_EVP_SYMV")) == 0;
+    static const int chunk_env = std::getenv("GS_EVP_CHUNK") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK")) : 0;
+    const bool use_tma = !tma_off && (sizeof(T) == 16 || vec) && aligned16(A);
+    SymvTmaParams<T> q{};
+    int sv_ctas = 0;
+    if (use_tma) {
+        int sms = 0;
+        GS_CUDA(plan, configure_symv(&sms));
+        sv_ctas = sms * SvCfg<T>::kCtasPerSm;
+        if (!make_symv_map(&q.mapA, A, N, int(sizeof(T) / 8))) return GS_ERR_CUDA;
+    }
     const int fgrid = std::max(1, std::min(64, (N + 255) / 256));
     auto finish = [&](int i, int jp, int mode) -> gs_status_t {
         p.i = i; p.jp = jp; p.mode = mode;
@@ -188,7 +239,21 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
         while (i >= 1 && jp < nb) {
             p.i = i; p.jp = jp; p.mode = 0;
             const int nJ = (i + TW - 1) / TW, nI = (i + TH - 1) / TH;
-            {
+            if (use_tma) {
+                // strips of K blocks: the longest that still leaves every persistent CTA about three work items
+                const long long nblocks = (long long)nJ * (nJ + 1) / 2;
+                int K = chunk_env == 1 || chunk_env == 2 || chunk_env == 4 ? chunk_env : (nblocks >= 12LL * sv_ctas ? 4 : nblocks >= 6LL * sv_ctas ? 2 : 1);
+                const int a = nJ / K, r = nJ % K, nitems = K * a * (a + 1) / 2 + r * (a + 1);
+                p.p2_chunk_rows = K * TW;
+                q.s = p; q.chunk_blocks = K; q.dot_ctas = jp > 0 ? nJ : 0;
+                LaunchTimer timer(plan, L_EVP_SYMV, stream);
+                const cudaError_t le = launch_pdl_smem(symv_tma_kernel<T>, dim3(q.dot_ctas + std::min(nitems, sv_ctas)), dim3(kSvThreads),
+                                                       SvCfg<T>::kSmemBytes, stream, q);
+                if (le != cudaSuccess) return cuda_fail(plan, le);
+                plan->launches += 1;
+                evp_trace(stream, "symv.tma", i, jp);
+            } else {
+                p.p2_chunk_rows = TH;
                 LaunchTimer timer(plan, L_EVP_SYMV, stream);
                 const dim3 grid(nJ, nI + (jp > 0 ? 1 : 0));
                 const cudaError_t le = vec ? evp_launch(symv_kernel<T, true>, grid, kSymvThreads, stream, p)

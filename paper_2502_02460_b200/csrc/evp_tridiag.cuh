@@ -126,8 +126,68 @@ struct StepParams {
     int lb;               // block order of R (= nb)
     int panel;            // panel number (block of R)
     int mode;             // F: 0 = lazy next column (stale A + panel corrections), 1 = fresh (A is up to date), 2 = none
+    int p2_chunk_rows;    // rows of A one P2 partial covers: TH (symv_kernel) or chunk_blocks * 128 (symv_tma_kernel)
     const int* info;
 };
+
+// ---------------------------------------------------------------------------------------------------------
+// Panel dots of S (CTA x of nx, >= 256 threads of which the first 256 work):
+//   Pt[x][c] = sum_{r in chunk x} Wt[c, r] u[r],  Pt[x][nb + c] likewise for Vt  (128-row chunks);
+// the last CTA to arrive finalises tW' = s (W^H u - beta Wt[:, i-1]), tV' likewise, and the new column of
+// M^H = conj(D) + striu(V^H V).  sm: 512 elements of shared memory.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last)
+{
+    constexpr int TW = kSymvTW;
+    const int m = p.i, jp = p.jp, nb = p.nb;
+    const int t = threadIdx.x;
+    if (jp == 0) return;
+    const int r0 = x * TW, r1 = min(r0 + TW, m);
+    const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
+    const int c = t % nb, g = t / nb;
+    T aw = zero_of(T{}), av = zero_of(T{});
+    if (t < kSymvThreads && c < jp) {
+        for (int r = r0 + g; r < r1; r += groups) {
+            const T ur = p.u[r];
+            aw = fmad(p.Wt[c + (long long)r * nb], ur, aw);
+            av = fmad(p.Vt[c + (long long)r * nb], ur, av);
+        }
+    }
+    if (t < kSymvThreads) { sm[t] = aw; sm[kSymvThreads + t] = av; }
+    __syncthreads();
+    if (t < nb) {
+        T sw = zero_of(T{}), sv = zero_of(T{});
+        for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
+        p.Pt[(long long)x * 2 * nb + t] = sw;
+        p.Pt[(long long)x * 2 * nb + nb + t] = sv;
+    }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) *s_last = (atomicAdd(&p.tickets[0], 1u) == unsigned(nx - 1)) ? 1u : 0u;
+    __syncthreads();
+    if (!*s_last) return;
+    __threadfence();
+    // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
+    const StepScalars<T> sc = *p.sc;
+    if (t < 2 * nb) {
+        const int cc = t % nb;
+        const bool isV = t >= nb;
+        T acc = zero_of(T{});
+        if (cc < jp) {
+            for (int xx = 0; xx < nx; ++xx) acc = add(acc, ldcg(&p.Pt[(long long)xx * 2 * nb + t]));
+            const T rowv = (isV ? p.Vt : p.Wt)[cc + (long long)(m - 1) * nb];   // conj(W(i-1, c))
+            acc = mul(sc.s, sub(acc, rscale(rowv, sc.beta)));
+        }
+        p.tfin[t] = acc;
+        if (isV && cc < jp) {
+            // G(a, b) = v_a^H v_b for a = itop - cc > b = i;  M^H(b - i0, a - i0) = conj(G(a, b)) with i0 = itop - lb + 1
+            const int lb = p.lb, rowb = lb - 1 - p.jp, cola = lb - 1 - cc;
+            p.R[(long long)p.panel * lb * (lb + 1) + rowb + (long long)cola * lb] = cj(acc);
+        }
+    }
+    if (t == 0) p.tickets[0] = 0u;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // S: partial sums of y = A[0:m, 0:m] u (m = i) from the UPPER triangle only, one CTA per (TH x 128) tile; the
@@ -147,55 +207,7 @@ __global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> 
     __shared__ unsigned int s_last;
 
     if (int(blockIdx.y) == nI) {
-        // ---- panel dots: Pt[x][c] = sum_{r in chunk} Wt[c, r] u[r],  Pt[x][nb + c] likewise for Vt ----
-        const int jp = p.jp, nb = p.nb;
-        if (jp == 0) return;
-        const int x = blockIdx.x;
-        const int r0 = x * TW, r1 = min(r0 + TW, m);
-        const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
-        const int c = t % nb, g = t / nb;
-        T aw = zero_of(T{}), av = zero_of(T{});
-        if (c < jp) {
-            for (int r = r0 + g; r < r1; r += groups) {
-                const T ur = p.u[r];
-                aw = fmad(p.Wt[c + (long long)r * nb], ur, aw);
-                av = fmad(p.Vt[c + (long long)r * nb], ur, av);
-            }
-        }
-        T* sm = &red[0][0];                               // 8 * TH elements >= 2 * 256
-        sm[t] = aw; sm[kSymvThreads + t] = av;
-        __syncthreads();
-        if (t < nb) {
-            T sw = zero_of(T{}), sv = zero_of(T{});
-            for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
-            p.Pt[(long long)x * 2 * nb + t] = sw;
-            p.Pt[(long long)x * 2 * nb + nb + t] = sv;
-        }
-        __threadfence();
-        __syncthreads();
-        if (t == 0) s_last = (atomicAdd(&p.tickets[0], 1u) == gridDim.x - 1) ? 1u : 0u;
-        __syncthreads();
-        if (!s_last) return;
-        __threadfence();
-        // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
-        const StepScalars<T> sc = *p.sc;
-        if (t < 2 * nb) {
-            const int cc = t % nb;
-            const bool isV = t >= nb;
-            T acc = zero_of(T{});
-            if (cc < jp) {
-                for (int xx = 0; xx < int(gridDim.x); ++xx) acc = add(acc, ldcg(&p.Pt[(long long)xx * 2 * nb + t]));
-                const T rowv = (isV ? p.Vt : p.Wt)[cc + (long long)(m - 1) * nb];   // conj(W(i-1, c))
-                acc = mul(sc.s, sub(acc, rscale(rowv, sc.beta)));
-            }
-            p.tfin[t] = acc;
-            if (isV && cc < jp) {
-                // G(a, b) = v_a^H v_b for a = itop - cc > b = i;  M^H(b - i0, a - i0) = conj(G(a, b)) with i0 = itop - lb + 1
-                const int lb = p.lb, rowb = lb - 1 - p.jp, cola = lb - 1 - cc;
-                p.R[(long long)p.panel * lb * (lb + 1) + rowb + (long long)cola * lb] = cj(acc);
-            }
-        }
-        if (t == 0) p.tickets[0] = 0u;
+        panel_dots(p, int(blockIdx.x), int(gridDim.x), &red[0][0], &s_last);
         return;
     }
 
@@ -269,6 +281,232 @@ __global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> 
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// S, TMA form (the default whenever A admits a tensor map: complex, or real with even N).  Same partial sums as
+// symv_kernel, other machinery -- the step is bound by the HBM stream of the triangle, so what matters is that
+// the stream never stops and that little else is issued beside it:
+//   * PERSISTENT CTAs (two per SM): a producer warp keeps a ring of 16 KB stages (TH rows x 16 columns, one TMA
+//     box each) full across tile and work-item boundaries; eight consumer warps read the stages from shared
+//     memory (conflict-free 16-byte loads), so no register is tied up by a load in flight.
+//   * a work item is a COLUMN STRIP: chunk_blocks * 128 rows of one 128-column block.  The column sums
+//     y(c) += conj(a(r,c)) u(r) stay in registers over the whole strip (a warp owns two columns of every stage,
+//     a lane four rows) and are reduced across lanes once per strip by a transposing butterfly (16 shuffles
+//     instead of 80); the row sums y(r) += a(r,c) u(c) of a tile are summed over the eight warps through shared
+//     memory (one named barrier per tile, double-buffered).
+//   * tiles strictly above the diagonal take a path without any per-element test; only the tiles that reach
+//     the diagonal select (r <= c: the strictly-lower part of the buffer is never used; real diagonal).
+//   Work items are dealt round-robin (item = cta, cta + G, ...): every partial has one owner and a fixed
+//   summation order, so the result does not depend on scheduling.
+// Leading CTAs (blockIdx.x < dot_ctas) form the panel dots instead (panel_dots).
+// P1[J][r]: row sums of column block J; P2[q][c]: column sums of strip q (p2_chunk_rows = chunk_blocks * 128).
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kSvStageBytes = 16384;                 // TH rows x 16 columns
+constexpr int kSvConsumerWarps = 8;
+constexpr int kSvThreads = (kSvConsumerWarps + 1) * 32;
+constexpr int kSvRedBytes = 2 * kSvConsumerWarps * 1024;   // two buffers of 8 warps x TH elements
+constexpr int kSvUcolBytes = 2 * kSymvTW * 16;             // u over the column block, two work items
+// real: 16 column sums = 32 registers -> two CTAs of 5 stages per SM; complex: 64 registers -> one CTA of 10 stages
+template <typename T> struct SvCfg {
+    static constexpr int kStages = sizeof(T) == 8 ? 5 : 10;
+    static constexpr int kCtasPerSm = sizeof(T) == 8 ? 2 : 1;
+    static constexpr int kSmemBytes = kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + 256 /*barriers*/ + 1024 /*alignment*/;
+};
+
+template <typename T>
+struct SymvTmaParams {
+    StepParams<T> s;
+    CUtensorMap mapA;     // A as an (N * sizeof(T)/8) x N FP64 tensor; box = 128 doubles (TH rows) x 16 columns, no swizzle
+    int chunk_blocks;     // 128-row blocks per work item (1, 2 or 4)
+    int dot_ctas;         // leading CTAs that form the panel dots (0 when the panel is empty)
+};
+
+// number of work items in the column blocks j < J:  sum_{j<J} ceil((j + 1) / K)
+__device__ __forceinline__ int sv_items_before(int J, int K)
+{
+    const int a = J / K, b = J - a * K;
+    return K * a * (a + 1) / 2 + b * (a + 1);
+}
+
+// v[16] per lane -> the sum over the 32 lanes of v[idx], idx = bits 4..1 of the lane (both lanes of a pair hold it)
+template <typename T>
+__device__ __forceinline__ T sv_transpose_reduce(const T (&v)[16], int lane)
+{
+    T w8[8], w4[4], w2[2];
+    const bool u16 = (lane & 16) != 0, u8 = (lane & 8) != 0, u4 = (lane & 4) != 0, u2 = (lane & 2) != 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) w8[i] = add(u16 ? v[i + 8] : v[i], shfl_xor(u16 ? v[i] : v[i + 8], 16));
+#pragma unroll
+    for (int i = 0; i < 4; ++i) w4[i] = add(u8 ? w8[i + 4] : w8[i], shfl_xor(u8 ? w8[i] : w8[i + 4], 8));
+#pragma unroll
+    for (int i = 0; i < 2; ++i) w2[i] = add(u4 ? w4[i + 2] : w4[i], shfl_xor(u4 ? w4[i] : w4[i + 2], 4));
+    T w1 = add(u2 ? w2[1] : w2[0], shfl_xor(u2 ? w2[0] : w2[1], 2));
+    return add(w1, shfl_xor(w1, 1));
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
+{
+    constexpr int kSvStages = SvCfg<T>::kStages;
+    constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW, H = RPT / 2;
+    constexpr int W8 = int(sizeof(T)) / 8;            // doubles per element
+    constexpr int R = TW / TH;                        // row tiles per 128-row block
+    const StepParams<T>& p = q.s;
+    extern __shared__ unsigned char sv_smem_raw[];
+    unsigned char* smem = sv_smem_raw + ((1024u - (smem_u32(sv_smem_raw) & 1023u)) & 1023u);
+    unsigned char* stages = smem;
+    T* red = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes);
+    T* ucol = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes + kSvRedBytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + kSvStages);
+    __shared__ unsigned int s_last;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    if (t == 0) {
+        for (int s = 0; s < kSvStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kSvConsumerWarps); }
+        mbar_fence_init();
+        tma_prefetch_desc(&q.mapA);
+    }
+    __syncthreads();
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const int m = p.i;
+    if (int(blockIdx.x) < q.dot_ctas) {
+        panel_dots(p, int(blockIdx.x), q.dot_ctas, red, &s_last);
+        return;
+    }
+    const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
+    const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH, K = q.chunk_blocks;
+    const int nitems = sv_items_before(nJ, K);
+
+    // item -> (column block J, first and one-past-last row tile): largest J with items_before(J) <= item
+    auto decode = [&](int item, int& J, int& I0, int& I1) {
+        int lo = 0, hi = nJ;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (sv_items_before(mid, K) <= item) lo = mid; else hi = mid;
+        }
+        J = lo;
+        const int qq = item - sv_items_before(lo, K);
+        I0 = qq * K * R;
+        I1 = min(min((qq + 1) * K * R, (J + 1) * R), nI);
+    };
+
+    if (warp == kSvConsumerWarps) {
+        // ---- producer: one lane streams every stage of every tile of this CTA's items ----
+        if (lane == 0) {
+            uint32_t cnt = 0;
+            for (int item = cta; item < nitems; item += G) {
+                int J, I0, I1;
+                decode(item, J, I0, I1);
+                for (int I = I0; I < I1; ++I) {
+                    for (int s = 0; s < TW / 16; ++s, ++cnt) {
+                        const uint32_t stage = cnt % kSvStages;
+                        if (cnt >= kSvStages) mbar_wait(empty0 + 8 * stage, ((cnt / kSvStages) - 1) & 1);
+                        mbar_arrive_expect_tx(full0 + 8 * stage, kSvStageBytes);
+                        tma_load_2d(smem_u32(stages + stage * kSvStageBytes), &q.mapA, I * TH * W8, J * TW + 16 * s, full0 + 8 * stage);
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    // ---- consumers: warp w owns columns 2w, 2w+1 of every stage; lane l owns rows {l H .. l H + H-1} of each half tile ----
+    auto row_of = [&](int k) { return (k / H) * (TH / 2) + lane * H + (k % H); };
+    auto load_u_rows = [&](int I, T (&dst)[RPT]) {
+#pragma unroll
+        for (int k = 0; k < RPT; ++k) {
+            const int r = I * TH + row_of(k);
+            dst[k] = (r < m) ? p.u[r] : zero_of(T{});
+        }
+    };
+    uint32_t cnt = 0;
+    int nitem = 0, ntile = 0;
+    for (int item = cta; item < nitems; item += G, ++nitem) {
+        int J, I0, I1;
+        decode(item, J, I0, I1);
+        T* uc = ucol + (nitem & 1) * TW;
+        if (t < TW) { const int c = J * TW + t; uc[t] = (c < m) ? p.u[c] : zero_of(T{}); }
+        named_bar_sync(1, kSvConsumerWarps * 32);
+        T yc[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) yc[i] = zero_of(T{});
+        T ur[RPT];
+        for (int I = I0; I < I1; ++I, ++ntile) {
+            load_u_rows(I, ur);
+            T yr[RPT];
+#pragma unroll
+            for (int k = 0; k < RPT; ++k) yr[k] = zero_of(T{});
+            const bool masked = I * TH + TH - 1 >= J * TW;     // some element of the tile lies below the diagonal
+#pragma unroll
+            for (int s = 0; s < TW / 16; ++s) {
+                const uint32_t stage = cnt % kSvStages;
+                mbar_wait(full0 + 8 * stage, (cnt / kSvStages) & 1);
+                if (cnt > 0) {                                   // release the previous stage (ptx.cuh: not right behind its loads)
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty0 + 8 * ((cnt - 1) % kSvStages));
+                }
+                ++cnt;
+                const unsigned char* sp = stages + stage * kSvStageBytes + (2 * warp) * (TH * int(sizeof(T)));
+                T a[2][RPT];
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double2 v = *reinterpret_cast<const double2*>(sp + j * (TH * int(sizeof(T))) + h * (TH / 2) * int(sizeof(T)) + lane * 16);
+                        if constexpr (sizeof(T) == 8) { a[j][2 * h] = v.x; a[j][2 * h + 1] = v.y; }
+                        else { a[j][h] = v; }
+                    }
+                }
+                const T u0 = uc[16 * s + 2 * warp], u1 = uc[16 * s + 2 * warp + 1];
+                if (!masked) {
+#pragma unroll
+                    for (int k = 0; k < RPT; ++k) {
+                        yr[k] = fmad(a[0][k], u0, yr[k]);
+                        yr[k] = fmad(a[1][k], u1, yr[k]);
+                        yc[2 * s] = cfmad(a[0][k], ur[k], yc[2 * s]);
+                        yc[2 * s + 1] = cfmad(a[1][k], ur[k], yc[2 * s + 1]);
+                    }
+                } else {
+                    const int c0 = J * TW + 16 * s + 2 * warp;
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const int c = c0 + j;
+#pragma unroll
+                        for (int k = 0; k < RPT; ++k) {
+                            const int r = I * TH + row_of(k);
+                            T av = (r <= c) ? a[j][k] : zero_of(T{});
+                            if (r == c) av = real_only(av);
+                            yr[k] = fmad(av, j == 0 ? u0 : u1, yr[k]);
+                            if (r < c) yc[2 * s + j] = cfmad(av, ur[k], yc[2 * s + j]);
+                        }
+                    }
+                }
+            }
+            // row sums of the tile over the eight warps
+            T* rb = red + ((ntile & 1) * kSvConsumerWarps + warp) * TH;
+#pragma unroll
+            for (int k = 0; k < RPT; ++k) rb[row_of(k)] = yr[k];
+            named_bar_sync(2, kSvConsumerWarps * 32);
+            if (t < TH) {
+                const T* rr = red + (ntile & 1) * kSvConsumerWarps * TH + t;
+                T sum = rr[0];
+#pragma unroll
+                for (int w = 1; w < kSvConsumerWarps; ++w) sum = add(sum, rr[w * TH]);
+                const int r = I * TH + t;
+                if (r < m) p.P1[(long long)J * p.ldp + r] = sum;
+            }
+        }
+        // column sums of the strip
+        const T ysum = sv_transpose_reduce(yc, lane);
+        if ((lane & 1) == 0) {
+            const int idx = lane >> 1;                          // = 2 s + j
+            const int c = J * TW + 16 * (idx >> 1) + 2 * warp + (idx & 1);
+            if (c < m) p.P2[(long long)(I0 / (K * R)) * p.ldp + c] = ysum;
+        }
+    }
+}
+
 // Householder scalars of a column with off-diagonal part (x, alpha):  H [x; alpha] = [0; beta]  (LAPACK xLARFG
 // without the safmin rescaling loop).
 __device__ __forceinline__ void householder_scalars(double alpha, double xnorm2, StepScalars<double>& sc)
@@ -327,7 +565,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
         // y(r): P1[J][r] for J >= r / TW, P2[I][r] for I <= r / TH
         const int nJ = (m + TW - 1) / TW;
         for (int J = r / TW + l8; J < nJ; J += 8) y = add(y, p.P1[(long long)J * p.ldp + r]);
-        for (int I = l8; I <= r / TH; I += 8) y = add(y, p.P2[(long long)I * p.ldp + r]);
+        for (int I = l8; I <= r / p.p2_chunk_rows; I += 8) y = add(y, p.P2[(long long)I * p.ldp + r]);
         const T* vt = p.Vt + (long long)r * nb;
         const T* wt = p.Wt + (long long)r * nb;
         for (int c = l8; c < jp; c += 8) {
@@ -371,9 +609,16 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    // the last CTA adds the partials up: every thread a strided share, then the fixed shuffle / warp order
+    T part = zero_of(T{});
+    for (int b = t; b < int(gridDim.x); b += 256) part = add(part, ldcg(&p.Pd[b]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part = add(part, shfl_xor(part, o));
+    if ((t & 31) == 0) s_dot[t >> 5] = part;
+    __syncthreads();
     if (t == 0) {
-        T dot = zero_of(T{});
-        for (int b = 0; b < int(gridDim.x); ++b) dot = add(dot, ldcg(&p.Pd[b]));
+        T dot = s_dot[0];
+        for (int w = 1; w < 8; ++w) dot = add(dot, s_dot[w]);
         p.sc->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
         p.d[m] = re(p.u[m]);
         p.e[m - 1] = sc.beta;
@@ -454,9 +699,15 @@ __global__ void __launch_bounds__(256) finish_kernel(const StepParams<T> p)
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    double xp = 0.0;
+    for (int b = t; b < int(gridDim.x); b += 256) xp += __ldcg(&reinterpret_cast<const double*>(p.Pd)[b]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) xp += __shfl_xor_sync(0xffffffffu, xp, o);
+    if ((t & 31) == 0) s_n[t >> 5] = xp;
+    __syncthreads();
     if (t == 0) {
         double x2 = 0.0;
-        for (int b = 0; b < int(gridDim.x); ++b) x2 += __ldcg(&reinterpret_cast<const double*>(p.Pd)[b]);
+        for (int w = 0; w < 8; ++w) x2 += s_n[w];
         if (inext >= 1) {
             StepScalars<T> nx;
             nx.alpha2 = zero_of(T{});
