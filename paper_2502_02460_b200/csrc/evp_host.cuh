@@ -211,6 +211,9 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     // GS_EVP_CHUNK fixes the strip length (128-row blocks per work item: 1, 2 or 4)
     static const bool tma_off = std::getenv("GS_EVP_SYMV") != nullptr && std::atoi(std::getenv("GS_EVP_SYMV")) == 0;
     static const int chunk_env = std::getenv("GS_EVP_CHUNK") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK")) : 0;
+    static const bool merge_off = std::getenv("GS_EVP_MERGE") != nullptr && std::atoi(std::getenv("GS_EVP_MERGE")) == 0;
+    static const int chunk_t = std::getenv("GS_EVP_CHUNK_T") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK_T")) : 4;
+    static const bool fuse_off = std::getenv("GS_EVP_FUSE") != nullptr && std::atoi(std::getenv("GS_EVP_FUSE")) == 0;
     const bool use_tma = !tma_off && (sizeof(T) == 16 || vec) && aligned16(A);
     SymvTmaParams<T> q{};
     int sv_ctas = 0;
@@ -237,17 +240,21 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
         int jp = 0;
         p.itop = itop; p.panel = panel;
         while (i >= 1 && jp < nb) {
-            p.i = i; p.jp = jp; p.mode = 0;
+            // TMA form: the F of the previous column (w, the next u, its norm and scalars) is formed inside this S
+            p.i = i; p.jp = jp; p.mode = 0; p.fuse = (use_tma && !fuse_off && jp > 0) ? 1 : 0;
             const int nJ = (i + TW - 1) / TW, nI = (i + TH - 1) / TH;
             if (use_tma) {
                 // strips of K blocks: the longest that still leaves every persistent CTA about three work items
                 const long long nblocks = (long long)nJ * (nJ + 1) / 2;
-                int K = chunk_env == 1 || chunk_env == 2 || chunk_env == 4 ? chunk_env : (nblocks >= 12LL * sv_ctas ? 4 : nblocks >= 6LL * sv_ctas ? 2 : 1);
+                int K = chunk_env == 1 || chunk_env == 2 || chunk_env == 4 || chunk_env == 8 ? chunk_env : (nblocks >= (long long)chunk_t * sv_ctas ? 4 : nblocks >= (long long)chunk_t * sv_ctas / 2 ? 2 : 1);
                 const int a = nJ / K, r = nJ % K, nitems = K * a * (a + 1) / 2 + r * (a + 1);
                 p.p2_chunk_rows = K * TW;
                 q.s = p; q.chunk_blocks = K; q.dot_ctas = jp > 0 ? nJ : 0;
+                // panel dots: CTAs of their own while there are free slots; otherwise the first streaming CTAs do them
+                const int stream_ctas = std::min(nitems, sv_ctas);
+                q.dots_merged = (q.dot_ctas > 0 && q.dot_ctas + stream_ctas > sv_ctas && q.dot_ctas <= stream_ctas && !merge_off) ? 1 : 0;
                 LaunchTimer timer(plan, L_EVP_SYMV, stream);
-                const cudaError_t le = launch_pdl_smem(symv_tma_kernel<T>, dim3(q.dot_ctas + std::min(nitems, sv_ctas)), dim3(kSvThreads),
+                const cudaError_t le = launch_pdl_smem(symv_tma_kernel<T>, dim3((q.dots_merged ? 0 : q.dot_ctas) + stream_ctas), dim3(kSvThreads),
                                                        SvCfg<T>::kSmemBytes, stream, q);
                 if (le != cudaSuccess) return cuda_fail(plan, le);
                 plan->launches += 1;
@@ -270,7 +277,8 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
                 evp_trace(stream, "combine", i, jp);
             }
             const bool last = (jp == nb - 1) || (i == 1);
-            GS_TRY(finish(i, jp, last ? 2 : 0));
+            if (last) GS_TRY(finish(i, jp, 2));
+            else if (!(use_tma && !fuse_off)) GS_TRY(finish(i, jp, 0));
             --i; ++jp;
         }
         // the panel's rank-2 jp update of the leading (i + 1) x (i + 1) block, then the next column from the updated matrix

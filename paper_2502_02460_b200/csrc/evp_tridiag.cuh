@@ -92,6 +92,33 @@ struct StepScalars {
     int pad[2];
 };
 
+// Householder scalars of a column with off-diagonal part (x, alpha):  H [x; alpha] = [0; beta]  (LAPACK xLARFG
+// without the safmin rescaling loop).
+__device__ __forceinline__ void householder_scalars(double alpha, double xnorm2, StepScalars<double>& sc)
+{
+    sc.xnorm2 = xnorm2;
+    if (xnorm2 == 0.0) { sc.tau = 0.0; sc.s = 0.0; sc.beta = alpha; return; }
+    const double beta = -copysign(sqrt(alpha * alpha + xnorm2), alpha);
+    sc.beta = beta;
+    sc.tau = (beta - alpha) / beta;
+    sc.s = 1.0 / (alpha - beta);
+}
+__device__ __forceinline__ void householder_scalars(double2 alpha, double xnorm2, StepScalars<double2>& sc)
+{
+    sc.xnorm2 = xnorm2;
+    if (xnorm2 == 0.0 && alpha.y == 0.0) { sc.tau = make_double2(0.0, 0.0); sc.s = make_double2(0.0, 0.0); sc.beta = alpha.x; return; }
+    const double beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
+    sc.beta = beta;
+    sc.tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
+    const double dr = alpha.x - beta, di = alpha.y, den = dr * dr + di * di;     // 1 / (alpha - beta)
+    sc.s = make_double2(dr / den, -di / den);
+}
+
+// the scalars of step i live in sc[i & 1]: a launch that derives the next step's scalars (F, or S with F fused in)
+// writes the other slot while its own CTAs may still be reading the current one
+template <typename T> struct StepParams;
+template <typename T> __device__ __forceinline__ StepScalars<T>* sc_of(const StepParams<T>& p, int step);
+
 constexpr int kSymvThreads = 256;
 constexpr int kSymvTW = 128;                        // tile width (columns): 8 warps x 16 columns
 template <typename T> struct SymvGeom { static constexpr int RPT = 32 / int(sizeof(T)); static constexpr int TH = 32 * RPT; };
@@ -127,7 +154,53 @@ struct StepParams {
     int panel;            // panel number (block of R)
     int mode;             // F: 0 = lazy next column (stale A + panel corrections), 1 = fresh (A is up to date), 2 = none
     int p2_chunk_rows;    // rows of A one P2 partial covers: TH (symv_kernel) or chunk_blocks * 128 (symv_tma_kernel)
+    int fuse;             // symv_tma_kernel: the previous step's F (mode 0) is formed inside this launch (u_next_value)
     const int* info;
+};
+
+template <typename T> __device__ __forceinline__ StepScalars<T>* sc_of(const StepParams<T>& p, int step) { return p.sc + (step & 1); }
+
+// ---- F (mode 0) inside S: the next column, formed wherever it is needed -------------------------------------
+// With io = p.i + 1 the step just combined (panel column jpo = p.jp - 1) and sc its scalars:
+//   w(r) = tau w'(r) + alpha2 v(r),   u(r) = A(r, p.i) - corr2(r) - v(r) conj(w(io-1)) - w(r) conj(v(io-1)),  r <= p.i.
+// Every operation is an explicit intrinsic (no contraction left to the compiler), so the CTAs that store u and
+// those that only use it get the same bits.
+__device__ __forceinline__ double fx_mul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double2 fx_mul(double2 a, double2 b)
+{
+    return make_double2(__fma_rn(-a.y, b.y, __dmul_rn(a.x, b.x)), __fma_rn(a.y, b.x, __dmul_rn(a.x, b.y)));
+}
+__device__ __forceinline__ double fx_add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double2 fx_add(double2 a, double2 b) { return make_double2(__dadd_rn(a.x, b.x), __dadd_rn(a.y, b.y)); }
+__device__ __forceinline__ double fx_sub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double2 fx_sub(double2 a, double2 b) { return make_double2(__dsub_rn(a.x, b.x), __dsub_rn(a.y, b.y)); }
+
+template <typename T>
+struct FusedF {
+    T tau, alpha2, cwlast, cvlast;      // conj(w(io-1)), conj(v(io-1))
+    int jpo;
+    __device__ __forceinline__ void init(const StepParams<T>& p)
+    {
+        const StepScalars<T> sc = *sc_of(p, p.i + 1);
+        tau = sc.tau; alpha2 = sc.alpha2; jpo = p.jp - 1;
+        const T vlast = cj(p.Vt[jpo + (long long)p.i * p.nb]);
+        const T wlast = fx_add(fx_mul(tau, p.wp[p.i]), fx_mul(alpha2, vlast));
+        cwlast = cj(wlast); cvlast = cj(vlast);
+    }
+    __device__ __forceinline__ T w_of(const StepParams<T>& p, int r, T& v) const
+    {
+        v = cj(p.Vt[jpo + (long long)r * p.nb]);
+        return fx_add(fx_mul(tau, p.wp[r]), fx_mul(alpha2, v));
+    }
+    __device__ __forceinline__ T u_of(const StepParams<T>& p, int r, T* w_out = nullptr) const
+    {
+        T v;
+        const T w = w_of(p, r, v);
+        T un = fx_sub(fx_sub(fx_sub(p.A[r + (long long)p.i * p.ld], p.corr2[r]), fx_mul(v, cwlast)), fx_mul(w, cvlast));
+        if (r == p.i) un = real_only(un);
+        if (w_out != nullptr) *w_out = w;
+        return un;
+    }
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -136,18 +209,54 @@ struct StepParams {
 // the last CTA to arrive finalises tW' = s (W^H u - beta Wt[:, i-1]), tV' likewise, and the new column of
 // M^H = conj(D) + striu(V^H V).  sm: 512 elements of shared memory.
 // ---------------------------------------------------------------------------------------------------------
+// bar_id == 0: every thread of the CTA calls (__syncthreads); otherwise the first nthr threads call and meet at
+// named barrier bar_id.
+__device__ __forceinline__ void cta_or_named_sync(int bar_id, int nthr)
+{
+    if (bar_id == 0) __syncthreads(); else named_bar_sync(bar_id, nthr);
+}
+
 template <typename T>
-__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last)
+__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last, int bar_id = 0, int nthr = 0)
 {
     constexpr int TW = kSymvTW;
     const int m = p.i, jp = p.jp, nb = p.nb;
     const int t = threadIdx.x;
     if (jp == 0) return;
     const int r0 = x * TW, r1 = min(r0 + TW, m);
+    if (p.fuse) {
+        // F of the previous step for the rows of this chunk (the last chunk also takes row m, the new diagonal entry):
+        // column jp-1 of W, the next column u, the partial of ||u(0 : m-2)||^2; rows >= io of the reflector column io = 0
+        FusedF<T> ff;
+        ff.init(p);
+        const int io = m + 1;
+        double nrm = 0.0;
+        const int r = (t < TW) ? r0 + t : ((t == TW && x == nx - 1) ? m : -1);
+        if (r >= 0 && (r < r1 || r == m)) {
+            T w;
+            const T un = ff.u_of(p, r, &w);
+            p.Wt[ff.jpo + (long long)r * nb] = cj(w);
+            p.u[r] = un;
+            if (r < m - 1) nrm = abs2(un);
+        }
+        for (int rz = io + x * kSymvThreads + t; rz < p.N && t < kSymvThreads; rz += nx * kSymvThreads) p.A[rz + (long long)io * p.ld] = zero_of(T{});
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+        double* sn = reinterpret_cast<double*>(sm);
+        if ((t & 31) == 0) sn[t >> 5] = nrm;
+        cta_or_named_sync(bar_id, nthr);
+        if (t == 0) {
+            double sum = 0.0;
+            for (int w = 0; w < (bar_id == 0 ? int(blockDim.x) : nthr) / 32; ++w) sum += sn[w];
+            reinterpret_cast<double*>(p.Pd)[x] = sum;
+        }
+        cta_or_named_sync(bar_id, nthr);      // the chunk's u and column jp-1 of Wt are read back below; sm is reused
+    }
     const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
     const int c = t % nb, g = t / nb;
     T aw = zero_of(T{}), av = zero_of(T{});
     if (t < kSymvThreads && c < jp) {
+#pragma unroll 8
         for (int r = r0 + g; r < r1; r += groups) {
             const T ur = p.u[r];
             aw = fmad(p.Wt[c + (long long)r * nb], ur, aw);
@@ -155,7 +264,7 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         }
     }
     if (t < kSymvThreads) { sm[t] = aw; sm[kSymvThreads + t] = av; }
-    __syncthreads();
+    cta_or_named_sync(bar_id, nthr);
     if (t < nb) {
         T sw = zero_of(T{}), sv = zero_of(T{});
         for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
@@ -163,13 +272,30 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         p.Pt[(long long)x * 2 * nb + nb + t] = sv;
     }
     __threadfence();
-    __syncthreads();
+    cta_or_named_sync(bar_id, nthr);
     if (t == 0) *s_last = (atomicAdd(&p.tickets[0], 1u) == unsigned(nx - 1)) ? 1u : 0u;
-    __syncthreads();
+    cta_or_named_sync(bar_id, nthr);
     if (!*s_last) return;
     __threadfence();
+    if (p.fuse) {
+        // the scalars of this step from the norm of the new column (F's finaliser)
+        if (t < 32) {
+            double x2 = 0.0;
+            for (int b = t; b < nx; b += 32) x2 += __ldcg(&reinterpret_cast<const double*>(p.Pd)[b]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x2 += __shfl_xor_sync(0xffffffffu, x2, o);
+            if (t == 0) {
+                StepScalars<T> nx_sc;
+                nx_sc.alpha2 = zero_of(T{});
+                householder_scalars(ldcg(&p.u[m - 1]), x2, nx_sc);
+                nx_sc.pad[0] = nx_sc.pad[1] = 0;
+                *sc_of(p, m) = nx_sc;
+            }
+        }
+        cta_or_named_sync(bar_id, nthr);
+    }
     // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
-    const StepScalars<T> sc = *p.sc;
+    const StepScalars<T> sc = *sc_of(p, m);
     if (t < 2 * nb) {
         const int cc = t % nb;
         const bool isV = t >= nb;
@@ -305,11 +431,13 @@ constexpr int kSvConsumerWarps = 8;
 constexpr int kSvThreads = (kSvConsumerWarps + 1) * 32;
 constexpr int kSvRedBytes = 2 * kSvConsumerWarps * 1024;   // two buffers of 8 warps x TH elements
 constexpr int kSvUcolBytes = 2 * kSymvTW * 16;             // u over the column block, two work items
+constexpr int kSvUrowBytes = 2 * 1024;                     // u over the rows of a tile (TH elements), two tiles
 // real: 16 column sums = 32 registers -> two CTAs of 5 stages per SM; complex: 64 registers -> one CTA of 10 stages
 template <typename T> struct SvCfg {
     static constexpr int kStages = sizeof(T) == 8 ? 5 : 10;
     static constexpr int kCtasPerSm = sizeof(T) == 8 ? 2 : 1;
-    static constexpr int kSmemBytes = kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + 256 /*barriers*/ + 1024 /*alignment*/;
+    static constexpr int kMaxRegs = sizeof(T) == 8 ? 112 : 224;      // 65536 / (kCtasPerSm * 288 threads), in units of 8
+    static constexpr int kSmemBytes = kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + kSvUrowBytes + 256 /*barriers*/ + 1024 /*alignment*/;
 };
 
 template <typename T>
@@ -317,7 +445,8 @@ struct SymvTmaParams {
     StepParams<T> s;
     CUtensorMap mapA;     // A as an (N * sizeof(T)/8) x N FP64 tensor; box = 128 doubles (TH rows) x 16 columns, no swizzle
     int chunk_blocks;     // 128-row blocks per work item (1, 2 or 4)
-    int dot_ctas;         // leading CTAs that form the panel dots (0 when the panel is empty)
+    int dot_ctas;         // number of panel-dot chunks (0 when the panel is empty): leading CTAs of their own, or
+    int dots_merged;      // (merged) work the first dot_ctas streaming CTAs do before their tiles
 };
 
 // number of work items in the column blocks j < J:  sum_{j<J} ceil((j + 1) / K)
@@ -344,7 +473,7 @@ __device__ __forceinline__ T sv_transpose_reduce(const T (&v)[16], int lane)
 }
 
 template <typename T>
-__global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
+__global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
 {
     constexpr int kSvStages = SvCfg<T>::kStages;
     constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW, H = RPT / 2;
@@ -356,12 +485,15 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     unsigned char* stages = smem;
     T* red = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes);
     T* ucol = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes + kSvRedBytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes);
-    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + kSvStages);
+    T* urow = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + kSvUrowBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + kSvStages), qfull0 = smem_u32(bars + 2 * kSvStages);
+    volatile int* item_q = reinterpret_cast<volatile int*>(bars + 2 * kSvStages + 4);
     __shared__ unsigned int s_last;
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     if (t == 0) {
         for (int s = 0; s < kSvStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kSvConsumerWarps); }
+        for (int s = 0; s < 4; ++s) mbar_init(qfull0 + 8 * s, 1);
         mbar_fence_init();
         tma_prefetch_desc(&q.mapA);
     }
@@ -370,11 +502,12 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     grid_dep_wait();
     if (*p.info != 0) return;
     const int m = p.i;
-    if (int(blockIdx.x) < q.dot_ctas) {
+    if (!q.dots_merged && int(blockIdx.x) < q.dot_ctas) {
         panel_dots(p, int(blockIdx.x), q.dot_ctas, red, &s_last);
         return;
     }
-    const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
+    const int lead = q.dots_merged ? 0 : q.dot_ctas;
+    const int cta = int(blockIdx.x) - lead, G = int(gridDim.x) - lead;
     const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH, K = q.chunk_blocks;
     const int nitems = sv_items_before(nJ, K);
 
@@ -391,11 +524,20 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
         I1 = min(min((qq + 1) * K * R, (J + 1) * R), nI);
     };
 
+    // Work items: the first one of a CTA is its own index, the rest comes from a global counter (tickets[3], reset by
+    // the C kernel that follows), so the CTAs that also form panel dots simply take fewer items.  The producer lane
+    // hands every item to the consumers through a four-slot queue in shared memory (the producer is never more than
+    // one item ahead: the stage ring holds less than a tile).
     if (warp == kSvConsumerWarps) {
-        // ---- producer: one lane streams every stage of every tile of this CTA's items ----
+        // ---- producer: one lane streams every stage of every tile of the CTA's items ----
         if (lane == 0) {
             uint32_t cnt = 0;
-            for (int item = cta; item < nitems; item += G) {
+            int item = cta;
+            for (int nq = 0;; ++nq) {
+                item_q[nq & 3] = item < nitems ? item : -1;
+                mbar_arrive(qfull0 + 8 * (nq & 3));
+                if (item >= nitems) break;
+                const int next = G + int(atomicAdd(p.tickets + 3, 1u));
                 int J, I0, I1;
                 decode(item, J, I0, I1);
                 for (int I = I0; I < I1; ++I) {
@@ -406,6 +548,7 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
                         tma_load_2d(smem_u32(stages + stage * kSvStageBytes), &q.mapA, I * TH * W8, J * TW + 16 * s, full0 + 8 * stage);
                     }
                 }
+                item = next;
             }
         }
         return;
@@ -413,27 +556,36 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
 
     // ---- consumers: warp w owns columns 2w, 2w+1 of every stage; lane l owns rows {l H .. l H + H-1} of each half tile ----
     auto row_of = [&](int k) { return (k / H) * (TH / 2) + lane * H + (k % H); };
-    auto load_u_rows = [&](int I, T (&dst)[RPT]) {
-#pragma unroll
-        for (int k = 0; k < RPT; ++k) {
-            const int r = I * TH + row_of(k);
-            dst[k] = (r < m) ? p.u[r] : zero_of(T{});
-        }
-    };
+    // merged form (every CTA slot is taken by a streaming CTA): the first dot_ctas CTAs form their panel-dot chunk
+    // here, while their producer warp is already filling the ring
+    if (q.dots_merged && cta < q.dot_ctas) panel_dots(p, cta, q.dot_ctas, red, &s_last, 3, kSvConsumerWarps * 32);
+    // u(r): stored by F, or (fuse) formed here from the previous step's vectors
+    FusedF<T> ff;
+    if (p.fuse) ff.init(p);
+    auto u_val = [&](int r) -> T { return (r < m) ? (p.fuse ? ff.u_of(p, r) : p.u[r]) : zero_of(T{}); };
     uint32_t cnt = 0;
     int nitem = 0, ntile = 0;
-    for (int item = cta; item < nitems; item += G, ++nitem) {
+    for (;; ++nitem) {
+        mbar_wait(qfull0 + 8 * (nitem & 3), (nitem >> 2) & 1);
+        const int item = item_q[nitem & 3];
+        if (item < 0) break;
         int J, I0, I1;
         decode(item, J, I0, I1);
         T* uc = ucol + (nitem & 1) * TW;
-        if (t < TW) { const int c = J * TW + t; uc[t] = (c < m) ? p.u[c] : zero_of(T{}); }
+        if (t < TW) uc[t] = u_val(J * TW + t);
+        if (t < TH) urow[(ntile & 1) * TH + t] = u_val(I0 * TH + t);
         named_bar_sync(1, kSvConsumerWarps * 32);
         T yc[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) yc[i] = zero_of(T{});
-        T ur[RPT];
         for (int I = I0; I < I1; ++I, ++ntile) {
-            load_u_rows(I, ur);
+            // the next tile's rows of u: loaded now, parked in shared memory before this tile's barrier
+            T unext = zero_of(T{});
+            const bool prefetch = (I + 1 < I1) && t < TH;
+            if (prefetch) unext = u_val((I + 1) * TH + t);
+            T ur[RPT];
+#pragma unroll
+            for (int k = 0; k < RPT; ++k) ur[k] = urow[(ntile & 1) * TH + row_of(k)];
             T yr[RPT];
 #pragma unroll
             for (int k = 0; k < RPT; ++k) yr[k] = zero_of(T{});
@@ -487,6 +639,7 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
             T* rb = red + ((ntile & 1) * kSvConsumerWarps + warp) * TH;
 #pragma unroll
             for (int k = 0; k < RPT; ++k) rb[row_of(k)] = yr[k];
+            if (prefetch) urow[((ntile + 1) & 1) * TH + t] = unext;
             named_bar_sync(2, kSvConsumerWarps * 32);
             if (t < TH) {
                 const T* rr = red + (ntile & 1) * kSvConsumerWarps * TH + t;
@@ -507,28 +660,6 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     }
 }
 
-// Householder scalars of a column with off-diagonal part (x, alpha):  H [x; alpha] = [0; beta]  (LAPACK xLARFG
-// without the safmin rescaling loop).
-__device__ __forceinline__ void householder_scalars(double alpha, double xnorm2, StepScalars<double>& sc)
-{
-    sc.xnorm2 = xnorm2;
-    if (xnorm2 == 0.0) { sc.tau = 0.0; sc.s = 0.0; sc.beta = alpha; return; }
-    const double beta = -copysign(sqrt(alpha * alpha + xnorm2), alpha);
-    sc.beta = beta;
-    sc.tau = (beta - alpha) / beta;
-    sc.s = 1.0 / (alpha - beta);
-}
-__device__ __forceinline__ void householder_scalars(double2 alpha, double xnorm2, StepScalars<double2>& sc)
-{
-    sc.xnorm2 = xnorm2;
-    if (xnorm2 == 0.0 && alpha.y == 0.0) { sc.tau = make_double2(0.0, 0.0); sc.s = make_double2(0.0, 0.0); sc.beta = alpha.x; return; }
-    const double beta = -copysign(sqrt(alpha.x * alpha.x + alpha.y * alpha.y + xnorm2), alpha.x);
-    sc.beta = beta;
-    sc.tau = make_double2((beta - alpha.x) / beta, -alpha.y / beta);
-    const double dr = alpha.x - beta, di = alpha.y, den = dr * dr + di * di;     // 1 / (alpha - beta)
-    sc.s = make_double2(dr / den, -di / den);
-}
-
 // ---------------------------------------------------------------------------------------------------------
 // C: per row r < m = i (32 rows per CTA, 8 threads per row):
 //   y      = sum of the partials of S
@@ -547,8 +678,9 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     if (*p.info != 0) return;
     const int m = p.i, jp = p.jp, nb = p.nb;
     const int t = threadIdx.x, l8 = t & 7, rr = t >> 3;
+    if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
     const int r = blockIdx.x * kCombineRows + rr;
-    const StepScalars<T> sc = *p.sc;
+    const StepScalars<T> sc = *sc_of(p, m);
     __shared__ T s_t[2 * 128];           // tW', tV'
     __shared__ T s_row[2 * 128];         // Wt[:, i-1], Vt[:, i-1]
     __shared__ T s_dot[8];
@@ -619,7 +751,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     if (t == 0) {
         T dot = s_dot[0];
         for (int w = 1; w < 8; ++w) dot = add(dot, s_dot[w]);
-        p.sc->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
+        sc_of(p, m)->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
         p.d[m] = re(p.u[m]);
         p.e[m - 1] = sc.beta;
         p.tau[m] = sc.tau;
@@ -650,7 +782,8 @@ __global__ void __launch_bounds__(256) finish_kernel(const StepParams<T> p)
     if (*p.info != 0) return;
     const int i = p.i, inext = i - 1, jp = p.jp, nb = p.nb, mode = p.mode;
     const int t = threadIdx.x;
-    const StepScalars<T> sc = *p.sc;
+    if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
+    const StepScalars<T> sc = *sc_of(p, i);          // (mode 1: not used)
     __shared__ double s_n[8];
     __shared__ unsigned int s_last;
     T wlast = zero_of(T{}), vlast = zero_of(T{});
@@ -713,7 +846,7 @@ __global__ void __launch_bounds__(256) finish_kernel(const StepParams<T> p)
             nx.alpha2 = zero_of(T{});
             householder_scalars(ldcg(&p.u[inext - 1]), x2, nx);
             nx.pad[0] = nx.pad[1] = 0;
-            *p.sc = nx;
+            *sc_of(p, inext) = nx;
         } else {
             p.d[0] = re(ldcg(&p.u[0]));
             p.tau[0] = zero_of(T{});
