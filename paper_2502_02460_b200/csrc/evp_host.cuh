@@ -168,6 +168,9 @@ inline cudaError_t configure_symv(int* sms)
     cudaError_t e = once.run([]() -> cudaError_t {
         cudaError_t r = cudaFuncSetAttribute(symv_tma_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, SvCfg<double>::kSmemBytes);
         if (r == cudaSuccess) r = cudaFuncSetAttribute(symv_tma_kernel<double2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SvCfg<double2>::kSmemBytes);
+        // two CTAs of the real kernel share an SM only if the whole shared-memory carve-out is granted
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(symv_tma_kernel<double>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (r == cudaSuccess) r = cudaFuncSetAttribute(symv_tma_kernel<double2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         return r;
     });
     if (e != cudaSuccess) return e;
@@ -211,7 +214,6 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     // GS_EVP_CHUNK fixes the strip length (128-row blocks per work item: 1, 2 or 4)
     static const bool tma_off = std::getenv("GS_EVP_SYMV") != nullptr && std::atoi(std::getenv("GS_EVP_SYMV")) == 0;
     static const int chunk_env = std::getenv("GS_EVP_CHUNK") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK")) : 0;
-    static const bool merge_off = std::getenv("GS_EVP_MERGE") != nullptr && std::atoi(std::getenv("GS_EVP_MERGE")) == 0;
     static const int chunk_t = std::getenv("GS_EVP_CHUNK_T") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK_T")) : 4;
     static const bool fuse_off = std::getenv("GS_EVP_FUSE") != nullptr && std::atoi(std::getenv("GS_EVP_FUSE")) == 0;
     const bool use_tma = !tma_off && (sizeof(T) == 16 || vec) && aligned16(A);
@@ -220,7 +222,8 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     if (use_tma) {
         int sms = 0;
         GS_CUDA(plan, configure_symv(&sms));
-        sv_ctas = sms * SvCfg<T>::kCtasPerSm;
+        static const int ctas_env = std::getenv("GS_EVP_CTAS") != nullptr ? std::atoi(std::getenv("GS_EVP_CTAS")) : 0;
+        sv_ctas = sms * (ctas_env > 0 ? ctas_env : SvCfg<T>::kCtasPerSm);
         if (!make_symv_map(&q.mapA, A, N, int(sizeof(T) / 8))) return GS_ERR_CUDA;
     }
     const int fgrid = std::max(1, std::min(64, (N + 255) / 256));
@@ -250,11 +253,9 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
                 const int a = nJ / K, r = nJ % K, nitems = K * a * (a + 1) / 2 + r * (a + 1);
                 p.p2_chunk_rows = K * TW;
                 q.s = p; q.chunk_blocks = K; q.dot_ctas = jp > 0 ? nJ : 0;
-                // panel dots: CTAs of their own while there are free slots; otherwise the first streaming CTAs do them
                 const int stream_ctas = std::min(nitems, sv_ctas);
-                q.dots_merged = (q.dot_ctas > 0 && q.dot_ctas + stream_ctas > sv_ctas && q.dot_ctas <= stream_ctas && !merge_off) ? 1 : 0;
                 LaunchTimer timer(plan, L_EVP_SYMV, stream);
-                const cudaError_t le = launch_pdl_smem(symv_tma_kernel<T>, dim3((q.dots_merged ? 0 : q.dot_ctas) + stream_ctas), dim3(kSvThreads),
+                const cudaError_t le = launch_pdl_smem(symv_tma_kernel<T>, dim3(q.dot_ctas + stream_ctas), dim3(kSvThreads),
                                                        SvCfg<T>::kSmemBytes, stream, q);
                 if (le != cudaSuccess) return cuda_fail(plan, le);
                 plan->launches += 1;

@@ -209,15 +209,8 @@ struct FusedF {
 // the last CTA to arrive finalises tW' = s (W^H u - beta Wt[:, i-1]), tV' likewise, and the new column of
 // M^H = conj(D) + striu(V^H V).  sm: 512 elements of shared memory.
 // ---------------------------------------------------------------------------------------------------------
-// bar_id == 0: every thread of the CTA calls (__syncthreads); otherwise the first nthr threads call and meet at
-// named barrier bar_id.
-__device__ __forceinline__ void cta_or_named_sync(int bar_id, int nthr)
-{
-    if (bar_id == 0) __syncthreads(); else named_bar_sync(bar_id, nthr);
-}
-
 template <typename T>
-__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last, int bar_id = 0, int nthr = 0)
+__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last)
 {
     constexpr int TW = kSymvTW;
     const int m = p.i, jp = p.jp, nb = p.nb;
@@ -244,13 +237,13 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
         double* sn = reinterpret_cast<double*>(sm);
         if ((t & 31) == 0) sn[t >> 5] = nrm;
-        cta_or_named_sync(bar_id, nthr);
+        __syncthreads();
         if (t == 0) {
             double sum = 0.0;
-            for (int w = 0; w < (bar_id == 0 ? int(blockDim.x) : nthr) / 32; ++w) sum += sn[w];
+            for (int w = 0; w < int(blockDim.x) / 32; ++w) sum += sn[w];
             reinterpret_cast<double*>(p.Pd)[x] = sum;
         }
-        cta_or_named_sync(bar_id, nthr);      // the chunk's u and column jp-1 of Wt are read back below; sm is reused
+        __syncthreads();      // the chunk's u and column jp-1 of Wt are read back below; sm is reused
     }
     const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
     const int c = t % nb, g = t / nb;
@@ -264,7 +257,7 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         }
     }
     if (t < kSymvThreads) { sm[t] = aw; sm[kSymvThreads + t] = av; }
-    cta_or_named_sync(bar_id, nthr);
+    __syncthreads();
     if (t < nb) {
         T sw = zero_of(T{}), sv = zero_of(T{});
         for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
@@ -272,9 +265,9 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         p.Pt[(long long)x * 2 * nb + nb + t] = sv;
     }
     __threadfence();
-    cta_or_named_sync(bar_id, nthr);
+    __syncthreads();
     if (t == 0) *s_last = (atomicAdd(&p.tickets[0], 1u) == unsigned(nx - 1)) ? 1u : 0u;
-    cta_or_named_sync(bar_id, nthr);
+    __syncthreads();
     if (!*s_last) return;
     __threadfence();
     if (p.fuse) {
@@ -292,7 +285,7 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
                 *sc_of(p, m) = nx_sc;
             }
         }
-        cta_or_named_sync(bar_id, nthr);
+        __syncthreads();
     }
     // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
     const StepScalars<T> sc = *sc_of(p, m);
@@ -436,7 +429,6 @@ constexpr int kSvUrowBytes = 2 * 1024;                     // u over the rows of
 template <typename T> struct SvCfg {
     static constexpr int kStages = sizeof(T) == 8 ? 5 : 10;
     static constexpr int kCtasPerSm = sizeof(T) == 8 ? 2 : 1;
-    static constexpr int kMaxRegs = sizeof(T) == 8 ? 112 : 224;      // 65536 / (kCtasPerSm * 288 threads), in units of 8
     static constexpr int kSmemBytes = kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + kSvUrowBytes + 256 /*barriers*/ + 1024 /*alignment*/;
 };
 
@@ -445,8 +437,7 @@ struct SymvTmaParams {
     StepParams<T> s;
     CUtensorMap mapA;     // A as an (N * sizeof(T)/8) x N FP64 tensor; box = 128 doubles (TH rows) x 16 columns, no swizzle
     int chunk_blocks;     // 128-row blocks per work item (1, 2 or 4)
-    int dot_ctas;         // number of panel-dot chunks (0 when the panel is empty): leading CTAs of their own, or
-    int dots_merged;      // (merged) work the first dot_ctas streaming CTAs do before their tiles
+    int dot_ctas;         // leading CTAs that form the panel dots (0 when the panel is empty)
 };
 
 // number of work items in the column blocks j < J:  sum_{j<J} ceil((j + 1) / K)
@@ -473,7 +464,7 @@ __device__ __forceinline__ T sv_transpose_reduce(const T (&v)[16], int lane)
 }
 
 template <typename T>
-__global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
+__global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
 {
     constexpr int kSvStages = SvCfg<T>::kStages;
     constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW, H = RPT / 2;
@@ -502,12 +493,11 @@ __global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) sy
     grid_dep_wait();
     if (*p.info != 0) return;
     const int m = p.i;
-    if (!q.dots_merged && int(blockIdx.x) < q.dot_ctas) {
+    if (int(blockIdx.x) < q.dot_ctas) {
         panel_dots(p, int(blockIdx.x), q.dot_ctas, red, &s_last);
         return;
     }
-    const int lead = q.dots_merged ? 0 : q.dot_ctas;
-    const int cta = int(blockIdx.x) - lead, G = int(gridDim.x) - lead;
+    const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
     const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH, K = q.chunk_blocks;
     const int nitems = sv_items_before(nJ, K);
 
@@ -525,7 +515,7 @@ __global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) sy
     };
 
     // Work items: the first one of a CTA is its own index, the rest comes from a global counter (tickets[3], reset by
-    // the C kernel that follows), so the CTAs that also form panel dots simply take fewer items.  The producer lane
+    // the C kernel that follows), so the CTAs that start late (behind the panel-dot CTAs) simply take fewer items.  The producer lane
     // hands every item to the consumers through a four-slot queue in shared memory (the producer is never more than
     // one item ahead: the stage ring holds less than a tile).
     if (warp == kSvConsumerWarps) {
@@ -556,9 +546,6 @@ __global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) sy
 
     // ---- consumers: warp w owns columns 2w, 2w+1 of every stage; lane l owns rows {l H .. l H + H-1} of each half tile ----
     auto row_of = [&](int k) { return (k / H) * (TH / 2) + lane * H + (k % H); };
-    // merged form (every CTA slot is taken by a streaming CTA): the first dot_ctas CTAs form their panel-dot chunk
-    // here, while their producer warp is already filling the ring
-    if (q.dots_merged && cta < q.dot_ctas) panel_dots(p, cta, q.dot_ctas, red, &s_last, 3, kSvConsumerWarps * 32);
     // u(r): stored by F, or (fuse) formed here from the previous step's vectors
     FusedF<T> ff;
     if (p.fuse) ff.init(p);
@@ -661,14 +648,15 @@ __global__ void __launch_bounds__(kSvThreads) __maxnreg__(SvCfg<T>::kMaxRegs) sy
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// C: per row r < m = i (32 rows per CTA, 8 threads per row):
+// C: per row r < m = i (16 rows per CTA, 16 threads per row):
 //   y      = sum of the partials of S
 //   v(r)   = s (u(r) - beta [r == i-1])                       -> Vt[jp, r] = conj(v), A(r, i) = v   (clean reflector)
 //   w'(r)  = s (y - beta A(r, i-1)) - sum_c ( V(r,c) tW'(c) + W(r,c) tV'(c) )
 //   corr2  = sum_c ( V(r,c) conj(W(i-1,c)) + W(r,c) conj(V(i-1,c)) )     (old panel columns of the next lazy update)
 //   partial of w'^H v; the last CTA sets alpha2 = -1/2 |tau|^2 (w'^H v) and records d(i), e(i-1), tau(i).
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kCombineRows = 32;
+constexpr int kCombineTPR = 16;                       // threads per row
+constexpr int kCombineRows = 256 / kCombineTPR;
 template <typename T>
 __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
 {
@@ -677,7 +665,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     grid_dep_wait();
     if (*p.info != 0) return;
     const int m = p.i, jp = p.jp, nb = p.nb;
-    const int t = threadIdx.x, l8 = t & 7, rr = t >> 3;
+    const int t = threadIdx.x, l8 = t % kCombineTPR, rr = t / kCombineTPR;
     if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
     const int r = blockIdx.x * kCombineRows + rr;
     const StepScalars<T> sc = *sc_of(p, m);
@@ -696,11 +684,14 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     if (r < m) {
         // y(r): P1[J][r] for J >= r / TW, P2[I][r] for I <= r / TH
         const int nJ = (m + TW - 1) / TW;
-        for (int J = r / TW + l8; J < nJ; J += 8) y = add(y, p.P1[(long long)J * p.ldp + r]);
-        for (int I = l8; I <= r / p.p2_chunk_rows; I += 8) y = add(y, p.P2[(long long)I * p.ldp + r]);
+#pragma unroll 4
+        for (int J = r / TW + l8; J < nJ; J += kCombineTPR) y = add(y, p.P1[(long long)J * p.ldp + r]);
+#pragma unroll 2
+        for (int I = l8; I <= r / p.p2_chunk_rows; I += kCombineTPR) y = add(y, p.P2[(long long)I * p.ldp + r]);
         const T* vt = p.Vt + (long long)r * nb;
         const T* wt = p.Wt + (long long)r * nb;
-        for (int c = l8; c < jp; c += 8) {
+#pragma unroll 4
+        for (int c = l8; c < jp; c += kCombineTPR) {
             const T vrc = cj(vt[c]), wrc = cj(wt[c]);             // V(r,c), W(r,c)
             c1 = fmad(vrc, s_t[c], c1);
             c1 = fmad(wrc, s_t[nb + c], c1);
@@ -708,9 +699,9 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
             c2 = fmad(wrc, s_row[nb + c], c2);
         }
     }
-    // (all 32 lanes take part in the shuffles: a warp holds four rows, some of which may lie beyond m)
+    // (all 32 lanes take part in the shuffles: a warp holds several rows, some of which may lie beyond m)
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) { y = add(y, shfl_xor(y, o)); c1 = add(c1, shfl_xor(c1, o)); c2 = add(c2, shfl_xor(c2, o)); }
+    for (int o = kCombineTPR / 2; o > 0; o >>= 1) { y = add(y, shfl_xor(y, o)); c1 = add(c1, shfl_xor(c1, o)); c2 = add(c2, shfl_xor(c2, o)); }
     if (r < m) {
         if (l8 == 0) {
             const T ur = p.u[r];
