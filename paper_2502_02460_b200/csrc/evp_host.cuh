@@ -26,10 +26,12 @@ struct EvpLayout {
     }
 };
 
+constexpr int kBackSplit = 3;   // the back-transformation forms Y = Vp^H C~ (one tile row, long k) in this many k-ranges
+
 struct EvpBuffers {
     // tridiagonalisation
     unsigned int* tickets; void* sc;
-    void *u, *wp, *corr2, *tfin, *Pd, *Vt, *Wt, *Pt, *P1, *P2, *R, *Rinv, *Y, *Y2;
+    void *u, *wp, *corr2, *tfin, *Pd, *Vt, *Wt, *Pt, *P1, *P2, *R, *Rinv, *Y, *Y2, *Ypart;
     long long ldp;
     int nb, npanels;
     // results kept for gs_standard_eigh
@@ -66,6 +68,7 @@ EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes, int64
     b.P1 = takeb(nJ * size_t(b.ldp)); b.P2 = takeb(nI * size_t(b.ldp));
     b.R = takeb(size_t(b.npanels) * nb * (nb + 1)); b.Rinv = takeb(size_t(b.npanels) * nb * (nb + 1));
     b.Y = takeb(size_t(nb) * (nev + 2)); b.Y2 = takeb(size_t(nb) * (nev + 2));
+    b.Ypart = takeb(size_t(kBackSplit) * nb * (((nev + size_t(nb) - 1) / nb) * nb + 2));   // split-k partials of Y, padded to whole tiles
     b.Z = L.take<double>(N * (nev > 0 ? nev : 1));
     DcArrays& a = b.dc;
     a.ldq = b.ldq;
@@ -322,6 +325,7 @@ gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const voi
     if (N < 2) return GS_OK;
     Stage st = make_stage(plan, stream);
     const int lb = st.lb, bk = st.bk;
+    static const bool back_split_off = std::getenv("GS_EVP_BACK_SPLIT") != nullptr && std::atoi(std::getenv("GS_EVP_BACK_SPLIT")) == 0;
     const int npan = (N - 1 + nb - 1) / nb;           // reflectors i = 1 .. N-1 in panels counted from the top
     const int tn = (nev + lb - 1) / lb;
     for (int pnl = npan - 1; pnl >= 0; --pnl) {
@@ -335,16 +339,35 @@ gs_status_t evp_backtransform_impl(gs_plan* plan, const EvpBuffers& b, const voi
         const MatView vA{A, m, i0 + cnt, N}, vC{Ct, m, nev, N};
         const MatView vY{b.Y, cnt, nev, nb}, vY2{b.Y2, cnt, nev, nb};
         const MatView vR{static_cast<const unsigned char*>(b.Rinv) + size_t(pnl) * nb * (nb + 1) * plan->es, nb, nb, nb};
-        {   // Y = Vp^H C~
+        {   // Y = Vp^H C~: ONE row of tiles with a k-extent of m -- too few CTAs for the device, so the k-range is split
+            // into kBackSplit batches (partials side by side in Ypart, summed in a fixed order by sum_parts_kernel)
+            const int ksteps = (m + bk - 1) / bk;
+            const int split = (back_split_off || ksteps < 8 * kBackSplit) ? 1 : kBackSplit;
+            const int kc = (ksteps + split - 1) / split;
+            const int ldpart = tn * lb;               // columns of one partial (whole tiles)
             EngineParams p = blank_params(plan);
             if (!set_operand(st, p, 0, vA, false) || !set_operand(st, p, 1, vC, false)) return GS_ERR_CUDA;
-            p.C = static_cast<double*>(b.Y); p.ldc = nb;
+            p.C = static_cast<double*>(split > 1 ? b.Ypart : b.Y); p.ldc = nb;
             p.tiles_m = 1; p.tiles_n = tn; p.order = ORDER_ROW;
-            p.c_rows = cnt; p.c_cols = nev;
-            p.khi_c = (m + bk - 1) / bk; p.kmax = p.khi_c;
+            p.c_rows = cnt; p.c_cols = split > 1 ? split * ldpart : nev;
+            p.khi_c = kc; p.kmax = kc;
             p.a.x0 = i0;
+            if (split > 1) { p.batch = split; p.c_bcol = ldpart; p.a.bk = kc * bk; p.b.bk = kc * bk; }
             GS_TRY(launch(st, p, false, L_EVP_BACK));
             evp_trace(stream, "back.y", pnl, cnt);
+            if (split > 1) {
+                LaunchTimer timer(plan, L_EVP_BACK, stream);
+                const long long total = (long long)nb * nev;
+                const int grid = int(std::min<long long>((total + 255) / 256, 4096));
+                cudaError_t le;
+                if (plan->z) le = launch_pdl(sum_parts_kernel<double2>, dim3(grid), dim3(256), 0, stream, static_cast<const double2*>(b.Ypart), (long long)nb * ldpart, split,
+                                             static_cast<double2*>(b.Y), total, static_cast<const int*>(info_ptr(plan)));
+                else le = launch_pdl(sum_parts_kernel<double>, dim3(grid), dim3(256), 0, stream, static_cast<const double*>(b.Ypart), (long long)nb * ldpart, split,
+                                     static_cast<double*>(b.Y), total, static_cast<const int*>(info_ptr(plan)));
+                if (le != cudaSuccess) return cuda_fail(plan, le);
+                plan->launches += 1;
+                evp_trace(stream, "back.ysum", pnl, split);
+            }
         }
         {   // Y2 = (Rp^-1)^H Y  (the panel's block of R^-1 is upper triangular with zeros below)
             Stage s2 = st;

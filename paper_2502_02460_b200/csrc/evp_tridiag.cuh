@@ -858,6 +858,21 @@ __global__ void init_r_kernel(T* R, int lb, int npanels)
     }
 }
 
+// out[i] = sum_s parts[s * stride + i] (s ascending: a fixed order), i < total -- the split-k partials of the
+// back-transformation's Y = Vp^H C~
+template <typename T>
+__global__ void sum_parts_kernel(const T* __restrict__ parts, long long stride, int nparts, T* __restrict__ out, long long total, const int* info)
+{
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*info != 0) return;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        T acc = parts[i];
+        for (int s = 1; s < nparts; ++s) acc = add(acc, parts[(long long)s * stride + i]);
+        out[i] = acc;
+    }
+}
+
 // C~(r, c) = Z(r, c) as T (real -> complex widening for the Hermitian path; a plain copy for the real one)
 template <typename T>
 __global__ void widen_kernel(const double* __restrict__ Z, long long ldz, T* __restrict__ C, long long ldc, int rows, int cols)

@@ -90,6 +90,7 @@ struct gs_plan {
     int leaf_mode = 2;               // 2: 32 x 32 sub-blocks, warp-level sweeps + in-CTA DMMA (leaf32_kernel.cuh, default); 1: 4-row panels; 0: rank-1 sweep over 256 threads
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
+    int super_syr2k = 4;             // the same for the SYR2K-shaped launch of gs_to_standard (four operand panels per tile)
     char cuda_error[256] = {0};
 };
 
@@ -653,6 +654,8 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     if (p->potrf_nb_tail > p->potrf_nb) p->potrf_nb_tail = p->potrf_nb;
     p->super_tile = p->z ? 16 : 8;
     knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
+    p->super_syr2k = p->super_tile > 4 ? 4 : p->super_tile;
+    knob("GS_SUPER_SYR2K", 0, 64, &p->super_syr2k);
     knob("GS_TILE64", 0, 2, &p->tile64_mode);
     knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);
@@ -818,7 +821,7 @@ static gs_status_t to_standard_rows(gs_plan* plan, Stage& st, const MatView& vV,
     if (whole) {
         p.tiles_m = nblk; p.tiles_n = nblk; p.order = ORDER_TRI_ROW_DESC;
         p.khi_c = kt; p.khi_i = kt;
-        if (!plan->z && plan->super_tile > 4) p.super = 4;   // four operand panels per tile: smaller super-tiles keep them in L2 (profiles/)
+        if (!plan->z) p.super = plan->super_syr2k;   // four operand panels per tile: its own super-tile edge (profiles/)
     } else {
         p.tiles_m = I1 - I0; p.tiles_n = nblk - I0; p.order = ORDER_TRAPEZOID;
         p.c_row0 = I0 * st.lb; p.c_col0 = I0 * st.lb;
