@@ -32,7 +32,7 @@ struct EvpBuffers {
     // tridiagonalisation
     unsigned int* tickets; void* sc;
     void *u, *wp, *corr2, *tfin, *Pd, *Vt, *Wt, *Pt, *P1, *P2, *R, *Rinv, *Y, *Y2, *Ypart;
-    long long ldp;
+    long long ldp, ldj;
     int nb, npanels;
     // results kept for gs_standard_eigh
     double *d, *e, *dwork; void* tau; double* Z;
@@ -65,7 +65,8 @@ EvpBuffers evp_carve(const gs_plan* p, unsigned char* base, size_t* bytes, int64
     b.u = takeb(N + 1); b.wp = takeb(N + 1); b.corr2 = takeb(N + 1); b.tfin = takeb(2 * size_t(nb)); b.Pd = takeb(N + 64);
     b.Vt = takeb(size_t(nb) * N); b.Wt = takeb(size_t(nb) * N);
     b.Pt = takeb(nJ * 2 * size_t(nb));
-    b.P1 = takeb(nJ * size_t(b.ldp)); b.P2 = takeb(nI * size_t(b.ldp));
+    b.ldj = (long long)(((nJ + 15) / 16) * 16);
+    b.P1 = takeb(N * size_t(b.ldj)); b.P2 = takeb(nI * size_t(b.ldp));
     b.R = takeb(size_t(b.npanels) * nb * (nb + 1)); b.Rinv = takeb(size_t(b.npanels) * nb * (nb + 1));
     b.Y = takeb(size_t(nb) * (nev + 2)); b.Y2 = takeb(size_t(nb) * (nev + 2));
     b.Ypart = takeb(size_t(kBackSplit) * nb * (((nev + size_t(nb) - 1) / nb) * nb + 2));   // split-k partials of Y, padded to whole tiles
@@ -103,7 +104,7 @@ StepParams<T> step_params(const gs_plan* plan, const EvpBuffers& b, void* A, dou
     p.A = static_cast<T*>(A); p.ld = plan->N; p.N = int(plan->N); p.nb = b.nb; p.lb = b.nb;
     p.u = static_cast<T*>(b.u); p.wp = static_cast<T*>(b.wp); p.corr2 = static_cast<T*>(b.corr2);
     p.Vt = static_cast<T*>(b.Vt); p.Wt = static_cast<T*>(b.Wt);
-    p.P1 = static_cast<T*>(b.P1); p.P2 = static_cast<T*>(b.P2); p.ldp = b.ldp;
+    p.P1 = static_cast<T*>(b.P1); p.P2 = static_cast<T*>(b.P2); p.ldp = b.ldp; p.ldj = b.ldj;
     p.Pt = static_cast<T*>(b.Pt); p.tfin = static_cast<T*>(b.tfin); p.Pd = static_cast<T*>(b.Pd);
     p.sc = static_cast<StepScalars<T>*>(b.sc); p.tickets = b.tickets;
     p.d = d; p.e = e; p.tau = static_cast<T*>(tau); p.R = static_cast<T*>(b.R);

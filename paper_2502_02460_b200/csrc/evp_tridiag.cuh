@@ -138,7 +138,8 @@ struct StepParams {
     T* corr2;             // N: old-panel part of the next column's lazy update (C -> F)
     T* Vt;                // nb x N (ld nb): V^H of the panel
     T* Wt;                // nb x N (ld nb): W^H of the panel
-    T* P1;                // [nJ][ldp] row-direction partials of y = A u, indexed by column block
+    T* P1;                // [N][ldj] row-direction partials of y = A u: row r, column block J (the partials of a row lie side by side)
+    long long ldj;
     T* P2;                // [nI][ldp] column-direction partials, indexed by row block
     long long ldp;
     T* Pt;                // [nJ][2 nb] partials of W^H u, V^H u
@@ -396,7 +397,7 @@ __global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> 
 #pragma unroll
         for (int w = 1; w < 8; ++w) s = add(s, red[w][t]);
         const int r = I * TH + t;
-        if (r < m) p.P1[(long long)J * p.ldp + r] = s;
+        if (r < m) p.P1[(long long)r * p.ldj + J] = s;
     }
 }
 
@@ -417,7 +418,7 @@ __global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> 
 //   Work items are dealt round-robin (item = cta, cta + G, ...): every partial has one owner and a fixed
 //   summation order, so the result does not depend on scheduling.
 // Leading CTAs (blockIdx.x < dot_ctas) form the panel dots instead (panel_dots).
-// P1[J][r]: row sums of column block J; P2[q][c]: column sums of strip q (p2_chunk_rows = chunk_blocks * 128).
+// P1[r][J]: row sums of column block J; P2[q][c]: column sums of strip q (p2_chunk_rows = chunk_blocks * 128).
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSvStageBytes = 16384;                 // TH rows x 16 columns
 constexpr int kSvConsumerWarps = 8;
@@ -634,7 +635,7 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
 #pragma unroll
                 for (int w = 1; w < kSvConsumerWarps; ++w) sum = add(sum, rr[w * TH]);
                 const int r = I * TH + t;
-                if (r < m) p.P1[(long long)J * p.ldp + r] = sum;
+                if (r < m) p.P1[(long long)r * p.ldj + J] = sum;
             }
         }
         // column sums of the strip
@@ -682,10 +683,10 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     T dotp = zero_of(T{});
     T y = zero_of(T{}), c1 = zero_of(T{}), c2 = zero_of(T{});
     if (r < m) {
-        // y(r): P1[J][r] for J >= r / TW, P2[I][r] for I <= r / TH
+        // y(r): P1[r][J] for J >= r / TW (one contiguous run per row), P2[I][r] for I <= r / p2_chunk_rows
         const int nJ = (m + TW - 1) / TW;
 #pragma unroll 4
-        for (int J = r / TW + l8; J < nJ; J += kCombineTPR) y = add(y, p.P1[(long long)J * p.ldp + r]);
+        for (int J = r / TW + l8; J < nJ; J += kCombineTPR) y = add(y, p.P1[(long long)r * p.ldj + J]);
 #pragma unroll 2
         for (int I = l8; I <= r / p.p2_chunk_rows; I += kCombineTPR) y = add(y, p.P2[(long long)I * p.ldp + r]);
         const T* vt = p.Vt + (long long)r * nb;
