@@ -13,8 +13,9 @@
  *   gs_backtransform         back-transformation C = U^-1 C~
  *
  * "A^T corresponds to the transpose or conjugate-transpose of a real- or complex-valued matrix"
- * (PAPER.md:67).  The standard eigensolve H~ C~ = eps C~ between steps 3 and 4 is NOT part of
- * this library.
+ * (PAPER.md:67).  The standard eigensolve H~ C~ = eps C~ between steps 3 and 4 is off the hot path of
+ * BASELINE.json; the library has its own (gs_standard_eigh and its three stages, further down), and any other
+ * eigensolver may be used instead.
  *
  * Conventions common to all calls
  * -------------------------------
