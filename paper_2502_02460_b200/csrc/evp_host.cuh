@@ -251,10 +251,8 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
             p.i = i; p.jp = jp; p.mode = 0; p.fuse = (use_tma && !fuse_off && jp > 0) ? 1 : 0;
             const int nJ = (i + TW - 1) / TW, nI = (i + TH - 1) / TH;
             if (use_tma) {
-                // strips of K blocks: the longest that still leaves every persistent CTA about three work items
-                const long long nblocks = (long long)nJ * (nJ + 1) / 2;
-                int K = chunk_env == 1 || chunk_env == 2 || chunk_env == 4 || chunk_env == 8 ? chunk_env : (nblocks >= (long long)chunk_t * sv_ctas ? 4 : nblocks >= (long long)chunk_t * sv_ctas / 2 ? 2 : 1);
-                const int a = nJ / K, r = nJ % K, nitems = K * a * (a + 1) / 2 + r * (a + 1);
+                const int K = chunk_env == 1 || chunk_env == 2 || chunk_env == 4 || chunk_env == 8 ? chunk_env : sv_chunk_blocks(nJ, chunk_t * sv_ctas);
+                const int nitems = sv_items_before(nJ, K);
                 p.p2_chunk_rows = K * TW;
                 q.s = p; q.chunk_blocks = K; q.dot_ctas = jp > 0 ? nJ : 0;
                 const int stream_ctas = std::min(nitems, sv_ctas);

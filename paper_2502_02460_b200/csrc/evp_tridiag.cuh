@@ -161,6 +161,20 @@ struct StepParams {
 
 template <typename T> __device__ __forceinline__ StepScalars<T>* sc_of(const StepParams<T>& p, int step) { return p.sc + (step & 1); }
 
+// Per-step indices of the device functions below; the step kernels take them from StepParams (step_idx).
+struct StepIdx {
+    int m;        // column i of this step = order of the active block
+    int jp;       // its column in the panel
+    int fuse;     // S: the F of the previous step is formed inside it
+    int bar_id;   // 0: the callers are the whole CTA (__syncthreads); else its first nthr threads, meeting at this named barrier
+    int nthr;
+};
+template <typename T> __device__ __forceinline__ StepIdx step_idx(const StepParams<T>& p) { return StepIdx{p.i, p.jp, p.fuse, 0, 0}; }
+__device__ __forceinline__ void step_sync(const StepIdx& ix)
+{
+    if (ix.bar_id == 0) __syncthreads(); else named_bar_sync(ix.bar_id, ix.nthr);
+}
+
 // ---- F (mode 0) inside S: the next column, formed wherever it is needed -------------------------------------
 // With io = p.i + 1 the step just combined (panel column jpo = p.jp - 1) and sc its scalars:
 //   w(r) = tau w'(r) + alpha2 v(r),   u(r) = A(r, p.i) - corr2(r) - v(r) conj(w(io-1)) - w(r) conj(v(io-1)),  r <= p.i.
@@ -179,13 +193,15 @@ __device__ __forceinline__ double2 fx_sub(double2 a, double2 b) { return make_do
 template <typename T>
 struct FusedF {
     T tau, alpha2, cwlast, cvlast;      // conj(w(io-1)), conj(v(io-1))
-    int jpo;
-    __device__ __forceinline__ void init(const StepParams<T>& p)
+    int jpo, col;
+    // alpha2_local: the caller's own copy of alpha2 of the step just combined; nullptr: read from sc
+    __device__ __forceinline__ void init(const StepParams<T>& p, const StepIdx& ix, const T* alpha2_local = nullptr)
     {
-        const StepScalars<T> sc = *sc_of(p, p.i + 1);
-        tau = sc.tau; alpha2 = sc.alpha2; jpo = p.jp - 1;
-        const T vlast = cj(p.Vt[jpo + (long long)p.i * p.nb]);
-        const T wlast = fx_add(fx_mul(tau, p.wp[p.i]), fx_mul(alpha2, vlast));
+        const StepScalars<T>* sc = sc_of(p, ix.m + 1);
+        tau = ldcg(&sc->tau); alpha2 = alpha2_local != nullptr ? *alpha2_local : ldcg(&sc->alpha2);
+        jpo = ix.jp - 1; col = ix.m;
+        const T vlast = cj(p.Vt[jpo + (long long)col * p.nb]);
+        const T wlast = fx_add(fx_mul(tau, p.wp[col]), fx_mul(alpha2, vlast));
         cwlast = cj(wlast); cvlast = cj(vlast);
     }
     __device__ __forceinline__ T w_of(const StepParams<T>& p, int r, T& v) const
@@ -197,8 +213,8 @@ struct FusedF {
     {
         T v;
         const T w = w_of(p, r, v);
-        T un = fx_sub(fx_sub(fx_sub(p.A[r + (long long)p.i * p.ld], p.corr2[r]), fx_mul(v, cwlast)), fx_mul(w, cvlast));
-        if (r == p.i) un = real_only(un);
+        T un = fx_sub(fx_sub(fx_sub(p.A[r + (long long)col * p.ld], p.corr2[r]), fx_mul(v, cwlast)), fx_mul(w, cvlast));
+        if (r == col) un = real_only(un);
         if (w_out != nullptr) *w_out = w;
         return un;
     }
@@ -211,18 +227,19 @@ struct FusedF {
 // M^H = conj(D) + striu(V^H V).  sm: 512 elements of shared memory.
 // ---------------------------------------------------------------------------------------------------------
 template <typename T>
-__device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx, T* sm, unsigned int* s_last)
+__device__ __forceinline__ void panel_dots(const StepParams<T>& p, const StepIdx& ix, int x, int nx, T* sm, unsigned int* s_last,
+                                           const T* alpha2_local = nullptr)
 {
     constexpr int TW = kSymvTW;
-    const int m = p.i, jp = p.jp, nb = p.nb;
+    const int m = ix.m, jp = ix.jp, nb = p.nb;
     const int t = threadIdx.x;
     if (jp == 0) return;
     const int r0 = x * TW, r1 = min(r0 + TW, m);
-    if (p.fuse) {
+    if (ix.fuse) {
         // F of the previous step for the rows of this chunk (the last chunk also takes row m, the new diagonal entry):
         // column jp-1 of W, the next column u, the partial of ||u(0 : m-2)||^2; rows >= io of the reflector column io = 0
         FusedF<T> ff;
-        ff.init(p);
+        ff.init(p, ix, alpha2_local);
         const int io = m + 1;
         double nrm = 0.0;
         const int r = (t < TW) ? r0 + t : ((t == TW && x == nx - 1) ? m : -1);
@@ -238,13 +255,13 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
         double* sn = reinterpret_cast<double*>(sm);
         if ((t & 31) == 0) sn[t >> 5] = nrm;
-        __syncthreads();
+        step_sync(ix);
         if (t == 0) {
             double sum = 0.0;
-            for (int w = 0; w < int(blockDim.x) / 32; ++w) sum += sn[w];
+            for (int w = 0; w < (ix.bar_id == 0 ? int(blockDim.x) : ix.nthr) / 32; ++w) sum += sn[w];
             reinterpret_cast<double*>(p.Pd)[x] = sum;
         }
-        __syncthreads();      // the chunk's u and column jp-1 of Wt are read back below; sm is reused
+        step_sync(ix);      // the chunk's u and column jp-1 of Wt are read back below; sm is reused
     }
     const int groups = kSymvThreads / nb;            // nb = 128: 2 row groups; nb = 64: 4
     const int c = t % nb, g = t / nb;
@@ -258,7 +275,7 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         }
     }
     if (t < kSymvThreads) { sm[t] = aw; sm[kSymvThreads + t] = av; }
-    __syncthreads();
+    step_sync(ix);
     if (t < nb) {
         T sw = zero_of(T{}), sv = zero_of(T{});
         for (int gg = 0; gg < groups; ++gg) { sw = add(sw, sm[gg * nb + t]); sv = add(sv, sm[kSymvThreads + gg * nb + t]); }
@@ -266,12 +283,12 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         p.Pt[(long long)x * 2 * nb + nb + t] = sv;
     }
     __threadfence();
-    __syncthreads();
+    step_sync(ix);
     if (t == 0) *s_last = (atomicAdd(&p.tickets[0], 1u) == unsigned(nx - 1)) ? 1u : 0u;
-    __syncthreads();
+    step_sync(ix);
     if (!*s_last) return;
     __threadfence();
-    if (p.fuse) {
+    if (ix.fuse) {
         // the scalars of this step from the norm of the new column (F's finaliser)
         if (t < 32) {
             double x2 = 0.0;
@@ -286,10 +303,10 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
                 *sc_of(p, m) = nx_sc;
             }
         }
-        __syncthreads();
+        step_sync(ix);
     }
     // last chunk CTA: tW' = s (W^H u - beta Wt[:, i-1]),  tV' likewise;  the new column of M^H = conj(D) + striu(V^H V)
-    const StepScalars<T> sc = *sc_of(p, m);
+    const StepScalars<T> sc = *sc_of(p, m);   // (written by this CTA just above, or by a kernel before this one)
     if (t < 2 * nb) {
         const int cc = t % nb;
         const bool isV = t >= nb;
@@ -302,7 +319,7 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, int x, int nx
         p.tfin[t] = acc;
         if (isV && cc < jp) {
             // G(a, b) = v_a^H v_b for a = itop - cc > b = i;  M^H(b - i0, a - i0) = conj(G(a, b)) with i0 = itop - lb + 1
-            const int lb = p.lb, rowb = lb - 1 - p.jp, cola = lb - 1 - cc;
+            const int lb = p.lb, rowb = lb - 1 - jp, cola = lb - 1 - cc;
             p.R[(long long)p.panel * lb * (lb + 1) + rowb + (long long)cola * lb] = cj(acc);
         }
     }
@@ -327,7 +344,7 @@ __global__ void __launch_bounds__(kSymvThreads) symv_kernel(const StepParams<T> 
     __shared__ unsigned int s_last;
 
     if (int(blockIdx.y) == nI) {
-        panel_dots(p, int(blockIdx.x), int(gridDim.x), &red[0][0], &s_last);
+        panel_dots(p, step_idx(p), int(blockIdx.x), int(gridDim.x), &red[0][0], &s_last);
         return;
     }
 
@@ -442,10 +459,16 @@ struct SymvTmaParams {
 };
 
 // number of work items in the column blocks j < J:  sum_{j<J} ceil((j + 1) / K)
-__device__ __forceinline__ int sv_items_before(int J, int K)
+__host__ __device__ __forceinline__ int sv_items_before(int J, int K)
 {
     const int a = J / K, b = J - a * K;
     return K * a * (a + 1) / 2 + b * (a + 1);
+}
+// strips of K blocks: the longest that still leaves every persistent CTA a few work items
+__host__ __device__ __forceinline__ int sv_chunk_blocks(int nJ, int chunk_thresh)
+{
+    const long long nblocks = (long long)nJ * (nJ + 1) / 2;
+    return nblocks >= chunk_thresh ? 4 : (2 * nblocks >= chunk_thresh ? 2 : 1);
 }
 
 // v[16] per lane -> the sum over the 32 lanes of v[idx], idx = bits 4..1 of the lane (both lanes of a pair hold it)
@@ -464,130 +487,135 @@ __device__ __forceinline__ T sv_transpose_reduce(const T (&v)[16], int lane)
     return add(w1, shfl_xor(w1, 1));
 }
 
+// Shared memory of a streaming CTA and the running counters of its two roles.
 template <typename T>
-__global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
-{
-    constexpr int kSvStages = SvCfg<T>::kStages;
-    constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW, H = RPT / 2;
-    constexpr int W8 = int(sizeof(T)) / 8;            // doubles per element
-    constexpr int R = TW / TH;                        // row tiles per 128-row block
-    const StepParams<T>& p = q.s;
-    extern __shared__ unsigned char sv_smem_raw[];
-    unsigned char* smem = sv_smem_raw + ((1024u - (smem_u32(sv_smem_raw) & 1023u)) & 1023u);
-    unsigned char* stages = smem;
-    T* red = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes);
-    T* ucol = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes + kSvRedBytes);
-    T* urow = reinterpret_cast<T*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kSvStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + kSvUrowBytes);
-    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + kSvStages), qfull0 = smem_u32(bars + 2 * kSvStages);
-    volatile int* item_q = reinterpret_cast<volatile int*>(bars + 2 * kSvStages + 4);
-    __shared__ unsigned int s_last;
-    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    if (t == 0) {
-        for (int s = 0; s < kSvStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kSvConsumerWarps); }
-        for (int s = 0; s < 4; ++s) mbar_init(qfull0 + 8 * s, 1);
+struct SvCta {
+    unsigned char* stages;
+    T *red, *ucol, *urow;
+    uint32_t full0, empty0, qfull0, qempty0;
+    volatile int* item_q;
+    uint32_t cnt;          // stages issued (producer) / consumed (consumers)
+    int nitem, ntile;      // queue slots written (producer) / read (consumers); tiles consumed
+    __device__ __forceinline__ void carve(unsigned char* raw)
+    {
+        constexpr int kStages = SvCfg<T>::kStages;
+        unsigned char* smem = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
+        stages = smem;
+        red = reinterpret_cast<T*>(smem + kStages * kSvStageBytes);
+        ucol = reinterpret_cast<T*>(smem + kStages * kSvStageBytes + kSvRedBytes);
+        urow = reinterpret_cast<T*>(smem + kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes);
+        uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kSvStageBytes + kSvRedBytes + kSvUcolBytes + kSvUrowBytes);
+        full0 = smem_u32(bars); empty0 = smem_u32(bars + kStages); qfull0 = smem_u32(bars + 2 * kStages); qempty0 = smem_u32(bars + 2 * kStages + 4);
+        item_q = reinterpret_cast<volatile int*>(bars + 2 * kStages + 8);
+        cnt = 0; nitem = 0; ntile = 0;
+    }
+    __device__ __forceinline__ void init_barriers() const      // one thread
+    {
+        constexpr int kStages = SvCfg<T>::kStages;
+        for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kSvConsumerWarps); }
+        for (int s = 0; s < 4; ++s) { mbar_init(qfull0 + 8 * s, 1); mbar_init(qempty0 + 8 * s, kSvConsumerWarps); }
         mbar_fence_init();
-        tma_prefetch_desc(&q.mapA);
     }
-    __syncthreads();
-    grid_dep_launch();
-    grid_dep_wait();
-    if (*p.info != 0) return;
-    const int m = p.i;
-    if (int(blockIdx.x) < q.dot_ctas) {
-        panel_dots(p, int(blockIdx.x), q.dot_ctas, red, &s_last);
-        return;
+};
+
+// item -> (column block J, first and one-past-last row tile): largest J with items_before(J) <= item
+template <typename T>
+__device__ __forceinline__ void sv_decode(int item, int nJ, int nI, int K, int& J, int& I0, int& I1)
+{
+    constexpr int R = kSymvTW / SymvGeom<T>::TH;      // row tiles per 128-row block
+    int lo = 0, hi = nJ;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (sv_items_before(mid, K) <= item) lo = mid; else hi = mid;
     }
-    const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
-    const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH, K = q.chunk_blocks;
+    J = lo;
+    const int qq = item - sv_items_before(lo, K);
+    I0 = qq * K * R;
+    I1 = min(min((qq + 1) * K * R, (J + 1) * R), nI);
+}
+
+// Producer lane, one step (order of the active block m): streams every stage of every tile of the CTA's work items.
+// The first item is `first` (< 0: none, the CTA starts with the counter), the others are dyn_base + the values of
+// the atomic counter; every item goes to the consumers through the four-slot queue (full / empty barriers per slot),
+// -1 ends the step.
+template <typename T>
+__device__ __forceinline__ void sv_produce_step(SvCta<T>& c, const CUtensorMap* map, int m, int K, int first, int dyn_base, unsigned int* counter)
+{
+    constexpr int kStages = SvCfg<T>::kStages;
+    constexpr int TH = SymvGeom<T>::TH, TW = kSymvTW, W8 = int(sizeof(T)) / 8;
+    const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH;
     const int nitems = sv_items_before(nJ, K);
-
-    // item -> (column block J, first and one-past-last row tile): largest J with items_before(J) <= item
-    auto decode = [&](int item, int& J, int& I0, int& I1) {
-        int lo = 0, hi = nJ;
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (sv_items_before(mid, K) <= item) lo = mid; else hi = mid;
-        }
-        J = lo;
-        const int qq = item - sv_items_before(lo, K);
-        I0 = qq * K * R;
-        I1 = min(min((qq + 1) * K * R, (J + 1) * R), nI);
-    };
-
-    // Work items: the first one of a CTA is its own index, the rest comes from a global counter (tickets[3], reset by
-    // the C kernel that follows), so the CTAs that start late (behind the panel-dot CTAs) simply take fewer items.  The producer lane
-    // hands every item to the consumers through a four-slot queue in shared memory (the producer is never more than
-    // one item ahead: the stage ring holds less than a tile).
-    if (warp == kSvConsumerWarps) {
-        // ---- producer: one lane streams every stage of every tile of the CTA's items ----
-        if (lane == 0) {
-            uint32_t cnt = 0;
-            int item = cta;
-            for (int nq = 0;; ++nq) {
-                item_q[nq & 3] = item < nitems ? item : -1;
-                mbar_arrive(qfull0 + 8 * (nq & 3));
-                if (item >= nitems) break;
-                const int next = G + int(atomicAdd(p.tickets + 3, 1u));
-                int J, I0, I1;
-                decode(item, J, I0, I1);
-                for (int I = I0; I < I1; ++I) {
-                    for (int s = 0; s < TW / 16; ++s, ++cnt) {
-                        const uint32_t stage = cnt % kSvStages;
-                        if (cnt >= kSvStages) mbar_wait(empty0 + 8 * stage, ((cnt / kSvStages) - 1) & 1);
-                        mbar_arrive_expect_tx(full0 + 8 * stage, kSvStageBytes);
-                        tma_load_2d(smem_u32(stages + stage * kSvStageBytes), &q.mapA, I * TH * W8, J * TW + 16 * s, full0 + 8 * stage);
-                    }
-                }
-                item = next;
+    int item = first >= 0 ? first : dyn_base + int(atomicAdd(counter, 1u));
+    for (;; ++c.nitem) {
+        if (c.nitem >= 4) mbar_wait(c.qempty0 + 8 * (c.nitem & 3), ((c.nitem >> 2) - 1) & 1);   // the slot has been read
+        c.item_q[c.nitem & 3] = item < nitems ? item : -1;
+        mbar_arrive(c.qfull0 + 8 * (c.nitem & 3));
+        if (item >= nitems) { ++c.nitem; break; }
+        const int next = dyn_base + int(atomicAdd(counter, 1u));
+        int J, I0, I1;
+        sv_decode<T>(item, nJ, nI, K, J, I0, I1);
+        for (int I = I0; I < I1; ++I) {
+            for (int s = 0; s < TW / 16; ++s, ++c.cnt) {
+                const uint32_t stage = c.cnt % kStages;
+                if (c.cnt >= kStages) mbar_wait(c.empty0 + 8 * stage, ((c.cnt / kStages) - 1) & 1);
+                mbar_arrive_expect_tx(c.full0 + 8 * stage, kSvStageBytes);
+                tma_load_2d(smem_u32(c.stages + stage * kSvStageBytes), map, I * TH * W8, J * TW + 16 * s, c.full0 + 8 * stage);
             }
         }
-        return;
+        item = next;
     }
+}
 
-    // ---- consumers: warp w owns columns 2w, 2w+1 of every stage; lane l owns rows {l H .. l H + H-1} of each half tile ----
+// Consumers (the first 256 threads), one step: warp w owns columns 2w, 2w+1 of every stage, lane l owns rows
+// {l H .. l H + H-1} of each half tile; u(r) is stored by F, or (fuse) formed here from the previous step's vectors.
+template <typename T>
+__device__ __forceinline__ void sv_consume_step(SvCta<T>& c, const StepParams<T>& p, const StepIdx& ix, const FusedF<T>& ff, int K)
+{
+    constexpr int kStages = SvCfg<T>::kStages;
+    constexpr int RPT = SymvGeom<T>::RPT, TH = SymvGeom<T>::TH, TW = kSymvTW, H = RPT / 2;
+    constexpr int R = TW / TH;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const int m = ix.m;
+    const int nJ = (m + TW - 1) / TW, nI = (m + TH - 1) / TH;
     auto row_of = [&](int k) { return (k / H) * (TH / 2) + lane * H + (k % H); };
-    // u(r): stored by F, or (fuse) formed here from the previous step's vectors
-    FusedF<T> ff;
-    if (p.fuse) ff.init(p);
-    auto u_val = [&](int r) -> T { return (r < m) ? (p.fuse ? ff.u_of(p, r) : p.u[r]) : zero_of(T{}); };
-    uint32_t cnt = 0;
-    int nitem = 0, ntile = 0;
-    for (;; ++nitem) {
-        mbar_wait(qfull0 + 8 * (nitem & 3), (nitem >> 2) & 1);
-        const int item = item_q[nitem & 3];
-        if (item < 0) break;
+    auto u_val = [&](int r) -> T { return (r < m) ? (ix.fuse ? ff.u_of(p, r) : p.u[r]) : zero_of(T{}); };
+    for (;; ++c.nitem) {
+        mbar_wait(c.qfull0 + 8 * (c.nitem & 3), (c.nitem >> 2) & 1);
+        const int item = c.item_q[c.nitem & 3];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(c.qempty0 + 8 * (c.nitem & 3));
+        if (item < 0) { ++c.nitem; break; }
         int J, I0, I1;
-        decode(item, J, I0, I1);
-        T* uc = ucol + (nitem & 1) * TW;
+        sv_decode<T>(item, nJ, nI, K, J, I0, I1);
+        T* uc = c.ucol + (c.nitem & 1) * TW;
         if (t < TW) uc[t] = u_val(J * TW + t);
-        if (t < TH) urow[(ntile & 1) * TH + t] = u_val(I0 * TH + t);
+        if (t < TH) c.urow[(c.ntile & 1) * TH + t] = u_val(I0 * TH + t);
         named_bar_sync(1, kSvConsumerWarps * 32);
         T yc[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) yc[i] = zero_of(T{});
-        for (int I = I0; I < I1; ++I, ++ntile) {
+        for (int I = I0; I < I1; ++I, ++c.ntile) {
             // the next tile's rows of u: loaded now, parked in shared memory before this tile's barrier
             T unext = zero_of(T{});
             const bool prefetch = (I + 1 < I1) && t < TH;
             if (prefetch) unext = u_val((I + 1) * TH + t);
             T ur[RPT];
 #pragma unroll
-            for (int k = 0; k < RPT; ++k) ur[k] = urow[(ntile & 1) * TH + row_of(k)];
+            for (int k = 0; k < RPT; ++k) ur[k] = c.urow[(c.ntile & 1) * TH + row_of(k)];
             T yr[RPT];
 #pragma unroll
             for (int k = 0; k < RPT; ++k) yr[k] = zero_of(T{});
             const bool masked = I * TH + TH - 1 >= J * TW;     // some element of the tile lies below the diagonal
 #pragma unroll
             for (int s = 0; s < TW / 16; ++s) {
-                const uint32_t stage = cnt % kSvStages;
-                mbar_wait(full0 + 8 * stage, (cnt / kSvStages) & 1);
-                if (cnt > 0) {                                   // release the previous stage (ptx.cuh: not right behind its loads)
+                const uint32_t stage = c.cnt % kStages;
+                mbar_wait(c.full0 + 8 * stage, (c.cnt / kStages) & 1);
+                if (c.cnt > 0) {                                 // release the previous stage (ptx.cuh: not right behind its loads)
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(empty0 + 8 * ((cnt - 1) % kSvStages));
+                    if (lane == 0) mbar_arrive(c.empty0 + 8 * ((c.cnt - 1) % kStages));
                 }
-                ++cnt;
-                const unsigned char* sp = stages + stage * kSvStageBytes + (2 * warp) * (TH * int(sizeof(T)));
+                ++c.cnt;
+                const unsigned char* sp = c.stages + stage * kSvStageBytes + (2 * warp) * (TH * int(sizeof(T)));
                 T a[2][RPT];
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
@@ -611,26 +639,26 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
                     const int c0 = J * TW + 16 * s + 2 * warp;
 #pragma unroll
                     for (int j = 0; j < 2; ++j) {
-                        const int c = c0 + j;
+                        const int cc = c0 + j;
 #pragma unroll
                         for (int k = 0; k < RPT; ++k) {
                             const int r = I * TH + row_of(k);
-                            T av = (r <= c) ? a[j][k] : zero_of(T{});
-                            if (r == c) av = real_only(av);
+                            T av = (r <= cc) ? a[j][k] : zero_of(T{});
+                            if (r == cc) av = real_only(av);
                             yr[k] = fmad(av, j == 0 ? u0 : u1, yr[k]);
-                            if (r < c) yc[2 * s + j] = cfmad(av, ur[k], yc[2 * s + j]);
+                            if (r < cc) yc[2 * s + j] = cfmad(av, ur[k], yc[2 * s + j]);
                         }
                     }
                 }
             }
             // row sums of the tile over the eight warps
-            T* rb = red + ((ntile & 1) * kSvConsumerWarps + warp) * TH;
+            T* rb = c.red + ((c.ntile & 1) * kSvConsumerWarps + warp) * TH;
 #pragma unroll
             for (int k = 0; k < RPT; ++k) rb[row_of(k)] = yr[k];
-            if (prefetch) urow[((ntile + 1) & 1) * TH + t] = unext;
+            if (prefetch) c.urow[((c.ntile + 1) & 1) * TH + t] = unext;
             named_bar_sync(2, kSvConsumerWarps * 32);
             if (t < TH) {
-                const T* rr = red + (ntile & 1) * kSvConsumerWarps * TH + t;
+                const T* rr = c.red + (c.ntile & 1) * kSvConsumerWarps * TH + t;
                 T sum = rr[0];
 #pragma unroll
                 for (int w = 1; w < kSvConsumerWarps; ++w) sum = add(sum, rr[w * TH]);
@@ -642,10 +670,44 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
         const T ysum = sv_transpose_reduce(yc, lane);
         if ((lane & 1) == 0) {
             const int idx = lane >> 1;                          // = 2 s + j
-            const int c = J * TW + 16 * (idx >> 1) + 2 * warp + (idx & 1);
-            if (c < m) p.P2[(long long)(I0 / (K * R)) * p.ldp + c] = ysum;
+            const int cc = J * TW + 16 * (idx >> 1) + 2 * warp + (idx & 1);
+            if (cc < m) p.P2[(long long)(I0 / (K * R)) * p.ldp + cc] = ysum;
         }
     }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
+{
+    const StepParams<T>& p = q.s;
+    extern __shared__ unsigned char sv_smem_raw[];
+    SvCta<T> c;
+    c.carve(sv_smem_raw);
+    __shared__ unsigned int s_last;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    if (t == 0) {
+        c.init_barriers();
+        tma_prefetch_desc(&q.mapA);
+    }
+    __syncthreads();
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const StepIdx ix = step_idx(p);
+    if (int(blockIdx.x) < q.dot_ctas) {
+        panel_dots(p, ix, int(blockIdx.x), q.dot_ctas, c.red, &s_last);
+        return;
+    }
+    // Work items: the first one of a CTA is its own index, the rest comes from a global counter (tickets[3], reset by
+    // the C kernel that follows), so the CTAs that start late (behind the panel-dot CTAs) simply take fewer items.
+    const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
+    if (warp == kSvConsumerWarps) {
+        if (lane == 0) sv_produce_step(c, &q.mapA, ix.m, q.chunk_blocks, cta, G, p.tickets + 3);
+        return;
+    }
+    FusedF<T> ff;
+    if (ix.fuse) ff.init(p, ix);
+    sv_consume_step(c, p, ix, ff, q.chunk_blocks);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -658,28 +720,28 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kCombineTPR = 16;                       // threads per row
 constexpr int kCombineRows = 256 / kCombineTPR;
+
+// tW', tV' and row i-1 of the panels into shared memory (2 * 128 elements each), by the first nthr threads of the CTA
 template <typename T>
-__global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
+__device__ __forceinline__ void combine_load(const StepParams<T>& p, const StepIdx& ix, T* s_t, T* s_row, int nthr)
 {
-    constexpr int TH = SymvGeom<T>::TH, TW = kSymvTW;
-    grid_dep_launch();
-    grid_dep_wait();
-    if (*p.info != 0) return;
-    const int m = p.i, jp = p.jp, nb = p.nb;
-    const int t = threadIdx.x, l8 = t % kCombineTPR, rr = t / kCombineTPR;
-    if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
-    const int r = blockIdx.x * kCombineRows + rr;
-    const StepScalars<T> sc = *sc_of(p, m);
-    __shared__ T s_t[2 * 128];           // tW', tV'
-    __shared__ T s_row[2 * 128];         // Wt[:, i-1], Vt[:, i-1]
-    __shared__ T s_dot[8];
-    __shared__ unsigned int s_last;
-    for (int c = t; c < 2 * nb; c += 256) {
+    const int nb = p.nb;
+    for (int c = threadIdx.x; c < 2 * nb; c += nthr) {
         const int cc = c % nb;
-        s_t[c] = (cc < jp) ? p.tfin[c] : zero_of(T{});
-        s_row[c] = (cc < jp) ? (c < nb ? p.Wt : p.Vt)[cc + (long long)(m - 1) * nb] : zero_of(T{});
+        s_t[c] = (cc < ix.jp) ? p.tfin[c] : zero_of(T{});
+        s_row[c] = (cc < ix.jp) ? (c < nb ? p.Wt : p.Vt)[cc + (long long)(ix.m - 1) * nb] : zero_of(T{});
     }
-    __syncthreads();
+}
+
+// rows [g * kCombineRows, (g + 1) * kCombineRows) by 256 threads; returns the thread's share of w'^H v (its row's
+// term in the threads that own a row, zero elsewhere)
+template <typename T>
+__device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx& ix, const StepScalars<T>& sc, const T* s_t, const T* s_row, int g)
+{
+    constexpr int TW = kSymvTW;
+    const int m = ix.m, jp = ix.jp, nb = p.nb;
+    const int t = threadIdx.x, l8 = t % kCombineTPR, rr = t / kCombineTPR;
+    const int r = g * kCombineRows + rr;
     T dotp = zero_of(T{});
     T y = zero_of(T{}), c1 = zero_of(T{}), c2 = zero_of(T{});
     if (r < m) {
@@ -703,22 +765,56 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     // (all 32 lanes take part in the shuffles: a warp holds several rows, some of which may lie beyond m)
 #pragma unroll
     for (int o = kCombineTPR / 2; o > 0; o >>= 1) { y = add(y, shfl_xor(y, o)); c1 = add(c1, shfl_xor(c1, o)); c2 = add(c2, shfl_xor(c2, o)); }
-    if (r < m) {
-        if (l8 == 0) {
-            const T ur = p.u[r];
-            T v = mul(sc.s, (r == m - 1) ? sub(ur, from_real(sc.beta, T{})) : ur);
-            if (r == m - 1 && !is_zero(sc.s)) v = from_real(1.0, T{});   // (an identity reflector keeps v = 0)
-            T acol = p.A[r + (long long)(m - 1) * p.ld];
-            if (r == m - 1) acol = real_only(acol);
-            T wpr = sub(mul(sc.s, sub(y, rscale(acol, sc.beta))), c1);
-            p.Vt[jp + (long long)r * nb] = cj(v);
-            p.A[r + (long long)m * p.ld] = v;
-            p.wp[r] = wpr;
-            p.corr2[r] = c2;
-            dotp = cfmad(wpr, v, dotp);
-        }
+    if (r < m && l8 == 0) {
+        const T ur = p.u[r];
+        T v = mul(sc.s, (r == m - 1) ? sub(ur, from_real(sc.beta, T{})) : ur);
+        if (r == m - 1 && !is_zero(sc.s)) v = from_real(1.0, T{});   // (an identity reflector keeps v = 0)
+        T acol = p.A[r + (long long)(m - 1) * p.ld];
+        if (r == m - 1) acol = real_only(acol);
+        T wpr = sub(mul(sc.s, sub(y, rscale(acol, sc.beta))), c1);
+        p.Vt[jp + (long long)r * nb] = cj(v);
+        p.A[r + (long long)m * p.ld] = v;
+        p.wp[r] = wpr;
+        p.corr2[r] = c2;
+        dotp = cfmad(wpr, v, dotp);
     }
-    // block partial of w'^H v: lanes with l8 == 0 hold one row each
+    return dotp;
+}
+
+// what the finaliser of C records besides alpha2: d(i), e(i-1), tau(i) and the diagonal of M^H = conj(D) + striu(V^H V)
+template <typename T>
+__device__ __forceinline__ void combine_record(const StepParams<T>& p, const StepIdx& ix, const StepScalars<T>& sc)
+{
+    const int m = ix.m;
+    p.d[m] = re(ldcg(&p.u[m]));
+    p.e[m - 1] = sc.beta;
+    p.tau[m] = sc.tau;
+    const int lb = p.lb, pos = lb - 1 - ix.jp;                 // conj(1 / tau) (1 for an identity reflector)
+    T dinv;
+    if (is_zero(sc.tau)) dinv = from_real(1.0, T{});
+    else { const double n2 = abs2(sc.tau); dinv = cj(rscale(cj(sc.tau), 1.0 / n2)); }   // conj(1/tau) = conj(conj(tau)/|tau|^2)
+    p.R[(long long)p.panel * lb * (lb + 1) + pos + (long long)pos * lb] = dinv;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
+{
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*p.info != 0) return;
+    const StepIdx ix = step_idx(p);
+    const int m = ix.m;
+    const int t = threadIdx.x;
+    if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
+    const StepScalars<T> sc = *sc_of(p, m);
+    __shared__ T s_t[2 * 128];           // tW', tV'
+    __shared__ T s_row[2 * 128];         // Wt[:, i-1], Vt[:, i-1]
+    __shared__ T s_dot[8];
+    __shared__ unsigned int s_last;
+    combine_load(p, ix, s_t, s_row, 256);
+    __syncthreads();
+    T dotp = combine_group(p, ix, sc, s_t, s_row, int(blockIdx.x));
+    // block partial of w'^H v
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dotp = add(dotp, shfl_xor(dotp, o));
     if ((t & 31) == 0) s_dot[t >> 5] = dotp;
@@ -744,15 +840,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
         T dot = s_dot[0];
         for (int w = 1; w < 8; ++w) dot = add(dot, s_dot[w]);
         sc_of(p, m)->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
-        p.d[m] = re(p.u[m]);
-        p.e[m - 1] = sc.beta;
-        p.tau[m] = sc.tau;
-        // diagonal of M^H = conj(D) + striu(V^H V): conj(1 / tau) (1 for an identity reflector)
-        const int lb = p.lb, pos = lb - 1 - jp;
-        T dinv;
-        if (is_zero(sc.tau)) dinv = from_real(1.0, T{});
-        else { const double n2 = abs2(sc.tau); dinv = cj(rscale(cj(sc.tau), 1.0 / n2)); }   // conj(1/tau) = conj(conj(tau)/|tau|^2)
-        p.R[(long long)p.panel * lb * (lb + 1) + pos + (long long)pos * lb] = dinv;
+        combine_record(p, ix, sc);
         p.tickets[1] = 0u;
     }
 }
