@@ -744,32 +744,56 @@ __device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx
     const int r = g * kCombineRows + rr;
     T dotp = zero_of(T{});
     T y = zero_of(T{}), c1 = zero_of(T{}), c2 = zero_of(T{});
+    T ur = zero_of(T{}), acol = zero_of(T{});
     if (r < m) {
+        // Every load of the row is independent of every other: they are issued in blocks of eight predicated loads
+        // per array (a dependent chain of L2 round trips is what this kernel's time consists of).
+        if (l8 == 0) { ur = p.u[r]; acol = p.A[r + (long long)(m - 1) * p.ld]; }
         // y(r): P1[r][J] for J >= r / TW (one contiguous run per row), P2[I][r] for I <= r / p2_chunk_rows
         const int nJ = (m + TW - 1) / TW;
-#pragma unroll 4
-        for (int J = r / TW + l8; J < nJ; J += kCombineTPR) y = add(y, p.P1[(long long)r * p.ldj + J]);
-#pragma unroll 2
-        for (int I = l8; I <= r / p.p2_chunk_rows; I += kCombineTPR) y = add(y, p.P2[(long long)I * p.ldp + r]);
+        const T* p1 = p.P1 + (long long)r * p.ldj;
+        for (int J0 = r / TW + l8; J0 < nJ; J0 += 8 * kCombineTPR) {
+            T v8[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { const int J = J0 + k * kCombineTPR; v8[k] = J < nJ ? p1[J] : zero_of(T{}); }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) y = add(y, v8[k]);
+        }
+        const int nP2 = r / p.p2_chunk_rows + 1;
+        for (int I0 = l8; I0 < nP2; I0 += 4 * kCombineTPR) {
+            T v4[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const int I = I0 + k * kCombineTPR; v4[k] = I < nP2 ? p.P2[(long long)I * p.ldp + r] : zero_of(T{}); }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) y = add(y, v4[k]);
+        }
         const T* vt = p.Vt + (long long)r * nb;
         const T* wt = p.Wt + (long long)r * nb;
-#pragma unroll 4
-        for (int c = l8; c < jp; c += kCombineTPR) {
-            const T vrc = cj(vt[c]), wrc = cj(wt[c]);             // V(r,c), W(r,c)
-            c1 = fmad(vrc, s_t[c], c1);
-            c1 = fmad(wrc, s_t[nb + c], c1);
-            c2 = fmad(vrc, s_row[c], c2);                          // V(r,c) conj(W(i-1,c)) : s_row[c] = Wt[c, i-1] = conj(W(i-1,c))
-            c2 = fmad(wrc, s_row[nb + c], c2);
+        for (int c0 = l8; c0 < jp; c0 += 8 * kCombineTPR) {
+            T vv[8], ww[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int c = c0 + k * kCombineTPR;
+                vv[k] = c < jp ? vt[c] : zero_of(T{});
+                ww[k] = c < jp ? wt[c] : zero_of(T{});
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int c = min(c0 + k * kCombineTPR, nb - 1);   // (beyond jp: vv = ww = 0 and the entries of s_t, s_row are zero)
+                const T vrc = cj(vv[k]), wrc = cj(ww[k]);             // V(r,c), W(r,c)
+                c1 = fmad(vrc, s_t[c], c1);
+                c1 = fmad(wrc, s_t[nb + c], c1);
+                c2 = fmad(vrc, s_row[c], c2);                          // V(r,c) conj(W(i-1,c)) : s_row[c] = Wt[c, i-1] = conj(W(i-1,c))
+                c2 = fmad(wrc, s_row[nb + c], c2);
+            }
         }
     }
     // (all 32 lanes take part in the shuffles: a warp holds several rows, some of which may lie beyond m)
 #pragma unroll
     for (int o = kCombineTPR / 2; o > 0; o >>= 1) { y = add(y, shfl_xor(y, o)); c1 = add(c1, shfl_xor(c1, o)); c2 = add(c2, shfl_xor(c2, o)); }
     if (r < m && l8 == 0) {
-        const T ur = p.u[r];
         T v = mul(sc.s, (r == m - 1) ? sub(ur, from_real(sc.beta, T{})) : ur);
         if (r == m - 1 && !is_zero(sc.s)) v = from_real(1.0, T{});   // (an identity reflector keeps v = 0)
-        T acol = p.A[r + (long long)(m - 1) * p.ld];
         if (r == m - 1) acol = real_only(acol);
         T wpr = sub(mul(sc.s, sub(y, rscale(acol, sc.beta))), c1);
         p.Vt[jp + (long long)r * nb] = cj(v);
