@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--shard-shares", type=int, default=0,
                     help="NEXT-3: time, on ONE GPU and one after the other, the share each of R ranks would run (not the headline)")
     ap.add_argument("--batch-complex", action="store_true")
+    ap.add_argument("--shard-chol", type=int, default=0,
+                    help="NEXT-3: gs_cholesky_sharded with R ranks emulated on ONE GPU (R plans, R streams) and the model projection")
     return ap.parse_args()
 
 
@@ -682,6 +684,104 @@ def run_sharded(args):
     replicas.finalize(info)
 
 
+def run_shard_chol(args):
+    """NEXT-3, step 1 over R ranks (gs_cholesky_sharded), on ONE GPU: (a) the look-ahead factorisation of the contract
+    path, (b) the same entry point with one rank (no look-ahead, one stream), (c) R emulated ranks = R plans on R streams
+    sharing the device (correctness and the total work incl. the copies -- NOT a parallel time), (d) the serial part:
+    the owner's diagonal-block chain, timed as a one-rank factorisation of one panel plus one block, times the number of
+    panels.  Projection at R GPUs, compute only: chain + (one-rank time - chain) / R."""
+    import torch
+
+    from paper_2502_02460_b200 import gs
+    from paper_2502_02460_b200 import workloads as wl
+
+    torch.cuda.set_device(0)
+    R = args.shard_chol
+    cfg = wl.CONFIGS[args.config]
+    N, cplx = cfg.N, cfg.complex
+    pen = wl.make_config(cfg, device="cuda")
+    dtc = gs.GS_COMPLEX128 if cplx else gs.GS_REAL64
+
+    def timed(fn, prep):
+        ts = []
+        for it in range(args.warmup + args.steps):
+            prep()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= args.warmup:
+                ts.append(e0.elapsed_time(e1))
+        return sum(ts) / len(ts)
+
+    plan = gs.Plan(N, 0, dtype=dtc)
+    U = wl.colmajor_empty(N, N, dtype=pen.S.dtype, device="cuda")
+    t_look = timed(lambda: plan.cholesky(U), lambda: U.copy_(pen.S))
+    t_one = timed(lambda: plan.cholesky_sharded(U, 0, 1), lambda: U.copy_(pen.S))
+    plan.last_info()
+    U_ref = U.clone()
+    panel = plan.block * 8
+    npanels = (N + panel - 1) // panel
+    Np = min(N, panel + plan.block)
+    pp = gs.Plan(Np, 0, dtype=dtc)
+    Sp = wl.to_colmajor(pen.S[:Np, :Np].contiguous())
+    Up = torch.empty_like(Sp)
+    t_panel = timed(lambda: pp.cholesky_sharded(Up, 0, 1), lambda: Up.copy_(Sp))
+    pp.last_info()
+    pp.close()
+    plans = [plan] + [gs.Plan(N, 0, dtype=dtc) for _ in range(R - 1)]
+    streams = [torch.cuda.Stream() for _ in range(R)]
+    Us = [U] + [wl.colmajor_empty(N, N, dtype=pen.S.dtype, device="cuda") for _ in range(R - 1)]
+    flags = [torch.zeros(R, dtype=torch.int32, device="cuda") for _ in range(R)]
+    nep = plan.cholesky_sharded_epochs()
+    state = {"epoch": 0}
+
+    def prep():
+        for x in Us:
+            x.copy_(pen.S)
+
+    def emul():
+        # one host thread per emulated rank (as one process per GPU would be): a rank's stream blocks on its waits, and a
+        # single thread that filled one stream's launch queue could never get to enqueue the rank it is waiting for
+        import threading
+        ev = torch.cuda.Event()
+        ev.record()
+
+        def rank_program(r):
+            torch.cuda.set_device(0)
+            streams[r].wait_event(ev)
+            plans[r].cholesky_sharded(Us[r], r, R, [x.data_ptr() for x in Us], [pl.workspace.data_ptr() for pl in plans],
+                                      [f.data_ptr() for f in flags], epoch0=state["epoch"], stream=streams[r])
+        th = [threading.Thread(target=rank_program, args=(r,)) for r in range(R)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        state["epoch"] += nep
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+    t_emul = timed(emul, prep) if R > 1 else t_one
+    for pl in plans:
+        pl.last_info()
+    same = all(bool(torch.equal(x, Us[0])) for x in Us)
+    err = float((torch.triu(Us[0]) - torch.triu(U_ref)).norm() / torch.triu(U_ref).norm())
+    t_chain = min(npanels * t_panel, t_one)
+    t_proj = t_chain + (t_one - t_chain) / R
+    flop = wl.nominal_flops(N, 0, cplx)["cholesky"]
+    print(json.dumps({"metric": "step 1 (Cholesky) over R ranks, gs_cholesky_sharded, emulated on one GPU + model projection (NEXT-3, not the headline)",
+                      "unit": "ms", "n_gpus": 1, "ranks": R, "steps": args.steps, "warmup": args.warmup, "dtype": "c128" if cplx else "f64",
+                      "data": "synthetic", "config": {"workload": f"shard_chol_R{R}_{cfg.name}"},
+                      "value": t_proj,
+                      "detail": {"cholesky_lookahead_ms": t_look, "sharded_one_rank_ms": t_one, "emulated_R_ranks_on_one_gpu_ms": t_emul,
+                                 "one_panel_ms": t_panel, "panels": npanels, "chain_ms": t_chain,
+                                 "projected_R_gpus_ms": t_proj, "projected_tflops": flop / (t_proj * 1e-3) / 1e12,
+                                 "all_ranks_bit_identical": same, "rel_frob_vs_one_rank": err,
+                                 "note": "projection = owner's diagonal-block chains (serial) + the rest / R; copies over NVLink and flag latency not included"}}))
+    assert same and err <= 1e-12
+
+
 def run_shard_shares(args):
     """NEXT-3: the column-range calls of every one of R ranks, timed on ONE GPU one rank
     after the other.  No multi-GPU hardware is available to this run, so the exchange is not timed: the
@@ -770,6 +870,9 @@ def main():
         return
     if args.shard_shares > 0:
         run_shard_shares(args)
+        return
+    if args.shard_chol > 0:
+        run_shard_chol(args)
         return
     if args.sharded and args.impl == "ours":
         run_sharded(args)

@@ -112,6 +112,32 @@ gs_status_t gs_to_standard(gs_plan_t* plan, const void* H, const void* Uinv, voi
 gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctilde, void* C,
                              void* cuda_stream);
 
+/* Step 1 over the GPUs of one NVSwitch domain (and the paper's
+ * multi-GPU direction PAPER.md:118): one process per GPU, every rank calls it with its own copy of S
+ * (N x N, ld N, upper triangle referenced) and on return -- in stream order -- holds the COMPLETE factor U in it
+ * (upper triangle; zeros below), the same bits on every rank.
+ * Panels of the plan's panel width (8 blocks of 128, 64 for GS_COMPLEX128) are dealt round-robin: panel p belongs
+ * to rank p mod nranks, which keeps the block columns of its panels up to date and nothing else.  Per panel the
+ * owner factors and inverts the diagonal block and copies both into every rank; every rank then forms its own
+ * pieces of the row panel U[p, q] = W_p^H S[p, q] and stores them into its own S AND into every peer's S (the
+ * all-gather of the row panel, fused into the producing side), and applies the trailing update to its own panels.
+ *   peer_S[s], peer_workspace[s]  rank s's S buffer and the workspace of its plan (same N, dtype: same layout) as
+ *                                 mapped in this process (gs_ipc_open; entry `rank` = this rank's own S_inout and
+ *                                 the plan's workspace);
+ *   flags[s]                      rank s's array of nranks 32-bit flags (zero before the first call; entry `rank`
+ *                                 local).  Rank r writes slot r of every peer's array and waits on its own array
+ *                                 (gs_exchange_signal / gs_exchange_wait: stream memory operations, no host
+ *                                 synchronisation, no spinning kernel);
+ *   epoch0                        the call uses the flag values epoch0 + 1 (every rank's S is in place: nothing is stored
+ *                                 into a buffer its owner is still filling) ... epoch0 + gs_cholesky_sharded_epochs();
+ *                                 every rank passes the same value and raises it by that count from call to call.
+ * nranks == 1 needs no peers (NULL) and is a plain, look-ahead-free factorisation.  nranks <= 8.  One stream per
+ * rank, no look-ahead: the owner's diagonal-block chain is exposed once per panel.  Every rank signals whatever its
+ * numerical status (a failed rank's kernels are no-ops, its signals are not): agree on gs_last_info afterwards. */
+gs_status_t gs_cholesky_sharded_epochs(const gs_plan_t* plan, uint32_t* count);
+gs_status_t gs_cholesky_sharded(gs_plan_t* plan, void* S_inout, int rank, int nranks, void* const* peer_S,
+                                void* const* peer_workspace, void* const* flags, uint32_t epoch0, void* cuda_stream);
+
 /* Column-range forms of steps 2, 3 and of the back-transformation: the path sharded over the
  * GPUs of one NVSwitch domain (the paper's multi-GPU direction,
  * PAPER.md:118).  Every rank holds U (step 1 is replicated) and owns a contiguous

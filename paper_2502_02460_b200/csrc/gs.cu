@@ -180,6 +180,34 @@ bool overlaps(const void* a, size_t na, const void* b, size_t nb)
 size_t mat_bytes(const gs_plan* p) { return size_t(p->N) * size_t(p->N) * p->es; }
 size_t vec_bytes(const gs_plan* p) { return size_t(p->N) * size_t(p->nev) * p->es; }
 
+// Device-side ordering of the fused exchange: stream memory operations (see include/gs.h).
+typedef CUresult (*StreamValue32Fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+StreamValue32Fn stream_value_fn(const char* name)
+{
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint(name, &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return nullptr;
+    return reinterpret_cast<StreamValue32Fn>(fn);
+}
+gs_status_t stream_values(gs_plan* plan, bool wait, int count, void* const* flags, uint32_t value, void* cuda_stream)
+{
+    if (plan == nullptr || count < 0 || count > 64 || (count > 0 && flags == nullptr)) return GS_ERR_INVALID_ARG;
+    for (int d = 0; d < count; ++d)
+        if (flags[d] == nullptr || (reinterpret_cast<uintptr_t>(flags[d]) & 3u) != 0) return GS_ERR_INVALID_ARG;
+    static StreamValue32Fn wr = stream_value_fn("cuStreamWriteValue32"), wt = stream_value_fn("cuStreamWaitValue32");
+    StreamValue32Fn fn = wait ? wt : wr;
+    if (fn == nullptr) return GS_ERR_CUDA;
+    for (int d = 0; d < count; ++d) {
+        const CUresult r = fn(static_cast<CUstream>(cuda_stream), reinterpret_cast<CUdeviceptr>(flags[d]), value,
+                              wait ? unsigned(CU_STREAM_WAIT_VALUE_GEQ) : unsigned(CU_STREAM_WRITE_VALUE_DEFAULT));
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(plan->cuda_error, sizeof(plan->cuda_error), "%s failed (CUresult %d)", wait ? "cuStreamWaitValue32" : "cuStreamWriteValue32", int(r));
+            return GS_ERR_CUDA;
+        }
+    }
+    return GS_OK;
+}
+
 // A stage under construction: knows whether every operand can go through TMA.
 struct Stage {
     gs_plan* plan;
@@ -583,6 +611,126 @@ struct Potrf {
         return GS_OK;
     }
 };
+
+// ------------------------------------------------------------------------------------------------
+// gs_cholesky_sharded: step 1 over the R GPUs of one NVSwitch domain.  Panels of potrf_nb blocks are dealt
+// round-robin (panel p belongs to rank p mod R); a rank keeps the block columns of its own panels up to date
+// and nothing else.  Per panel p = block rows [s1, s2), owner o:
+//   o     : factor the diagonal block and invert it (the single-GPU chain: leaf kernels, one-tile solves, doubling),
+//           copy U_pp and W_p = U_pp^-1 into every rank (copy_block_push_kernel), signal a_p
+//   all   : wait a_p; for each own panel q > p:  U[p, q] = W_p^T S[p, q]  (one engine launch into the workspace),
+//           copied into the own S AND into every peer's S -- the all-gather of the row panel, rank by rank, piece
+//           by piece; signal b_p; wait for b_p of every rank
+//   all   : for each own panel q > p:  S[(p, q], q] -= U[p, (p, q]]^T U[p, q]   (rectangle + upper diagonal block)
+// (before the first panel every rank signals that its S is in place and waits for the others: nothing is stored into a
+// buffer its owner is still filling)
+// Ordering is on the device (gs_exchange_signal / gs_exchange_wait on flags[rank][source]); one stream per rank,
+// no look-ahead.  On return (stream order) every rank holds the complete U.
+// ------------------------------------------------------------------------------------------------
+struct ShardedChol {
+    int rank, nranks;
+    void* const* peer_S;       // nranks entries (own entry = the rank's S)
+    void* const* peer_ws;      // nranks entries: workspace base of every rank's plan (same geometry)
+    void* const* flags;        // nranks entries: flag array (nranks x uint32) of every rank, own entry local
+    uint32_t epoch0;
+};
+
+gs_status_t sharded_copy(Potrf& f, const void* src, long long lds, int srow0, int scol0, const PushTargets& dst, long long ldd,
+                         int drow0, int dcol0, int rows, int cols, bool upper_only)
+{
+    gs_plan* plan = f.st.plan;
+    if (rows <= 0 || cols <= 0 || dst.n == 0) return GS_OK;
+    dim3 grid(cols, (rows + 255) / 256);
+    LaunchTimer timer(plan, L_POTRF_TRSM, f.st.stream);
+    cudaError_t e;
+    if (f.st.z)
+        e = launch_pdl(copy_block_push_kernel<double2>, grid, 256, 0, f.st.stream, static_cast<const double2*>(src), lds, srow0, scol0, dst, ldd,
+                       drow0, dcol0, rows, upper_only ? 1 : 0, static_cast<const int*>(info_ptr(plan)));
+    else
+        e = launch_pdl(copy_block_push_kernel<double>, grid, 256, 0, f.st.stream, static_cast<const double*>(src), lds, srow0, scol0, dst, ldd,
+                       drow0, dcol0, rows, upper_only ? 1 : 0, static_cast<const int*>(info_ptr(plan)));
+    if (e != cudaSuccess) return cuda_fail(plan, e);
+    plan->launches += 1;
+    return GS_OK;
+}
+
+gs_status_t factor_sharded(Potrf& f, const ShardedChol& sh, cudaStream_t stream)
+{
+    gs_plan* plan = f.st.plan;
+    const int N = int(plan->N), n = plan->nblk, lb = f.st.lb, R = sh.nranks, me = sh.rank;
+    const int nbp = plan->potrf_nb < n ? plan->potrf_nb : n;
+    const int np = (n + nbp - 1) / nbp;
+    const int ldw = wp_ld(plan);
+    auto start = [&](int p) { return p * nbp < n ? p * nbp : n; };
+    auto el = [&](int b) { return b * lb < N ? b * lb : N; };      // first element of block b, clipped
+    // flags: slot `me` of every other rank's array; own slots of every other rank
+    std::vector<void*> sig, wt_all;
+    for (int s = 0; s < R; ++s) {
+        if (s == me) continue;
+        sig.push_back(static_cast<unsigned char*>(sh.flags[s]) + 4 * size_t(me));
+        wt_all.push_back(static_cast<unsigned char*>(sh.flags[me]) + 4 * size_t(s));
+    }
+    f.st.stream = stream;
+    GS_TRY(zero_lower(f.st, f.S));
+    // every rank's S is in place (whatever the caller enqueued before this call) before anything is stored into it
+    if (!sig.empty()) {
+        GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), sh.epoch0 + 1u, stream));
+        GS_TRY(stream_values(plan, true, int(wt_all.size()), wt_all.data(), sh.epoch0 + 1u, stream));
+    }
+    for (int p = 0; p < np; ++p) {
+        const int s1 = start(p), s2 = start(p + 1), o = p % R;
+        const uint32_t a_p = sh.epoch0 + 2u * uint32_t(p) + 2u, b_p = a_p + 1u;
+        const MatView W{wp_ptr(plan, p), ldw, ldw, ldw};
+        if (me == o) {
+            f.vW = W;
+            GS_TRY(f.panel_diag(s1, s2, n));
+            // U_pp (upper triangle) and, if a row panel follows, W_p into every other rank
+            PushTargets ts{}, tw{};
+            for (int s = 0; s < R; ++s) {
+                if (s == me) continue;
+                ts.ptr[ts.n++] = sh.peer_S[s];
+                tw.ptr[tw.n++] = static_cast<unsigned char*>(sh.peer_ws[s]) + (static_cast<unsigned char*>(wp_ptr(plan, p)) - plan->ws);
+            }
+            const int rows = el(s2) - el(s1);
+            GS_TRY(sharded_copy(f, f.S, plan->N, el(s1), el(s1), ts, plan->N, el(s1), el(s1), rows, rows, false));   // (with the zeros below its diagonal)
+            if (s2 < n) GS_TRY(sharded_copy(f, W.ptr, ldw, 0, 0, tw, ldw, 0, 0, rows, rows, false));
+            if (!sig.empty()) GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), a_p, stream));
+        } else {
+            void* w = static_cast<unsigned char*>(sh.flags[me]) + 4 * size_t(o);
+            GS_TRY(stream_values(plan, true, 1, &w, a_p, stream));
+        }
+        if (s2 >= n) break;
+        // own pieces of row panel p: into the workspace, then into the own S and every peer's S
+        PushTargets all{};
+        for (int s = 0; s < R; ++s) all.ptr[all.n++] = sh.peer_S[s];
+        for (int q = p + 1; q < np; ++q) {
+            if (q % R != me) continue;
+            const int c0 = start(q), c1 = start(q + 1);
+            EngineParams ep = blank_params(plan);
+            if (!set_operand(f.st, ep, 0, W, false) || !set_operand(f.st, ep, 1, f.vS, false)) return GS_ERR_CUDA;
+            ep.C = static_cast<double*>(const_cast<void*>(f.vT.ptr)); ep.ldc = f.vT.ld;
+            ep.tiles_m = s2 - s1; ep.tiles_n = c1 - c0; ep.order = ORDER_ROW_REV;
+            ep.c_row0 = s1 * lb; ep.c_col0 = c0 * lb; ep.c_rows = int(f.vT.rows); ep.c_cols = int(f.vT.cols);
+            ep.khi_c = KPB; ep.khi_i = KPB; ep.kmax = (s2 - s1) * (KPB);
+            ep.a.k0 = 0; ep.a.x0 = 0;
+            ep.b.k0 = s1 * lb; ep.b.x0 = c0 * lb;
+            GS_TRY(launch(f.st, ep, false, L_POTRF_TRSM));
+            GS_TRY(sharded_copy(f, f.vT.ptr, f.vT.ld, el(s1), el(c0), all, plan->N, el(s1), el(c0), el(s2) - el(s1), el(c1) - el(c0), false));
+        }
+        if (!sig.empty()) {
+            GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), b_p, stream));
+            GS_TRY(stream_values(plan, true, int(wt_all.size()), wt_all.data(), b_p, stream));
+        }
+        // trailing update of the own panels
+        for (int q = p + 1; q < np; ++q) {
+            if (q % R != me) continue;
+            const int c0 = start(q), c1 = start(q + 1);
+            if (c0 > s2) GS_TRY(f.gemm_update(s1, s2, c0, c0, c1));        // rows (p, q) of the block columns of q
+            GS_TRY(f.syrk(s1, s2, c0, c1));                                  // the diagonal block of q, upper tiles
+        }
+    }
+    return GS_OK;
+}
 
 gs_status_t ensure_side_stream(gs_plan* plan)
 {
@@ -1085,36 +1233,6 @@ gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int c
     return GS_OK;
 }
 
-// Device-side ordering of the fused exchange: stream memory operations (see include/gs.h).
-namespace {
-typedef CUresult (*StreamValue32Fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
-StreamValue32Fn stream_value_fn(const char* name)
-{
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint(name, &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return nullptr;
-    return reinterpret_cast<StreamValue32Fn>(fn);
-}
-gs_status_t stream_values(gs_plan* plan, bool wait, int count, void* const* flags, uint32_t value, void* cuda_stream)
-{
-    if (plan == nullptr || count < 0 || count > 64 || (count > 0 && flags == nullptr)) return GS_ERR_INVALID_ARG;
-    for (int d = 0; d < count; ++d)
-        if (flags[d] == nullptr || (reinterpret_cast<uintptr_t>(flags[d]) & 3u) != 0) return GS_ERR_INVALID_ARG;
-    static StreamValue32Fn wr = stream_value_fn("cuStreamWriteValue32"), wt = stream_value_fn("cuStreamWaitValue32");
-    StreamValue32Fn fn = wait ? wt : wr;
-    if (fn == nullptr) return GS_ERR_CUDA;
-    for (int d = 0; d < count; ++d) {
-        const CUresult r = fn(static_cast<CUstream>(cuda_stream), reinterpret_cast<CUdeviceptr>(flags[d]), value,
-                              wait ? unsigned(CU_STREAM_WAIT_VALUE_GEQ) : unsigned(CU_STREAM_WRITE_VALUE_DEFAULT));
-        if (r != CUDA_SUCCESS) {
-            std::snprintf(plan->cuda_error, sizeof(plan->cuda_error), "%s failed (CUresult %d)", wait ? "cuStreamWaitValue32" : "cuStreamWriteValue32", int(r));
-            return GS_ERR_CUDA;
-        }
-    }
-    return GS_OK;
-}
-}  // namespace
-
 gs_status_t gs_exchange_signal(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream)
 {
     return stream_values(plan, false, count, flags, value, cuda_stream);
@@ -1199,6 +1317,60 @@ gs_status_t gs_density_matrix(gs_plan_t* plan, const void* C_, const double* f, 
     p.khi_c = (nev + st.bk - 1) / st.bk; p.kmax = p.khi_c;
     p.flags = F_STORE_UPPER | F_REAL_DIAG;
     return launch(st, p, false, L_DENS_SYRK);
+}
+
+gs_status_t gs_cholesky_sharded_epochs(const gs_plan_t* plan, uint32_t* count)
+{
+    if (plan == nullptr || count == nullptr) return GS_ERR_INVALID_ARG;
+    const int nbp = plan->potrf_nb < plan->nblk ? plan->potrf_nb : plan->nblk;
+    *count = 2u * uint32_t((plan->nblk + nbp - 1) / nbp) + 1u;
+    return GS_OK;
+}
+
+gs_status_t gs_cholesky_sharded(gs_plan_t* plan, void* S_inout, int rank, int nranks, void* const* peer_S, void* const* peer_workspace,
+                                void* const* flags, uint32_t epoch0, void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (S_inout == nullptr || !aligned16(S_inout) || nranks < 1 || nranks > kMaxPeers || rank < 0 || rank >= nranks) return GS_ERR_INVALID_ARG;
+    if (nranks > 1) {
+        if (peer_S == nullptr || peer_workspace == nullptr || flags == nullptr) return GS_ERR_INVALID_ARG;
+        for (int s = 0; s < nranks; ++s) {
+            if (peer_S[s] == nullptr || !aligned16(peer_S[s]) || peer_workspace[s] == nullptr || (reinterpret_cast<uintptr_t>(peer_workspace[s]) & 255u) != 0 ||
+                flags[s] == nullptr || (reinterpret_cast<uintptr_t>(flags[s]) & 3u) != 0)
+                return GS_ERR_INVALID_ARG;
+        }
+        if (peer_S[rank] != S_inout || peer_workspace[rank] != plan->ws) return GS_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    GS_TRY(configure_leaf(plan));
+    // Every kernel of the call is loaded BEFORE the first wait is enqueued: with lazy module loading the first launch of
+    // a kernel may synchronise with the device, and a stream that sits in a wait for a rank whose work this very host
+    // thread has yet to enqueue would never let it return.
+    {
+        static PerDeviceOnce once;
+        const cudaError_t pe = once.run([]() -> cudaError_t {
+            cudaError_t r = engine_configure();
+            cudaFuncAttributes fa;
+            if (r == cudaSuccess) r = cudaFuncGetAttributes(&fa, copy_block_push_kernel<double>);
+            if (r == cudaSuccess) r = cudaFuncGetAttributes(&fa, copy_block_push_kernel<double2>);
+            if (r == cudaSuccess) r = cudaFuncGetAttributes(&fa, zero_lower_blocks_kernel<double, LB>);
+            if (r == cudaSuccess) r = cudaFuncGetAttributes(&fa, zero_lower_blocks_kernel<double2, CLB>);
+            return r;
+        });
+        if (pe != cudaSuccess) return cuda_fail(plan, pe);
+    }
+    GS_CUDA(plan, cudaMemsetAsync(info_ptr(plan), 0, sizeof(int), stream));
+    Potrf f;
+    f.st = make_stage(plan, stream);
+    f.S = S_inout;
+    f.vS = MatView{S_inout, plan->N, plan->N, plan->N};
+    f.vT = MatView{big_ptr(plan), plan->N, plan->N, plan->N};
+    f.pb = 0;
+    void* self_S[1] = {S_inout};
+    void* self_ws[1] = {plan->ws};
+    void* self_flags[1] = {plan->ws};     // (never used with one rank)
+    ShardedChol sh{rank, nranks, nranks > 1 ? peer_S : self_S, nranks > 1 ? peer_workspace : self_ws, nranks > 1 ? flags : self_flags, epoch0};
+    return factor_sharded(f, sh, stream);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -524,6 +524,26 @@ __global__ void push_band_kernel(const T* __restrict__ src, PushTargets dst, lon
     }
 }
 
+// dst_d[drow0 + r, dcol0 + c] = src[srow0 + r, scol0 + c] for r < rows, c = blockIdx.x, for each of the n targets
+// (all with leading dimension ldd): the pieces of the sharded factorisation (gs_cholesky_sharded) that no engine
+// epilogue carries -- a finished row-panel piece, copied out of the workspace into the rank's own S and into every
+// peer's S; the factored diagonal block and its inverse.  upper_only: only rows r <= c (a triangular block).
+template <typename T>
+__global__ void copy_block_push_kernel(const T* __restrict__ src, long long lds, int srow0, int scol0, PushTargets dst, long long ldd,
+                                       int drow0, int dcol0, int rows, int upper_only, const int* info)
+{
+    grid_dep_launch();
+    grid_dep_wait();
+    if (*info != 0) return;
+    const int c = blockIdx.x;
+    const int r = blockIdx.y * blockDim.x + threadIdx.x;
+    if (r < rows && (!upper_only || r <= c)) {
+        const T v = src[srow0 + r + (long long)(scol0 + c) * lds];
+        const long long off = drow0 + r + (long long)(dcol0 + c) * ldd;
+        for (int d = 0; d < dst.n; ++d) static_cast<T*>(dst.ptr[d])[off] = v;
+    }
+}
+
 // dst[row0 + r, col0 + c] = src[row0 + r, col0 + c] for r < rows; one grid column (blockIdx.x) per column c.
 template <typename T>
 __global__ void copy_block_kernel(const T* __restrict__ src, T* __restrict__ dst, long long ld, int row0, int rows,

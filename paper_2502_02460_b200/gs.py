@@ -28,7 +28,7 @@ STATUS_NAMES = {
 }
 EXPORTS = (
     "gs_plan_create", "gs_plan_destroy", "gs_plan_workspace_bytes", "gs_plan_set_workspace",
-    "gs_cholesky", "gs_cholesky_leading", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_density_matrix_static", "gs_last_info", "gs_plan_clear_info",
+    "gs_cholesky", "gs_cholesky_leading", "gs_cholesky_sharded", "gs_cholesky_sharded_epochs", "gs_invert_triangular", "gs_to_standard", "gs_backtransform", "gs_density_matrix", "gs_density_matrix_static", "gs_last_info", "gs_plan_clear_info",
     "gs_invert_triangular_cols", "gs_to_standard_g_cols", "gs_to_standard_cols", "gs_backtransform_cols",
     "gs_plan_set_push_targets", "gs_ipc_export", "gs_ipc_open", "gs_ipc_close", "gs_exchange_signal", "gs_exchange_wait",
     "gs_reduce_host_scratch_bytes", "gs_reduce_host_h2d_bytes", "gs_reduce_host_d2h_bytes", "gs_reduce_host", "gs_backtransform_host",
@@ -79,6 +79,8 @@ def lib() -> ctypes.CDLL:
         L.gs_cholesky.argtypes = [vp, vp, vp]
         L.gs_cholesky_leading.argtypes = [vp, vp, i64, vp]
         L.gs_invert_triangular.argtypes = [vp, vp, vp, vp]
+        L.gs_cholesky_sharded.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.c_uint32, vp]
+        L.gs_cholesky_sharded_epochs.argtypes = [vp, ctypes.POINTER(ctypes.c_uint32)]
         L.gs_to_standard.argtypes = [vp, vp, vp, vp, vp]
         L.gs_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_density_matrix.argtypes = [vp, vp, vp, vp, vp]
@@ -204,6 +206,19 @@ class Plan:
     def cholesky_leading(self, S: torch.Tensor, ncols: int, stream=None):
         """Step 1 on the leading ncols x ncols block only (sharded path)."""
         self._check(lib().gs_cholesky_leading(self._h, _dev_ptr(S, self.N, self.N, self.tdtype), ncols, _stream_ptr(stream)))
+
+    def cholesky_sharded_epochs(self) -> int:
+        n = ctypes.c_uint32(0)
+        self._check(lib().gs_cholesky_sharded_epochs(self._h, ctypes.byref(n)))
+        return int(n.value)
+
+    def cholesky_sharded(self, S: torch.Tensor, rank: int, nranks: int, peer_S=None, peer_workspace=None, flags=None, epoch0: int = 0, stream=None):
+        """Step 1 over `nranks` GPUs (gs_cholesky_sharded): peer_S / peer_workspace / flags are lists of nranks device
+        addresses (ints) as mapped in this process; entry `rank` = S.data_ptr() / self.workspace.data_ptr() / the local flags."""
+        def arr(v):
+            return None if v is None else (ctypes.c_void_p * nranks)(*[int(x) for x in v])
+        self._check(lib().gs_cholesky_sharded(self._h, _dev_ptr(S, self.N, self.N, self.tdtype), rank, nranks, arr(peer_S), arr(peer_workspace),
+                                              arr(flags), epoch0 & 0xFFFFFFFF, _stream_ptr(stream)))
 
     def invert_triangular(self, U: torch.Tensor, Uinv: torch.Tensor, stream=None):
         self._check(lib().gs_invert_triangular(self._h, _dev_ptr(U, self.N, self.N, self.tdtype),

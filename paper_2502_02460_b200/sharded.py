@@ -2,11 +2,13 @@
 (SURVEY.md section 8(f) NEXT-3; the paper's multi-GPU direction, PAPER.md:118, PAPER.md:138;
 DESIGN.md section 9).
 
-One process per GPU.  Every rank holds H, S and forms the part of U it needs itself: step 1 does not
-shard (each panel depends on all earlier trailing updates), but the leading principal blocks of a
-Cholesky factor nest -- chol(S[:k,:k]) = U[:k,:k] -- and a rank that owns columns up to k needs no more
-than that block (gs_cholesky_leading; the same kernels give the same bits on every rank).  After that
-the work is split by COLUMN RANGES, which need no exchange while they are formed:
+One process per GPU.  Every rank holds H, S.  Step 1, two forms: chol="leading" -- every rank forms the part of
+U it needs itself: the leading principal blocks of a Cholesky factor nest, chol(S[:k,:k]) = U[:k,:k], and a rank
+that owns columns up to k needs no more than that block (gs_cholesky_leading; the same kernels give the same bits
+on every rank; the last rank factors all of S) -- or chol="sharded" (push exchange with device-side ordering
+only) -- gs_cholesky_sharded: the panels are dealt round-robin over the ranks, the owner's factored diagonal block
+and every rank's pieces of the row panel are stored into all ranks, the trailing update of a panel's block columns
+is its owner's.  After that the work is split by COLUMN RANGES, which need no exchange while they are formed:
 
     rank r owns the block columns J_r = [c_r, c_{r+1}) of U^-1, of G = T U^-1 and of H~
       1. V[:, J_r]  = (U^-1)[:, J_r]                (gs_invert_triangular_cols)
@@ -163,15 +165,27 @@ class ShardedReduction:
     """Host driver of the sharded path for one rank.  `plan` is a gs.Plan (or, in the CPU test of this
     host logic, an object with the same column-range methods -- exchange="collective" only)."""
 
-    def __init__(self, plan, rank: int = 0, world: int = 1, group=None, exchange: str = "collective", sync: str = "host"):
+    def __init__(self, plan, rank: int = 0, world: int = 1, group=None, exchange: str = "collective", sync: str = "host",
+                 chol: str = "leading"):
         if exchange not in ("collective", "push"):
             raise ValueError("exchange must be 'collective' or 'push'")
         if sync not in ("host", "device"):
             raise ValueError("sync must be 'host' or 'device'")
+        if chol not in ("leading", "sharded"):
+            raise ValueError("chol must be 'leading' (every rank factors the leading block it needs) or 'sharded' "
+                             "(gs_cholesky_sharded: panels dealt round-robin over the ranks)")
+        if chol == "sharded" and world > 1 and not (exchange == "push" and sync == "device"):
+            raise ValueError("chol='sharded' stores into the peers' buffers and orders itself by device-side flags: "
+                             "it needs exchange='push' and sync='device'")
+        if chol == "sharded" and world > 8:
+            raise ValueError("chol='sharded': at most 8 ranks (one NVSwitch domain)")
         self.plan = plan
         self.rank, self.world, self.group = int(rank), int(world), group
         self.push = exchange == "push" and self.world > 1
         self.device_sync = self.push and sync == "device"
+        self.chol_sharded = chol == "sharded" and self.world > 1
+        self.chol_epoch = 0
+        self.U_ptrs = self.ws_ptrs = self.chol_flags = self.chol_flag_ptrs = None
         self.epoch = 0
         self.flags = None            # int32[2 * world]: ready slots, then done slots (device sync)
         self.flag_ptrs = None        # this rank's view of every rank's flag array
@@ -234,6 +248,15 @@ class ShardedReduction:
                 torch.cuda.synchronize(like.device)
                 self.flag_ptrs = self.peers.map_all(self.flags)
                 self.epoch = 0
+            if self.chol_sharded:
+                # step 1 over the ranks: the peers' U buffers and plan workspaces (the inverted diagonal blocks travel
+                # through them) and a flag array of its own
+                self.U_ptrs = self.peers.map_all(res.U)
+                self.ws_ptrs = self.peers.map_all(self.plan.workspace)
+                self.chol_flags = torch.zeros(self.world, dtype=torch.int32, device=like.device)
+                torch.cuda.synchronize(like.device)
+                self.chol_flag_ptrs = self.peers.map_all(self.chol_flags)
+                self.chol_epoch = 0
             self._barrier()
         return res
 
@@ -298,9 +321,16 @@ class ShardedReduction:
         done_out, done_in = self._slots(1)
         if e > 1:
             plan.exchange_wait(done_in, e - 1, stream=stream)     # the peers have read what the last round pushed
-        if c1 > c0:
+        if self.chol_sharded:
+            # every rank takes part (it owns panels whatever its column range) and ends up with ALL of U
+            res.U.copy_(S)
+            plan.cholesky_sharded(res.U, self.rank, self.world, self.U_ptrs, self.ws_ptrs, self.chol_flag_ptrs,
+                                  epoch0=self.chol_epoch, stream=stream)
+            self.chol_epoch += plan.cholesky_sharded_epochs()
+        elif c1 > c0:
             res.U.copy_(S)
             plan.cholesky_leading(res.U, c1, stream=stream)
+        if c1 > c0:
             plan.invert_triangular_cols(res.U, res.Uinv_work, c0, c1 - c0, stream=stream)
             plan.to_standard_g_cols(H, res.Uinv_work, res.G, c0, c1 - c0, stream=stream)
         plan.exchange_signal(ready_out, e, stream=stream)          # behind the kernels whose epilogues pushed the slabs

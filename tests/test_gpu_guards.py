@@ -59,7 +59,7 @@ def test_no_call_writes_outside_its_buffers(N, cplx):
     plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
     L = gs.lib()
     ws_bytes = plan.workspace.numel()
-    arena = Arena(20 * (N * N * es + 2 * GUARD) + ws_bytes + plan.evp_workspace_bytes() + 8 * GUARD)
+    arena = Arena(22 * (N * N * es + 2 * GUARD) + ws_bytes + plan.evp_workspace_bytes() + 8 * GUARD)
     ws = arena.take(ws_bytes)
     assert L.gs_plan_set_workspace(plan._h, ws.data_ptr(), ws_bytes) == 0
     H, S, U, V, Ht, G, Vw, Vx, Htx, P = (arena.matrix(N, N, dt) for _ in range(10))
@@ -93,6 +93,17 @@ def test_no_call_writes_outside_its_buffers(N, cplx):
     plan.backtransform_cols(V, Ct, C, 0, nev)
     assert plan.last_info() == 0
     plan.set_push_targets(gs.GS_PUSH_UINV, [])
+    # step 1 in its sharded form: two emulated ranks on this one stream would wait for each other, so one rank here (the
+    # same launches minus the copies; tests/test_gpu_sharded_chol.py runs the ranks), and the allocation-free density matrix
+    Us = arena.matrix(N, N, dt)
+    Us.copy_(S)
+    plan.cholesky_sharded(Us, 0, 1)
+    Ps = arena.matrix(N, N, dt)
+    Ps.copy_(P)
+    plan.density_matrix_static(C, f, Ps)
+    assert plan.last_info() == 0
+    assert torch.equal(torch.triu(Ps), torch.triu(P))
+    assert ((torch.triu(Us) - torch.triu(U)).norm() / torch.triu(U).norm()).item() < 1e-13
     # the standard eigensolver (NEXT-4), when the library has it
     if hasattr(plan, "standard_eigh"):
         A = arena.matrix(N, N, dt)

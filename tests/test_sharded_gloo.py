@@ -206,3 +206,20 @@ def _failing_worker(rank, world, port, out):
 def test_a_failing_rank_stops_every_rank():
     res = _spawn(_failing_worker, 2, ())
     assert res == [(0, (2, 77)), (1, (2, 77))]
+
+
+def test_sharded_cholesky_option_needs_the_push_exchange_with_device_ordering():
+    """chol='sharded' (gs_cholesky_sharded) stores into the peers' buffers: only with exchange='push', sync='device'."""
+    from paper_2502_02460_b200 import sharded
+
+    class P:
+        N, nev, block = 1024, 0, 128
+    for kw in ({"exchange": "collective"}, {"exchange": "push", "sync": "host"}):
+        with pytest.raises(ValueError):
+            sharded.ShardedReduction(P(), rank=0, world=2, chol="sharded", **kw)
+    with pytest.raises(ValueError):
+        sharded.ShardedReduction(P(), rank=0, world=2, chol="cyclic")
+    with pytest.raises(ValueError):
+        sharded.ShardedReduction(P(), rank=0, world=9, exchange="push", sync="device", chol="sharded")
+    r = sharded.ShardedReduction(P(), rank=0, world=1, chol="sharded")      # one rank: nothing to shard
+    assert not r.chol_sharded
