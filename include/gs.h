@@ -131,8 +131,9 @@ gs_status_t gs_backtransform(gs_plan_t* plan, const void* Uinv, const void* Ctil
  *   epoch0                        the call uses the flag values epoch0 + 1 (every rank's S is in place: nothing is stored
  *                                 into a buffer its owner is still filling) ... epoch0 + gs_cholesky_sharded_epochs();
  *                                 every rank passes the same value and raises it by that count from call to call.
- * nranks == 1 needs no peers (NULL) and is a plain, look-ahead-free factorisation.  nranks <= 8.  One stream per
- * rank, no look-ahead: the owner's diagonal-block chain is exposed once per panel.  Every rank signals whatever its
+ * nranks == 1 needs no peers (NULL).  nranks <= 8.  One stream per rank; the owner of the next panel updates that
+ * panel first and factors its diagonal block before its other updates (one panel of look-ahead), so the chain of a
+ * diagonal block runs beside the other ranks' trailing updates.  Every rank signals whatever its
  * numerical status (a failed rank's kernels are no-ops, its signals are not): agree on gs_last_info afterwards. */
 gs_status_t gs_cholesky_sharded_epochs(const gs_plan_t* plan, uint32_t* count);
 gs_status_t gs_cholesky_sharded(gs_plan_t* plan, void* S_inout, int rank, int nranks, void* const* peer_S,

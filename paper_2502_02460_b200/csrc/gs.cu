@@ -624,8 +624,10 @@ struct Potrf {
 //   all   : for each own panel q > p:  S[(p, q], q] -= U[p, (p, q]]^T U[p, q]   (rectangle + upper diagonal block)
 // (before the first panel every rank signals that its S is in place and waits for the others: nothing is stored into a
 // buffer its owner is still filling)
-// Ordering is on the device (gs_exchange_signal / gs_exchange_wait on flags[rank][source]); one stream per rank,
-// no look-ahead.  On return (stream order) every rank holds the complete U.
+// Look-ahead: the owner of panel p + 1 updates that panel first and factors its diagonal block before its other updates,
+// so a_{p+1} is usually there when the other ranks have finished their updates of panel p.
+// Ordering is on the device (gs_exchange_signal / gs_exchange_wait on flags[rank][source]); one stream per rank.
+// On return (stream order) every rank holds the complete U.
 // ------------------------------------------------------------------------------------------------
 struct ShardedChol {
     int rank, nranks;
@@ -677,28 +679,43 @@ gs_status_t factor_sharded(Potrf& f, const ShardedChol& sh, cudaStream_t stream)
         GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), sh.epoch0 + 1u, stream));
         GS_TRY(stream_values(plan, true, int(wt_all.size()), wt_all.data(), sh.epoch0 + 1u, stream));
     }
+    auto a_of = [&](int p) { return sh.epoch0 + 2u * uint32_t(p) + 2u; };
+    auto Wof = [&](int p) { return MatView{wp_ptr(plan, p), ldw, ldw, ldw}; };
+    // owner: factor and invert the diagonal block of panel p, copy U_pp and (if a row panel follows) W_p into every other
+    // rank, signal a_p
+    auto diag_block = [&](int p) -> gs_status_t {
+        const int s1 = start(p), s2 = start(p + 1);
+        f.vW = Wof(p);
+        GS_TRY(f.panel_diag(s1, s2, n));
+        PushTargets ts{}, tw{};
+        for (int s = 0; s < R; ++s) {
+            if (s == me) continue;
+            ts.ptr[ts.n++] = sh.peer_S[s];
+            tw.ptr[tw.n++] = static_cast<unsigned char*>(sh.peer_ws[s]) + (static_cast<unsigned char*>(wp_ptr(plan, p)) - plan->ws);
+        }
+        const int rows = el(s2) - el(s1);
+        GS_TRY(sharded_copy(f, f.S, plan->N, el(s1), el(s1), ts, plan->N, el(s1), el(s1), rows, rows, false));   // (with the zeros below its diagonal)
+        if (s2 < n) GS_TRY(sharded_copy(f, Wof(p).ptr, ldw, 0, 0, tw, ldw, 0, 0, rows, rows, false));
+        if (!sig.empty()) GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), a_of(p), stream));
+        return GS_OK;
+    };
+    auto update_panel = [&](int p, int q) -> gs_status_t {     // S[(p, q], q] -= U[p, (p, q]]^H U[p, q]
+        const int s1 = start(p), s2 = start(p + 1), c0 = start(q), c1 = start(q + 1);
+        if (c0 > s2) GS_TRY(f.gemm_update(s1, s2, c0, c0, c1));        // rows (p, q) of the block columns of q
+        return f.syrk(s1, s2, c0, c1);                                  // the diagonal block of q, upper tiles
+    };
+    bool have_diag = false;     // this rank factored the diagonal block of the current panel one iteration early
     for (int p = 0; p < np; ++p) {
         const int s1 = start(p), s2 = start(p + 1), o = p % R;
-        const uint32_t a_p = sh.epoch0 + 2u * uint32_t(p) + 2u, b_p = a_p + 1u;
-        const MatView W{wp_ptr(plan, p), ldw, ldw, ldw};
+        const uint32_t b_p = a_of(p) + 1u;
+        const MatView W = Wof(p);
         if (me == o) {
-            f.vW = W;
-            GS_TRY(f.panel_diag(s1, s2, n));
-            // U_pp (upper triangle) and, if a row panel follows, W_p into every other rank
-            PushTargets ts{}, tw{};
-            for (int s = 0; s < R; ++s) {
-                if (s == me) continue;
-                ts.ptr[ts.n++] = sh.peer_S[s];
-                tw.ptr[tw.n++] = static_cast<unsigned char*>(sh.peer_ws[s]) + (static_cast<unsigned char*>(wp_ptr(plan, p)) - plan->ws);
-            }
-            const int rows = el(s2) - el(s1);
-            GS_TRY(sharded_copy(f, f.S, plan->N, el(s1), el(s1), ts, plan->N, el(s1), el(s1), rows, rows, false));   // (with the zeros below its diagonal)
-            if (s2 < n) GS_TRY(sharded_copy(f, W.ptr, ldw, 0, 0, tw, ldw, 0, 0, rows, rows, false));
-            if (!sig.empty()) GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), a_p, stream));
+            if (!have_diag) GS_TRY(diag_block(p));
         } else {
             void* w = static_cast<unsigned char*>(sh.flags[me]) + 4 * size_t(o);
-            GS_TRY(stream_values(plan, true, 1, &w, a_p, stream));
+            GS_TRY(stream_values(plan, true, 1, &w, a_of(p), stream));
         }
+        have_diag = false;
         if (s2 >= n) break;
         // own pieces of row panel p: into the workspace, then into the own S and every peer's S
         PushTargets all{};
@@ -721,12 +738,17 @@ gs_status_t factor_sharded(Potrf& f, const ShardedChol& sh, cudaStream_t stream)
             GS_TRY(stream_values(plan, false, int(sig.size()), sig.data(), b_p, stream));
             GS_TRY(stream_values(plan, true, int(wt_all.size()), wt_all.data(), b_p, stream));
         }
-        // trailing update of the own panels
+        // look-ahead: the owner of the NEXT panel updates that panel first and factors its diagonal block at once, so that
+        // its chain runs beside the other ranks' (and its own remaining) trailing updates
+        const int pn = p + 1;
+        if (pn < np && pn % R == me) {
+            GS_TRY(update_panel(p, pn));
+            GS_TRY(diag_block(pn));
+            have_diag = true;
+        }
         for (int q = p + 1; q < np; ++q) {
-            if (q % R != me) continue;
-            const int c0 = start(q), c1 = start(q + 1);
-            if (c0 > s2) GS_TRY(f.gemm_update(s1, s2, c0, c0, c1));        // rows (p, q) of the block columns of q
-            GS_TRY(f.syrk(s1, s2, c0, c1));                                  // the diagonal block of q, upper tiles
+            if (q % R != me || (q == pn && have_diag)) continue;
+            GS_TRY(update_panel(p, q));
         }
     }
     return GS_OK;

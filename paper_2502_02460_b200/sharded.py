@@ -190,7 +190,8 @@ class ShardedReduction:
         self.flags = None            # int32[2 * world]: ready slots, then done slots (device sync)
         self.flag_ptrs = None        # this rank's view of every rank's flag array
         self.N, self.nev = plan.N, plan.nev
-        self.ranges = column_ranges(self.N, self.world, plan.block)
+        # (chol='sharded': step 1 costs every rank the same, whatever its columns -- the plain cube rule balances steps 2-3)
+        self.ranges = column_ranges(self.N, self.world, plan.block, 0.0 if chol == "sharded" and self.world > 1 else CHOL_WEIGHT)
         self.eig_ranges = even_ranges(self.nev, self.world, 2)
         self.peers = None
 
