@@ -29,6 +29,7 @@ namespace gs {
 namespace evp {
 
 constexpr int kDcLeaf = 128;
+constexpr int kDcLeafSmemBytes = kDcLeaf * kDcLeaf * 8;     // the leaf's Q block
 
 struct MergeDesc {
     int off, n1, n2;     // block [off, off + n1 + n2): children [off, off + n1), [off + n1, off + n1 + n2)
@@ -71,9 +72,9 @@ __global__ void dc_cut_kernel(double* d, const double* e, int N)
 // ---------------------------------------------------------------------------------------------------------
 // Leaf: all eigenpairs of the n x n (n <= 128) tridiagonal block at offset off by the implicit QL iteration with
 // Wilkinson shifts (EISPACK tql2 / LAPACK xSTEQR scheme).  Thread 0 runs the scalar recurrences of one sweep and
-// leaves its rotations in shared memory; then every thread applies them to its own ROW of Q (kept in registers?
-// no: in the Q block in global memory, 128 KB per leaf, L2-resident; loads of successive columns are coalesced
-// over the rows).  Result: dcur ascending, idx = physical column.
+// leaves its rotations in shared memory; then every thread applies them to its own ROW of Q, which lives in dynamic
+// shared memory (128 KB per leaf; in global memory every rotation was an L2 round trip: 7.75 -> see profiles/) and is
+// written out once at the end.  Result: dcur ascending, idx = physical column.
 // ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restrict__ dd, const double* __restrict__ ee, int N, DcArrays a)
 {
@@ -83,10 +84,12 @@ __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restri
     const int t = threadIdx.x;
     __shared__ double d[kDcLeaf], e[kDcLeaf], cs[kDcLeaf], sn[kDcLeaf];
     __shared__ int s_l, s_m, s_cnt, s_fail;
+    extern __shared__ double dc_leaf_q[];        // the leaf's Q block (128 x 128, column-major, ld kDcLeaf): every sweep rewrites it
     if (t < n) { d[t] = dd[off + t]; e[t] = (t + 1 < n) ? ee[off + t] : 0.0; }
-    double* Q = a.Qcur + off + (long long)off * a.ldq;
+    double* Q = dc_leaf_q;
+    constexpr long long ldq = kDcLeaf;
     for (int c = 0; c < n; ++c)
-        if (t < n) Q[t + (long long)c * a.ldq] = (t == c) ? 1.0 : 0.0;
+        if (t < n) Q[t + (long long)c * ldq] = (t == c) ? 1.0 : 0.0;
     if (t == 0) { s_fail = 0; }
     __syncthreads();
     for (int l = 0; l < n; ++l) {
@@ -111,11 +114,15 @@ __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restri
                     for (; i >= l; --i) {
                         double f = s * e[i];
                         const double b = c * e[i];
-                        r = hypot(f, g);
+                        // (this single-thread recurrence is the leaf's critical path: a plain square root and one
+                        // reciprocal where they are safe, hypot and the divisions where f^2 + g^2 leaves the normal range)
+                        const double q2 = f * f + g * g;
+                        const bool plain = q2 > 1e-280 && q2 < 1e280;
+                        r = plain ? sqrt(q2) : hypot(f, g);
                         e[i + 1] = r;
                         if (r == 0.0) { d[i + 1] -= p; e[m] = 0.0; early = true; break; }
-                        s = f / r;
-                        c = g / r;
+                        if (plain) { const double rr = 1.0 / r; s = f * rr; c = g * rr; }
+                        else { s = f / r; c = g / r; }
                         g = d[i + 1] - p;
                         r = (d[i] - g) * s + 2.0 * c * b;
                         p = s * r;
@@ -135,14 +142,14 @@ __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restri
             // apply the sweep's rotations, i = m-1 down to s_l, to row t of Q
             if (t < n && s_cnt > 0) {
                 const int lo = s_l;
-                double hi_val = Q[t + (long long)m * a.ldq];            // z(t, i+1)
+                double hi_val = Q[t + (long long)m * ldq];            // z(t, i+1)
                 for (int i = m - 1; i >= lo; --i) {
-                    const double zi = Q[t + (long long)i * a.ldq];
+                    const double zi = Q[t + (long long)i * ldq];
                     const double c = cs[i], s = sn[i];
-                    Q[t + (long long)(i + 1) * a.ldq] = s * zi + c * hi_val;
+                    Q[t + (long long)(i + 1) * ldq] = s * zi + c * hi_val;
                     hi_val = c * zi - s * hi_val;
                 }
-                Q[t + (long long)lo * a.ldq] = hi_val;
+                Q[t + (long long)lo * ldq] = hi_val;
             }
             ++iter;
             __syncthreads();
@@ -151,6 +158,11 @@ __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restri
     }
     __syncthreads();
     if (s_fail) { if (t == 0) atomicCAS(a.info, 0, -(1 << 30)); return; }
+    {   // the eigenvector block goes out once (rows over the threads: coalesced)
+        double* Qg = a.Qcur + off + (long long)off * a.ldq;
+        for (int c = 0; c < n; ++c)
+            if (t < n) Qg[t + (long long)c * a.ldq] = Q[t + (long long)c * ldq];
+    }
     // ascending order through an index (rank sort, ties by position)
     if (t < n) {
         const double v = d[t];

@@ -408,7 +408,13 @@ gs_status_t evp_solve_impl(gs_plan* plan, EvpBuffers& b, double* d, const double
     {
         LaunchTimer timer(plan, L_EVP_DC, stream);
         if (nleaf > 1) { dc_cut_kernel<<<(nleaf + 255) / 256, 256, 0, stream>>>(d, e, N); GS_LAUNCH_OK(plan); }
-        dc_leaf_kernel<<<nleaf, kDcLeaf, 0, stream>>>(d, e, N, a);
+        {
+            static PerDeviceOnce once;
+            GS_CUDA(plan, once.run([]() -> cudaError_t {
+                return cudaFuncSetAttribute(dc_leaf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDcLeafSmemBytes);
+            }));
+        }
+        dc_leaf_kernel<<<nleaf, kDcLeaf, kDcLeafSmemBytes, stream>>>(d, e, N, a);
         GS_LAUNCH_OK(plan);
     }
     // real engine launches, also inside a complex plan
