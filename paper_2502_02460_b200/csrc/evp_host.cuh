@@ -219,6 +219,14 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     static const bool tma_off = std::getenv("GS_EVP_SYMV") != nullptr && std::atoi(std::getenv("GS_EVP_SYMV")) == 0;
     static const int chunk_env = std::getenv("GS_EVP_CHUNK") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK")) : 0;
     static const int chunk_t = std::getenv("GS_EVP_CHUNK_T") != nullptr ? std::atoi(std::getenv("GS_EVP_CHUNK_T")) : 4;
+    static const int comb_env = std::getenv("GS_EVP_COMBINE_THREADS") != nullptr ? std::atoi(std::getenv("GS_EVP_COMBINE_THREADS")) : 0;
+    int comb_threads = comb_env;
+    if (comb_threads <= 0) {
+        int dev = 0, sms = 0;
+        GS_CUDA(plan, cudaGetDevice(&dev));
+        GS_CUDA(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        comb_threads = sms * 3 * 256;
+    }
     static const bool fuse_off = std::getenv("GS_EVP_FUSE") != nullptr && std::atoi(std::getenv("GS_EVP_FUSE")) == 0;
     const bool use_tma = !tma_off && (sizeof(T) == 16 || vec) && aligned16(A);
     SymvTmaParams<T> q{};
@@ -274,7 +282,11 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
             }
             {
                 LaunchTimer timer(plan, L_EVP_STEP, stream);
-                const cudaError_t le = evp_launch(combine_kernel<T>, (i + kCombineRows - 1) / kCombineRows, 256, stream, p);
+                // 16 threads per row while that is one wave of CTAs (three per SM at its register count), 8 beyond
+                const bool wide = (long long)i * 16 <= (long long)comb_threads;
+                const int rows_per_cta = wide ? 16 : 32;
+                const cudaError_t le = wide ? evp_launch(combine_kernel<T, 16>, (i + rows_per_cta - 1) / rows_per_cta, 256, stream, p)
+                                            : evp_launch(combine_kernel<T, 8>, (i + rows_per_cta - 1) / rows_per_cta, 256, stream, p);
                 if (le != cudaSuccess) return cuda_fail(plan, le);
                 plan->launches += 1;
                 evp_trace(stream, "combine", i, jp);

@@ -718,8 +718,7 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
 //   corr2  = sum_c ( V(r,c) conj(W(i-1,c)) + W(r,c) conj(V(i-1,c)) )     (old panel columns of the next lazy update)
 //   partial of w'^H v; the last CTA sets alpha2 = -1/2 |tau|^2 (w'^H v) and records d(i), e(i-1), tau(i).
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kCombineTPR = 16;                       // threads per row
-constexpr int kCombineRows = 256 / kCombineTPR;
+// threads per row: 16 up to mid sizes; 8 for the largest blocks, where 16 would make the launch more than one wave of CTAs
 
 // tW', tV' and row i-1 of the panels into shared memory (2 * 128 elements each), by the first nthr threads of the CTA
 template <typename T>
@@ -733,12 +732,13 @@ __device__ __forceinline__ void combine_load(const StepParams<T>& p, const StepI
     }
 }
 
-// rows [g * kCombineRows, (g + 1) * kCombineRows) by 256 threads; returns the thread's share of w'^H v (its row's
+// rows [g * kCombineRows, (g + 1) * kCombineRows), kCombineRows = 256 / kCombineTPR, by 256 threads; returns the thread's share of w'^H v (its row's
 // term in the threads that own a row, zero elsewhere)
-template <typename T>
+template <typename T, int kCombineTPR>
 __device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx& ix, const StepScalars<T>& sc, const T* s_t, const T* s_row, int g)
 {
     constexpr int TW = kSymvTW;
+    constexpr int kCombineRows = 256 / kCombineTPR;
     const int m = ix.m, jp = ix.jp, nb = p.nb;
     const int t = threadIdx.x, l8 = t % kCombineTPR, rr = t / kCombineTPR;
     const int r = g * kCombineRows + rr;
@@ -820,7 +820,7 @@ __device__ __forceinline__ void combine_record(const StepParams<T>& p, const Ste
     p.R[(long long)p.panel * lb * (lb + 1) + pos + (long long)pos * lb] = dinv;
 }
 
-template <typename T>
+template <typename T, int kCombineTPR>
 __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
 {
     grid_dep_launch();
@@ -837,7 +837,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     __shared__ unsigned int s_last;
     combine_load(p, ix, s_t, s_row, 256);
     __syncthreads();
-    T dotp = combine_group(p, ix, sc, s_t, s_row, int(blockIdx.x));
+    T dotp = combine_group<T, kCombineTPR>(p, ix, sc, s_t, s_row, int(blockIdx.x));
     // block partial of w'^H v
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dotp = add(dotp, shfl_xor(dotp, o));
