@@ -199,7 +199,12 @@ gs_status_t gs_plan_set_push_targets(gs_plan_t* plan, gs_push_kind_t kind, int c
  * Both are stream memory operations of the driver (cuStreamWriteValue32 / cuStreamWaitValue32): no kernel spins, no SM
  * is held, the host is not synchronised.  Flags are 4-byte aligned device addresses; use increasing epochs as values.
  * A wait whose signal is never enqueued blocks its stream for good: every rank must signal, also after a numerical
- * failure (the compute calls are no-ops then, the signals are not). */
+ * failure (the compute calls are no-ops then, the signals are not).
+ * With CUDA's lazy module loading the FIRST launch of a kernel may synchronise with the device: behind a pending wait it
+ * returns only once the wait is satisfied.  Across processes that is a delay in the first round; ranks emulated in ONE
+ * process by one host thread would deadlock (the thread never gets to enqueue the signalling rank).  gs_cholesky_sharded
+ * therefore loads its kernels before it enqueues its first wait; callers that build their own sequences around
+ * gs_exchange_wait should run each call once before the first wait, or set CUDA_MODULE_LOADING=EAGER. */
 gs_status_t gs_exchange_signal(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream);
 gs_status_t gs_exchange_wait(gs_plan_t* plan, int count, void* const* flags, uint32_t value, void* cuda_stream);
 
