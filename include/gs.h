@@ -284,6 +284,19 @@ gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double*
 gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream);
 gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream);
 
+/* The whole generalized solve  H C = eps S C  of PAPER.md:61-67 in ONE call, for the lowest nev eigenpairs of the plan
+ * (ELPA's own interface offers the one call and the individual steps): gs_cholesky, gs_invert_triangular,
+ * gs_to_standard, gs_standard_eigh and gs_backtransform enqueued one after the other on `cuda_stream`, with the
+ * arguments, triangles, aliasing rules and failure behaviour of those calls.
+ *   H        N x N, both triangles, not modified        S_inout  N x N: S (upper triangle) on entry, U on return
+ *   Uinv     N x N out: U^-1                            Htilde   N x N scratch (H~, then the Householder vectors)
+ *   Ctilde   N x nev scratch (the eigenvectors of H~)   eps      nev eigenvalues, ascending
+ *   C        N x nev out: the eigenvectors, C^H S C = I
+ * All device pointers, caller-owned; both workspaces (gs_plan_set_workspace, gs_evp_set_workspace) must be set.
+ * SYNCHRONISES the stream inside (the divide and conquer of gs_evp_tridiag_solve, once per level). */
+gs_status_t gs_generalized_eigh(gs_plan_t* plan, const void* H, void* S_inout, void* Uinv, void* Htilde, void* Ctilde,
+                                double* eps, void* C, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------------
  * (5) Ill-conditioned overlap matrix.  "In the latter case (high condition number of S),
  * electronic structure calculations can then be carried out by transforming the eigenproblem (2) to the basis of

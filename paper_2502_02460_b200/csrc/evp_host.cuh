@@ -585,6 +585,22 @@ gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, v
     return evp_eigh_impl(plan, b, Htilde_inout, eps, Ctilde, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
 }
 
+// The whole generalized solve of PAPER.md:61-67 on one stream: steps 1-3, the standard eigensolver, the back-transformation.
+gs_status_t gs_generalized_eigh(gs_plan_t* plan, const void* H, void* S_inout, void* Uinv, void* Htilde, void* Ctilde, double* eps, void* C,
+                                void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));                       // both workspaces, before anything is enqueued
+    if (plan->nev > 0 && (Ctilde == nullptr || C == nullptr || eps == nullptr || overlaps(Ctilde, vec_bytes(plan), C, vec_bytes(plan))))
+        return GS_ERR_INVALID_ARG;
+    GS_TRY(gs_cholesky(plan, S_inout, cuda_stream));
+    GS_TRY(gs_invert_triangular(plan, S_inout, Uinv, cuda_stream));
+    GS_TRY(gs_to_standard(plan, H, Uinv, Htilde, cuda_stream));
+    GS_TRY(gs_standard_eigh(plan, Htilde, eps, Ctilde, cuda_stream));
+    return gs_backtransform(plan, Uinv, Ctilde, C, cuda_stream);
+}
+
 // ------------------------------------------------------------------------------------------------------
 // (5) Ill-conditioned overlap: "electronic structure calculations can then be carried out by
 // transforming the eigenproblem (2) to the basis of eigenvectors D_i of the overlap matrix, but omitting any D_i

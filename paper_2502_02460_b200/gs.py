@@ -35,7 +35,7 @@ EXPORTS = (
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
     "gs_evp_workspace_bytes", "gs_evp_set_workspace", "gs_evp_tridiagonalize", "gs_evp_tridiag_solve", "gs_evp_backtransform",
-    "gs_standard_eigh", "gs_truncated_workspace_bytes", "gs_truncated_to_standard", "gs_truncated_rank", "gs_backtransform_dense",
+    "gs_standard_eigh", "gs_generalized_eigh", "gs_truncated_workspace_bytes", "gs_truncated_to_standard", "gs_truncated_rank", "gs_backtransform_dense",
 )
 
 
@@ -112,6 +112,7 @@ def lib() -> ctypes.CDLL:
         L.gs_evp_tridiag_solve.argtypes = [vp, vp, vp, vp, vp, vp]
         L.gs_evp_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_standard_eigh.argtypes = [vp, vp, vp, vp, vp]
+        L.gs_generalized_eigh.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gs_truncated_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_truncated_to_standard.argtypes = [vp, vp, vp, ctypes.c_double, vp, vp, vp, vp]
         L.gs_truncated_rank.argtypes = [vp, vp, ctypes.POINTER(i64)]
@@ -363,6 +364,24 @@ class Plan:
                                            _dev_ptr(Ct, self.N, self.nev, self.tdtype) if self.nev > 0 else None,
                                            _stream_ptr(stream)))
         return eps, Ct
+
+    def generalized_eigh(self, H: torch.Tensor, S: torch.Tensor, stream=None):
+        """gs_generalized_eigh: the whole solve H C = eps S C in one call.  S is not modified (a copy is
+        factored).  Returns (eps, C, U, Uinv): the lowest nev eigenvalues, their eigenvectors, the factor and its inverse."""
+        from .workloads import colmajor_empty, colmajor_zeros
+        self.ensure_evp_workspace()
+        N, nev, dt = self.N, self.nev, self.tdtype
+        U = colmajor_empty(N, N, dtype=dt, device=self.device)
+        U.copy_(S)
+        Uinv = colmajor_empty(N, N, dtype=dt, device=self.device)
+        Ht = colmajor_zeros(N, N, dtype=dt, device=self.device)
+        Ct = colmajor_empty(N, max(nev, 1), dtype=dt, device=self.device)[:, :nev]
+        C = colmajor_empty(N, max(nev, 1), dtype=dt, device=self.device)[:, :nev]
+        eps = self._vec(max(nev, 1))[:nev]
+        self._check(lib().gs_generalized_eigh(self._h, _dev_ptr(H, N, N, dt), _dev_ptr(U, N, N, dt), _dev_ptr(Uinv, N, N, dt), _dev_ptr(Ht, N, N, dt),
+                                              Ct.data_ptr() if nev > 0 else None, eps.data_ptr() if nev > 0 else None,
+                                              C.data_ptr() if nev > 0 else None, _stream_ptr(stream)))
+        return eps, C, U, Uinv
 
     # ---- (5) ill-conditioned S: the truncated-basis route of PAPER.md:73 ----
     def truncated_to_standard(self, H: torch.Tensor, S: torch.Tensor, delta: float, stream=None):

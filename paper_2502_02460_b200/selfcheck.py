@@ -64,6 +64,16 @@ def check_size(N: int, cplx: bool, standard_evp: bool = False) -> dict:
     plan.set_push_targets(gs.GS_PUSH_UINV, [])
     out["cols_inv"] = _rel(torch.triu(Vx), torch.triu(V))
     out["cols_std"] = _rel(torch.triu(Htx), torch.triu(Ht))
+    # step 1 in its sharded form (one rank: no peers) and the allocation-free density matrix
+    Us = wl.colmajor_empty(N, N, dtype=dt, device="cuda")
+    Us.copy_(p.S)
+    plan.cholesky_sharded(Us, 0, 1)
+    Ps = wl.colmajor_zeros(N, N, dtype=dt, device="cuda")
+    plan.density_matrix_static(C, f, Ps)
+    plan.last_info()
+    Ust = torch.triu(Us)
+    out["chol_sharded"] = _rel(Ust.conj().t() @ Ust, p.S)
+    out["dens_static"] = _rel(torch.triu(Ps), torch.triu(Pref))
     if standard_evp and hasattr(plan, "standard_eigh"):
         eps, Q = plan.standard_eigh(Ht.clone())
         plan.last_info()
@@ -72,6 +82,14 @@ def check_size(N: int, cplx: bool, standard_evp: bool = False) -> dict:
         G = Q.conj().t() @ Q
         G.diagonal().sub_(1.0)
         out["evp_orth"] = G.abs().max().item()
+        # the whole generalized solve in one call: H C = S C eps, C^H S C = I
+        eps_g, Cg, _, _ = plan.generalized_eigh(p.H, p.S)
+        plan.last_info()
+        Rg = p.H @ Cg - (p.S @ Cg) * eps_g.to(dt).unsqueeze(0)
+        out["gen_resid"] = (Rg.norm() / (p.H.norm() * N * 2.0 ** -52)).item()
+        Gg = Cg.conj().t() @ (p.S @ Cg)
+        Gg.diagonal().sub_(1.0)
+        out["gen_sorth"] = Gg.abs().max().item()
     plan.close()
     return out
 
@@ -89,7 +107,7 @@ def main(argv=None) -> int:
         for cplx in (False, True):
             r = check_size(N, cplx, args.standard_evp)
             tol = {"chol": 1e-13, "inv": 1e-11, "std": 1e-9, "back": 1e-11, "dens": 1e-12, "cols_inv": 1e-11, "cols_std": 1e-11,
-                   "evp_resid": 100.0, "evp_orth": 1e-11}
+                   "evp_resid": 100.0, "evp_orth": 1e-11, "chol_sharded": 1e-13, "dens_static": 1e-12, "gen_resid": 100.0, "gen_sorth": 1e-10}
             ok = all(v <= tol[k] for k, v in r.items())
             bad += 0 if ok else 1
             print(f"selfcheck N={N} {'c128' if cplx else 'f64'} {'ok' if ok else 'FAILED'} " +

@@ -269,3 +269,30 @@ def test_configs_2_and_3_generalized_solve(index):
     sigma = 0.5 * (lam[cfg.nev - 1] + lam[cfg.nev]).item()
     assert int((eps < sigma).sum().item()) == cfg.nev and int((lam < sigma).sum().item()) == cfg.nev
     plan.close()
+
+
+@pytest.mark.parametrize("cplx,N,nev", [(False, 256, 256), (False, 300, 77), (True, 150, 150), (False, 1, 1)])
+def test_generalized_eigh_one_call(cplx, N, nev):
+    """gs_generalized_eigh = the five calls in a row: eigenvalues against the oracle's chain (unblocked
+    Cholesky, substitution, triple loops, Jacobi), eigenvectors by the residual of the ORIGINAL pencil and S-orthonormality."""
+    gs = _gs()
+    p = wl.small_pencil(N, seed=900 + N, complex=cplx)
+    H, S = p.H.numpy(), p.S.numpy()
+    V_o = oracle.invert_upper(oracle.cholesky(S))
+    eps_o, _, _ = oracle.jacobi(oracle.to_standard(H, V_o))
+    plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
+    Hd, Sd = wl.to_colmajor(p.H.cuda()), wl.to_colmajor(p.S.cuda())
+    S_before = Sd.clone()
+    eps, C, U, Uinv = plan.generalized_eigh(Hd, Sd)
+    assert plan.last_info() == 0
+    assert torch.equal(Sd, S_before)
+    scale = max(1.0, np.abs(eps_o).max())
+    assert np.abs(eps.cpu().numpy() - eps_o[:nev]).max() <= 1e-11 * scale
+    assert M.eig_residual(H, S, C.cpu().numpy(), eps.cpu().numpy()) <= M.TOL_RESIDUAL
+    assert M.s_orthonormality(S, C.cpu().numpy()) <= M.TOL_SORTH
+    assert M.rel_frob_upper(U.cpu(), oracle.cholesky(S)) <= M.TOL_FROB and M.rel_frob_upper(Uinv.cpu(), V_o) <= M.TOL_FROB
+    # argument errors come back before anything is enqueued
+    L = gs.lib()
+    assert L.gs_generalized_eigh(None, Hd.data_ptr(), U.data_ptr(), Uinv.data_ptr(), Hd.data_ptr(), C.data_ptr(), eps.data_ptr(), C.data_ptr(), None) == 1
+    assert L.gs_generalized_eigh(plan._h, Hd.data_ptr(), U.data_ptr(), Uinv.data_ptr(), Hd.data_ptr(), C.data_ptr(), eps.data_ptr(), C.data_ptr(), None) == 1   # C~ = C
+    plan.close()
