@@ -91,6 +91,7 @@ struct gs_plan {
     int shard_panel = 8;             // column-range inversion: panel of the back substitution in blocks (power of two)
     int super_tile = 12;             // super-tile edge of triangular launches (about one wave of CTAs per super-tile)
     int super_syr2k = 4;             // the same for the SYR2K-shaped launch of gs_to_standard (four operand panels per tile)
+    int potrf_flat = 1;              // diagonal panel blocks factored right-looking block by block (default) instead of recursively
     char cuda_error[256] = {0};
 };
 
@@ -484,6 +485,18 @@ struct Potrf {
     gs_status_t potrf(int b0, int b1)
     {
         if (b1 - b0 == 1) return leaf(b0);
+        if (st.plan->potrf_flat != 0) {
+            // flat right-looking form: per block the leaf, ONE in-place solve of its row inside the panel, ONE update of the
+            // rest of the panel block (3 launches per block instead of the recursion's 4: fewer, but K = 128 everywhere)
+            for (int k = b0; k < b1; ++k) {
+                GS_TRY(leaf(k));
+                if (k + 1 < b1) {
+                    GS_TRY(trsm_leaf(k, k + 1, b1));
+                    GS_TRY(syrk(k, k + 1, k + 1, b1));
+                }
+            }
+            return GS_OK;
+        }
         const int mid = b0 + (b1 - b0 + 1) / 2;
         GS_TRY(potrf(b0, mid));
         GS_TRY(trsm(b0, mid, mid, b1));
@@ -826,6 +839,7 @@ gs_status_t gs_plan_create(gs_plan_t** plan, int64_t N, gs_dtype_t dtype, int64_
     knob("GS_SUPER_TILE", 0, 64, &p->super_tile);
     p->super_syr2k = p->super_tile > 4 ? 4 : p->super_tile;
     knob("GS_SUPER_SYR2K", 0, 64, &p->super_syr2k);
+    knob("GS_POTRF_FLAT", 0, 1, &p->potrf_flat);
     knob("GS_TILE64", 0, 2, &p->tile64_mode);
     knob("GS_CTILE_HALF", 0, 1, &p->ctile_half);
     knob("GS_TILE64_BELOW", 0, 1 << 30, &p->tile64_below);

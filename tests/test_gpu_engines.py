@@ -1,6 +1,6 @@
 """The alternative engine configurations stay correct: the 128 x 128-tile real engine (GS_TILE64=0),
 the 64 x 64-tile complex engine (GS_CTILE_HALF=0), no super-tile rasterisation, other POTRF panel
-schedules, the alternative diagonal-block kernels (GS_LEAF=0: rank-1 sweep over 256 threads; GS_LEAF_BLOCKED=1: 4-row panels).  The knobs are read at plan creation, so each configuration runs in its own process."""
+schedules, the recursive form of the panel's diagonal block (GS_POTRF_FLAT=0), the alternative diagonal-block kernels (GS_LEAF=0: rank-1 sweep over 256 threads; GS_LEAF_BLOCKED=1: 4-row panels).  The knobs are read at plan creation, so each configuration runs in its own process."""
 import os
 import subprocess
 import sys
@@ -46,6 +46,7 @@ print("OK" if bad == 0 else "FAILED")
     {"GS_POTRF_NB": "16", "GS_POTRF_TAIL": "0", "GS_POTRF_END": "0"},
     {"GS_LEAF_BLOCKED": "1"},
     {"GS_LEAF": "0"},
+    {"GS_POTRF_FLAT": "0"},
 ])
 def test_engine_configuration(env):
     e = dict(os.environ)
