@@ -54,6 +54,10 @@ def parse_args():
                     help="NEXT-3: ONE pencil over all ranks (steps 2-4 by column ranges, one exchange); strong scaling, not the headline mode")
     ap.add_argument("--exchange", default="push", choices=["push", "collective"],
                     help="--sharded: slabs stored into the peers' buffers from the kernel epilogues (push) or NCCL broadcasts after the kernels")
+    ap.add_argument("--shard-sync", default="host", choices=["host", "device"],
+                    help="--sharded with the push exchange: order producing and consuming launches by host barriers or by device-side flags")
+    ap.add_argument("--shard-chol-mode", default="leading", choices=["leading", "sharded"],
+                    help="--sharded: step 1 per rank on the leading block it needs, or over the ranks (gs_cholesky_sharded; needs --exchange push --shard-sync device)")
     ap.add_argument("--shard-shares", type=int, default=0,
                     help="NEXT-3: time, on ONE GPU and one after the other, the share each of R ranks would run (not the headline)")
     ap.add_argument("--batch-complex", action="store_true")
@@ -634,7 +638,7 @@ def run_sharded(args):
     N, nev, cplx = cfg.N, cfg.nev, cfg.complex
     pen = wl.make_pencil(N, cfg.box, cfg.seed, complex=cplx, device=dev)      # the same on every rank
     plan = gs.Plan(N, nev, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64, device=dev)
-    drv = sharded.ShardedReduction(plan, info.rank, info.world, exchange=args.exchange)
+    drv = sharded.ShardedReduction(plan, info.rank, info.world, exchange=args.exchange, sync=args.shard_sync, chol=args.shard_chol_mode)
     bufs = drv.alloc(pen.H)
     Ct = wl.dense_rhs(N, nev, seed=0, complex=cplx, device=dev)
     C = bufs.C if drv.push else wl.colmajor_empty(N, nev, dtype=pen.H.dtype, device=dev)
@@ -674,8 +678,10 @@ def run_sharded(args):
                           "scaling": "strong", "vs_baseline": None, "dtype": "c128 (FP64 arithmetic)" if cplx else "f64",
                           "data": "synthetic",
                           "config": {"workload": cfg.name, "N": N, "nev": nev, "seed": cfg.seed,
-                                     "parallelism": f"sharded x{info.world}: step 1 replicated, steps 2-4 by column ranges, "
-                                                    "one exchange of the U^-1 and G slabs (NEXT-3)",
+                                     "parallelism": f"sharded x{info.world}: step 1 " +
+                                                    ("over the ranks (gs_cholesky_sharded)" if drv.chol_sharded else "per rank on the leading block it needs") +
+                                                    ", steps 2-4 by column ranges, one exchange of the U^-1 and G slabs (NEXT-3)",
+                                     "sync": "device-side flags" if drv.device_sync else "host barriers",
                                      "exchange": ("push: fused into the kernel epilogues over peer memory" if drv.push else
                                                   "collective: broadcasts after the kernels" if info.world > 1 else "none (one rank)"),
                                      "column_ranges": drv.ranges},
