@@ -13,9 +13,11 @@
 // traffic, not arithmetic: the symmetric product reads ONE triangle (4 m^2 bytes per step instead of 8 m^2:
 // 4N^3/3 bytes over the whole reduction), every element feeding both y(r) += a u(c) and y(c) += conj(a) u(r).
 //
-// A step is three launches (S, C, F) because it contains three global reductions that depend on each other
-// (the matrix-vector product, the dot product w'^H v, the norm of the next column).  Two identities shorten
-// that chain:
+// A step contains three global reductions that depend on each other (the matrix-vector product, the dot product
+// w'^H v, the norm of the next column): S, C, F.  With a tensor map on A (complex, or real with even N) it is TWO
+// launches -- symv_tma_kernel (S, with the F of the previous column formed inside it) and combine_kernel (C);
+// finish_kernel (F) then runs only at the panel boundaries.  Without one (odd real N): symv_kernel, combine_kernel,
+// finish_kernel, three launches per column.  Two identities shorten the chain:
 //   * with u = the updated column a(0:i) BEFORE scaling, v = s (u - beta e_{i-1}), s = 1 / (alpha - beta): every
 //     product with v is linear in u, so S multiplies by u and never waits for the norm; the scaling is applied
 //     in C:  A v = s (A u - beta A(:, i-1)),  W^H v = s (W^H u - beta conj(W(i-1, :)));
