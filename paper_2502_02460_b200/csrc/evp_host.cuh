@@ -230,6 +230,10 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
     // L2 policy of the streamed tiles: 0 plain, 1 evict-first always, 2 evict-first while the triangle exceeds evict_bytes
     static const int evict_mode = std::getenv("GS_EVP_EVICT") != nullptr ? std::atoi(std::getenv("GS_EVP_EVICT")) : 2;
     static const double evict_bytes = std::getenv("GS_EVP_EVICT_MB") != nullptr ? 1e6 * std::atof(std::getenv("GS_EVP_EVICT_MB")) : 100e6;
+    // ... except the tiles of the leading column blocks (27 MB: the same tiles in every column of the reduction), which stay
+    // in the L2 from column to column with the plain policy: real 20 blocks, complex 14
+    static const int keep_env = std::getenv("GS_EVP_KEEP") != nullptr ? std::atoi(std::getenv("GS_EVP_KEEP")) : -1;
+    const int keep_blocks = keep_env >= 0 ? keep_env : (sizeof(T) == 8 ? 20 : 14);
     static const bool fuse_off = std::getenv("GS_EVP_FUSE") != nullptr && std::atoi(std::getenv("GS_EVP_FUSE")) == 0;
     const bool use_tma = !tma_off && (sizeof(T) == 16 || vec) && aligned16(A);
     SymvTmaParams<T> q{};
@@ -266,6 +270,7 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
                 const int nitems = sv_items_before(nJ, K);
                 p.p2_chunk_rows = K * TW;
                 q.s = p; q.chunk_blocks = K; q.dot_ctas = jp > 0 ? nJ : 0;
+                q.keep_blocks = keep_blocks;
                 q.evict_first = evict_mode == 1 || (evict_mode == 2 && (double)i * i * 4.0 * (sizeof(T) / 8) > evict_bytes) ? 1 : 0;
                 const int stream_ctas = std::min(nitems, sv_ctas);
                 LaunchTimer timer(plan, L_EVP_SYMV, stream);

@@ -459,6 +459,7 @@ struct SymvTmaParams {
     int chunk_blocks;     // 128-row blocks per work item (1, 2 or 4)
     int dot_ctas;         // leading CTAs that form the panel dots (0 when the panel is empty)
     int evict_first;      // the tiles of A are loaded with the L2 evict-first policy (the triangle does not fit the L2 anyway)
+    int keep_blocks;      // ... except those of the column blocks below this one: the same tiles in every column of the reduction, kept in L2
 };
 
 // number of work items in the column blocks j < J:  sum_{j<J} ceil((j + 1) / K)
@@ -543,7 +544,7 @@ __device__ __forceinline__ void sv_decode(int item, int nJ, int nI, int K, int& 
 // -1 ends the step.
 template <typename T>
 __device__ __forceinline__ void sv_produce_step(SvCta<T>& c, const CUtensorMap* map, int m, int K, int first, int dyn_base, unsigned int* counter,
-                                                bool evict_first)
+                                                bool evict_first, int keep_blocks)
 {
     const uint64_t policy = l2_policy_evict_first();
     constexpr int kStages = SvCfg<T>::kStages;
@@ -564,7 +565,7 @@ __device__ __forceinline__ void sv_produce_step(SvCta<T>& c, const CUtensorMap* 
                 const uint32_t stage = c.cnt % kStages;
                 if (c.cnt >= kStages) mbar_wait(c.empty0 + 8 * stage, ((c.cnt / kStages) - 1) & 1);
                 mbar_arrive_expect_tx(c.full0 + 8 * stage, kSvStageBytes);
-                if (evict_first) tma_load_2d_hint(smem_u32(c.stages + stage * kSvStageBytes), map, I * TH * W8, J * TW + 16 * s, c.full0 + 8 * stage, policy);
+                if (evict_first && J >= keep_blocks) tma_load_2d_hint(smem_u32(c.stages + stage * kSvStageBytes), map, I * TH * W8, J * TW + 16 * s, c.full0 + 8 * stage, policy);
                 else tma_load_2d(smem_u32(c.stages + stage * kSvStageBytes), map, I * TH * W8, J * TW + 16 * s, c.full0 + 8 * stage);
             }
         }
@@ -708,7 +709,7 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     // the C kernel that follows), so the CTAs that start late (behind the panel-dot CTAs) simply take fewer items.
     const int cta = int(blockIdx.x) - q.dot_ctas, G = int(gridDim.x) - q.dot_ctas;
     if (warp == kSvConsumerWarps) {
-        if (lane == 0) sv_produce_step(c, &q.mapA, ix.m, q.chunk_blocks, cta, G, p.tickets + 3, q.evict_first != 0);
+        if (lane == 0) sv_produce_step(c, &q.mapA, ix.m, q.chunk_blocks, cta, G, p.tickets + 3, q.evict_first != 0, q.keep_blocks);
         return;
     }
     FusedF<T> ff;
