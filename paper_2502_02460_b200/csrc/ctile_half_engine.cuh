@@ -235,7 +235,8 @@ __global__ void __launch_bounds__(kCThreads, 3) ctile_half_engine_kernel(const _
                     Cz[row + col * p.ldc] = v;
                 }
             }
-    }    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
+    }
+    for (int d = 0; d < p.npeer; ++d) {   // fused exchange (tile_engine.cuh: EngineParams::peer)
         double2* Cd = reinterpret_cast<double2*>(p.peer[d]);
 #pragma unroll
         for (int mg = 0; mg < 4; ++mg) {
