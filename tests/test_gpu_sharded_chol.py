@@ -59,6 +59,31 @@ for cplx, N, R in ((False, 1500, 2), (False, 1100, 3), (True, 700, 2), (False, 1
             ok = ok and e <= M.TOL_FROB and z and same
     for pl in plans:
         pl.close()
+# a pivot that is not positive on ONE rank's panel: nobody hangs (every rank signals whatever its status: its kernels are
+# no-ops, its signals are not), the owner of the bad block reports the pivot, and the flags reach their final values
+N, R = 900, 2
+p = wl.small_pencil(N, seed=77)
+Sbad = p.S.clone()
+Sbad[400, 400] = -1.0                                  # block 3 = panel 1 (panels of GS_POTRF_NB blocks) or panel 3 (nb = 1)
+S0 = wl.to_colmajor(Sbad.cuda())
+plans = [gs.Plan(N, 0) for _ in range(R)]
+streams = [torch.cuda.Stream() for _ in range(R)]
+S = [S0.clone() for _ in range(R)]
+flags = [torch.zeros(R, dtype=torch.int32, device="cuda") for _ in range(R)]
+torch.cuda.synchronize()
+def bad_program(r):
+    torch.cuda.set_device(0)
+    plans[r].cholesky_sharded(S[r], r, R, [x.data_ptr() for x in S], [pl.workspace.data_ptr() for pl in plans],
+                              [f.data_ptr() for f in flags], epoch0=0, stream=streams[r])
+th = [threading.Thread(target=bad_program, args=(r,)) for r in range(R)]
+for t in th: t.start()
+for t in th: t.join()
+torch.cuda.synchronize()                               # returns: no stream is left waiting
+infos = [pl.last_info(raise_on_failure=False) for pl in plans]
+print("non-PD: infos", infos, "statuses", [getattr(pl, "last_status", None) for pl in plans], "flags", [f.tolist() for f in flags], flush=True)
+ok = ok and 401 in [abs(int(i)) for i in infos]
+for pl in plans:
+    pl.close()
 # nranks = 1: no peers, no flags
 N = 900
 p = wl.small_pencil(N, seed=7)
