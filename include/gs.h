@@ -284,6 +284,19 @@ gs_status_t gs_evp_tridiag_solve(gs_plan_t* plan, const double* d, const double*
 gs_status_t gs_evp_backtransform(gs_plan_t* plan, const void* A_reflectors, const double* Z, void* Ctilde, void* cuda_stream);
 gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, void* Ctilde, void* cuda_stream);
 
+/* Eigenvalues only ("If the eigenvectors are needed, one has to perform the backtransformation", PAPER.md:67 -- if they
+ * are not, the divide and conquer and both back-transformations are not needed either):
+ *   gs_evp_tridiag_eigenvalues  the `count` smallest eigenvalues (ascending, 0 <= count <= N) of the real symmetric
+ *                               tridiagonal matrix tridiag(e, d, e) of order N by bisection on the Sturm count
+ *                               (Sylvester's inertia of T - x I), each to the last bit the interval can be halved to.
+ *                               d (N), e (N - 1 used), eps (count): device pointers; d, e are not modified.  Needs the
+ *                               plan's ordinary workspace only; does not synchronise.
+ *   gs_standard_eigenvalues     the `count` smallest eigenvalues of the Hermitian matrix whose upper triangle is in
+ *                               Htilde_inout: gs_evp_tridiagonalize (Htilde_inout is destroyed: it holds the Householder
+ *                               vectors afterwards) + gs_evp_tridiag_eigenvalues.  Needs the eigensolver workspace. */
+gs_status_t gs_evp_tridiag_eigenvalues(gs_plan_t* plan, const double* d, const double* e, int64_t count, double* eps, void* cuda_stream);
+gs_status_t gs_standard_eigenvalues(gs_plan_t* plan, void* Htilde_inout, int64_t count, double* eps, void* cuda_stream);
+
 /* The whole generalized solve  H C = eps S C  of PAPER.md:61-67 in ONE call, for the lowest nev eigenpairs of the plan
  * (ELPA's own interface offers the one call and the individual steps): gs_cholesky, gs_invert_triangular,
  * gs_to_standard, gs_standard_eigh and gs_backtransform enqueued one after the other on `cuda_stream`, with the

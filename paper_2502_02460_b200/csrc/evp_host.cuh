@@ -594,6 +594,32 @@ gs_status_t gs_standard_eigh(gs_plan_t* plan, void* Htilde_inout, double* eps, v
     return evp_eigh_impl(plan, b, Htilde_inout, eps, Ctilde, int(plan->nev), static_cast<cudaStream_t>(cuda_stream));
 }
 
+// Eigenvalues only: bisection on the tridiagonal matrix (evp_dc.cuh: tridiag_bisect_kernel); no eigensolver workspace needed
+gs_status_t gs_evp_tridiag_eigenvalues(gs_plan_t* plan, const double* d, const double* e, int64_t count, double* eps, void* cuda_stream)
+{
+    GS_TRY(check_ready(plan));
+    if (count < 0 || count > plan->N || d == nullptr || (plan->N > 1 && e == nullptr) || (count > 0 && eps == nullptr)) return GS_ERR_INVALID_ARG;
+    if (count == 0) return GS_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    LaunchTimer timer(plan, L_EVP_DC, stream);
+    tridiag_bisect_kernel<<<unsigned((count + kBisectThreads - 1) / kBisectThreads), kBisectThreads, 0, stream>>>(d, e, int(plan->N), int(count), eps, info_ptr(plan));
+    GS_LAUNCH_OK(plan);
+    return GS_OK;
+}
+
+// ... of a Hermitian matrix: tridiagonalise, then bisection (H~ is destroyed as by gs_evp_tridiagonalize)
+gs_status_t gs_standard_eigenvalues(gs_plan_t* plan, void* Htilde_inout, int64_t count, double* eps, void* cuda_stream)
+{
+    if (plan == nullptr) return GS_ERR_INVALID_ARG;
+    EvpBuffers b;
+    GS_TRY(evp_ready(plan, &b));
+    if (Htilde_inout == nullptr || !aligned16(Htilde_inout) || count < 0 || count > plan->N || (count > 0 && eps == nullptr)) return GS_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    GS_TRY(plan->z ? evp_tridiagonalize_t<double2>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream)
+                   : evp_tridiagonalize_t<double>(plan, b, Htilde_inout, b.d, b.e, b.tau, stream));
+    return gs_evp_tridiag_eigenvalues(plan, b.d, b.e, count, eps, cuda_stream);
+}
+
 // The whole generalized solve of PAPER.md:61-67 on one stream: steps 1-3, the standard eigensolver, the back-transformation.
 gs_status_t gs_generalized_eigh(gs_plan_t* plan, const void* H, void* S_inout, void* Uinv, void* Htilde, void* Ctilde, double* eps, void* C,
                                 void* cuda_stream)

@@ -35,7 +35,7 @@ EXPORTS = (
     "gs_plan_launch_count", "gs_status_string", "gs_plan_last_cuda_error",
     "gs_plan_set_timing", "gs_plan_launch_times", "gs_plan_launch_trace",
     "gs_evp_workspace_bytes", "gs_evp_set_workspace", "gs_evp_tridiagonalize", "gs_evp_tridiag_solve", "gs_evp_backtransform",
-    "gs_standard_eigh", "gs_generalized_eigh", "gs_truncated_workspace_bytes", "gs_truncated_to_standard", "gs_truncated_rank", "gs_backtransform_dense",
+    "gs_standard_eigh", "gs_generalized_eigh", "gs_evp_tridiag_eigenvalues", "gs_standard_eigenvalues", "gs_truncated_workspace_bytes", "gs_truncated_to_standard", "gs_truncated_rank", "gs_backtransform_dense",
 )
 
 
@@ -113,6 +113,8 @@ def lib() -> ctypes.CDLL:
         L.gs_evp_backtransform.argtypes = [vp, vp, vp, vp, vp]
         L.gs_standard_eigh.argtypes = [vp, vp, vp, vp, vp]
         L.gs_generalized_eigh.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gs_evp_tridiag_eigenvalues.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.gs_standard_eigenvalues.argtypes = [vp, vp, i64, vp, vp]
         L.gs_truncated_workspace_bytes.argtypes = [vp, ctypes.POINTER(sz)]
         L.gs_truncated_to_standard.argtypes = [vp, vp, vp, ctypes.c_double, vp, vp, vp, vp]
         L.gs_truncated_rank.argtypes = [vp, vp, ctypes.POINTER(i64)]
@@ -364,6 +366,25 @@ class Plan:
                                            _dev_ptr(Ct, self.N, self.nev, self.tdtype) if self.nev > 0 else None,
                                            _stream_ptr(stream)))
         return eps, Ct
+
+    def evp_tridiag_eigenvalues(self, d: torch.Tensor, e: torch.Tensor, count: int | None = None, stream=None) -> torch.Tensor:
+        """The `count` (default N) smallest eigenvalues of tridiag(e, d, e) by bisection (gs_evp_tridiag_eigenvalues)."""
+        count = self.N if count is None else int(count)
+        ebuf = self._vec(max(self.N, 1))
+        ebuf[:e.numel()].copy_(e)
+        eps = self._vec(max(count, 1))[:count]
+        self._check(lib().gs_evp_tridiag_eigenvalues(self._h, d.data_ptr(), ebuf.data_ptr(), count, eps.data_ptr() if count > 0 else None,
+                                                     _stream_ptr(stream)))
+        return eps
+
+    def standard_eigenvalues(self, Htilde: torch.Tensor, count: int | None = None, stream=None) -> torch.Tensor:
+        """The `count` (default N) smallest eigenvalues of the Hermitian matrix in the upper triangle of Htilde (DESTROYED)."""
+        self.ensure_evp_workspace()
+        count = self.N if count is None else int(count)
+        eps = self._vec(max(count, 1))[:count]
+        self._check(lib().gs_standard_eigenvalues(self._h, _dev_ptr(Htilde, self.N, self.N, self.tdtype), count,
+                                                  eps.data_ptr() if count > 0 else None, _stream_ptr(stream)))
+        return eps
 
     def generalized_eigh(self, H: torch.Tensor, S: torch.Tensor, stream=None):
         """gs_generalized_eigh: the whole solve H C = eps S C in one call.  S is not modified (a copy is

@@ -296,3 +296,55 @@ def test_generalized_eigh_one_call(cplx, N, nev):
     assert L.gs_generalized_eigh(None, Hd.data_ptr(), U.data_ptr(), Uinv.data_ptr(), Hd.data_ptr(), C.data_ptr(), eps.data_ptr(), C.data_ptr(), None) == 1
     assert L.gs_generalized_eigh(plan._h, Hd.data_ptr(), U.data_ptr(), Uinv.data_ptr(), Hd.data_ptr(), C.data_ptr(), eps.data_ptr(), C.data_ptr(), None) == 1   # C~ = C
     plan.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 17, 257, 1000])
+def test_tridiag_eigenvalues_by_bisection_against_the_oracle(N):
+    """gs_evp_tridiag_eigenvalues (eigenvalues only: PAPER.md:67) against the oracle's Sturm bisection (O8/O9, pinned by the
+    closed-form spectrum of tridiag(-1, 2, -1)) and, for that matrix, against the closed form itself; partial counts."""
+    gs = _gs()
+    rng = np.random.default_rng(N)
+    cases = {"toeplitz": (np.full(N, 2.0), np.full(max(N - 1, 0), -1.0)),
+             "random": (rng.standard_normal(N), rng.standard_normal(max(N - 1, 0))),
+             "wilkinson": (np.abs(np.arange(N) - (N - 1) / 2.0), np.ones(max(N - 1, 0))),
+             "graded": (10.0 ** -np.linspace(0, 8, N), 1e-3 * 10.0 ** -np.linspace(0, 8, max(N - 1, 1))[:max(N - 1, 0)]),
+             "decoupled": (rng.standard_normal(N), np.where(np.arange(max(N - 1, 0)) % 5 == 4, 0.0, 0.3))}
+    plan = gs.Plan(N, N)
+    for name, (d, e) in cases.items():
+        ref = oracle.tridiag_eigenvalues(d, e)
+        dd, ee = torch.from_numpy(np.ascontiguousarray(d)).cuda(), torch.from_numpy(np.ascontiguousarray(e)).cuda()
+        lam = plan.evp_tridiag_eigenvalues(dd, ee).cpu().numpy()
+        assert plan.last_info() == 0
+        scale = max(1.0, np.abs(ref).max())
+        assert np.abs(lam - ref).max() <= 1e-13 * scale, name
+        assert np.all(np.diff(lam) >= 0)
+        if name == "toeplitz":
+            exact = 2.0 - 2.0 * np.cos(np.arange(1, N + 1) * np.pi / (N + 1))
+            assert np.abs(lam - exact).max() <= 1e-13 * 4.0
+        k = max(1, N // 3)
+        part = plan.evp_tridiag_eigenvalues(dd, ee, count=k).cpu().numpy()
+        assert np.array_equal(part, lam[:k])
+    assert plan.evp_tridiag_eigenvalues(dd, ee, count=0).numel() == 0
+    L = gs.lib()
+    assert L.gs_evp_tridiag_eigenvalues(plan._h, dd.data_ptr(), ee.data_ptr() if N > 1 else None, N + 1, dd.data_ptr(), None) == 1
+    assert L.gs_evp_tridiag_eigenvalues(plan._h, None, None, 1, dd.data_ptr(), None) == 1
+    plan.close()
+
+
+@pytest.mark.parametrize("cplx,N", [(False, 257), (True, 150), (False, 512)])
+def test_standard_eigenvalues_only(cplx, N):
+    """gs_standard_eigenvalues = tridiagonalisation + bisection: against the oracle's Jacobi on the same H~ and against the
+    eigenvalues gs_standard_eigh (divide and conquer) returns."""
+    gs = _gs()
+    _, _, Ht = _htilde(N, cplx, seed=700 + N)
+    eps_o, _, _ = oracle.jacobi(Ht)
+    scale = max(1.0, np.abs(eps_o).max())
+    plan = gs.Plan(N, N, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
+    lam = plan.standard_eigenvalues(_upper_poisoned(Ht)).cpu().numpy()
+    assert plan.last_info() == 0
+    assert np.abs(lam - eps_o).max() <= 1e-12 * scale
+    eps_dc, _ = plan.standard_eigh(_upper_poisoned(Ht))
+    assert np.abs(lam - eps_dc.cpu().numpy()).max() <= 1e-12 * scale
+    few = plan.standard_eigenvalues(_upper_poisoned(Ht), count=7).cpu().numpy()
+    assert np.abs(few - eps_o[:7]).max() <= 1e-12 * scale
+    plan.close()
