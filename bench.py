@@ -529,6 +529,15 @@ def standard_evp_block(plan, H, S0, U, V, Ht, C, N, nev, cplx, fp64_peak, hbm_gb
     tri_bytes = 4.0 * float(N) ** 3 / 3.0 * (es / 8.0)       # one triangle of the leading block per step: sum_m 4 m^2 (x2 complex)
     back_flop = f * 2.0 * float(N) ** 2 * nev
     her2k_flop = f * 2.0 * float(N) ** 3 / 3.0
+    # eigenvalues only: bisection on (d, e) instead of Solve and Back
+    evb = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    plan.evp_tridiag_eigenvalues(d, e, count=nev)                # warm-up (loads the kernel)
+    evb[0].record()
+    lam = plan.evp_tridiag_eigenvalues(d, e, count=nev)
+    evb[1].record()
+    plan.last_info()
+    t_bisect = evb[0].elapsed_time(evb[1])
+    bisect_diff = float((lam - eps).abs().max() / max(1.0, float(eps.abs().max())))
     # per-label device times of one more pass
     A.copy_(Ht)
     plan.set_timing(1)
@@ -548,6 +557,8 @@ def standard_evp_block(plan, H, S0, U, V, Ht, C, N, nev, cplx, fp64_peak, hbm_gb
                   "gemm_ms": kern.get("evp.solve.gemm", {}).get("ms")},
         "back": {"ms": round(t_back, 3), "bound": "tensor", "nominal_flop": back_flop,
                  "tflops": back_flop / (t_back * 1e-3) / 1e12, "frac_of_fp64_peak": back_flop / (t_back * 1e-3) / 1e12 / fp64_peak},
+        "eigenvalues_only": {"bisect_ms": round(t_bisect, 3), "total_ms": round(t_tri + t_bisect, 3), "bound": "latency (one dependent FMA per row and count)",
+                             "max_diff_to_solve_rel": bisect_diff},
         "total_ms": round(t_tri + t_solve + t_back, 3), "kernels": kern,
     }
     # the whole generalized solve, one chain on one stream

@@ -82,6 +82,9 @@ def check_size(N: int, cplx: bool, standard_evp: bool = False) -> dict:
         G = Q.conj().t() @ Q
         G.diagonal().sub_(1.0)
         out["evp_orth"] = G.abs().max().item()
+        lam = plan.standard_eigenvalues(Ht.clone(), count=eps.numel())   # eigenvalues only: bisection instead of Solve and Back
+        plan.last_info()
+        out["evp_bisect"] = ((lam - eps).abs().max() / max(1.0, eps.abs().max().item())).item()
         # the whole generalized solve in one call: H C = S C eps, C^H S C = I
         eps_g, Cg, _, _ = plan.generalized_eigh(p.H, p.S)
         plan.last_info()
@@ -107,7 +110,7 @@ def main(argv=None) -> int:
         for cplx in (False, True):
             r = check_size(N, cplx, args.standard_evp)
             tol = {"chol": 1e-13, "inv": 1e-11, "std": 1e-9, "back": 1e-11, "dens": 1e-12, "cols_inv": 1e-11, "cols_std": 1e-11,
-                   "evp_resid": 100.0, "evp_orth": 1e-11, "chol_sharded": 1e-13, "dens_static": 1e-12, "gen_resid": 100.0, "gen_sorth": 1e-10}
+                   "evp_resid": 100.0, "evp_orth": 1e-11, "chol_sharded": 1e-13, "dens_static": 1e-12, "gen_resid": 100.0, "gen_sorth": 1e-10, "evp_bisect": 1e-12}
             ok = all(v <= tol[k] for k, v in r.items())
             bad += 0 if ok else 1
             print(f"selfcheck N={N} {'c128' if cplx else 'f64'} {'ok' if ok else 'FAILED'} " +
