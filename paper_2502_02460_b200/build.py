@@ -33,21 +33,27 @@ def _sources_mtime() -> float:
     return m
 
 
-def build(force: bool = False, verbose: bool = False) -> list[str]:
+# a diagnostic build of libgs.so with per-CTA time stamps in the tridiagonalisation's step kernels (trace_tridiag.py);
+# built only on request, never loaded by gs.py
+TRACE_TARGET = ("libgs_trace.so", ["gs.cu"], ["-DGS_SV_TRACE"])
+
+
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> list[str]:
     nvcc = os.environ.get("NVCC", "nvcc")
     out = []
     newest = _sources_mtime()
-    for lib, srcs in TARGETS.items():
+    targets = [(lib, srcs, []) for lib, srcs in TARGETS.items()] + ([TRACE_TARGET] if trace else [])
+    for lib, srcs, defines in targets:
         path = os.path.join(HERE, lib)
         out.append(path)
         if not force and os.path.exists(path) and os.path.getmtime(path) >= newest:
             continue
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = [nvcc] + NVCC_FLAGS + defines + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", path] + [os.path.join(CSRC, s) for s in srcs]
         subprocess.run(cmd, check=True)
     return out
 
 
 if __name__ == "__main__":
-    for p in build(force="--force" in sys.argv, verbose="-v" in sys.argv):
+    for p in build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv):
         print(p)

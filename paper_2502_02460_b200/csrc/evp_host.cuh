@@ -740,3 +740,21 @@ gs_status_t gs_backtransform_dense(gs_plan_t* plan, const void* X, const void* C
 }
 
 }  // extern "C"
+
+#ifdef GS_SV_TRACE
+// Trace build only (evp_tridiag.cuh, "Timeline of one column"): arm the stamps for the blocks of order m and m - 1; read them back.
+extern "C" int gs_trace_tridiag_arm(int m)
+{
+    unsigned long long init[2][4] = {{~0ull, ~0ull, 0ull, 0ull}, {~0ull, ~0ull, 0ull, 0ull}};
+    void* ptr = nullptr;
+    if (cudaMemcpyToSymbol(g_c_trace, init, sizeof(init)) != cudaSuccess || cudaGetSymbolAddress(&ptr, g_sv_trace) != cudaSuccess) return GS_ERR_CUDA;
+    if (cudaMemset(ptr, 0, sizeof(unsigned long long) * 2 * kTraceCtas * 8) != cudaSuccess) return GS_ERR_CUDA;
+    return cudaMemcpyToSymbol(g_sv_trace_m, &m, sizeof(int)) == cudaSuccess ? GS_OK : GS_ERR_CUDA;
+}
+extern "C" int gs_trace_tridiag_read(unsigned long long* s_stamps /* [2][600][8] */, unsigned long long* c_stamps /* [2][4] */)
+{
+    if (cudaDeviceSynchronize() != cudaSuccess) return GS_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(s_stamps, g_sv_trace, sizeof(unsigned long long) * 2 * kTraceCtas * 8) != cudaSuccess) return GS_ERR_CUDA;
+    return cudaMemcpyFromSymbol(c_stamps, g_c_trace, sizeof(unsigned long long) * 2 * 4) == cudaSuccess ? GS_OK : GS_ERR_CUDA;
+}
+#endif

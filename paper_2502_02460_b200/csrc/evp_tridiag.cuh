@@ -557,7 +557,6 @@ __device__ __forceinline__ void sv_produce_step(SvCta<T>& c, const CUtensorMap* 
         c.item_q[c.nitem & 3] = item < nitems ? item : -1;
         mbar_arrive(c.qfull0 + 8 * (c.nitem & 3));
         if (item >= nitems) { ++c.nitem; break; }
-        const int next = dyn_base + int(atomicAdd(counter, 1u));
         int J, I0, I1;
         sv_decode<T>(item, nJ, nI, K, J, I0, I1);
         for (int I = I0; I < I1; ++I) {
@@ -569,7 +568,9 @@ __device__ __forceinline__ void sv_produce_step(SvCta<T>& c, const CUtensorMap* 
                 else tma_load_2d(smem_u32(c.stages + stage * kSvStageBytes), map, I * TH * W8, J * TW + 16 * s, c.full0 + 8 * stage);
             }
         }
-        item = next;
+        // the next item is taken only now (the ring holds five stages of look-ahead, more than the counter's round
+        // trip): a CTA that reserves its next item before streaming the current one leaves a tail of two items
+        item = dyn_base + int(atomicAdd(counter, 1u));
     }
 }
 
@@ -683,6 +684,21 @@ __device__ __forceinline__ void sv_consume_step(SvCta<T>& c, const StepParams<T>
     }
 }
 
+// ---- Timeline of one column (trace build only: `python -m paper_2502_02460_b200.trace_tridiag`, -DGS_SV_TRACE) ----
+// %globaltimer stamps of the S launches of the blocks of order trace_m and trace_m - 1, per CTA: [0] entry (before the
+// grid dependency), [1] dependency resolved, [2] first work item, [3] end, [4] items, [5] tiles, [6] SM, [7] 1 = panel-dot
+// CTA; of the C launches: earliest entry, earliest start after the dependency, latest end.
+#ifdef GS_SV_TRACE
+constexpr int kTraceCtas = 600;
+__device__ unsigned long long g_sv_trace[2][kTraceCtas][8];
+__device__ unsigned long long g_c_trace[2][4];
+__device__ int g_sv_trace_m = -1;
+__device__ __forceinline__ unsigned long long trace_time() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define GS_TRACE(...) __VA_ARGS__
+#else
+#define GS_TRACE(...)
+#endif
+
 template <typename T>
 __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_kernel(const __grid_constant__ SymvTmaParams<T> q)
 {
@@ -697,12 +713,17 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
         tma_prefetch_desc(&q.mapA);
     }
     __syncthreads();
+    GS_TRACE(const unsigned long long tr_entry = trace_time();)
     grid_dep_launch();
     grid_dep_wait();
     if (*p.info != 0) return;
     const StepIdx ix = step_idx(p);
+    GS_TRACE(const int tr_slot = g_sv_trace_m - ix.m;
+             unsigned long long* tr = ((tr_slot == 0 || tr_slot == 1) && blockIdx.x < kTraceCtas && t == 0) ? g_sv_trace[tr_slot][blockIdx.x] : nullptr;
+             if (tr) { tr[0] = tr_entry; tr[1] = trace_time(); tr[7] = int(blockIdx.x) < q.dot_ctas ? 1 : 0; })
     if (int(blockIdx.x) < q.dot_ctas) {
         panel_dots(p, ix, int(blockIdx.x), q.dot_ctas, c.red, &s_last);
+        GS_TRACE(if (tr) tr[3] = trace_time();)
         return;
     }
     // Work items: the first one of a CTA is its own index, the rest comes from a global counter (tickets[3], reset by
@@ -714,7 +735,9 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     }
     FusedF<T> ff;
     if (ix.fuse) ff.init(p, ix);
+    GS_TRACE(if (tr) tr[2] = trace_time();)
     sv_consume_step(c, p, ix, ff, q.chunk_blocks);
+    GS_TRACE(if (tr) { unsigned int sm; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); tr[3] = trace_time(); tr[4] = c.nitem; tr[5] = c.ntile; tr[6] = sm; })
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -830,12 +853,16 @@ __device__ __forceinline__ void combine_record(const StepParams<T>& p, const Ste
 template <typename T, int kCombineTPR>
 __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
 {
+    GS_TRACE(const unsigned long long tr_entry = trace_time();)
     grid_dep_launch();
     grid_dep_wait();
     if (*p.info != 0) return;
     const StepIdx ix = step_idx(p);
     const int m = ix.m;
     const int t = threadIdx.x;
+    GS_TRACE(struct TraceEnd { unsigned long long* c; __device__ ~TraceEnd() { if (c) atomicMax(c + 2, trace_time()); } }
+                 tr_end{((g_sv_trace_m - m == 0 || g_sv_trace_m - m == 1) && t == 0) ? g_c_trace[g_sv_trace_m - m] : nullptr};
+             if (tr_end.c) { atomicMin(tr_end.c + 0, tr_entry); atomicMin(tr_end.c + 1, trace_time()); })
     if (blockIdx.x == 0 && t == 0) p.tickets[3] = 0u;      // work counter of symv_tma_kernel
     const StepScalars<T> sc = *sc_of(p, m);
     __shared__ T s_t[2 * 128];           // tW', tV'
