@@ -1,6 +1,6 @@
 """Timeline of one column of the tridiagonalisation (csrc/evp_tridiag.cuh, "Timeline of one column").
 
-    python -m paper_2502_02460_b200.trace_tridiag N m [m ...]
+    python -m paper_2502_02460_b200.trace_tridiag [--complex] N m [m ...]
 
 Builds the diagnostic library libgs_trace.so (libgs.so compiled with -DGS_SV_TRACE: %globaltimer stamps in the step
 kernels S = symv_tma_kernel and C = combine_kernel), runs gs_evp_tridiagonalize on a random symmetric N x N matrix and
@@ -24,7 +24,9 @@ TRACE_CTAS = 600
 
 
 def main(argv=None) -> int:
-    argv = sys.argv[1:] if argv is None else argv
+    argv = sys.argv[1:] if argv is None else list(argv)
+    cplx = "--complex" in argv
+    argv = [a for a in argv if a != "--complex"]
     if len(argv) < 2:
         print(__doc__, file=sys.stderr)
         return 2
@@ -37,11 +39,12 @@ def main(argv=None) -> int:
     L.gs_trace_tridiag_arm.argtypes = [ctypes.c_int]
     L.gs_trace_tridiag_read.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
     hbm = gs.measured_hbm_gbs() if hasattr(gs, "measured_hbm_gbs") else None
-    plan = gs.Plan(N, max(N // 4, 1))
+    plan = gs.Plan(N, max(N // 4, 1), dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
     g = torch.Generator(device="cpu")
     g.manual_seed(1)
-    A0 = torch.randn(N, N, dtype=torch.float64, generator=g)
-    A0 = wl.to_colmajor((A0 + A0.t()).cuda())
+    A0 = torch.randn(N, N, dtype=torch.complex128 if cplx else torch.float64, generator=g)
+    A0 = wl.to_colmajor((A0 + A0.conj().t()).cuda())
+    es = 16 if cplx else 8
     A = A0.clone()
     plan.evp_tridiagonalize(A)                       # warm-up: modules loaded, attributes set
     torch.cuda.synchronize()
@@ -64,7 +67,7 @@ def main(argv=None) -> int:
             us = lambda x: (x - base) / 1e3
             starts.append(s[:, 1].min())
             q = lambda a, f: us(np.percentile(a, f))
-            bytes_ = 4.0 * (m - slot) ** 2
+            bytes_ = 0.5 * es * (m - slot) ** 2
             span = (st[:, 3].max() - st[:, 2].min()) / 1e3
             print(f"m={m - slot}: S {len(st)} streaming + {len(dots)} panel-dot CTAs | dependency resolved at {us(s[:, 1].min()):.1f}"
                   f" | first item at {q(st[:, 2], 50):.1f} (median) | stream end min / median / max {us(st[:, 3].min()):.1f} / {q(st[:, 3], 50):.1f} / {us(st[:, 3].max()):.1f}"
@@ -73,8 +76,8 @@ def main(argv=None) -> int:
                   f" | items per CTA {st[:, 4].min()}..{st[:, 4].max()}, tiles {st[:, 5].min()}..{st[:, 5].max()}"
                   f" | C entry {us(cc[slot][0]):.1f}, start {us(cc[slot][1]):.1f}, end {us(cc[slot][2]):.1f}")
         if len(starts) == 2:
-            print(f"   period (dependency resolved -> resolved): {(starts[1] - starts[0]) / 1e3:.1f} us;  4 m^2 bytes at the HBM copy rate"
-                  f" ({hbm or 6549:.0f} GB/s): {4.0 * m * m / (hbm or 6549) / 1e3:.1f} us")
+            print(f"   period (dependency resolved -> resolved): {(starts[1] - starts[0]) / 1e3:.1f} us;  the triangle's {0.5 * es * m * m / 1e9:.3f} GB at the HBM copy rate"
+                  f" ({hbm or 6549:.0f} GB/s): {0.5 * es * m * m / (hbm or 6549) / 1e3:.1f} us")
     plan.close()
     return 0
 
