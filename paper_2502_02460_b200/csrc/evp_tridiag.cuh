@@ -797,15 +797,29 @@ __device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx
 #pragma unroll
             for (int k = 0; k < 4; ++k) y = add(y, v4[k]);
         }
-        const T* vt = p.Vt + (long long)r * nb;
-        const T* wt = p.Wt + (long long)r * nb;
-        for (int c0 = l8; c0 < jp; c0 += 8 * kCombineTPR) {
-            T vv[8], ww[8];
+    }
+    // The first block of the row's panel entries is loaded before the barrier that publishes s_t and s_row (staged by
+    // combine_load), so that the staging and the row's own loads are one round trip to the L2, not two.
+    const T* vt = p.Vt + (long long)r * nb;
+    const T* wt = p.Wt + (long long)r * nb;
+    T vv[8], ww[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const int c = c0 + k * kCombineTPR;
-                vv[k] = c < jp ? vt[c] : zero_of(T{});
-                ww[k] = c < jp ? wt[c] : zero_of(T{});
+    for (int k = 0; k < 8; ++k) {
+        const int c = l8 + k * kCombineTPR;
+        const bool in = r < m && c < jp;
+        vv[k] = in ? vt[c] : zero_of(T{});
+        ww[k] = in ? wt[c] : zero_of(T{});
+    }
+    __syncthreads();
+    if (r < m) {
+        for (int c0 = l8; c0 < jp; c0 += 8 * kCombineTPR) {
+            if (c0 != l8) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int c = c0 + k * kCombineTPR;
+                    vv[k] = c < jp ? vt[c] : zero_of(T{});
+                    ww[k] = c < jp ? wt[c] : zero_of(T{});
+                }
             }
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
@@ -870,8 +884,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     __shared__ T s_dot[8];
     __shared__ unsigned int s_last;
     combine_load(p, ix, s_t, s_row, 256);
-    __syncthreads();
-    T dotp = combine_group<T, kCombineTPR>(p, ix, sc, s_t, s_row, int(blockIdx.x));
+    T dotp = combine_group<T, kCombineTPR>(p, ix, sc, s_t, s_row, int(blockIdx.x));      // (holds the barrier for s_t, s_row)
     // block partial of w'^H v
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dotp = add(dotp, shfl_xor(dotp, o));
