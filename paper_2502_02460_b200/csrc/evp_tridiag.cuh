@@ -230,7 +230,7 @@ struct FusedF {
 // ---------------------------------------------------------------------------------------------------------
 template <typename T>
 __device__ __forceinline__ void panel_dots(const StepParams<T>& p, const StepIdx& ix, int x, int nx, T* sm, unsigned int* s_last,
-                                           const T* alpha2_local = nullptr)
+                                           const T* alpha2_local = nullptr, int failed = 0)
 {
     constexpr int TW = kSymvTW;
     const int m = ix.m, jp = ix.jp, nb = p.nb;
@@ -252,7 +252,8 @@ __device__ __forceinline__ void panel_dots(const StepParams<T>& p, const StepIdx
             p.u[r] = un;
             if (r < m - 1) nrm = abs2(un);
         }
-        for (int rz = io + x * kSymvThreads + t; rz < p.N && t < kSymvThreads; rz += nx * kSymvThreads) p.A[rz + (long long)io * p.ld] = zero_of(T{});
+        if (failed == 0)      // (the only store of this function outside the workspace)
+            for (int rz = io + x * kSymvThreads + t; rz < p.N && t < kSymvThreads; rz += nx * kSymvThreads) p.A[rz + (long long)io * p.ld] = zero_of(T{});
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
         double* sn = reinterpret_cast<double*>(sm);
@@ -716,13 +717,16 @@ __global__ void __launch_bounds__(kSvThreads, SvCfg<T>::kCtasPerSm) symv_tma_ker
     GS_TRACE(const unsigned long long tr_entry = trace_time();)
     grid_dep_launch();
     grid_dep_wait();
-    if (*p.info != 0) return;
+    // The info flag is read here and consumed only where something outside the workspace is stored (the panel-dot CTAs
+    // zero a column of A): a branch on it at this point would put one more L2 round trip in front of every column.  With
+    // the flag set the kernel runs on whatever the workspace holds -- fixed trip counts, stores into the workspace only.
+    const int failed = *reinterpret_cast<const volatile int*>(p.info);
     const StepIdx ix = step_idx(p);
     GS_TRACE(const int tr_slot = g_sv_trace_m - ix.m;
              unsigned long long* tr = ((tr_slot == 0 || tr_slot == 1) && blockIdx.x < kTraceCtas && t == 0) ? g_sv_trace[tr_slot][blockIdx.x] : nullptr;
              if (tr) { tr[0] = tr_entry; tr[1] = trace_time(); tr[7] = int(blockIdx.x) < q.dot_ctas ? 1 : 0; })
     if (int(blockIdx.x) < q.dot_ctas) {
-        panel_dots(p, ix, int(blockIdx.x), q.dot_ctas, c.red, &s_last);
+        panel_dots(p, ix, int(blockIdx.x), q.dot_ctas, c.red, &s_last, static_cast<const T*>(nullptr), failed);
         GS_TRACE(if (tr) tr[3] = trace_time();)
         return;
     }
@@ -765,7 +769,7 @@ __device__ __forceinline__ void combine_load(const StepParams<T>& p, const StepI
 // rows [g * kCombineRows, (g + 1) * kCombineRows), kCombineRows = 256 / kCombineTPR, by 256 threads; returns the thread's share of w'^H v (its row's
 // term in the threads that own a row, zero elsewhere)
 template <typename T, int kCombineTPR>
-__device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx& ix, const StepScalars<T>& sc, const T* s_t, const T* s_row, int g)
+__device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx& ix, const StepScalars<T>& sc, const T* s_t, const T* s_row, int g, int failed)
 {
     constexpr int TW = kSymvTW;
     constexpr int kCombineRows = 256 / kCombineTPR;
@@ -841,7 +845,7 @@ __device__ __forceinline__ T combine_group(const StepParams<T>& p, const StepIdx
         if (r == m - 1) acol = real_only(acol);
         T wpr = sub(mul(sc.s, sub(y, rscale(acol, sc.beta))), c1);
         p.Vt[jp + (long long)r * nb] = cj(v);
-        p.A[r + (long long)m * p.ld] = v;
+        if (failed == 0) p.A[r + (long long)m * p.ld] = v;          // (with d, e, tau the only stores of C outside the workspace)
         p.wp[r] = wpr;
         p.corr2[r] = c2;
         dotp = cfmad(wpr, v, dotp);
@@ -870,7 +874,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     GS_TRACE(const unsigned long long tr_entry = trace_time();)
     grid_dep_launch();
     grid_dep_wait();
-    if (*p.info != 0) return;
+    const int failed = *reinterpret_cast<const volatile int*>(p.info);      // consumed at the stores (symv_tma_kernel says why)
     const StepIdx ix = step_idx(p);
     const int m = ix.m;
     const int t = threadIdx.x;
@@ -884,7 +888,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
     __shared__ T s_dot[8];
     __shared__ unsigned int s_last;
     combine_load(p, ix, s_t, s_row, 256);
-    T dotp = combine_group<T, kCombineTPR>(p, ix, sc, s_t, s_row, int(blockIdx.x));      // (holds the barrier for s_t, s_row)
+    T dotp = combine_group<T, kCombineTPR>(p, ix, sc, s_t, s_row, int(blockIdx.x), failed);      // (holds the barrier for s_t, s_row)
     // block partial of w'^H v
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dotp = add(dotp, shfl_xor(dotp, o));
@@ -911,7 +915,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const StepParams<T> p)
         T dot = s_dot[0];
         for (int w = 1; w < 8; ++w) dot = add(dot, s_dot[w]);
         sc_of(p, m)->alpha2 = rscale(dot, -0.5 * abs2(sc.tau));
-        combine_record(p, ix, sc);
+        if (failed == 0) combine_record(p, ix, sc);
         p.tickets[1] = 0u;
     }
 }

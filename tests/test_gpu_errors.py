@@ -273,3 +273,43 @@ def test_evp_and_truncated_argument_errors():
     torch.cuda.synchronize()
     assert plan.last_info() == 0 and plan.launch_count() == 0
     plan.close()
+
+
+@pytest.mark.parametrize("cplx,N", [(False, 300), (True, 200), (False, 129)])
+def test_eigensolver_stages_are_noops_while_the_flag_is_set(cplx, N):
+    """include/gs.h, "Errors": all later compute calls on the plan are no-ops while the flag is set.  The step kernels of
+    the tridiagonalisation read the flag late (csrc/evp_tridiag.cuh: off the critical path) and must still leave the
+    matrix and d, e, tau alone; so must the eigenvalues-only calls.  Even N: the TMA loader, several panels."""
+    gs = _gs()
+    L = gs.lib()
+    dt = torch.complex128 if cplx else torch.float64
+    plan = gs.Plan(N, N, dtype=gs.GS_COMPLEX128 if cplx else gs.GS_REAL64)
+    plan.ensure_evp_workspace()
+    bad = np.eye(N) * (1.0 + 0j if cplx else 1.0)
+    bad[N // 2, N // 2] = -1.0
+    S = wl.to_colmajor(torch.from_numpy(bad).to(dt).cuda())
+    plan.cholesky(S)
+    assert plan.last_info(raise_on_failure=False) == N // 2 + 1
+    g = torch.Generator(device="cpu")
+    g.manual_seed(N)
+    A0 = torch.randn(N, N, dtype=dt, generator=g)
+    A0 = wl.to_colmajor((A0 + A0.conj().t()).cuda())
+    A = A0.clone()
+    d = torch.full((N,), 5.0, dtype=torch.float64, device="cuda")
+    e = torch.full((N,), 6.0, dtype=torch.float64, device="cuda")
+    tau = torch.full((N,), 7.0, dtype=dt, device="cuda")
+    assert L.gs_evp_tridiagonalize(plan._h, A.data_ptr(), d.data_ptr(), e.data_ptr(), tau.data_ptr(), None) == gs.GS_OK
+    lam = torch.full((N,), 8.0, dtype=torch.float64, device="cuda")
+    assert L.gs_evp_tridiag_eigenvalues(plan._h, d.data_ptr(), e.data_ptr(), N, lam.data_ptr(), None) == gs.GS_OK
+    assert L.gs_standard_eigenvalues(plan._h, A.data_ptr(), N, lam.data_ptr(), None) == gs.GS_OK
+    assert plan.last_info(raise_on_failure=False) == N // 2 + 1
+    assert torch.equal(A, A0)
+    assert torch.all(d == 5.0) and torch.all(e == 6.0) and torch.all(tau == 7.0) and torch.all(lam == 8.0)
+    # and the same plan works again once the flag is cleared
+    plan.clear_info()
+    d2, e2, _ = plan.evp_tridiagonalize(A)
+    assert plan.last_info() == 0
+    ref = torch.linalg.eigvalsh(A0.cpu() if not cplx else A0.cpu())          # (a check of the recovery only; parity is in test_gpu_evp.py)
+    got = plan.evp_tridiag_eigenvalues(d2, e2).cpu()
+    assert (got - ref).abs().max().item() <= 1e-11 * max(1.0, ref.abs().max().item())
+    plan.close()
