@@ -285,65 +285,106 @@ __global__ void __launch_bounds__(256) dc_setup_kernel(const double* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// M2: deflation scan (sequential in the sorted order: one thread per merge after a parallel max-reduction).
+// M2: deflation scan, one CTA per merge.  The scan is sequential in the sorted order (an entry is compared with the
+// last survivor, which a rotation may have changed), so one thread runs it -- but out of shared memory, which all
+// threads fill in chunks, with the survivor's entry in registers (448 -> ~40 ns per entry: the loop used to be a chain
+// of global-memory round trips), and with the hypot and the two divisions of the rotation test only where the test is
+// not decided by a factor of two without them.  The grouped order of the survivors is then formed by all threads.
 // ---------------------------------------------------------------------------------------------------------
+constexpr int kDeflChunk = 1024;
 __global__ void __launch_bounds__(256) dc_deflate_kernel(DcArrays a)
 {
     if (*a.info != 0) return;
     MergeDesc& ds = a.desc[blockIdx.x];
     const int off = ds.off, n = ds.n1 + ds.n2;
+    const int t = threadIdx.x;
     __shared__ double s_max[256];
+    __shared__ double s_dm[kDeflChunk], s_z[kDeflChunk];
+    __shared__ int s_src[kDeflChunk], s_typ[kDeflChunk];
+    __shared__ int s_c[3][256];
+    __shared__ int s_k;
     double mx = 0.0;
-    for (int j = threadIdx.x; j < n; j += 256) mx = fmax(mx, fmax(fabs(a.dm[off + j]), fabs(a.zs[off + j])));
-    s_max[threadIdx.x] = mx;
+    for (int j = t; j < n; j += 256) mx = fmax(mx, fmax(fabs(a.dm[off + j]), fabs(a.zs[off + j])));
+    s_max[t] = mx;
     __syncthreads();
     for (int o = 128; o > 0; o >>= 1) {
-        if (threadIdx.x < o) s_max[threadIdx.x] = fmax(s_max[threadIdx.x], s_max[threadIdx.x + o]);
+        if (t < o) s_max[t] = fmax(s_max[t], s_max[t + o]);
         __syncthreads();
     }
-    if (threadIdx.x != 0) return;
     const double tol = 8.0 * (DBL_EPSILON * 0.5) * s_max[0];
     const double rho = ds.rho;
-    double* dm = a.dm + off; double* z = a.zs + off; int* src = a.srcm + off; int* typ = a.typ + off;
-    int k = 0, ndef = 0, nrot = 0, pj = -1;
-    // non-deflated entries are compacted in place at the front (index k <= j always), deflated ones go to dval
-    auto defl = [&](int j) { a.dval[off + ndef] = dm[j]; a.dsrc[off + ndef] = src[j]; a.dtyp[off + ndef] = typ[j]; ++ndef; };
-    auto keep = [&](int j) { a.dlam[off + k] = dm[j]; a.wz[off + k] = z[j]; a.gsrc[off + k] = src[j]; a.gtyp[off + k] = typ[j]; ++k; };
-    for (int j = 0; j < n; ++j) {
-        if (rho * fabs(z[j]) <= tol) { defl(j); continue; }
-        if (pj < 0) { pj = j; continue; }
-        double s = z[pj], c = z[j];
-        const double tau = hypot(c, s);
-        const double tdiff = dm[j] - dm[pj];
-        c /= tau;
-        s = -s / tau;
-        if (fabs(tdiff * c * s) <= tol) {
-            z[j] = tau; z[pj] = 0.0;
-            a.rota[off + nrot] = src[pj]; a.rotb[off + nrot] = src[j];
-            a.rotta[off + nrot] = typ[pj]; a.rottb[off + nrot] = typ[j];
-            a.rotc[off + nrot] = c; a.rots[off + nrot] = s;
-            ++nrot;
-            if (typ[pj] != typ[j]) { typ[pj] = 2; typ[j] = 2; }
-            const double tt = dm[pj] * c * c + dm[j] * s * s;
-            dm[j] = dm[pj] * s * s + dm[j] * c * c;
-            dm[pj] = tt;
-            defl(pj);
-            pj = j;
-        } else {
-            keep(pj);
-            pj = j;
+    // thread 0: k survivors (compacted into dlam, wz, gsrc, gtyp), ndef deflated entries (dval, dsrc, dtyp), nrot rotations;
+    // (p_*) = the last survivor so far, not yet written out
+    int k = 0, ndef = 0, nrot = 0;
+    bool have = false;
+    double p_dm = 0.0, p_z = 0.0;
+    int p_src = 0, p_typ = 0;
+    auto defl = [&](double dv, int sv, int tv) { a.dval[off + ndef] = dv; a.dsrc[off + ndef] = sv; a.dtyp[off + ndef] = tv; ++ndef; };
+    auto keep = [&](double dv, double zv, int sv, int tv) { a.dlam[off + k] = dv; a.wz[off + k] = zv; a.gsrc[off + k] = sv; a.gtyp[off + k] = tv; ++k; };
+    for (int c0 = 0; c0 < n; c0 += kDeflChunk) {
+        const int cn = min(kDeflChunk, n - c0);
+        for (int i = t; i < cn; i += 256) {
+            s_dm[i] = a.dm[off + c0 + i]; s_z[i] = a.zs[off + c0 + i]; s_src[i] = a.srcm[off + c0 + i]; s_typ[i] = a.typ[off + c0 + i];
         }
+        __syncthreads();
+        if (t == 0) {
+            for (int jj = 0; jj < cn; ++jj) {
+                const double dj = s_dm[jj], zj = s_z[jj];
+                const int sj = s_src[jj], tj = s_typ[jj];
+                if (rho * fabs(zj) <= tol) { defl(dj, sj, tj); continue; }
+                if (!have) { have = true; p_dm = dj; p_z = zj; p_src = sj; p_typ = tj; continue; }
+                const double tdiff = dj - p_dm;
+                // |tdiff c s| = |tdiff| |z_j z_p| / (z_j^2 + z_p^2): beyond twice the tolerance the rotation test below fails for sure
+                bool rotate = false;
+                double c = zj, sn = p_z, tau = 0.0;
+                if (!(fabs(tdiff) * fabs(zj * p_z) > 2.0 * tol * fma(zj, zj, p_z * p_z))) {
+                    tau = hypot(c, sn);
+                    c /= tau;
+                    sn = -sn / tau;
+                    rotate = fabs(tdiff * c * sn) <= tol;
+                }
+                if (rotate) {
+                    a.rota[off + nrot] = p_src; a.rotb[off + nrot] = sj;
+                    a.rotta[off + nrot] = p_typ; a.rottb[off + nrot] = tj;
+                    a.rotc[off + nrot] = c; a.rots[off + nrot] = sn;
+                    ++nrot;
+                    const int ty = (p_typ != tj) ? 2 : tj;
+                    const double tt = p_dm * c * c + dj * sn * sn;
+                    const double dn = p_dm * sn * sn + dj * c * c;
+                    defl(tt, p_src, ty);
+                    p_dm = dn; p_z = tau; p_src = sj; p_typ = ty;
+                } else {
+                    keep(p_dm, p_z, p_src, p_typ);
+                    p_dm = dj; p_z = zj; p_src = sj; p_typ = tj;
+                }
+            }
+        }
+        __syncthreads();
     }
-    if (pj >= 0) keep(pj);
-    // grouped order of the non-deflated columns: [from Q1 only | mixed | from Q2 only]
-    int c1 = 0, c2 = 0, c3 = 0;
-    for (int q = 0; q < k; ++q) { const int ty = a.gtyp[off + q]; c1 += ty == 1; c2 += ty == 2; c3 += ty == 3; }
-    int p1 = 0, p2 = c1, p3 = c1 + c2;
-    for (int q = 0; q < k; ++q) {
+    if (t == 0) {
+        if (have) keep(p_dm, p_z, p_src, p_typ);
+        s_k = k;
+    }
+    __syncthreads();
+    // grouped order of the non-deflated columns: [from Q1 only | mixed | from Q2 only]; thread t owns a run of them
+    k = s_k;
+    const int len = (k + 255) / 256, q0 = min(t * len, k), q1 = min(q0 + len, k);
+    int n1 = 0, n2 = 0, n3 = 0;
+    for (int q = q0; q < q1; ++q) { const int ty = a.gtyp[off + q]; n1 += ty == 1; n2 += ty == 2; n3 += ty == 3; }
+    s_c[0][t] = n1; s_c[1][t] = n2; s_c[2][t] = n3;
+    __syncthreads();
+    int c1 = 0, c2 = 0, c3 = 0, b1 = 0, b2 = 0, b3 = 0;       // totals, and the counts of the runs before this thread's
+    for (int u = 0; u < 256; ++u) {
+        const int v1 = s_c[0][u], v2 = s_c[1][u], v3 = s_c[2][u];
+        if (u < t) { b1 += v1; b2 += v2; b3 += v3; }
+        c1 += v1; c2 += v2; c3 += v3;
+    }
+    int p1 = b1, p2 = c1 + b2, p3 = c1 + c2 + b3;
+    for (int q = q0; q < q1; ++q) {
         const int ty = a.gtyp[off + q];
         a.gpos[off + q] = ty == 1 ? p1++ : ty == 2 ? p2++ : p3++;
     }
-    ds.k = k; ds.c1 = c1; ds.c2 = c2; ds.c3 = c3; ds.nrot = nrot; ds.fail = 0;
+    if (t == 0) { ds.k = k; ds.c1 = c1; ds.c2 = c2; ds.c3 = c3; ds.nrot = nrot; ds.fail = 0; }
 }
 
 // ---------------------------------------------------------------------------------------------------------
