@@ -15,7 +15,7 @@
 //     eigenvectors x_j = (D - lambda_j)^-1 z^ / ||.|| are then orthogonal to working precision;
 //   * the new eigenvector block is  Q X: two GEMMs on the FP64 tensor-core tile engine (top rows use only the
 //     columns that come from Q1 or were mixed by a deflation rotation, bottom rows likewise) -- all the O(N^3) work.
-// Leaves (128 x 128) are solved by the implicit QL iteration, one CTA each.
+// Leaves (kDcLeaf x kDcLeaf = 64 x 64) are solved by the implicit QL iteration, one CTA each.
 //
 // Eigenvalues of a solved block are kept sorted through an index (dcur ascending, idx -> physical column of Q),
 // so no column is ever moved for the sake of ordering.  All arrays below are indexed by GLOBAL position
@@ -28,7 +28,7 @@
 namespace gs {
 namespace evp {
 
-constexpr int kDcLeaf = 128;
+constexpr int kDcLeaf = 64;       // (128: the leaves' QL iteration is 6 ms at any N; 32: one more level of small GEMMs costs more than the leaves gain from N = 8192 on)
 constexpr int kDcLeafSmemBytes = kDcLeaf * kDcLeaf * 8;     // the leaf's Q block
 
 struct MergeDesc {
@@ -70,10 +70,10 @@ __global__ void dc_cut_kernel(double* d, const double* e, int N)
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Leaf: all eigenpairs of the n x n (n <= 128) tridiagonal block at offset off by the implicit QL iteration with
+// Leaf: all eigenpairs of the n x n (n <= kDcLeaf) tridiagonal block at offset off by the implicit QL iteration with
 // Wilkinson shifts (EISPACK tql2 / LAPACK xSTEQR scheme).  Thread 0 runs the scalar recurrences of one sweep and
 // leaves its rotations in shared memory; then every thread applies them to its own ROW of Q, which lives in dynamic
-// shared memory (128 KB per leaf; in global memory every rotation was an L2 round trip: 7.75 -> see profiles/) and is
+// shared memory (kDcLeaf^2 x 8 B = 32 KB per leaf; with 128 x 128 leaves in global memory every rotation was an L2 round trip: 7.75 -> see profiles/) and is
 // written out once at the end.  Result: dcur ascending, idx = physical column.
 // ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restrict__ dd, const double* __restrict__ ee, int N, DcArrays a)
@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(kDcLeaf) dc_leaf_kernel(const double* __restri
     const int t = threadIdx.x;
     __shared__ double d[kDcLeaf], e[kDcLeaf], cs[kDcLeaf], sn[kDcLeaf];
     __shared__ int s_l, s_m, s_cnt, s_fail;
-    extern __shared__ double dc_leaf_q[];        // the leaf's Q block (128 x 128, column-major, ld kDcLeaf): every sweep rewrites it
+    extern __shared__ double dc_leaf_q[];        // the leaf's Q block (kDcLeaf x kDcLeaf, column-major): every sweep rewrites it
     if (t < n) { d[t] = dd[off + t]; e[t] = (t + 1 < n) ? ee[off + t] : 0.0; }
     double* Q = dc_leaf_q;
     constexpr long long ldq = kDcLeaf;
