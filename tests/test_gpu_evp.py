@@ -152,7 +152,7 @@ def test_solve_exact_multiplicities_and_decoupled_blocks():
     # (b) zero couplings exactly at the cut points (rho = 0) and tiny ones elsewhere
     d = rng.standard_normal(N)
     e = rng.standard_normal(N - 1)
-    e[127::128] = 0.0
+    e[63::64] = 0.0                                     # (the leaves are 64 wide: every cut of every level)
     e[300] = 1e-200
     eps, Z = _solve(d, e)
     _check_tridiag_pairs(d, e, eps, Z)
@@ -166,6 +166,21 @@ def test_solve_exact_multiplicities_and_decoupled_blocks():
     e = 10.0 ** rng.uniform(-10, 2, N - 1)
     eps, Z = _solve(d, e, N // 2)
     _check_tridiag_pairs(d, e, eps, Z)
+
+
+@pytest.mark.parametrize("glue", [1e-4, 1e-8, 1e-14])
+def test_solve_glued_wilkinson(glue):
+    """Copies of W21+ glued by a small coupling: clusters of nearly equal eigenvalues whose secular equations have roots
+    next to their poles and nearly coincident poles -- the hard case for the root finder (regula falsi on f |mu| with a
+    bisection safeguard, csrc/evp_dc.cuh) and for the deflation test."""
+    copies, m = 24, 10
+    d = np.tile(np.abs(np.arange(-m, m + 1)).astype(float), copies)
+    e = np.ones(len(d) - 1)
+    e[2 * m::2 * m + 1] = glue
+    eps, Z = _solve(d, e)
+    _check_tridiag_pairs(d, e, eps, Z)
+    eps_k, Z_k = _solve(d, e, len(d) // 3)
+    _check_tridiag_pairs(d, e, eps_k, Z_k)
 
 
 def test_stage_calls_chain_like_standard_eigh():
