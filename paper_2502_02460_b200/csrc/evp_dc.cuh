@@ -9,8 +9,9 @@
 //   * deflation: entries with rho |z_j| tiny, and pairs of (nearly) equal d rotated so that one z vanishes, are
 //     eigenpairs already;
 //   * the other k eigenvalues are the roots of  1 + rho sum_i z_i^2 / (d_i - lambda) = 0, one per interval
-//     (d_j, d_j+1): found by bisection on mu = lambda - d_origin with the origin at the NEARER pole, so that every
-//     difference d_i - lambda_j = (d_i - d_origin) - mu is formed without cancellation;
+//     (d_j, d_j+1): found in mu = lambda - d_origin with the origin at the NEARER pole, so that every difference
+//     d_i - lambda_j = (d_i - d_origin) - mu is formed without cancellation (a bracket shrunk until it cannot be halved:
+//     regula falsi on f |mu| with a bisection safeguard, dc_secular_kernel);
 //   * z is replaced by the z^ for which the computed lambda are the EXACT eigenvalues (Loewner's formula): the
 //     eigenvectors x_j = (D - lambda_j)^-1 z^ / ||.|| are then orthogonal to working precision;
 //   * the new eigenvector block is  Q X: two GEMMs on the FP64 tensor-core tile engine (top rows use only the
