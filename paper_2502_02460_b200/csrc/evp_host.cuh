@@ -225,7 +225,7 @@ gs_status_t evp_tridiagonalize_t(gs_plan* plan, const EvpBuffers& b, void* A, do
         int dev = 0, sms = 0;
         GS_CUDA(plan, cudaGetDevice(&dev));
         GS_CUDA(plan, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        comb_threads = sms * 3 * 256;
+        comb_threads = sms * (plan->z ? 2 : 3) * 256;      // one wave of C: three CTAs per SM at the real kernel's register count, two at the complex one's
     }
     // L2 policy of the streamed tiles: 0 plain, 1 evict-first always, 2 evict-first while the triangle exceeds evict_bytes
     static const int evict_mode = std::getenv("GS_EVP_EVICT") != nullptr ? std::atoi(std::getenv("GS_EVP_EVICT")) : 2;
